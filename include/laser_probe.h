@@ -1,0 +1,183 @@
+/*
+ * laser_probe.h — C ABI of the B200-native LASER confidence probe.
+ *
+ * One call, laser_probe_confidence(), runs the whole data-parallel hot path of LASER's serving loop
+ * (arxiv/paper_2606_31580; citations are /root/reference/PAPER.md line numbers) for every in-flight
+ * request at a probe point (an "action transition point"):
+ *
+ *   a1  logits[n,v] = sum_k hidden[n,k] * W[v,k]          LM-head projection of the trial-answer
+ *                                                         tokens' final hidden states
+ *   a2  pmax[n] = max_v softmax(logits[n,:]),  argmax[n]  online softmax over the vocabulary; the
+ *                                                         [N,V] logits never leave the SM
+ *   a3  conf[r] = mean_{n in request r} pmax[n]           confidence C_i^(k)
+ *   a4  tau[r]  = clamp(lambda_base - beta*tanh(gamma*(load[r]-L_target)/L_target),
+ *                       lambda_min, lambda_max)           Eq. 5 + clamp
+ *   a5  exit[r] = conf[r] > tau[r]   (strict)             PAPER.md:61, 70, 122 (Algorithm 1 step 6)
+ *
+ * Device code is sm_100a only (TMA + tcgen05/TMEM).  There is no fallback of any kind: on another
+ * device the call returns LASER_E_ARCH.  The library never allocates device memory, never
+ * synchronises the host with the device and never reads device data on the host; all work is
+ * enqueued on the caller's stream.  The only internal state is a small host-side cache of encoded
+ * TMA descriptors, released by laser_shutdown().
+ *
+ * All functions return an int status (LASER_OK == 0, errors negative); none throws or aborts.
+ */
+#ifndef LASER_PROBE_H_
+#define LASER_PROBE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    LASER_OK = 0,
+    LASER_E_NULL = -1,      /* a required pointer is NULL                                             */
+    LASER_E_DIMS = -2,      /* d <= 0, V <= 0, N < 0, R < 0, d % 8 != 0 (TMA row pitch must be 16 B)  */
+    LASER_E_ALIGN = -3,     /* hidden / W not 16-byte aligned                                         */
+    LASER_E_PARAMS = -4,    /* lambda_min > lambda_max, l_target <= 0, or a non-finite parameter      */
+    LASER_E_WORKSPACE = -5, /* workspace NULL or smaller than laser_probe_workspace_bytes()           */
+    LASER_E_ARCH = -6,      /* current device is not compute capability 10.0 (B200)                   */
+    LASER_E_CUDA = -7,      /* a CUDA runtime / driver call failed; see laser_last_error()            */
+    LASER_E_MODE = -8       /* unknown aggregate mode                                                 */
+};
+
+/* Hyper-parameters of Eq. 5; defaults are the paper's.  `l_target` and load[] share
+ * one unit: the paper counts active requests (L_target = 10); only the ratio enters Eq. 5. */
+typedef struct {
+    float lambda_base; /* 0.95 */
+    float beta;        /* 0.04 */
+    float gamma;       /* 1.0  */
+    float l_target;    /* 10   */
+    float lambda_min;  /* 0.88 */
+    float lambda_max;  /* 0.97 */
+} laser_tau_params;
+
+/* N = rows allocated in `hidden` (valid rows are [0, req_offsets[R])), d = hidden size,
+ * V = vocabulary size, R = number of requests. */
+typedef struct {
+    int32_t N, d, V, R;
+} laser_probe_dims;
+
+/* How a call is laid out on the GPU (informational; filled by laser_probe_plan_query). */
+typedef struct {
+    int32_t num_sms;         /* SMs the plan was made for                                             */
+    int32_t m_tiles;         /* ceil(N / 128) token tiles                                             */
+    int32_t splits;          /* vocabulary splits S                                                   */
+    int32_t tiles_per_split; /* vocab tiles per split T                                               */
+    int32_t tile_n;          /* vocab rows per tile BN (multiple of 16, <= 256)                       */
+    int32_t k_blocks;        /* ceil(d / 64)                                                          */
+    int32_t stages;          /* shared-memory pipeline depth                                          */
+    int32_t grid;            /* CTAs of the fused kernel (persistent, <= num_sms)                     */
+    int32_t work_items;      /* m_tiles * splits                                                      */
+    int32_t smem_bytes;      /* dynamic shared memory per CTA                                         */
+    int32_t kernel_launches; /* kernels one laser_probe_confidence call enqueues                      */
+} laser_probe_plan;
+
+/* Aggregate that turns the per-token max probabilities of a request into its confidence.
+ * The paper does not fix it; MEAN is the default reading (A1). */
+enum { LASER_AGG_MEAN = 0, LASER_AGG_GEOMEAN = 1, LASER_AGG_MIN = 2 };
+
+/* Writes the paper's defaults.  Host. */
+int laser_tau_params_default(laser_tau_params* out);
+
+/* Device scratch laser_probe_confidence needs for `dims`, in bytes (12 * splits * m_tiles * 128,
+ * at least 16).  Returns 0 for invalid dims.  Host; needs no GPU. */
+size_t laser_probe_workspace_bytes(const laser_probe_dims* dims);
+
+/* Fills *plan for `dims`.  Host; needs no GPU (assumes 148 SMs when no device is present). */
+int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan);
+
+/*
+ * The hot path a1-a5.  Asynchronous on `stream`; returns after enqueueing.
+ *
+ *   hidden       device, bf16 [N, d] row-major, 16-byte aligned, d % 8 == 0.  Post-final-norm states.
+ *   W            device, bf16 [V, d] row-major, 16-byte aligned (LM-head / unembedding matrix).
+ *   req_offsets  device, int32 [R+1], non-decreasing, [0] == 0, [R] <= N (CSR over rows; a
+ *                precondition, not checked: the library never reads device data on the host).
+ *                Rows >= req_offsets[R] are padding.
+ *   load         device, float [R]: smoothed load Lbar of each request's probe point, unit of l_target.
+ *   tau_params   HOST pointer; copied by value into the launch.
+ *   out_conf     device, float [R].   Empty request -> 0.  NaN in a request's rows -> NaN.
+ *   out_argmax   device, int32 [N].   Lowest vocabulary index attaining the row maximum; -1 for
+ *                padding rows.
+ *   out_exit     device, uint8 [R].   1 iff conf > tau (strict); NaN conf -> 0.
+ *   dims         HOST pointer.
+ *   workspace    device scratch >= laser_probe_workspace_bytes(dims), 16-byte aligned; contents are
+ *                overwritten; may be reused by the next call on the same stream.
+ *   stream       cudaStream_t (NULL = legacy default stream).
+ *   out_tau_opt  device float [R] or NULL: the thresholds.
+ *   out_pmax_opt device float [N] or NULL: per-row max probability (NaN for padding rows).
+ *
+ * All buffers are caller-owned.  N == 0 or R == 0 is a successful no-op on conf/exit (argmax of all
+ * N rows is still set to -1 when R == 0).
+ */
+int laser_probe_confidence(const void* hidden, const void* W, const int32_t* req_offsets,
+                           const float* load, const laser_tau_params* tau_params, float* out_conf,
+                           int32_t* out_argmax, uint8_t* out_exit, const laser_probe_dims* dims,
+                           void* workspace, size_t workspace_bytes, void* stream,
+                           float* out_tau_opt, float* out_pmax_opt);
+
+/* Same, with an explicit aggregate (LASER_AGG_*). */
+int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t* req_offsets,
+                               const float* load, const laser_tau_params* tau_params,
+                               float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+                               const laser_probe_dims* dims, void* workspace,
+                               size_t workspace_bytes, void* stream, float* out_tau_opt,
+                               float* out_pmax_opt, int aggregate_mode);
+
+/*
+ * End-to-end form with HOST buffers for the per-step tensors (W stays resident on the device: it is
+ * the model's weight, not a per-step input).  Copies hidden / req_offsets / load to the device
+ * staging buffers, runs laser_probe_confidence, copies conf / argmax / exit back, and synchronises
+ * `stream` before returning.  Host buffers should be pinned for the copies to be asynchronous.
+ *
+ *   h_*          host pointers (same shapes and dtypes as above)
+ *   d_staging    device scratch >= laser_probe_staging_bytes(dims), 256-byte aligned
+ *   W, workspace as above (device)
+ */
+size_t laser_probe_staging_bytes(const laser_probe_dims* dims);
+int laser_probe_confidence_host(const void* h_hidden, const void* W, const int32_t* h_req_offsets,
+                                const float* h_load, const laser_tau_params* tau_params,
+                                float* h_out_conf, int32_t* h_out_argmax, uint8_t* h_out_exit,
+                                const laser_probe_dims* dims, void* workspace,
+                                size_t workspace_bytes, void* d_staging, size_t staging_bytes,
+                                void* stream);
+
+/* Host, scalar-array version of a4 (Eq. 5 + clamp) in the same float arithmetic as the kernel. */
+int laser_tau_from_load(const float* load, int32_t R, const laser_tau_params* tau_params,
+                        float* out_tau);
+
+/* Control-plane helpers either side of the probe in Algorithm 1 (host scalars, "O(1)").
+ * EMA: lbar <- alpha*L + (1-alpha)*lbar, in place over R independent trackers. */
+int laser_ema_update(float* lbar, const float* L, int32_t R, float alpha);
+
+/* Budget pre-allocation, Eq. 6-8; defaults PAPER.md:166, 195. */
+typedef struct {
+    float b_base;   /* 10  */
+    float b_min;    /* 2   */
+    float f_min;    /* 0.6 */
+    float f_max;    /* 1.5 */
+    float p_min;    /* 50  */
+    float p_max;    /* 275 */
+    float l_target; /* 10  */
+} laser_budget_params;
+int laser_budget_params_default(laser_budget_params* out);
+int laser_allocate_budget(const int32_t* prompt_tokens, const float* L, int32_t R,
+                          const laser_budget_params* params, int32_t* out_budget);
+
+/* Text for a status code; never NULL. */
+const char* laser_status_string(int status);
+/* Detail of the last LASER_E_CUDA on this thread ("" if none). */
+const char* laser_last_error(void);
+/* Number of kernels this library has enqueued since load (all threads). */
+uint64_t laser_kernel_launch_count(void);
+/* Drops the TMA descriptor cache. */
+int laser_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LASER_PROBE_H_ */

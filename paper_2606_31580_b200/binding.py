@@ -1,0 +1,241 @@
+"""Thin ctypes binding of include/laser_probe.h — argument marshalling only.
+
+Every step of the path (projection, online softmax, aggregate, threshold, exit mask) runs in the CUDA
+kernels of csrc/.  torch is used for device memory and streams, nothing else.  There is no CPU or
+eager fallback: if liblaser_probe.so is missing this module raises on first use, and on a device
+that is not sm_100 the library returns LASER_E_ARCH, which is raised as an error.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass
+from pathlib import Path
+
+_SO = Path(__file__).resolve().parent / "liblaser_probe.so"
+_lib = None
+
+AGG_MEAN, AGG_GEOMEAN, AGG_MIN = 0, 1, 2
+
+EXPORTS = [
+    "laser_tau_params_default", "laser_probe_workspace_bytes", "laser_probe_plan_query",
+    "laser_probe_confidence", "laser_probe_confidence_agg", "laser_probe_staging_bytes",
+    "laser_probe_confidence_host", "laser_tau_from_load", "laser_ema_update",
+    "laser_budget_params_default", "laser_allocate_budget", "laser_status_string",
+    "laser_last_error", "laser_kernel_launch_count", "laser_shutdown",
+]
+
+
+class TauParams(C.Structure):
+    """laser_tau_params; defaults are the paper's."""
+    _fields_ = [(n, C.c_float) for n in
+                ("lambda_base", "beta", "gamma", "l_target", "lambda_min", "lambda_max")]
+
+    def __init__(self, lambda_base=0.95, beta=0.04, gamma=1.0, l_target=10.0, lambda_min=0.88,
+                 lambda_max=0.97):
+        super().__init__(lambda_base, beta, gamma, l_target, lambda_min, lambda_max)
+
+
+class BudgetParams(C.Structure):
+    """laser_budget_params; defaults PAPER.md:166, 195."""
+    _fields_ = [(n, C.c_float) for n in
+                ("b_base", "b_min", "f_min", "f_max", "p_min", "p_max", "l_target")]
+
+    def __init__(self, b_base=10.0, b_min=2.0, f_min=0.6, f_max=1.5, p_min=50.0, p_max=275.0,
+                 l_target=10.0):
+        super().__init__(b_base, b_min, f_min, f_max, p_min, p_max, l_target)
+
+
+class Dims(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("N", "d", "V", "R")]
+
+
+class Plan(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in
+                ("num_sms", "m_tiles", "splits", "tiles_per_split", "tile_n", "k_blocks", "stages",
+                 "grid", "work_items", "smem_bytes", "kernel_launches")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+class LaserError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"laser_probe status {status}: {text}")
+        self.status = status
+
+
+def lib():
+    """Load liblaser_probe.so (built by paper_2606_31580_b200.build).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not _SO.exists():
+            raise FileNotFoundError(
+                f"{_SO} not found: run `python -m paper_2606_31580_b200.build` "
+                "(there is no fallback implementation)")
+        L = C.CDLL(str(_SO))
+        vp, i32p, fp, u8p = C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p
+        tp, dp = C.POINTER(TauParams), C.POINTER(Dims)
+        L.laser_tau_params_default.argtypes = [tp]
+        L.laser_probe_workspace_bytes.argtypes = [dp]
+        L.laser_probe_workspace_bytes.restype = C.c_size_t
+        L.laser_probe_staging_bytes.argtypes = [dp]
+        L.laser_probe_staging_bytes.restype = C.c_size_t
+        L.laser_probe_plan_query.argtypes = [dp, C.POINTER(Plan)]
+        common = [vp, vp, i32p, fp, tp, fp, i32p, u8p, dp, vp, C.c_size_t, vp, fp, fp]
+        L.laser_probe_confidence.argtypes = common
+        L.laser_probe_confidence_agg.argtypes = common + [C.c_int]
+        L.laser_probe_confidence_host.argtypes = [vp, vp, i32p, fp, tp, fp, i32p, u8p, dp, vp,
+                                                  C.c_size_t, vp, C.c_size_t, vp]
+        L.laser_tau_from_load.argtypes = [fp, C.c_int32, tp, fp]
+        L.laser_ema_update.argtypes = [fp, fp, C.c_int32, C.c_float]
+        L.laser_budget_params_default.argtypes = [C.POINTER(BudgetParams)]
+        L.laser_allocate_budget.argtypes = [i32p, fp, C.c_int32, C.POINTER(BudgetParams), i32p]
+        L.laser_status_string.argtypes = [C.c_int]
+        L.laser_status_string.restype = C.c_char_p
+        L.laser_last_error.restype = C.c_char_p
+        L.laser_kernel_launch_count.restype = C.c_uint64
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        L = lib()
+        txt = L.laser_status_string(rc).decode()
+        if rc == -7:
+            txt += " — " + L.laser_last_error().decode()
+        raise LaserError(rc, txt)
+
+
+def plan_query(N, d, V, R) -> dict:
+    p = Plan()
+    _check(lib().laser_probe_plan_query(C.byref(Dims(N, d, V, R)), C.byref(p)))
+    return p.as_dict()
+
+
+def workspace_bytes(N, d, V, R) -> int:
+    return int(lib().laser_probe_workspace_bytes(C.byref(Dims(N, d, V, R))))
+
+
+def staging_bytes(N, d, V, R) -> int:
+    return int(lib().laser_probe_staging_bytes(C.byref(Dims(N, d, V, R))))
+
+
+def kernel_launch_count() -> int:
+    return int(lib().laser_kernel_launch_count())
+
+
+def tau_from_load(load, params: TauParams):
+    """Host arrays (numpy float32) -> numpy float32; laser_tau_from_load."""
+    import numpy as np
+    load = np.ascontiguousarray(load, np.float32).reshape(-1)
+    out = np.empty_like(load)
+    _check(lib().laser_tau_from_load(load.ctypes.data, load.shape[0], C.byref(params), out.ctypes.data))
+    return out
+
+
+def ema_update(lbar, L, alpha=0.3):
+    """In place on a numpy float32 array `lbar`; laser_ema_update."""
+    import numpy as np
+    assert lbar.dtype == np.float32 and lbar.flags.c_contiguous
+    L = np.ascontiguousarray(L, np.float32).reshape(-1)
+    _check(lib().laser_ema_update(lbar.ctypes.data, L.ctypes.data, lbar.shape[0], alpha))
+    return lbar
+
+
+def allocate_budget(prompt_tokens, L, params: BudgetParams | None = None):
+    """laser_allocate_budget, Eq. 6-8."""
+    import numpy as np
+    pt = np.ascontiguousarray(prompt_tokens, np.int32).reshape(-1)
+    L = np.ascontiguousarray(L, np.float32).reshape(-1)
+    out = np.empty(pt.shape[0], np.int32)
+    q = params or BudgetParams()
+    _check(lib().laser_allocate_budget(pt.ctypes.data, L.ctypes.data, pt.shape[0], C.byref(q), out.ctypes.data))
+    return out
+
+
+@dataclass
+class ProbeOutputs:
+    conf: "torch.Tensor"      # float32 [R]
+    argmax: "torch.Tensor"    # int32 [N]
+    exit: "torch.Tensor"      # uint8 [R]
+    tau: "torch.Tensor | None"
+    pmax: "torch.Tensor | None"
+
+
+class Probe:
+    """Caller-owned buffers for repeated laser_probe_confidence calls of one shape (device memory
+    from torch; the library itself allocates nothing)."""
+
+    def __init__(self, N, d, V, R, device="cuda", debug_outputs=True):
+        import torch
+        self.torch = torch
+        self.dims = Dims(N, d, V, R)
+        self.device = torch.device(device)
+        wb = workspace_bytes(N, d, V, R)
+        if wb == 0:
+            raise LaserError(-2, "invalid dimensions")
+        self.workspace = torch.empty(wb, dtype=torch.uint8, device=self.device)
+        self.conf = torch.empty(R, dtype=torch.float32, device=self.device)
+        self.argmax = torch.empty(N, dtype=torch.int32, device=self.device)
+        self.exit = torch.empty(R, dtype=torch.uint8, device=self.device)
+        self.tau = torch.empty(R, dtype=torch.float32, device=self.device) if debug_outputs else None
+        self.pmax = torch.empty(N, dtype=torch.float32, device=self.device) if debug_outputs else None
+        self.plan = plan_query(N, d, V, R)
+
+    def __call__(self, hidden, W, req_offsets, load, params: TauParams, stream=None, agg=AGG_MEAN):
+        """hidden bf16 [N,d], W bf16 [V,d], req_offsets int32 [R+1], load float32 [R] — device
+        tensors.  Enqueues on `stream` (default: torch's current stream); does not synchronise."""
+        torch = self.torch
+        d = self.dims
+        assert hidden.dtype == torch.bfloat16 and W.dtype == torch.bfloat16
+        assert hidden.is_contiguous() and W.is_contiguous()
+        assert tuple(hidden.shape) == (d.N, d.d) and tuple(W.shape) == (d.V, d.d)
+        assert req_offsets.dtype == torch.int32 and req_offsets.numel() == d.R + 1
+        assert load.dtype == torch.float32 and load.numel() == d.R
+        s = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+        _check(lib().laser_probe_confidence_agg(
+            hidden.data_ptr(), W.data_ptr(), req_offsets.data_ptr(), load.data_ptr(),
+            C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(),
+            C.byref(d), self.workspace.data_ptr(), self.workspace.numel(), s,
+            self.tau.data_ptr() if self.tau is not None else None,
+            self.pmax.data_ptr() if self.pmax is not None else None, agg))
+        return ProbeOutputs(self.conf, self.argmax, self.exit, self.tau, self.pmax)
+
+
+class HostProbe:
+    """laser_probe_confidence_host: per-step tensors in pinned HOST memory, W resident on device."""
+
+    def __init__(self, N, d, V, R, device="cuda"):
+        import torch
+        self.torch = torch
+        self.dims = Dims(N, d, V, R)
+        self.device = torch.device(device)
+        self.workspace = torch.empty(workspace_bytes(N, d, V, R), dtype=torch.uint8, device=self.device)
+        self.staging = torch.empty(staging_bytes(N, d, V, R), dtype=torch.uint8, device=self.device)
+        self.conf = torch.empty(R, dtype=torch.float32).pin_memory()
+        self.argmax = torch.empty(N, dtype=torch.int32).pin_memory()
+        self.exit = torch.empty(R, dtype=torch.uint8).pin_memory()
+        self.h2d_bytes = N * d * 2 + (R + 1) * 4 + R * 4
+        self.d2h_bytes = R * 4 + N * 4 + R
+
+    def __call__(self, h_hidden, W, h_req_offsets, h_load, params: TauParams, stream=None):
+        torch = self.torch
+        assert not h_hidden.is_cuda and W.is_cuda
+        s = (stream or torch.cuda.current_stream(self.device)).cuda_stream
+        _check(lib().laser_probe_confidence_host(
+            h_hidden.data_ptr(), W.data_ptr(), h_req_offsets.data_ptr(), h_load.data_ptr(),
+            C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(),
+            C.byref(self.dims), self.workspace.data_ptr(), self.workspace.numel(),
+            self.staging.data_ptr(), self.staging.numel(), s))
+        return ProbeOutputs(self.conf, self.argmax, self.exit, None, None)
+
+
+def bf16_tensor_from_bits(bits, device=None, pin=False):
+    """numpy uint16 bf16 bit patterns -> torch.bfloat16 tensor (no value conversion)."""
+    import numpy as np
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)
+    if pin:
+        t = t.pin_memory()
+    return t.to(device) if device is not None else t

@@ -1,0 +1,481 @@
+// laser_probe.cu — host side of the C ABI declared in include/laser_probe.h: argument validation,
+// launch planning, TMA descriptor encoding (driver entry point fetched through the runtime, no
+// -lcuda), and the two kernel launches.  No device allocation, no host<->device synchronisation
+// (except in the explicit *_host entry point), no fallback path.
+#include "../../include/laser_probe.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <mutex>
+#include <string>
+#include <unordered_map>
+
+#include "probe_kernels.cuh"
+
+namespace {
+
+using namespace laser;
+
+thread_local std::string g_last_error;
+std::atomic<uint64_t> g_launches{0};
+
+constexpr int kDefaultSMs = 148;             // B200
+constexpr int kMaxDynSmem = 227 * 1024;      // per-CTA opt-in limit on sm_100
+constexpr int kSmemSlack = 1024 + 256;       // alignment slack + barrier block
+
+int set_cuda_error(const char* what, cudaError_t e) {
+    g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+    return LASER_E_CUDA;
+}
+
+// ---------------------------------------------------------------------------------------- device
+struct DeviceInfo {
+    bool queried = false, ok = false;
+    int sms = kDefaultSMs, cc_major = 0, cc_minor = 0;
+    bool attr_set = false;
+};
+std::mutex g_mu;
+DeviceInfo g_dev[64];
+
+// Returns the cached info of the current device; cuda_ok = false if no device can be queried.
+DeviceInfo* current_device(bool* cuda_ok) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+        (void)cudaGetLastError();
+        *cuda_ok = false;
+        return nullptr;
+    }
+    std::lock_guard<std::mutex> lk(g_mu);
+    DeviceInfo& d = g_dev[dev];
+    if (!d.queried) {
+        d.queried = true;
+        d.ok = cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+               cudaDeviceGetAttribute(&d.cc_major, cudaDevAttrComputeCapabilityMajor, dev) == cudaSuccess &&
+               cudaDeviceGetAttribute(&d.cc_minor, cudaDevAttrComputeCapabilityMinor, dev) == cudaSuccess;
+        if (!d.ok) (void)cudaGetLastError();
+    }
+    *cuda_ok = d.ok;
+    return &d;
+}
+
+// ---------------------------------------------------------------------------------------- plan
+int ceil_div(int a, int b) { return (a + b - 1) / b; }
+int round_up(int a, int b) { return ceil_div(a, b) * b; }
+int gcd_i(int a, int b) { while (b) { int t = a % b; a = b; b = t; } return a; }
+
+bool dims_valid(const laser_probe_dims* d) {
+    return d && d->d > 0 && d->V > 0 && d->N >= 0 && d->R >= 0 && (d->d % 8) == 0;
+}
+
+// Choose (splits, tiles_per_split, tile_n): the vocabulary is cut into splits of T*BN rows, BN a
+// multiple of 16 and <= 256.  m_tiles*splits should fill the SMs in whole rounds; among such
+// choices minimise the busiest CTA's work, counted in W rows plus a charge per tile for re-streaming
+// the 128 hidden rows from L2.
+void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
+    const int m_tiles = dm.N > 0 ? ceil_div(dm.N, kTileM) : 1;
+    const int s_unit = num_sms / gcd_i(num_sms, m_tiles);
+    const double kTileCharge = 32.0;  // W-row equivalents per tile (hidden re-stream, pipeline bubble)
+    double best = 1e300;
+    int bS = 1, bT = 1, bBN = 16;
+    for (int k = 1; k <= 4; ++k) {
+        const int s_try = s_unit * k;
+        const int L = ceil_div(dm.V, s_try);
+        const int t_min = ceil_div(L, kMaxTileN);
+        for (int T = t_min; T <= t_min + 3; ++T) {
+            const int BN = round_up(ceil_div(L, T), 16);
+            if (BN > kMaxTileN) continue;
+            const int S = ceil_div(dm.V, T * BN);
+            const long items = static_cast<long>(m_tiles) * S;
+            const long rounds = (items + num_sms - 1) / num_sms;
+            const double cost = static_cast<double>(rounds) * T * (BN + kTileCharge);
+            if (cost < best - 1e-9) { best = cost; bS = S; bT = T; bBN = BN; }
+        }
+    }
+    pl->num_sms = num_sms;
+    pl->m_tiles = m_tiles;
+    pl->splits = bS;
+    pl->tiles_per_split = bT;
+    pl->tile_n = bBN;
+    pl->k_blocks = ceil_div(dm.d, kBlockK);
+    const int stage_bytes = kABytes + bBN * 128;
+    int stages = (kMaxDynSmem - kSmemSlack) / stage_bytes;
+    if (stages > kMaxStages) stages = kMaxStages;
+    pl->stages = stages;
+    pl->work_items = m_tiles * bS;
+    pl->grid = pl->work_items < num_sms ? pl->work_items : num_sms;
+    pl->smem_bytes = stages * stage_bytes + kSmemSlack;
+    pl->kernel_launches = 2;
+}
+
+size_t workspace_bytes_for(const laser_probe_plan& pl) {
+    size_t b = static_cast<size_t>(12) * pl.splits * pl.m_tiles * kTileM;
+    return b < 16 ? 16 : b;
+}
+
+// ---------------------------------------------------------------------------------------- TMA maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+struct MapKey {
+    const void* ptr;
+    int rows, cols, box_rows;
+    bool operator==(const MapKey& o) const {
+        return ptr == o.ptr && rows == o.rows && cols == o.cols && box_rows == o.box_rows;
+    }
+};
+struct MapKeyHash {
+    size_t operator()(const MapKey& k) const {
+        size_t h = reinterpret_cast<size_t>(k.ptr);
+        h ^= (static_cast<size_t>(k.rows) * 0x9E3779B97F4A7C15ull) ^ (static_cast<size_t>(k.cols) << 20) ^
+             (static_cast<size_t>(k.box_rows) << 44);
+        return h;
+    }
+};
+std::unordered_map<MapKey, CUtensorMap, MapKeyHash> g_maps;
+
+// bf16 [rows, cols] row-major; box = 64 columns (128 B, the swizzle span) x box_rows rows.
+int get_tensor_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMap* out) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!g_encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+            (void)cudaGetLastError();
+            g_last_error = "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled) failed";
+            return LASER_E_CUDA;
+        }
+        g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    const MapKey key{ptr, rows, cols, box_rows};
+    auto it = g_maps.find(key);
+    if (it != g_maps.end()) { *out = it->second; return LASER_OK; }
+    const cuuint64_t gdim[2] = {static_cast<cuuint64_t>(cols), static_cast<cuuint64_t>(rows)};
+    const cuuint64_t gstride[1] = {static_cast<cuuint64_t>(cols) * 2};
+    const cuuint32_t box[2] = {static_cast<cuuint32_t>(kBlockK), static_cast<cuuint32_t>(box_rows)};
+    const cuuint32_t estr[2] = {1, 1};
+    CUtensorMap m;
+    CUresult r = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim,
+                          gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d) rows=%d cols=%d box_rows=%d",
+                 static_cast<int>(r), rows, cols, box_rows);
+        g_last_error = buf;
+        return LASER_E_CUDA;
+    }
+    if (g_maps.size() > 256) g_maps.clear();
+    g_maps.emplace(key, m);
+    *out = m;
+    return LASER_OK;
+}
+
+bool params_valid(const laser_tau_params* t) {
+    return std::isfinite(t->lambda_base) && std::isfinite(t->beta) && std::isfinite(t->gamma) &&
+           std::isfinite(t->l_target) && std::isfinite(t->lambda_min) && std::isfinite(t->lambda_max) &&
+           t->l_target > 0.f && t->lambda_min <= t->lambda_max;
+}
+
+TauParamsDev to_dev(const laser_tau_params* t) {
+    return TauParamsDev{t->lambda_base, t->beta, t->gamma, t->l_target, t->lambda_min, t->lambda_max};
+}
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Staging {
+    size_t hidden, offsets, load, conf, argmax, exit_, total;
+};
+Staging staging_layout(const laser_probe_dims& d) {
+    Staging s;
+    size_t o = 0;
+    s.hidden = o;  o = align_up(o + static_cast<size_t>(d.N) * d.d * 2, 256);
+    s.offsets = o; o = align_up(o + static_cast<size_t>(d.R + 1) * 4, 256);
+    s.load = o;    o = align_up(o + static_cast<size_t>(d.R) * 4, 256);
+    s.conf = o;    o = align_up(o + static_cast<size_t>(d.R) * 4, 256);
+    s.argmax = o;  o = align_up(o + static_cast<size_t>(d.N) * 4, 256);
+    s.exit_ = o;   o = align_up(o + static_cast<size_t>(d.R), 256);
+    s.total = o < 256 ? 256 : o;
+    return s;
+}
+
+}  // namespace
+
+// ============================================================================================ ABI
+extern "C" {
+
+int laser_tau_params_default(laser_tau_params* out) {
+    if (!out) return LASER_E_NULL;
+    *out = laser_tau_params{0.95f, 0.04f, 1.0f, 10.0f, 0.88f, 0.97f};
+    return LASER_OK;
+}
+
+int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan) {
+    if (!dims || !plan) return LASER_E_NULL;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
+    bool ok = false;
+    DeviceInfo* di = current_device(&ok);
+    make_plan(*dims, (ok && di) ? di->sms : kDefaultSMs, plan);
+    return LASER_OK;
+}
+
+size_t laser_probe_workspace_bytes(const laser_probe_dims* dims) {
+    laser_probe_plan pl;
+    if (laser_probe_plan_query(dims, &pl) != LASER_OK) return 0;
+    return workspace_bytes_for(pl);
+}
+
+int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t* req_offsets,
+                               const float* load, const laser_tau_params* tau_params,
+                               float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+                               const laser_probe_dims* dims, void* workspace,
+                               size_t workspace_bytes, void* stream_v, float* out_tau_opt,
+                               float* out_pmax_opt, int aggregate_mode) {
+    if (!dims || !tau_params) return LASER_E_NULL;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
+    if (!params_valid(tau_params)) return LASER_E_PARAMS;
+    if (aggregate_mode < LASER_AGG_MEAN || aggregate_mode > LASER_AGG_MIN) return LASER_E_MODE;
+    const int N = dims->N, R = dims->R;
+    if (N == 0 && R == 0) return LASER_OK;
+    if (N > 0 && (!hidden || !W || !out_argmax)) return LASER_E_NULL;
+    if (R > 0 && (!req_offsets || !load || !out_conf || !out_exit)) return LASER_E_NULL;
+    if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(W) & 15))
+        return LASER_E_ALIGN;
+
+    bool ok = false;
+    DeviceInfo* di = current_device(&ok);
+    if (!ok || !di) { g_last_error = "no usable CUDA device"; return LASER_E_CUDA; }
+    if (di->cc_major != 10 || di->cc_minor != 0) return LASER_E_ARCH;  // sm_100a only, no fallback
+
+    laser_probe_plan pl;
+    make_plan(*dims, di->sms, &pl);
+    if (!workspace || workspace_bytes < workspace_bytes_for(pl) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 15))
+        return LASER_E_WORKSPACE;
+
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+    const int n_pad = pl.m_tiles * kTileM;
+    float* ws_m = static_cast<float*>(workspace);
+    int32_t* ws_a = reinterpret_cast<int32_t*>(ws_m + static_cast<size_t>(pl.splits) * n_pad);
+    float* ws_s = reinterpret_cast<float*>(ws_a + static_cast<size_t>(pl.splits) * n_pad);
+
+    const bool run_fused = (N > 0 && R > 0);
+    if (run_fused) {
+        if (!di->attr_set) {
+            cudaError_t e = cudaFuncSetAttribute(laser_probe_fused_kernel,
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
+            if (e != cudaSuccess) return set_cuda_error("cudaFuncSetAttribute", e);
+            di->attr_set = true;
+        }
+        CUtensorMap tm_h, tm_w;
+        int rc = get_tensor_map(hidden, N, dims->d, kTileM, &tm_h);
+        if (rc != LASER_OK) return rc;
+        rc = get_tensor_map(W, dims->V, dims->d, pl.tile_n, &tm_w);
+        if (rc != LASER_OK) return rc;
+
+        FusedParams fp;
+        fp.n_alloc = N; fp.d = dims->d; fp.V = dims->V;
+        fp.m_tiles = pl.m_tiles; fp.splits = pl.splits; fp.tiles_per_split = pl.tiles_per_split;
+        fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
+        fp.work_items = pl.work_items; fp.n_pad = n_pad;
+        fp.stage_bytes = static_cast<uint32_t>(kABytes + pl.tile_n * 128);
+        fp.tx_bytes = fp.stage_bytes;  // OOB rows are zero-filled and still counted
+        // W is streamed once when a single token tile exists; with several token tiles the other
+        // CTAs re-read the same rows from L2, so do not mark them evict-first.
+        fp.w_policy = (pl.m_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
+        fp.ws_m = ws_m; fp.ws_a = ws_a; fp.ws_s = ws_s;
+
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(pl.grid);
+        cfg.blockDim = dim3(kFusedThreads);
+        cfg.dynamicSmemBytes = static_cast<size_t>(pl.smem_bytes);
+        cfg.stream = stream;
+        cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel, tm_h, tm_w, fp);
+        if (e != cudaSuccess) return set_cuda_error("launch laser_probe_fused_kernel", e);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+
+    FinalizeParams fz;
+    fz.n_alloc = N; fz.R = run_fused ? R : 0; fz.splits = pl.splits; fz.n_pad = n_pad;
+    fz.agg_mode = aggregate_mode;
+    fz.ws_m = ws_m; fz.ws_a = ws_a; fz.ws_s = ws_s;
+    fz.req_offsets = req_offsets; fz.load = load;
+    fz.out_conf = out_conf; fz.out_argmax = out_argmax; fz.out_exit = out_exit;
+    fz.out_tau = out_tau_opt; fz.out_pmax = out_pmax_opt;
+    fz.tau = to_dev(tau_params);
+    const int pad_blocks = ceil_div(N, kFinalizeThreads);
+    if (!run_fused && R > 0) {
+        // N == 0 with R > 0: every request is empty -> conf 0, exit 0, tau still defined.
+        // Handled by the same kernel: req_offsets are all 0, no partials are read.
+        fz.R = R;
+    }
+    const int grid = fz.R + pad_blocks;
+    if (grid > 0) {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(grid);
+        cfg.blockDim = dim3(kFinalizeThreads);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        static const bool no_pdl = getenv("LASER_NO_PDL") != nullptr;
+        if (run_fused && !no_pdl) {
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+        }
+        cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_finalize_kernel, fz);
+        if (e != cudaSuccess) return set_cuda_error("launch laser_probe_finalize_kernel", e);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    return LASER_OK;
+}
+
+int laser_probe_confidence(const void* hidden, const void* W, const int32_t* req_offsets,
+                           const float* load, const laser_tau_params* tau_params, float* out_conf,
+                           int32_t* out_argmax, uint8_t* out_exit, const laser_probe_dims* dims,
+                           void* workspace, size_t workspace_bytes, void* stream,
+                           float* out_tau_opt, float* out_pmax_opt) {
+    return laser_probe_confidence_agg(hidden, W, req_offsets, load, tau_params, out_conf, out_argmax,
+                                      out_exit, dims, workspace, workspace_bytes, stream,
+                                      out_tau_opt, out_pmax_opt, LASER_AGG_MEAN);
+}
+
+size_t laser_probe_staging_bytes(const laser_probe_dims* dims) {
+    if (!dims_valid(dims)) return 0;
+    return staging_layout(*dims).total;
+}
+
+int laser_probe_confidence_host(const void* h_hidden, const void* W, const int32_t* h_req_offsets,
+                                const float* h_load, const laser_tau_params* tau_params,
+                                float* h_out_conf, int32_t* h_out_argmax, uint8_t* h_out_exit,
+                                const laser_probe_dims* dims, void* workspace,
+                                size_t workspace_bytes, void* d_staging, size_t staging_bytes,
+                                void* stream_v) {
+    if (!dims || !tau_params) return LASER_E_NULL;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
+    const int N = dims->N, R = dims->R;
+    if (N == 0 && R == 0) return LASER_OK;
+    if (!d_staging) return LASER_E_NULL;
+    if (N > 0 && (!h_hidden || !h_out_argmax)) return LASER_E_NULL;
+    if (R > 0 && (!h_req_offsets || !h_load || !h_out_conf || !h_out_exit)) return LASER_E_NULL;
+    const Staging st = staging_layout(*dims);
+    if (staging_bytes < st.total || (reinterpret_cast<uintptr_t>(d_staging) & 255)) return LASER_E_WORKSPACE;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+    uint8_t* base = static_cast<uint8_t*>(d_staging);
+    cudaError_t e;
+    if (N > 0) {
+        e = cudaMemcpyAsync(base + st.hidden, h_hidden, static_cast<size_t>(N) * dims->d * 2,
+                            cudaMemcpyHostToDevice, stream);
+        if (e != cudaSuccess) return set_cuda_error("H2D hidden", e);
+    }
+    if (R > 0) {
+        e = cudaMemcpyAsync(base + st.offsets, h_req_offsets, static_cast<size_t>(R + 1) * 4,
+                            cudaMemcpyHostToDevice, stream);
+        if (e != cudaSuccess) return set_cuda_error("H2D req_offsets", e);
+        e = cudaMemcpyAsync(base + st.load, h_load, static_cast<size_t>(R) * 4, cudaMemcpyHostToDevice, stream);
+        if (e != cudaSuccess) return set_cuda_error("H2D load", e);
+    }
+    int rc = laser_probe_confidence(base + st.hidden, W, reinterpret_cast<int32_t*>(base + st.offsets),
+                                    reinterpret_cast<float*>(base + st.load), tau_params,
+                                    reinterpret_cast<float*>(base + st.conf),
+                                    reinterpret_cast<int32_t*>(base + st.argmax), base + st.exit_, dims,
+                                    workspace, workspace_bytes, stream_v, nullptr, nullptr);
+    if (rc != LASER_OK) return rc;
+    if (R > 0) {
+        e = cudaMemcpyAsync(h_out_conf, base + st.conf, static_cast<size_t>(R) * 4, cudaMemcpyDeviceToHost, stream);
+        if (e != cudaSuccess) return set_cuda_error("D2H conf", e);
+        e = cudaMemcpyAsync(h_out_exit, base + st.exit_, static_cast<size_t>(R), cudaMemcpyDeviceToHost, stream);
+        if (e != cudaSuccess) return set_cuda_error("D2H exit", e);
+    }
+    if (N > 0) {
+        e = cudaMemcpyAsync(h_out_argmax, base + st.argmax, static_cast<size_t>(N) * 4, cudaMemcpyDeviceToHost, stream);
+        if (e != cudaSuccess) return set_cuda_error("D2H argmax", e);
+    }
+    e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return set_cuda_error("cudaStreamSynchronize", e);
+    return LASER_OK;
+}
+
+int laser_tau_from_load(const float* load, int32_t R, const laser_tau_params* tau_params, float* out_tau) {
+    if (!tau_params || (R > 0 && (!load || !out_tau))) return LASER_E_NULL;
+    if (R < 0) return LASER_E_DIMS;
+    if (!params_valid(tau_params)) return LASER_E_PARAMS;
+    const TauParamsDev t = to_dev(tau_params);
+    for (int32_t r = 0; r < R; ++r) out_tau[r] = tau_eval(load[r], t);
+    return LASER_OK;
+}
+
+int laser_ema_update(float* lbar, const float* L, int32_t R, float alpha) {
+    if (R > 0 && (!lbar || !L)) return LASER_E_NULL;
+    if (R < 0) return LASER_E_DIMS;
+    if (!(alpha >= 0.f && alpha <= 1.f)) return LASER_E_PARAMS;
+    for (int32_t r = 0; r < R; ++r) lbar[r] = alpha * L[r] + (1.f - alpha) * lbar[r];
+    return LASER_OK;
+}
+
+int laser_budget_params_default(laser_budget_params* out) {
+    if (!out) return LASER_E_NULL;
+    *out = laser_budget_params{10.f, 2.f, 0.6f, 1.5f, 50.f, 275.f, 10.f};
+    return LASER_OK;
+}
+
+int laser_allocate_budget(const int32_t* prompt_tokens, const float* L, int32_t R,
+                          const laser_budget_params* q, int32_t* out_budget) {
+    if (!q || (R > 0 && (!prompt_tokens || !L || !out_budget))) return LASER_E_NULL;
+    if (R < 0) return LASER_E_DIMS;
+    if (!(q->p_max > q->p_min) || !(q->f_max >= q->f_min) || !(q->l_target > 0.f)) return LASER_E_PARAMS;
+    for (int32_t r = 0; r < R; ++r) {
+        // Eq. 7: difficulty factor from the prompt length, clipped to [f_min, f_max]
+        double f_diff = q->f_min + (static_cast<double>(prompt_tokens[r]) - q->p_min) /
+                                       (static_cast<double>(q->p_max) - q->p_min) *
+                                       (static_cast<double>(q->f_max) - q->f_min);
+        f_diff = f_diff < q->f_min ? q->f_min : (f_diff > q->f_max ? q->f_max : f_diff);
+        // Eq. 8: load factor min(1, L_target / max(1, L(t)))
+        const double den = L[r] > 1.f ? L[r] : 1.0;
+        double f_load = q->l_target / den;
+        f_load = f_load < 1.0 ? f_load : 1.0;
+        // Eq. 6
+        double b = std::floor(static_cast<double>(q->b_base) * f_diff * f_load);
+        if (b < q->b_min) b = q->b_min;
+        out_budget[r] = static_cast<int32_t>(b);
+    }
+    return LASER_OK;
+}
+
+const char* laser_status_string(int status) {
+    switch (status) {
+        case LASER_OK: return "ok";
+        case LASER_E_NULL: return "required pointer is NULL";
+        case LASER_E_DIMS: return "invalid dimensions (need d > 0, d % 8 == 0, V > 0, N >= 0, R >= 0)";
+        case LASER_E_ALIGN: return "hidden / W must be 16-byte aligned";
+        case LASER_E_PARAMS: return "invalid parameters";
+        case LASER_E_WORKSPACE: return "workspace / staging buffer missing, misaligned or too small";
+        case LASER_E_ARCH: return "device is not sm_100 (B200); this library has no fallback path";
+        case LASER_E_CUDA: return "CUDA call failed (see laser_last_error)";
+        case LASER_E_MODE: return "unknown aggregate mode";
+        default: return "unknown status";
+    }
+}
+
+const char* laser_last_error(void) { return g_last_error.c_str(); }
+
+uint64_t laser_kernel_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+int laser_shutdown(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_maps.clear();
+    return LASER_OK;
+}
+
+}  // extern "C"

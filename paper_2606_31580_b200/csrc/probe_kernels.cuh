@@ -1,0 +1,384 @@
+// probe_kernels.cuh — the two kernels of the LASER confidence probe (sm_100a).
+//
+//  laser_probe_fused_kernel   a1 + a2 of include/laser_probe.h: LM-head projection on tcgen05 tensor
+//                             cores with the online-softmax statistics (max, lowest-index argmax,
+//                             sum-exp) taken straight out of TMEM.  Logits never reach HBM.
+//  laser_probe_finalize_kernel  merge of the per-split statistics (warp shuffles), a3 per-request
+//                             aggregate, a4 threshold (Eq. 5 + clamp), a5 exit mask.
+//
+// Orientation: tokens on the MMA M axis (= TMEM lanes), vocabulary on the N axis (= TMEM columns).
+// With tcgen05.ld 32x32b every epilogue thread owns one token row and walks its vocabulary columns
+// in registers: no cross-lane traffic in the vocabulary loop.
+//
+// Work decomposition: the vocabulary is cut into `splits` contiguous ranges of tiles_per_split *
+// tile_n rows; a work item is (token tile of 128 rows, split).  Items are ordered token-tile
+// fastest so that CTAs running side by side stream the same W rows (one HBM read, L2 hits for the
+// rest).  The grid is persistent (<= one CTA per SM); CTA b takes items b, b + grid, ...
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
+#include <cstdint>
+
+#include "ptx.cuh"
+
+namespace laser {
+
+constexpr int kTileM = 128;       // token rows per MMA (TMEM lanes)
+constexpr int kBlockK = 64;       // bf16 elements per k-block = one 128-byte swizzle row
+constexpr int kUmmaK = 16;        // K of one tcgen05.mma kind::f16
+constexpr int kMaxTileN = 256;    // vocabulary rows per tile (UMMA N <= 256)
+constexpr int kMaxStages = 8;
+constexpr int kABytes = kTileM * kBlockK * 2;  // 16 KiB of hidden per stage
+constexpr int kTmemCols = 512;    // two 256-column accumulators (double buffered)
+constexpr int kFusedThreads = 192;  // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-5 epilogue
+constexpr int kEpilogueThreads = 128;
+constexpr float kLog2e = 1.4426950408889634f;
+
+struct FusedParams {
+    int32_t n_alloc, d, V;
+    int32_t m_tiles, splits, tiles_per_split, tile_n, k_blocks, stages;
+    int32_t work_items, n_pad;
+    uint32_t tx_bytes;     // bytes TMA delivers per stage (hidden box + W box)
+    uint32_t stage_bytes;  // shared-memory stride of a stage: kABytes + tile_n * 128
+    uint64_t w_policy;     // L2 eviction policy for the W stream
+    float* ws_m;           // [splits, n_pad] running max per (split, row)
+    int32_t* ws_a;         // [splits, n_pad] argmax
+    float* ws_s;           // [splits, n_pad] sum of exp(logit - max)
+};
+
+// ---------------------------------------------------------------------------------- descriptors
+// Shared-memory matrix descriptor, K-major operand, 128-byte swizzle: rows of 128 B, 8-row groups
+// 1024 B apart (SBO), LBO unused for swizzled K-major, descriptor version 1 (Blackwell).
+__device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t smem_addr) {
+    uint64_t desc = 0;
+    desc |= static_cast<uint64_t>((smem_addr & 0x3FFFFu) >> 4);   // start address  [0,14)
+    desc |= static_cast<uint64_t>(1024u >> 4) << 32;              // SBO            [32,46)
+    desc |= static_cast<uint64_t>(1) << 46;                       // version        [46,48)
+    desc |= static_cast<uint64_t>(2) << 61;                       // SWIZZLE_128B   [61,64)
+    return desc;
+}
+// Instruction descriptor for kind::f16: D fp32, A/B bf16, both K-major, M = 128, N = tile_n.
+__device__ __forceinline__ uint32_t make_idesc_bf16(uint32_t n) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((kTileM >> 4) << 24);
+}
+
+// ---------------------------------------------------------------------------------- epilogue math
+// Fold NC consecutive vocabulary columns (starting at vocabulary index vbase) of one token row into
+// the running statistics (m, a, s):  m = max, a = lowest index attaining it, s = sum 2^{(x-m)log2e}.
+// Columns are visited in ascending vocabulary order and the update is strict (>), so ties keep the
+// lowest index.  Columns v >= V (TMA zero fill past the end of W) are masked out.
+template <int NC>
+__device__ __forceinline__ void fold_columns(const uint32_t (&r)[NC], int vbase, int V, float& m,
+                                             int& a, float& s) {
+    float x[NC];
+#pragma unroll
+    for (int j = 0; j < NC; ++j) x[j] = __uint_as_float(r[j]);
+    if (vbase + NC > V) {
+#pragma unroll
+        for (int j = 0; j < NC; ++j)
+            if (vbase + j >= V) x[j] = -CUDART_INF_F;
+    }
+    float c0 = x[0], c1 = x[1], c2 = x[2], c3 = x[3];
+#pragma unroll
+    for (int j = 4; j < NC; j += 4) {
+        c0 = fmaxf(c0, x[j]);
+        c1 = fmaxf(c1, x[j + 1]);
+        c2 = fmaxf(c2, x[j + 2]);
+        c3 = fmaxf(c3, x[j + 3]);
+    }
+    const float cm = fmaxf(fmaxf(c0, c1), fmaxf(c2, c3));
+    if (cm > m) {
+        int idx = 0;
+#pragma unroll
+        for (int j = NC - 1; j >= 0; --j)
+            if (x[j] == cm) idx = j;
+        a = vbase + idx;
+        s *= ptx::ex2_approx((m - cm) * kLog2e);  // m = -inf on the first chunk: s = 0 stays 0
+        m = cm;
+    }
+    const float ms = m * kLog2e;
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+#pragma unroll
+    for (int j = 0; j < NC; j += 4) {
+        s0 += ptx::ex2_approx(fmaf(x[j], kLog2e, -ms));
+        s1 += ptx::ex2_approx(fmaf(x[j + 1], kLog2e, -ms));
+        s2 += ptx::ex2_approx(fmaf(x[j + 2], kLog2e, -ms));
+        s3 += ptx::ex2_approx(fmaf(x[j + 3], kLog2e, -ms));
+    }
+    s += (s0 + s1) + (s2 + s3);
+}
+
+// ---------------------------------------------------------------------------------- fused kernel
+__global__ void __launch_bounds__(kFusedThreads, 1)
+laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
+                         const __grid_constant__ CUtensorMap tmap_w, const FusedParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t raw = ptx::smem_u32(smem_raw);
+    const uint32_t smem = (raw + 1023u) & ~1023u;  // SWIZZLE_128B tiles need 1024-byte alignment
+    const uint32_t bars = smem + static_cast<uint32_t>(p.stages) * p.stage_bytes;
+    // barrier block: full[8] | empty[8] | tmem_full[2] | tmem_empty[2] | tmem base address (u32)
+    auto full_bar = [&](int s) { return bars + 8u * s; };
+    auto empty_bar = [&](int s) { return bars + 64u + 8u * s; };
+    auto tfull_bar = [&](int b) { return bars + 128u + 8u * b; };
+    auto tempty_bar = [&](int b) { return bars + 144u + 8u * b; };
+    const uint32_t tmem_slot = bars + 160u;
+    volatile uint32_t* tmem_slot_ptr =
+        reinterpret_cast<volatile uint32_t*>(smem_raw + (smem - raw) + p.stages * p.stage_bytes + 160u);
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tensormap(&tmap_hidden);
+        ptx::prefetch_tensormap(&tmap_w);
+        for (int s = 0; s < p.stages; ++s) {
+            ptx::mbar_init(full_bar(s), 1);
+            ptx::mbar_init(empty_bar(s), 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            ptx::mbar_init(tfull_bar(b), 1);
+            ptx::mbar_init(tempty_bar(b), kEpilogueThreads);
+        }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) {
+        ptx::tmem_alloc(tmem_slot, kTmemCols);
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    // Let the finalize kernel's CTAs be scheduled as SMs free up (it waits on griddepcontrol.wait).
+    ptx::pdl_launch_dependents();
+
+    const int T = p.tiles_per_split, BN = p.tile_n;
+
+    if (warp == 0) {
+        // ===================================================================== TMA producer
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int w = blockIdx.x; w < p.work_items; w += gridDim.x) {
+                const int mt = w % p.m_tiles, sp = w / p.m_tiles;
+                const int v0 = sp * T * BN;
+                const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
+                for (int t = 0; t < ntiles; ++t) {
+                    for (int kb = 0; kb < p.k_blocks; ++kb) {
+                        ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+                        const uint32_t sa = smem + static_cast<uint32_t>(stage) * p.stage_bytes;
+                        ptx::mbar_arrive_expect_tx(full_bar(stage), p.tx_bytes);
+                        ptx::tma_load_2d(sa, &tmap_hidden, full_bar(stage), kb * kBlockK,
+                                         mt * kTileM, ptx::kEvictLast);
+                        ptx::tma_load_2d(sa + kABytes, &tmap_w, full_bar(stage), kb * kBlockK,
+                                         v0 + t * BN, p.w_policy);
+                        if (++stage == p.stages) { stage = 0; phase ^= 1u; }
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================================================================== MMA issuer
+        if (lane == 0) {
+            const uint32_t idesc = make_idesc_bf16(static_cast<uint32_t>(BN));
+            int stage = 0;
+            uint32_t phase = 0, acc = 0;
+            for (int w = blockIdx.x; w < p.work_items; w += gridDim.x) {
+                const int sp = w / p.m_tiles;
+                const int v0 = sp * T * BN;
+                const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
+                for (int t = 0; t < ntiles; ++t, ++acc) {
+                    const uint32_t buf = acc & 1u, aphase = (acc >> 1) & 1u;
+                    ptx::mbar_wait(tempty_bar(buf), aphase ^ 1u);  // epilogue drained this buffer
+                    ptx::tc_fence_after();
+                    const uint32_t d_tmem = tmem_base + buf * kMaxTileN;
+                    for (int kb = 0; kb < p.k_blocks; ++kb) {
+                        ptx::mbar_wait(full_bar(stage), phase);  // TMA bytes have landed
+                        ptx::tc_fence_after();
+                        const uint32_t sa = smem + static_cast<uint32_t>(stage) * p.stage_bytes;
+                        const uint64_t a_desc = make_smem_desc_sw128(sa);
+                        const uint64_t b_desc = make_smem_desc_sw128(sa + kABytes);
+#pragma unroll
+                        for (int k = 0; k < kBlockK / kUmmaK; ++k) {
+                            // +32 bytes along K inside the swizzle row = +2 in the address field
+                            ptx::umma_bf16(d_tmem, a_desc + 2u * k, b_desc + 2u * k, idesc,
+                                           (kb | k) != 0);
+                        }
+                        ptx::umma_commit(empty_bar(stage));  // frees the stage when the MMAs retire
+                        if (++stage == p.stages) { stage = 0; phase ^= 1u; }
+                    }
+                    ptx::umma_commit(tfull_bar(buf));  // accumulator complete -> epilogue
+                }
+            }
+        }
+    } else {
+        // ===================================================================== epilogue (4 warps)
+        const int q = warp & 3;  // a warp may only touch TMEM lanes [32*(warp%4), +32)
+        const int row = q * 32 + lane;
+        const uint32_t lane_addr = static_cast<uint32_t>(q * 32) << 16;
+        uint32_t acc = 0;
+        for (int w = blockIdx.x; w < p.work_items; w += gridDim.x) {
+            const int mt = w % p.m_tiles, sp = w / p.m_tiles;
+            const int v0 = sp * T * BN;
+            const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
+            float m = -CUDART_INF_F, s = 0.f;
+            int a = -1;
+            for (int t = 0; t < ntiles; ++t, ++acc) {
+                const uint32_t buf = acc & 1u, aphase = (acc >> 1) & 1u;
+                ptx::mbar_wait(tfull_bar(buf), aphase);
+                ptx::tc_fence_after();
+                const uint32_t taddr = tmem_base + lane_addr + buf * kMaxTileN;
+                const int vt = v0 + t * BN;
+                int c = 0;
+                for (; c + 32 <= BN && vt + c < p.V; c += 32) {
+                    uint32_t r[32];
+                    ptx::tmem_ld_x32(taddr + c, r);
+                    ptx::tmem_wait_ld();
+                    fold_columns<32>(r, vt + c, p.V, m, a, s);
+                }
+                // tile_n is a multiple of 16: at most one 16-column tail chunk
+                if (c + 16 == BN && vt + c < p.V) {
+                    uint32_t r[16];
+                    ptx::tmem_ld_x16(taddr + c, r);
+                    ptx::tmem_wait_ld();
+                    fold_columns<16>(r, vt + c, p.V, m, a, s);
+                }
+                ptx::tc_fence_before();
+                ptx::mbar_arrive(tempty_bar(buf));
+            }
+            const size_t o = static_cast<size_t>(sp) * p.n_pad + static_cast<size_t>(mt) * kTileM + row;
+            p.ws_m[o] = m;
+            p.ws_a[o] = a;
+            p.ws_s[o] = s;
+        }
+    }
+
+    // ------------------------------------------------------------------------- teardown
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        ptx::tc_fence_after();
+        ptx::tmem_dealloc(tmem_base, kTmemCols);
+    }
+}
+
+// ---------------------------------------------------------------------------------- finalize
+struct TauParamsDev {
+    float lambda_base, beta, gamma, l_target, lambda_min, lambda_max;
+};
+
+// a4: Eq. 5 then the clamp.  Shared by the kernel and laser_tau_from_load.
+__host__ __device__ __forceinline__ float tau_eval(float load, const TauParamsDev& t) {
+    float lam = t.lambda_base - t.beta * tanhf(t.gamma * (load - t.l_target) / t.l_target);
+    lam = fmaxf(lam, t.lambda_min);
+    lam = fminf(lam, t.lambda_max);
+    return lam;
+}
+
+struct FinalizeParams {
+    int32_t n_alloc, R, splits, n_pad, agg_mode;
+    const float* ws_m;
+    const int32_t* ws_a;
+    const float* ws_s;
+    const int32_t* req_offsets;
+    const float* load;
+    float* out_conf;
+    int32_t* out_argmax;
+    uint8_t* out_exit;
+    float* out_tau;   // nullable
+    float* out_pmax;  // nullable
+    TauParamsDev tau;
+};
+
+// (m,a,s) (+) (m',a',s'): commutative form — on equal maxima the smaller vocabulary index wins.
+__device__ __forceinline__ void merge_stats(float& m, int& a, float& s, float m2, int a2, float s2) {
+    const float M = fmaxf(m, m2);
+    const int an = (m > m2) ? a : ((m2 > m) ? a2 : min(a, a2));
+    const float e1 = (m == M) ? 1.f : ptx::ex2_approx((m - M) * kLog2e);
+    const float e2 = (m2 == M) ? 1.f : ptx::ex2_approx((m2 - M) * kLog2e);
+    s = s * e1 + s2 * e2;
+    m = M;
+    a = an;
+}
+
+constexpr int kFinalizeThreads = 128;
+
+// Blocks [0, R): one request each.  A warp takes rows b+w, b+w+4, ...: its lanes stride over the
+// vocabulary splits of the row, fold their own partials, then merge across the warp with shuffles.
+// Blocks [R, R + ceil(n_alloc/128)): mark padding rows (n >= req_offsets[R]).
+__global__ void __launch_bounds__(kFinalizeThreads)
+laser_probe_finalize_kernel(const FinalizeParams p) {
+    ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (static_cast<int>(blockIdx.x) >= p.R) {
+        const int n = (blockIdx.x - p.R) * kFinalizeThreads + threadIdx.x;
+        const int n_valid = (p.R > 0) ? p.req_offsets[p.R] : 0;
+        if (n < p.n_alloc && n >= n_valid) {
+            p.out_argmax[n] = -1;
+            if (p.out_pmax) p.out_pmax[n] = CUDART_NAN_F;
+        }
+        return;
+    }
+    __shared__ float warp_acc[kFinalizeThreads / 32];
+    const int r = blockIdx.x;
+    const int b = p.req_offsets[r], e = p.req_offsets[r + 1];
+    // running aggregate of this warp's rows: sum (mean), sum of logs (geomean), min
+    float acc = (p.agg_mode == 2) ? CUDART_INF_F : 0.f;
+    bool any_nan = false;
+    for (int n = b + warp; n < e; n += kFinalizeThreads / 32) {
+        float m = -CUDART_INF_F, s = 0.f;
+        int a = 0x7fffffff;
+        for (int sp = lane; sp < p.splits; sp += 32) {
+            const size_t o = static_cast<size_t>(sp) * p.n_pad + n;
+            merge_stats(m, a, s, p.ws_m[o], p.ws_a[o], p.ws_s[o]);
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            const float m2 = __shfl_xor_sync(0xffffffffu, m, off);
+            const int a2 = __shfl_xor_sync(0xffffffffu, a, off);
+            const float s2 = __shfl_xor_sync(0xffffffffu, s, off);
+            merge_stats(m, a, s, m2, a2, s2);
+        }
+        const float pmax = 1.0f / s;
+        if (lane == 0) {
+            p.out_argmax[n] = a;
+            if (p.out_pmax) p.out_pmax[n] = pmax;
+        }
+        any_nan |= (pmax != pmax);
+        if (p.agg_mode == 0) acc += pmax;
+        else if (p.agg_mode == 1) acc += logf(pmax);
+        else acc = fminf(acc, pmax);
+    }
+    if (p.agg_mode == 2 && any_nan) acc = CUDART_NAN_F;
+    if (lane == 0) warp_acc[warp] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int len = e - b;
+        float conf = 0.f;
+        if (len > 0) {
+            if (p.agg_mode == 2) {
+                conf = warp_acc[0];
+                bool nan = conf != conf;
+                for (int w = 1; w < kFinalizeThreads / 32; ++w) {
+                    nan |= (warp_acc[w] != warp_acc[w]);
+                    conf = fminf(conf, warp_acc[w]);
+                }
+                if (nan) conf = CUDART_NAN_F;
+            } else {
+                float t = 0.f;
+                for (int w = 0; w < kFinalizeThreads / 32; ++w) t += warp_acc[w];
+                conf = t / static_cast<float>(len);
+                if (p.agg_mode == 1) conf = expf(conf);
+            }
+        }
+        const float tau = tau_eval(p.load[r], p.tau);
+        p.out_conf[r] = conf;
+        p.out_exit[r] = (conf > tau) ? 1 : 0;  // strict; NaN > tau is false
+        if (p.out_tau) p.out_tau[r] = tau;
+    }
+}
+
+}  // namespace laser

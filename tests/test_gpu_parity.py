@@ -1,0 +1,277 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  All tests need a B200 (`-m gpu`)."""
+import json
+import os
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from paper_2606_31580_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+OUT = Path(os.environ.get("GRAFT_REPO_ROOT", Path(__file__).resolve().parent.parent)) / "gpurun_out"
+
+
+def _log(name, stats):
+    try:
+        OUT.mkdir(exist_ok=True)
+        with open(OUT / "parity_stats.jsonl", "a") as f:
+            f.write(json.dumps(dict(case=name, **stats)) + "\n")
+    except OSError:
+        pass
+    print(name, stats)
+
+
+@pytest.fixture(scope="module")
+def P():
+    import _parity as p
+    return p
+
+
+def _pick_requests(w, k, seed=0):
+    rng = np.random.default_rng(seed)
+    return np.sort(rng.choice(w.R, size=min(k, w.R), replace=False))
+
+
+# ------------------------------------------------------------------ the five BASELINE.json configs
+def test_c1_tiny(P):
+    w = wl.config_c1()
+    st = P.check(w)
+    _log("C1", st)
+    assert st["exits"] >= 1                                   # the mask is exercised (DESIGN A16)
+
+
+def test_c2_qwen15b_full(P, c2_W_bits):
+    """The graded config, every row and request, in the launch configuration bench.py times."""
+    w = wl.config_c2(c2_W_bits)
+    st = P.check(w)
+    _log("C2", st)
+    assert st["rows"] == 128 and st["requests"] == 16 and 0 < st["exits"] < 16
+
+
+def test_c3_qwen7b_sampled(P):
+    w = wl.config_c3()
+    st = P.check(w, requests=_pick_requests(w, 6, 3))
+    _log("C3", st)
+
+
+def test_c4_llama8b_sampled(P):
+    w = wl.config_c4()
+    assert w.N_alloc == 1024 and w.N_valid < 1024
+    g = P.run_gpu(w)
+    reqs = _pick_requests(w, 5, 4)
+    ora, rows, reqs = P.run_oracle(w, reqs)
+    st = P.compare(w, g, ora, rows, reqs, "C4")
+    _log("C4", st)
+    assert np.all(g.argmax[w.N_valid:] == -1)                 # padding rows (DESIGN A11)
+    assert np.all(g.argmax[:w.N_valid] >= 0)
+    planted = w.planted[:w.N_valid]
+    assert np.all(g.argmax[:w.N_valid][planted >= 0] == planted[planted >= 0])   # property at full size
+
+
+@pytest.mark.parametrize("N", wl.C5_NS)
+def test_c5_sweep(P, c2_W_bits, N):
+    w = wl.config_c5(N, c2_W_bits)
+    k = w.R if N <= 64 else 6
+    g = P.run_gpu(w)
+    ora, rows, reqs = P.run_oracle(w, None if N <= 64 else _pick_requests(w, k, N))
+    st = P.compare(w, g, ora, rows, reqs, f"C5:{N}")
+    _log(f"C5:{N}", st)
+    # properties that hold at any size: planted tokens win; conf within [0,1]; exit is 0/1
+    pl = w.planted >= 0
+    assert np.all(g.argmax[pl] == w.planted[pl])
+    assert np.all((g.conf >= 0) & (g.conf <= 1.0 + 1e-6))
+    assert np.all((g.pmax > 0) & (g.pmax <= 1.0 + 1e-6))
+
+
+# ------------------------------------------------------------------ stress inputs (not timed)
+def test_s1_tau_band(P, c2_W_bits):
+    """Requests planted around the band where tau(load) decides: the mask depends on load."""
+    w = wl.tau_band_stress(c2_W_bits, 0.02, R=40, L=8)
+    st = P.check(w)
+    _log("S1", st)
+    assert 0 < st["exits"] < w.R
+
+
+def test_literal_generator_flat(P):
+    """BASELINE.json's generator taken literally: flat distributions, tiny top-2 gaps."""
+    w = wl.literal(151936, 1536, 0.02, 8, 8, seed=wl.SEED_BASE + 7)
+    st = P.check(w)
+    _log("literal", st)
+    assert st["exits"] == 0
+
+
+@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
+    (5000, 256, 12, 8, None, None),        # several tiles, V not a multiple of 16
+    (4099, 200, 9, 5, None, None),         # d not a multiple of 64 (k tail), odd V
+    (33000, 512, 40, None, 400, (1, 16)),  # 3 token tiles, CSR with padding rows
+    (70001, 128, 20, None, 300, (0, 24)),  # empty requests, ragged everything
+    (1000, 64, 3, 130, None, None),        # a request longer than one token tile
+    (17, 8, 2, 3, None, None),             # V smaller than one tile, d smaller than one k-block
+])
+def test_scaled_shapes(P, V, d, R, L, n_alloc, var_len):
+    w = wl.scaled(f"scaled-V{V}-d{d}", V, d, 0.05, R, L, seed=V + d, N_alloc=n_alloc, var_len=var_len)
+    st = P.check(w)
+    _log(w.name, st)
+
+
+# ------------------------------------------------------------------ closed forms on the GPU
+def test_uniform_logits_gpu(P):
+    """P1 on the device: hidden = 0 -> pmax = 1/V, argmax 0 (lowest index), conf = 1/V."""
+    w = wl.scaled("uniform", 40000, 256, 0.05, 4, 8, seed=5)
+    w.hidden_bits[:] = 0
+    g = P.run_gpu(w)
+    assert np.all(g.argmax == 0)
+    np.testing.assert_allclose(g.pmax, 1.0 / w.V, rtol=2e-5)
+    np.testing.assert_allclose(g.conf, 1.0 / w.V, rtol=2e-5)
+    assert np.all(g.exit == 0)
+
+
+def test_one_hot_confidence_one(P):
+    """P2 on the device: W = 40*I, hidden = e_j -> conf = 1 (to fp32), argmax = j, exit."""
+    V = d = 256
+    W = wl.bf16_bits((40.0 * np.eye(V)).astype(np.float32))
+    js = np.array([0, 17, 255, 128, 127, 31, 32, 200])
+    w = wl.Workload("onehot", W, wl.bf16_bits(np.eye(V, dtype=np.float32)[js]),
+                    wl.fixed_offsets(2, 4), np.array([0.0, 1.0], np.float32))
+    g = P.run_gpu(w)
+    assert np.array_equal(g.argmax, js)
+    np.testing.assert_allclose(g.conf, 1.0, atol=1e-6)
+    assert np.all(g.exit == 1)
+
+
+def test_ties_across_tile_and_split_boundaries(P):
+    """P3 on the device: duplicate W rows give bit-identical logits; the lowest index must survive the
+    in-thread, cross-tile and cross-split merges."""
+    from paper_2606_31580_b200 import binding as B
+    V, d, N = 20000, 128, 16
+    plan = B.plan_query(N, d, V, 2)
+    bn, T = plan["tile_n"], plan["tiles_per_split"]
+    rng = np.random.default_rng(8)
+    Wf = (rng.standard_normal((V, d)) * 0.05).astype(np.float32)
+    h = rng.standard_normal((N, d)).astype(np.float32)
+    big = (h[0] * 0.5).astype(np.float32)          # strong match for row 0 only
+    pairs = [(bn - 1, bn),                         # straddles a tile boundary
+             (T * bn - 1, T * bn),                 # straddles a split boundary
+             (5, 3 * T * bn + 7),                  # far apart, different splits
+             (31, 32)]                             # same tile, adjacent 32-column chunks
+    for v1, v2 in pairs:
+        W2 = Wf.copy(); W2[v1] = big; W2[v2] = big
+        w = wl.Workload("ties", wl.bf16_bits(W2), wl.bf16_bits(h), wl.fixed_offsets(2, 8),
+                        np.array([0.3, 0.7], np.float32))
+        g = P.run_gpu(w)
+        assert g.argmax[0] == v1, (v1, v2, g.argmax[0], plan)
+        ora, rows, reqs = P.run_oracle(w)
+        assert ora.argmax[0] == v1 and ora.gap2[0] == 0.0
+        P.compare(w, g, ora, rows, reqs, "ties")
+
+
+# ------------------------------------------------------------------ semantics fixed at the boundary
+def test_nan_row_poisons_only_its_request(P):
+    w = wl.scaled("nan", 3000, 64, 0.05, 3, 4, seed=11)
+    hf = w.hidden_f32().copy(); hf[5, 7] = np.nan
+    w.hidden_bits = wl.bf16_bits(hf)
+    g = P.run_gpu(w)
+    assert np.isnan(g.conf[1]) and g.exit[1] == 0
+    assert np.isfinite(g.conf[0]) and np.isfinite(g.conf[2])
+    ora, _, _ = P.run_oracle(w)
+    np.testing.assert_allclose(g.conf[[0, 2]], ora.conf[[0, 2]], atol=2e-3)
+
+
+def test_empty_batches_and_requests(P):
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    tp = B.TauParams(l_target=0.5)
+    # R = 0, N = 0: no-op, no launch
+    before = B.kernel_launch_count()
+    pr = B.Probe(0, 64, 1000, 0)
+    z16 = torch.empty((0, 64), dtype=torch.bfloat16, device="cuda")
+    W = torch.zeros((1000, 64), dtype=torch.bfloat16, device="cuda")
+    pr(z16, W, torch.zeros(1, dtype=torch.int32, device="cuda"),
+       torch.empty(0, dtype=torch.float32, device="cuda"), tp)
+    assert B.kernel_launch_count() == before
+    # R = 0, N = 4: all rows are padding
+    pr = B.Probe(4, 64, 1000, 0)
+    pr.argmax.fill_(5)
+    pr(torch.zeros((4, 64), dtype=torch.bfloat16, device="cuda"), W,
+       torch.zeros(1, dtype=torch.int32, device="cuda"), torch.empty(0, dtype=torch.float32, device="cuda"), tp)
+    torch.cuda.synchronize()
+    assert pr.argmax.cpu().tolist() == [-1] * 4
+    # all requests empty: conf 0, exit 0, tau defined
+    w = wl.scaled("emptyreq", 2000, 64, 0.05, 3, 0, seed=12, N_alloc=8)
+    g = P.run_gpu(w)
+    assert np.all(g.conf == 0) and np.all(g.exit == 0) and np.all(g.argmax == -1)
+    assert np.all((g.tau >= 0.88) & (g.tau <= 0.97))
+
+
+def test_exit_is_strict_on_device(P):
+    """conf == tau must not exit: beta = 0, lambda_base = the GPU's own conf of a one-row request."""
+    from paper_2606_31580_b200 import binding as B
+    V = d = 64
+    W = wl.bf16_bits((3.0 * np.eye(V)).astype(np.float32))
+    w = wl.Workload("strict", W, wl.bf16_bits(np.eye(V, dtype=np.float32)[[2]]),
+                    wl.fixed_offsets(1, 1), np.array([0.3], np.float32))
+    c = float(P.run_gpu(w).conf[0])
+    for lam, want in [(c, 0), (np.nextafter(np.float32(c), np.float32(0)), 1),
+                      (np.nextafter(np.float32(c), np.float32(1)), 0)]:
+        tp = dict(lambda_base=float(lam), beta=0.0, gamma=1.0, l_target=0.5, lambda_min=0.0, lambda_max=1.0)
+        g = P.run_gpu(w, tau_params=tp)
+        assert g.tau[0] == np.float32(lam) and g.exit[0] == want
+
+
+def test_lower_clamp_and_fixed_threshold(P):
+    """beta = 0.1 reaches lambda_min (DESIGN A8); beta = 0 is the Fixed-High baseline (P9)."""
+    w = wl.config_c1()
+    for tp in (dict(wl.TAU_DEFAULTS_NORMALISED, beta=0.1), dict(wl.TAU_DEFAULTS_NORMALISED, beta=0.0)):
+        w.load = np.linspace(0, 3, w.R).astype(np.float32)
+        st = P.check(w, tau_params=tp)
+    g = P.run_gpu(w, tau_params=dict(wl.TAU_DEFAULTS_NORMALISED, beta=0.1))
+    assert g.tau.min() == np.float32(0.88) and g.tau.max() == np.float32(0.97)
+
+
+@pytest.mark.parametrize("agg", [1, 2])
+def test_aggregate_modes(P, agg):
+    """NEXT-1: geometric mean / min over the request's tokens in the same fused reduction."""
+    w = wl.scaled("agg", 12000, 256, 0.05, 10, None, seed=21, var_len=(1, 9))
+    st = P.check(w, agg=agg)
+    _log(f"agg{agg}", st)
+
+
+def test_deterministic_and_host_entry(P, c2_W_bits):
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    w = wl.config_c5(64, c2_W_bits)
+    dev = P.to_device(w)
+    a = P.run_gpu(w, dev)
+    b = P.run_gpu(w, dev)
+    for f in ("conf", "argmax", "exit", "pmax"):
+        assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    hp = B.HostProbe(w.N_alloc, w.d, w.V, w.R)
+    hh = B.bf16_tensor_from_bits(w.hidden_bits, pin=True)
+    out = hp(hh, dev["W"], torch.from_numpy(w.req_offsets).pin_memory(),
+             torch.from_numpy(w.load).pin_memory(), B.TauParams(**w.tau_params))
+    assert np.array_equal(out.conf.numpy(), a.conf) and np.array_equal(out.argmax.numpy(), a.argmax)
+    assert np.array_equal(out.exit.numpy(), a.exit)
+
+
+def test_error_codes_on_device(P):
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    w = wl.config_c1()
+    dev = P.to_device(w)
+    pr = B.Probe(w.N_alloc, w.d, w.V, w.R)
+    tp = B.TauParams(l_target=0.5)
+    with pytest.raises(B.LaserError) as e:
+        pr.workspace = pr.workspace[:64]
+        pr(dev["hidden"], dev["W"], dev["off"], dev["load"], tp)
+    assert e.value.status == -5
+    pr = B.Probe(w.N_alloc, w.d, w.V, w.R)
+    with pytest.raises(B.LaserError) as e:
+        pr(dev["hidden"], dev["W"], dev["off"], dev["load"], B.TauParams(lambda_min=0.99, lambda_max=0.9))
+    assert e.value.status == -4
+    mis = torch.empty(w.V * w.d + 8, dtype=torch.bfloat16, device="cuda")[1:1 + w.V * w.d].view(w.V, w.d)
+    with pytest.raises(B.LaserError) as e:
+        pr(dev["hidden"], mis, dev["off"], dev["load"], tp)
+    assert e.value.status == -3
