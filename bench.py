@@ -1,0 +1,441 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the LASER confidence probe on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload C2|C3|C4|C5:<N>] [--no-sweep] [--no-cpu-baseline]
+
+A "step" is one pass of the whole hot path (a1-a5 of include/laser_probe.h: projection, online
+softmax, per-request confidence, threshold, exit mask) over one batch of seeded synthetic input —
+one laser_probe_confidence() call, two kernel launches.  Default workload: BASELINE.json configs[1]
+(Qwen-1.5B-shaped, d=1536, V=151936, 16 requests x 8 tokens), the config the metric is quoted on.
+
+`value`    rows/s with every input already resident in HBM (device-timed, CUDA events on the launch
+           stream, barrier + synchronize either side, max over ranks).
+`e2e`      rows/s through laser_probe_confidence_host(): per-step inputs (hidden, req_offsets, load)
+           in pinned HOST memory, H2D + kernels + D2H of conf/argmax/exit + sync inside the timed
+           region.  W, the model's LM-head weight, stays resident (it is not a per-step input).
+`roofline` for the dominant (fused) kernel: algorithmic bytes per launch / its own average duration
+           (events recorded by the library either side of that kernel, second pass of K steps).
+`cpu_baseline` the fp64 oracle, as it stands, on this box's host cores (rank 0, N=1 only).
+
+--impl reference times the oracle itself (the reference arm of this tier): each step is the oracle
+on a bounded sample of the same workload.  Under torchrun only rank 0 runs it.
+
+Multi-GPU (--gpus N under torchrun): the probe's batches are independent, so ranks shard requests
+(each rank probes its own batch against its own replica of W) with no data-path collective: weak
+scaling.  torch.distributed is used for the barrier and the max-over-ranks reduction only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2606_31580_b200 import workloads as wl  # noqa: E402
+
+METRIC = "probe_rows_per_sec"
+UNIT = "rows/s"
+NOMINAL_HBM_GBS = 8000.0
+NOMINAL_BF16_TFLOPS = 2250.0
+
+
+# ----------------------------------------------------------------------------------------- helpers
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            j = json.loads(p.read_text())
+            return dict(hbm_gbs=float(j["hbm_gbs"]), bf16_tflops=float(j["bf16_tflops"]),
+                        bf16_tflops_sustained=float(j.get("bf16_tflops_sustained", j["bf16_tflops"])),
+                        source="measured")
+        except Exception:
+            pass
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
+
+
+def ncu_traffic_bytes(workload_name: str):
+    """dram read+write bytes per launch of the fused kernel from the committed ncu summary, or None."""
+    f = ROOT / "profiles" / "fused_kernel_dram_traffic.csv"
+    if not f.exists():
+        return None
+    for line in f.read_text().splitlines():
+        parts = [t.strip() for t in line.split(",")]
+        if len(parts) >= 2 and parts[0] == workload_name:
+            try:
+                return float(parts[1])
+            except ValueError:
+                return None
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML every ~5 ms while the GPU works."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self._stop_evt, self.err = index, [], threading.Event(), None
+        self.sm_max = None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.sm_max = int(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            get_reasons = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+                nv.nvmlDeviceGetCurrentClocksThrottleReasons
+            while not self._stop_evt.is_set():
+                self.samples.append((time.perf_counter(), int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)),
+                                     int(get_reasons(h))))
+                time.sleep(0.004)
+        except Exception as e:  # NVML missing: report it, do not fail the bench
+            self.err = repr(e)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+
+    def summary(self, t0, t1):
+        names = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap",
+                 0x8: "hw_slowdown", 0x10: "sync_boost", 0x20: "sw_thermal_slowdown",
+                 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+        inside = [s for s in self.samples if t0 <= s[0] <= t1]
+        window = "timed"
+        if len(inside) < 3:
+            inside, window = list(self.samples), "warmup+timed"
+        if not inside:
+            return dict(sm_mhz=None, sm_max_mhz=self.sm_max, reasons=[], window="none", error=self.err)
+        bits = 0
+        for s in inside:
+            bits |= s[2]
+        reasons = [n for b, n in names.items() if bits & b and n != "gpu_idle"]
+        return dict(sm_mhz=float(np.median([s[1] for s in inside])), sm_max_mhz=self.sm_max,
+                    reasons=reasons, samples=len(inside), window=window)
+
+
+def physical_gpu_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except (ValueError, IndexError):
+            pass
+    return local_rank
+
+
+def make_workload(name: str, rank: int, W_cache: dict) -> wl.Workload:
+    """Rank r > 0 draws its own hidden/load batch (seed + 7919*r) against the same W."""
+    if rank == 0:
+        return wl.by_name(name, W_cache)
+    base = wl.by_name(name, W_cache)
+    if name == "C2":
+        return wl.config_c2(base.W_bits, seed=wl.SEED_BASE + 2 + 7919 * rank)
+    if name == "C3":
+        return wl.config_c3(base.W_bits, seed=wl.SEED_BASE + 3 + 7919 * rank)
+    if name == "C4":
+        return wl.config_c4(base.W_bits, seed=wl.SEED_BASE + 4 + 7919 * rank)
+    return base
+
+
+def describe(w: wl.Workload) -> str:
+    return (f"{w.name}: d={w.d} V={w.V} N={w.N_alloc} rows (valid {w.N_valid}) R={w.R} requests, bf16 W/hidden, "
+            f"polarised synthetic generator (DESIGN.md §4)")
+
+
+def roofline_for(w: wl.Workload, fused_us: float, peaks: dict, sustained: bool):
+    """Slower of (algorithmic bytes / HBM) and (flops / bf16 tensor peak) bounds the path."""
+    by, fl = w.algorithmic_bytes(), w.flops()
+    tc_peak = peaks["bf16_tflops_sustained"] if sustained else peaks["bf16_tflops"]
+    t_hbm = by / (peaks["hbm_gbs"] * 1e9)
+    t_tc = fl / (tc_peak * 1e12)
+    if t_hbm >= t_tc:
+        ach = by / (fused_us * 1e-6) / 1e9
+        return dict(bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"],
+                    frac_of_nominal=ach / NOMINAL_HBM_GBS, peak_source=f"of {peaks['source']}")
+    ach = fl / (fused_us * 1e-6) / 1e12
+    return dict(bound="tensor", achieved=ach, peak=tc_peak, unit="TFLOP/s", frac=ach / tc_peak,
+                frac_of_nominal=ach / NOMINAL_BF16_TFLOPS,
+                peak_source=f"of {peaks['source']} ({'sustained' if sustained else 'burst'})")
+
+
+# ----------------------------------------------------------------------------------------- GPU arm
+class GpuCase:
+    def __init__(self, w: wl.Workload, device, two_w_copies: bool = False, Ws=None):
+        import torch
+        from paper_2606_31580_b200 import binding as B
+        self.torch, self.B, self.w = torch, B, w
+        self.hidden = B.bf16_tensor_from_bits(w.hidden_bits, device)
+        if Ws is None:
+            Ws = [B.bf16_tensor_from_bits(w.W_bits, device)]
+            if two_w_copies:
+                Ws.append(Ws[0].clone())
+        self.Ws = Ws
+        self.off = torch.from_numpy(w.req_offsets).to(device)
+        self.load = torch.from_numpy(w.load).to(device)
+        self.tp = B.TauParams(**w.tau_params)
+        self.probe = B.Probe(w.N_alloc, w.d, w.V, w.R, device=device, debug_outputs=False)
+        self.i = 0
+
+    def step(self):
+        W = self.Ws[self.i % len(self.Ws)]
+        self.i += 1
+        return self.probe(self.hidden, W, self.off, self.load, self.tp)
+
+    def time_steps(self, steps: int, sync_fn=None):
+        """K steps bracketed by events on the launch stream; returns total milliseconds."""
+        torch = self.torch
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if sync_fn:
+            sync_fn()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(steps):
+            self.step()
+        e1.record()
+        torch.cuda.synchronize()
+        if sync_fn:
+            sync_fn()
+        return e0.elapsed_time(e1)
+
+    def kernel_times(self, steps: int):
+        """Average duration (us) of the fused and the finalize kernel over `steps` calls."""
+        B = self.B
+        fused = fin = 0.0
+        n = 0
+        left = steps
+        B.profile_enable(True)
+        try:
+            while left > 0:
+                k = min(left, 256)
+                for _ in range(k):
+                    self.step()
+                a, b, c = B.profile_read()
+                fused += a; fin += b; n += c; left -= k
+        finally:
+            B.profile_enable(False)
+        return fused / n * 1e3, fin / n * 1e3
+
+
+def run_ours(args):
+    import torch
+    from paper_2606_31580_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", 0))
+    local_rank = int(os.environ.get("LOCAL_RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — this library has no CPU path (use --impl reference "
+                         "for the oracle's CPU timing)")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    peaks = measured_peaks()
+    W_cache: dict = {}
+    w = make_workload(args.workload, rank, W_cache)
+    case = GpuCase(w, device, two_w_copies=(w.V * w.d * 2 < 2_000_000_000))
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    sampler.start()
+
+    for _ in range(args.warmup):
+        case.step()
+    torch.cuda.synchronize()
+    barrier()
+    launches0 = B.kernel_launch_count()
+    t0 = time.perf_counter()
+    ms = case.time_steps(args.steps, barrier)
+    t1 = time.perf_counter()
+    launches = B.kernel_launch_count() - launches0
+    clocks = sampler.summary(t0, t1)
+    sampler.stop()
+
+    # dominant kernel on its own (second pass, same stream, library-recorded events)
+    fused_us, fin_us = case.kernel_times(args.steps)
+
+    # end to end through the host-buffer entry point
+    hp = B.HostProbe(w.N_alloc, w.d, w.V, w.R, device=device)
+    hh = B.bf16_tensor_from_bits(w.hidden_bits, pin=True)
+    hoff = torch.from_numpy(w.req_offsets).pin_memory()
+    hload = torch.from_numpy(w.load).pin_memory()
+    for _ in range(args.warmup):
+        hp(hh, case.Ws[0], hoff, hload, case.tp)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    te0 = time.perf_counter()
+    for i in range(args.steps):
+        hp(hh, case.Ws[i % len(case.Ws)], hoff, hload, case.tp)
+    te1 = time.perf_counter()
+    e1.record()
+    torch.cuda.synchronize()
+    e2e_ms = max(e0.elapsed_time(e1), (te1 - te0) * 1e3)   # host-synchronous: wall == device span
+
+    if dist is not None:
+        t = torch.tensor([ms, e2e_ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = float(t[0]), float(t[1])
+        rows_t = torch.tensor([w.N_valid, w.R], device=device, dtype=torch.float64)
+        dist.all_reduce(rows_t, op=dist.ReduceOp.SUM)
+        rows_all, reqs_all = float(rows_t[0]), float(rows_t[1])
+    else:
+        rows_all, reqs_all = float(w.N_valid), float(w.R)
+
+    out = None
+    if rank == 0:
+        ms_per_step = ms / args.steps
+        value = rows_all / (ms_per_step * 1e-3)
+        roof = roofline_for(w, fused_us, peaks, sustained=False)
+        roof["traffic"] = ncu_traffic_bytes(args.workload)
+        roof["kernel"] = "laser_probe_fused_kernel"
+        roof["kernel_us"] = fused_us
+        roof["finalize_kernel_us"] = fin_us
+        roof["algorithmic_bytes"] = w.algorithmic_bytes()
+        roof["step_frac"] = (w.algorithmic_bytes() / (ms_per_step * 1e-3) / 1e9 / peaks["hbm_gbs"]
+                             if roof["bound"] == "hbm" else
+                             w.flops() / (ms_per_step * 1e-3) / 1e12 / peaks["bf16_tflops"])
+        out = dict(
+            metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+            ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None,
+            dtype="bf16", data="synthetic",
+            config=dict(workload=describe(w), plan=case.probe.plan,
+                        l2="W (%.0f MB) exceeds the 126 MB L2; two W copies alternate between steps"
+                           % (w.V * w.d * 2 / 1e6) if len(case.Ws) > 1 else
+                           "W (%.0f MB) exceeds the 126 MB L2" % (w.V * w.d * 2 / 1e6),
+                        sharding="requests sharded across ranks, W replicated, no collective" if world > 1 else "single GPU",
+                        e2e_w_resident=True),
+            requests_per_sec=reqs_all / (ms_per_step * 1e-3),
+            clocks=clocks,
+            e2e=dict(value=rows_all / (e2e_ms / args.steps * 1e-3), unit=UNIT,
+                     h2d_bytes_per_step=hp.h2d_bytes, d2h_bytes_per_step=hp.d2h_bytes,
+                     ms_per_step=e2e_ms / args.steps),
+            gpu_launches=int(launches),
+            roofline=roof,
+        )
+
+    # heavy-load sweep (configs[4]) — rank 0, single GPU only; W shared with C2
+    if rank == 0 and world == 1 and not args.no_sweep and args.workload == "C2":
+        sweep = []
+        for N in wl.C5_NS:
+            ws = wl.config_c5(N, W_cache["C2"])
+            c = GpuCase(ws, device, Ws=case.Ws)
+            k = max(5, min(args.steps, int(2e5 / max(N, 128))))
+            for _ in range(3):
+                c.step()
+            t_ms = c.time_steps(k) / k
+            f_us, z_us = c.kernel_times(min(k, 64))
+            r = roofline_for(ws, f_us, peaks, sustained=(N >= 4096))
+            sweep.append(dict(N=N, us_per_step=t_ms * 1e3, rows_per_sec=N / (t_ms * 1e-3), fused_us=f_us,
+                              finalize_us=z_us, bound=r["bound"], achieved=r["achieved"], unit=r["unit"],
+                              frac=r["frac"], frac_of_nominal=r["frac_of_nominal"], plan=c.probe.plan))
+            del c
+        out["sweep"] = sweep
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(w, target_s=10.0)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+
+
+# ----------------------------------------------------------------------------------------- CPU arm
+def cpu_baseline(w: wl.Workload, target_s: float):
+    """The fp64 oracle, as it stands, on this box's host cores, on the same workload (a bounded sample
+    for the large configs).  bench.py's cpu_baseline / --impl reference legs are, with tests/ and
+    smoke(), the only callers of oracle/ in the repo."""
+    import oracle
+    tp = oracle.TauParams(**w.tau_params)
+    budget_rows = max(8, int(120e9 / (2.0 * w.V * w.d)))   # ~120 GFLOP per repetition
+    reqs = 0
+    while reqs < w.R and int(w.req_offsets[reqs + 1]) <= budget_rows:
+        reqs += 1
+    reqs = max(reqs, 1)
+    rows = int(w.req_offsets[reqs])
+    hid, off, load = w.hidden_f32()[:rows], w.req_offsets[:reqs + 1], w.load[:reqs]
+    Wf = w.W_f32()
+    best, spent, reps = None, 0.0, 0
+    while spent < target_s and reps < 5:
+        r = oracle.probe(hid, Wf, off, load, tp)
+        best = r.seconds if best is None else min(best, r.seconds)
+        spent += r.seconds
+        reps += 1
+    return dict(value=rows / best, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                sample=f"first {reqs} requests ({rows} rows) of {w.name}, full V and d; best of {reps} runs "
+                       f"({best:.2f} s each), fp64, OpenMP over rows",
+                requests_per_sec=reqs / best)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    if rank != 0:
+        return
+    import oracle
+    w = wl.by_name(args.workload, {})
+    tp = oracle.TauParams(**w.tau_params)
+    # bounded sample per step: whole requests, about 4 GFLOP of fp64 (a fraction of a second of CPU
+    # time), so that --steps 200 still ends within a minute or two
+    budget_rows = max(4, int(4e9 / (2.0 * w.V * w.d)))
+    reqs = 0
+    while reqs < w.R and int(w.req_offsets[reqs + 1]) <= budget_rows:
+        reqs += 1
+    reqs = max(reqs, 1)
+    rows = int(w.req_offsets[reqs])
+    hid, off, load = w.hidden_f32()[:rows], w.req_offsets[:reqs + 1], w.load[:reqs]
+    Wf = w.W_f32()
+    steps, warm = args.steps, args.warmup
+    for _ in range(warm):
+        oracle.probe(hid, Wf, off, load, tp)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.probe(hid, Wf, off, load, tp)
+    dt = time.perf_counter() - t0
+    value = rows * steps / dt
+    sample = (f"each step = fp64 oracle on the first {reqs} requests ({rows} rows) of {w.name}, full V and d")
+    print(json.dumps(dict(
+        impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=steps, warmup=warm,
+        ms_per_step=dt / steps * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+        data="synthetic", config=dict(workload=describe(w)),
+        cpu_baseline=dict(value=value, unit=UNIT, cores=oracle.num_threads(), kind="oracle", sample=sample),
+        e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+        gpu_launches=0)), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C2")
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    args.steps = max(args.steps, 1)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -168,6 +168,16 @@ int laser_budget_params_default(laser_budget_params* out);
 int laser_allocate_budget(const int32_t* prompt_tokens, const float* L, int32_t R,
                           const laser_budget_params* params, int32_t* out_budget);
 
+/*
+ * Per-kernel timing for bench / profiling (thread-local; off by default).  While enabled, each
+ * laser_probe_confidence* call on this thread records CUDA events on its stream before the fused
+ * kernel, between the two kernels and after the finalize kernel (up to 512 calls; programmatic
+ * dependent launch is not used for those calls).  laser_profile_read() waits for the last recorded
+ * call, returns the summed durations in milliseconds and the number of calls, and resets the count.
+ */
+int laser_profile_enable(int on);
+int laser_profile_read(float* ms_fused_sum, float* ms_finalize_sum, int32_t* calls);
+
 /* Text for a status code; never NULL. */
 const char* laser_status_string(int status);
 /* Detail of the last LASER_E_CUDA on this thread ("" if none). */

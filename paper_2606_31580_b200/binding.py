@@ -21,7 +21,8 @@ EXPORTS = [
     "laser_probe_confidence", "laser_probe_confidence_agg", "laser_probe_staging_bytes",
     "laser_probe_confidence_host", "laser_tau_from_load", "laser_ema_update",
     "laser_budget_params_default", "laser_allocate_budget", "laser_status_string",
-    "laser_last_error", "laser_kernel_launch_count", "laser_shutdown",
+    "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
+    "laser_profile_read",
 ]
 
 
@@ -94,6 +95,8 @@ def lib():
         L.laser_status_string.restype = C.c_char_p
         L.laser_last_error.restype = C.c_char_p
         L.laser_kernel_launch_count.restype = C.c_uint64
+        L.laser_profile_enable.argtypes = [C.c_int]
+        L.laser_profile_read.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_int32)]
         _lib = L
     return _lib
 
@@ -123,6 +126,17 @@ def staging_bytes(N, d, V, R) -> int:
 
 def kernel_launch_count() -> int:
     return int(lib().laser_kernel_launch_count())
+
+
+def profile_enable(on: bool):
+    _check(lib().laser_profile_enable(1 if on else 0))
+
+
+def profile_read():
+    """-> (fused kernel ms summed, finalize kernel ms summed, calls) since the last read."""
+    a, b, n = C.c_float(), C.c_float(), C.c_int32()
+    _check(lib().laser_profile_read(C.byref(a), C.byref(b), C.byref(n)))
+    return a.value, b.value, n.value
 
 
 def tau_from_load(load, params: TauParams):

@@ -25,6 +25,17 @@ using namespace laser;
 thread_local std::string g_last_error;
 std::atomic<uint64_t> g_launches{0};
 
+// Optional per-kernel timing (bench / profiling only): when enabled on this thread, every call
+// records events before the fused kernel, between the kernels and after the finalize kernel.
+constexpr int kProfRing = 512;
+struct ProfState {
+    bool on = false;
+    int calls = 0;
+    cudaEvent_t ev[kProfRing][3] = {};
+    bool created = false;
+};
+thread_local ProfState g_prof;
+
 constexpr int kDefaultSMs = 148;             // B200
 constexpr int kMaxDynSmem = 227 * 1024;      // per-CTA opt-in limit on sm_100
 constexpr int kSmemSlack = 1024 + 256;       // alignment slack + barrier block
@@ -270,6 +281,8 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
     float* ws_s = reinterpret_cast<float*>(ws_a + static_cast<size_t>(pl.splits) * n_pad);
 
     const bool run_fused = (N > 0 && R > 0);
+    const bool prof = g_prof.on && g_prof.created && run_fused && g_prof.calls < kProfRing;
+    const int prof_slot = g_prof.calls;
     if (run_fused) {
         if (!di->attr_set) {
             cudaError_t e = cudaFuncSetAttribute(laser_probe_fused_kernel,
@@ -295,6 +308,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         fp.w_policy = (pl.m_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
         fp.ws_m = ws_m; fp.ws_a = ws_a; fp.ws_s = ws_s;
 
+        if (prof) cudaEventRecord(g_prof.ev[prof_slot][0], stream);
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(pl.grid);
         cfg.blockDim = dim3(kFusedThreads);
@@ -328,7 +342,8 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         cfg.stream = stream;
         cudaLaunchAttribute attr[1];
         static const bool no_pdl = getenv("LASER_NO_PDL") != nullptr;
-        if (run_fused && !no_pdl) {
+        if (prof) cudaEventRecord(g_prof.ev[prof_slot][1], stream);
+        if (run_fused && !no_pdl && !prof) {
             attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
             attr[0].val.programmaticStreamSerializationAllowed = 1;
             cfg.attrs = attr;
@@ -337,6 +352,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_finalize_kernel, fz);
         if (e != cudaSuccess) return set_cuda_error("launch laser_probe_finalize_kernel", e);
         g_launches.fetch_add(1, std::memory_order_relaxed);
+        if (prof) { cudaEventRecord(g_prof.ev[prof_slot][2], stream); g_prof.calls++; }
     }
     return LASER_OK;
 }
@@ -466,6 +482,36 @@ const char* laser_status_string(int status) {
         case LASER_E_MODE: return "unknown aggregate mode";
         default: return "unknown status";
     }
+}
+
+int laser_profile_enable(int on) {
+    if (on && !g_prof.created) {
+        for (int i = 0; i < kProfRing; ++i)
+            for (int j = 0; j < 3; ++j) {
+                cudaError_t e = cudaEventCreate(&g_prof.ev[i][j]);
+                if (e != cudaSuccess) return set_cuda_error("cudaEventCreate", e);
+            }
+        g_prof.created = true;
+    }
+    g_prof.on = on != 0;
+    g_prof.calls = 0;
+    return LASER_OK;
+}
+
+int laser_profile_read(float* ms_fused_sum, float* ms_finalize_sum, int32_t* calls) {
+    if (!ms_fused_sum || !ms_finalize_sum || !calls) return LASER_E_NULL;
+    *ms_fused_sum = 0.f; *ms_finalize_sum = 0.f; *calls = g_prof.calls;
+    if (!g_prof.created || g_prof.calls == 0) return LASER_OK;
+    cudaError_t e = cudaEventSynchronize(g_prof.ev[g_prof.calls - 1][2]);
+    if (e != cudaSuccess) return set_cuda_error("cudaEventSynchronize", e);
+    for (int i = 0; i < g_prof.calls; ++i) {
+        float a = 0.f, b = 0.f;
+        cudaEventElapsedTime(&a, g_prof.ev[i][0], g_prof.ev[i][1]);
+        cudaEventElapsedTime(&b, g_prof.ev[i][1], g_prof.ev[i][2]);
+        *ms_fused_sum += a; *ms_finalize_sum += b;
+    }
+    g_prof.calls = 0;
+    return LASER_OK;
 }
 
 const char* laser_last_error(void) { return g_last_error.c_str(); }

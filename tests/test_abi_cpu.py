@@ -1,0 +1,141 @@
+"""CPU-only checks of the C-ABI library: it loads without a GPU, exports every symbol the header
+declares, validates arguments, plans launches sanely, and refuses (loudly) to compute without a
+B200.  The host-side scalar helpers (tau, EMA, budget) are compared with the oracle."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_31580_b200 import binding as B
+from paper_2606_31580_b200 import build as build_mod
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build_mod.build()
+
+
+def test_header_symbols_all_exported():
+    hdr = (ROOT / "include" / "laser_probe.h").read_text()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(laser_[a-z_]+)\s*\(", hdr))
+    assert declared, "no declarations found"
+    L = B.lib()
+    missing = [s for s in sorted(declared) if not hasattr(L, s)]
+    assert not missing, missing
+    assert declared == set(B.EXPORTS), declared ^ set(B.EXPORTS)
+
+
+def test_library_is_sm100a_with_tcgen05_and_tma():
+    """The shipped binary holds sm_100a SASS with the Blackwell tensor / TMA instructions."""
+    import shutil, subprocess
+    if not shutil.which("cuobjdump"):
+        pytest.skip("cuobjdump not on PATH")
+    so = ROOT / "paper_2606_31580_b200" / "liblaser_probe.so"
+    sass = subprocess.run(["cuobjdump", "-sass", str(so)], capture_output=True, text=True).stdout
+    assert "sm_100a" in sass
+    for mnemonic in ("UTCHMMA", "LDTM", "UTMALDG"):
+        assert mnemonic in sass, mnemonic
+    assert "HMMA." not in sass.replace("UTCHMMA", "")       # no legacy mma.sync path
+
+
+@pytest.mark.parametrize("dims", [(128, 1536, 151936, 16), (256, 3584, 152064, 32), (1024, 4096, 128256, 64),
+                                  (32, 64, 1000, 8), (8, 1536, 151936, 1), (64, 1536, 151936, 8),
+                                  (512, 1536, 151936, 64), (4096, 1536, 151936, 512),
+                                  (16384, 1536, 151936, 2048), (1, 8, 1, 1), (300, 72, 70001, 20)])
+def test_plan_invariants(dims):
+    N, d, V, R = dims
+    p = B.plan_query(*dims)
+    bn, T, S = p["tile_n"], p["tiles_per_split"], p["splits"]
+    assert bn % 16 == 0 and 16 <= bn <= 256
+    assert S * T * bn >= V and (S - 1) * T * bn < V          # splits tile the vocabulary exactly once
+    assert p["m_tiles"] == max(1, -(-N // 128)) and p["k_blocks"] == -(-d // 64)
+    assert p["work_items"] == p["m_tiles"] * S and 1 <= p["grid"] <= min(p["num_sms"], p["work_items"])
+    assert 2 <= p["stages"] <= 8
+    assert p["stages"] * (16384 + bn * 128) + 1280 == p["smem_bytes"] <= 227 * 1024
+    assert B.workspace_bytes(*dims) == max(16, 12 * S * p["m_tiles"] * 128)
+    # the busiest CTA does at most ~8 % more than an even share of W rows (+ one tile of slack)
+    rounds = -(-p["work_items"] // p["grid"])
+    assert rounds * T * bn <= 1.08 * (p["m_tiles"] * V / p["grid"]) + bn
+
+
+def test_c2_plan_is_the_documented_one():
+    p = B.plan_query(128, 1536, 151936, 16)
+    assert (p["splits"], p["tiles_per_split"], p["tile_n"], p["stages"], p["grid"]) == (147, 5, 208, 5, 147)
+
+
+def test_argument_validation_needs_no_gpu():
+    L = B.lib()
+    tp = B.TauParams()
+    assert B.workspace_bytes(128, 1537, 1000, 4) == 0                      # d % 8 != 0
+    assert B.workspace_bytes(128, 0, 1000, 4) == 0 and B.workspace_bytes(-1, 64, 1000, 4) == 0
+    buf = (C.c_char * 4096)()
+    a = C.addressof(buf)
+    args = lambda dims, t=tp, mode=0: (a, a, a, a, C.byref(t), a, a, a, C.byref(dims), a, 4096, None, None, None, mode)
+    assert L.laser_probe_confidence_agg(*args(B.Dims(32, 60, 1000, 8))) == -2    # LASER_E_DIMS
+    assert L.laser_probe_confidence_agg(*args(B.Dims(32, 64, 1000, 8), B.TauParams(l_target=0.0))) == -4
+    assert L.laser_probe_confidence_agg(*args(B.Dims(32, 64, 1000, 8), B.TauParams(lambda_min=0.98))) == -4
+    assert L.laser_probe_confidence_agg(*args(B.Dims(32, 64, 1000, 8), B.TauParams(beta=float("nan")))) == -4
+    assert L.laser_probe_confidence_agg(*args(B.Dims(32, 64, 1000, 8), tp, 7)) == -8     # LASER_E_MODE
+    assert L.laser_probe_confidence_agg(*args(B.Dims(0, 64, 1000, 0))) == 0             # empty batch: no-op
+    bad = list(args(B.Dims(32, 64, 1000, 8))); bad[0] = None
+    assert L.laser_probe_confidence_agg(*bad) == -1                                     # LASER_E_NULL
+    assert L.laser_probe_confidence_agg(*args(B.Dims(32, 64, 1000, 8))[:0], *[a + 2] + list(args(B.Dims(32, 64, 1000, 8)))[1:]) == -3
+    for code in range(-8, 1):
+        assert L.laser_status_string(code)
+
+
+def test_no_cpu_fallback():
+    """Without a B200 the compute entry point must fail loudly, never compute."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present; covered by the gpu tests")
+    L = B.lib()
+    buf = (C.c_char * (1 << 20))()
+    a = (C.addressof(buf) + 255) // 256 * 256
+    rc = L.laser_probe_confidence(a, a, a, a, C.byref(B.TauParams()), a, a, a, C.byref(B.Dims(32, 64, 1000, 8)),
+                                  a, 1 << 19, None, None, None)
+    assert rc in (-7, -6)                                                  # LASER_E_CUDA / LASER_E_ARCH
+    with pytest.raises(B.LaserError):
+        B._check(rc)
+
+
+def test_tau_from_load_matches_oracle():
+    rng = np.random.default_rng(0)
+    for kw in (dict(), dict(l_target=0.5), dict(beta=0.1, gamma=2.0, l_target=8.0), dict(beta=0.0, lambda_base=0.9)):
+        load = (rng.random(257) * 4 * kw.get("l_target", 10.0)).astype(np.float32)
+        got = B.tau_from_load(load, B.TauParams(**kw))
+        want = oracle.tau(load, oracle.TauParams(**kw))
+        np.testing.assert_allclose(got, want, atol=2e-7)
+        assert got.min() >= np.float32(0.88) and got.max() <= np.float32(0.97)
+    d = B.TauParams()
+    B.lib().laser_tau_params_default(C.byref(d))
+    assert [round(getattr(d, f), 6) for f, _ in d._fields_] == [0.95, 0.04, 1.0, 10.0, 0.88, 0.97]
+
+
+def test_ema_and_budget_match_oracle():
+    rng = np.random.default_rng(1)
+    L = (rng.random((50, 6)) * 30).astype(np.float32)
+    lbar = np.zeros(6, np.float32)                                        # Alg. 1 line 1: Lbar <- 0
+    traj = []
+    for t in range(50):
+        B.ema_update(lbar, L[t], alpha=0.3)
+        traj.append(lbar.copy())
+    traj = np.stack(traj)
+    for j in range(6):
+        np.testing.assert_allclose(traj[:, j], oracle.ema(L[:, j].astype(np.float64), 0.3), rtol=2e-6)
+    pt = rng.integers(1, 600, 500)
+    Lr = (rng.random(500) * 60).astype(np.float32)
+    got = B.allocate_budget(pt, Lr)
+    # same inputs on both sides: the ABI's parameters are floats, so the oracle gets the float32-rounded
+    # defaults (a floor() decides an integer here; both sides then decide it in double)
+    f32 = lambda x: float(np.float32(x))
+    q = oracle.BudgetParams(f_min=f32(0.6), f_max=f32(1.5))
+    want = oracle.budget(pt.astype(np.float64), Lr.astype(np.float64), q)
+    assert np.array_equal(got, want)
+    assert got.min() >= 2 and got.max() <= 15
