@@ -281,6 +281,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
     float* ws_s = reinterpret_cast<float*>(ws_a + static_cast<size_t>(pl.splits) * n_pad);
 
     const bool run_fused = (N > 0 && R > 0);
+    static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
     const bool prof = g_prof.on && g_prof.created && run_fused && g_prof.calls < kProfRing;
     const int prof_slot = g_prof.calls;
     if (run_fused) {
@@ -314,6 +315,16 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         cfg.blockDim = dim3(kFusedThreads);
         cfg.dynamicSmemBytes = static_cast<size_t>(pl.smem_bytes);
         cfg.stream = stream;
+        // Programmatic dependent launch: the prologue (barrier init, TMEM allocation, descriptor
+        // prefetch) may overlap the tail of the previous kernel in the stream; the kernel executes
+        // griddepcontrol.wait before its first global-memory access.
+        cudaLaunchAttribute fattr[1];
+        if (use_pdl && !prof) {
+            fattr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            fattr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = fattr;
+            cfg.numAttrs = 1;
+        }
         cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel, tm_h, tm_w, fp);
         if (e != cudaSuccess) return set_cuda_error("launch laser_probe_fused_kernel", e);
         g_launches.fetch_add(1, std::memory_order_relaxed);
@@ -341,9 +352,8 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         cfg.dynamicSmemBytes = 0;
         cfg.stream = stream;
         cudaLaunchAttribute attr[1];
-        static const bool no_pdl = getenv("LASER_NO_PDL") != nullptr;
         if (prof) cudaEventRecord(g_prof.ev[prof_slot][1], stream);
-        if (run_fused && !no_pdl && !prof) {
+        if (run_fused && use_pdl && !prof) {
             attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
             attr[0].val.programmaticStreamSerializationAllowed = 1;
             cfg.attrs = attr;

@@ -152,7 +152,10 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
-    // Let the finalize kernel's CTAs be scheduled as SMs free up (it waits on griddepcontrol.wait).
+    // Programmatic dependent launch: everything above overlapped the previous kernel in the stream;
+    // nothing below may touch global memory before that kernel has completed.
+    ptx::pdl_wait();
+    // Let the finalize kernel's CTAs become resident now (they block in griddepcontrol.wait).
     ptx::pdl_launch_dependents();
 
     const int T = p.tiles_per_split, BN = p.tile_n;
@@ -304,36 +307,57 @@ __device__ __forceinline__ void merge_stats(float& m, int& a, float& s, float m2
     a = an;
 }
 
-constexpr int kFinalizeThreads = 128;
+constexpr int kFinalizeThreads = 256;
+constexpr int kFinalizeWarps = kFinalizeThreads / 32;
+constexpr int kMergeBatch = 4;  // partials a lane loads before it starts merging
 
-// Blocks [0, R): one request each.  A warp takes rows b+w, b+w+4, ...: its lanes stride over the
-// vocabulary splits of the row, fold their own partials, then merge across the warp with shuffles.
-// Blocks [R, R + ceil(n_alloc/128)): mark padding rows (n >= req_offsets[R]).
+// Blocks [0, R): one request each.  A warp takes rows b+w, b+w+8, ...: its lanes stride over the
+// vocabulary splits of the row (loads issued in batches so that they overlap), fold their own
+// partials, then merge across the warp with shuffles.
+// Blocks [R, R + ceil(n_alloc/256)): mark padding rows (n >= req_offsets[R]).
+// Everything that does not depend on the fused kernel (offsets, load, threshold) is read before
+// griddepcontrol.wait so that under programmatic dependent launch it overlaps the fused kernel.
 __global__ void __launch_bounds__(kFinalizeThreads)
 laser_probe_finalize_kernel(const FinalizeParams p) {
-    ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (static_cast<int>(blockIdx.x) >= p.R) {
         const int n = (blockIdx.x - p.R) * kFinalizeThreads + threadIdx.x;
-        const int n_valid = (p.R > 0) ? p.req_offsets[p.R] : 0;
-        if (n < p.n_alloc && n >= n_valid) {
+        const int n_valid = (p.R > 0) ? __ldg(p.req_offsets + p.R) : 0;
+        if (n < p.n_alloc && n >= n_valid) {   // outputs of padding rows: independent of the fused kernel
             p.out_argmax[n] = -1;
             if (p.out_pmax) p.out_pmax[n] = CUDART_NAN_F;
         }
         return;
     }
-    __shared__ float warp_acc[kFinalizeThreads / 32];
+    __shared__ float warp_acc[kFinalizeWarps];
     const int r = blockIdx.x;
-    const int b = p.req_offsets[r], e = p.req_offsets[r + 1];
+    const int b = __ldg(p.req_offsets + r), e = __ldg(p.req_offsets + r + 1);
+    float tau = 0.f;
+    if (threadIdx.x == 0) tau = tau_eval(__ldg(p.load + r), p.tau);   // a4
+
+    ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
+    ptx::pdl_launch_dependents();  // the next kernel's prologue may overlap the rest of this one
+
     // running aggregate of this warp's rows: sum (mean), sum of logs (geomean), min
     float acc = (p.agg_mode == 2) ? CUDART_INF_F : 0.f;
     bool any_nan = false;
-    for (int n = b + warp; n < e; n += kFinalizeThreads / 32) {
+    for (int n = b + warp; n < e; n += kFinalizeWarps) {
         float m = -CUDART_INF_F, s = 0.f;
         int a = 0x7fffffff;
-        for (int sp = lane; sp < p.splits; sp += 32) {
-            const size_t o = static_cast<size_t>(sp) * p.n_pad + n;
-            merge_stats(m, a, s, p.ws_m[o], p.ws_a[o], p.ws_s[o]);
+        for (int sp0 = lane; sp0 < p.splits; sp0 += 32 * kMergeBatch) {
+            float pm[kMergeBatch], ps[kMergeBatch];
+            int pa[kMergeBatch];
+#pragma unroll
+            for (int j = 0; j < kMergeBatch; ++j) {
+                const int sp = sp0 + 32 * j;
+                const bool ok = sp < p.splits;
+                const size_t o = static_cast<size_t>(ok ? sp : 0) * p.n_pad + n;
+                pm[j] = ok ? p.ws_m[o] : -CUDART_INF_F;
+                pa[j] = ok ? p.ws_a[o] : 0x7fffffff;
+                ps[j] = ok ? p.ws_s[o] : 0.f;
+            }
+#pragma unroll
+            for (int j = 0; j < kMergeBatch; ++j) merge_stats(m, a, s, pm[j], pa[j], ps[j]);
         }
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
@@ -342,7 +366,8 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
             const float s2 = __shfl_xor_sync(0xffffffffu, s, off);
             merge_stats(m, a, s, m2, a2, s2);
         }
-        const float pmax = 1.0f / s;
+        // s >= 1 up to the rounding of ex2.approx; a probability does not exceed 1.  NaN stays NaN.
+        const float pmax = (s == s) ? fminf(1.0f / s, 1.0f) : CUDART_NAN_F;
         if (lane == 0) {
             p.out_argmax[n] = a;
             if (p.out_pmax) p.out_pmax[n] = pmax;
@@ -362,21 +387,20 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
             if (p.agg_mode == 2) {
                 conf = warp_acc[0];
                 bool nan = conf != conf;
-                for (int w = 1; w < kFinalizeThreads / 32; ++w) {
+                for (int w = 1; w < kFinalizeWarps; ++w) {
                     nan |= (warp_acc[w] != warp_acc[w]);
                     conf = fminf(conf, warp_acc[w]);
                 }
                 if (nan) conf = CUDART_NAN_F;
             } else {
                 float t = 0.f;
-                for (int w = 0; w < kFinalizeThreads / 32; ++w) t += warp_acc[w];
+                for (int w = 0; w < kFinalizeWarps; ++w) t += warp_acc[w];
                 conf = t / static_cast<float>(len);
                 if (p.agg_mode == 1) conf = expf(conf);
             }
         }
-        const float tau = tau_eval(p.load[r], p.tau);
-        p.out_conf[r] = conf;
-        p.out_exit[r] = (conf > tau) ? 1 : 0;  // strict; NaN > tau is false
+        p.out_conf[r] = conf;                  // a3
+        p.out_exit[r] = (conf > tau) ? 1 : 0;  // a5: strict; NaN > tau is false
         if (p.out_tau) p.out_tau[r] = tau;
     }
 }
