@@ -64,17 +64,25 @@ typedef struct {
 /* How a call is laid out on the GPU (informational; filled by laser_probe_plan_query). */
 typedef struct {
     int32_t num_sms;         /* SMs the plan was made for                                             */
-    int32_t m_tiles;         /* ceil(N / 128) token tiles                                             */
+    int32_t m_tiles;         /* ceil(N / tile_m) token tiles                                          */
     int32_t splits;          /* vocabulary splits S                                                   */
     int32_t tiles_per_split; /* vocab tiles per split T                                               */
-    int32_t tile_n;          /* vocab rows per tile BN (multiple of 16, <= 256)                       */
+    int32_t tile_n;          /* vocab rows per tile BN (multiple of 16; 32 in pair mode; <= 256)      */
     int32_t k_blocks;        /* ceil(d / 64)                                                          */
     int32_t stages;          /* shared-memory pipeline depth                                          */
     int32_t grid;            /* CTAs of the fused kernel (persistent, <= num_sms)                     */
     int32_t work_items;      /* m_tiles * splits                                                      */
     int32_t smem_bytes;      /* dynamic shared memory per CTA                                         */
     int32_t kernel_launches; /* kernels one laser_probe_confidence call enqueues                      */
+    int32_t tile_m;          /* token rows per work item: 128 (one CTA) or 256 (CTA pair)             */
+    int32_t cta_pair;        /* 1: clusters of two CTAs, tcgen05 cta_group::2; 0: one CTA per item    */
 } laser_probe_plan;
+
+/* Kernel variant selection.  AUTO (default): one CTA per work item for N <= 128 rows and for small
+ * odd counts of 128-row tiles (< 10), CTA pairs otherwise.  SINGLE / PAIR force one variant for every shape (tuning and tests; both are exact).
+ * Process-wide; affects laser_probe_plan_query / workspace_bytes and subsequent calls. */
+enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2 };
+int laser_probe_set_mode(int mode);
 
 /* Aggregate that turns the per-token max probabilities of a request into its confidence.
  * The paper does not fix it; MEAN is the default reading (A1). */
@@ -83,7 +91,7 @@ enum { LASER_AGG_MEAN = 0, LASER_AGG_GEOMEAN = 1, LASER_AGG_MIN = 2 };
 /* Writes the paper's defaults.  Host. */
 int laser_tau_params_default(laser_tau_params* out);
 
-/* Device scratch laser_probe_confidence needs for `dims`, in bytes (12 * splits * m_tiles * 128,
+/* Device scratch laser_probe_confidence needs for `dims`, in bytes (12 * splits * m_tiles * tile_m,
  * at least 16).  Returns 0 for invalid dims.  Host; needs no GPU. */
 size_t laser_probe_workspace_bytes(const laser_probe_dims* dims);
 

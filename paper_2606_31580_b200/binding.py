@@ -15,6 +15,7 @@ _SO = Path(__file__).resolve().parent / "liblaser_probe.so"
 _lib = None
 
 AGG_MEAN, AGG_GEOMEAN, AGG_MIN = 0, 1, 2
+MODE_AUTO, MODE_SINGLE, MODE_PAIR = 0, 1, 2
 
 EXPORTS = [
     "laser_tau_params_default", "laser_probe_workspace_bytes", "laser_probe_plan_query",
@@ -22,7 +23,7 @@ EXPORTS = [
     "laser_probe_confidence_host", "laser_tau_from_load", "laser_ema_update",
     "laser_budget_params_default", "laser_allocate_budget", "laser_status_string",
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
-    "laser_profile_read",
+    "laser_profile_read", "laser_probe_set_mode",
 ]
 
 
@@ -53,7 +54,7 @@ class Dims(C.Structure):
 class Plan(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("num_sms", "m_tiles", "splits", "tiles_per_split", "tile_n", "k_blocks", "stages",
-                 "grid", "work_items", "smem_bytes", "kernel_launches")]
+                 "grid", "work_items", "smem_bytes", "kernel_launches", "tile_m", "cta_pair")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -95,6 +96,7 @@ def lib():
         L.laser_status_string.restype = C.c_char_p
         L.laser_last_error.restype = C.c_char_p
         L.laser_kernel_launch_count.restype = C.c_uint64
+        L.laser_probe_set_mode.argtypes = [C.c_int]
         L.laser_profile_enable.argtypes = [C.c_int]
         L.laser_profile_read.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_int32)]
         _lib = L
@@ -122,6 +124,11 @@ def workspace_bytes(N, d, V, R) -> int:
 
 def staging_bytes(N, d, V, R) -> int:
     return int(lib().laser_probe_staging_bytes(C.byref(Dims(N, d, V, R))))
+
+
+def set_mode(mode: int):
+    """laser_probe_set_mode: MODE_AUTO / MODE_SINGLE / MODE_PAIR (process-wide kernel variant)."""
+    _check(lib().laser_probe_set_mode(mode))
 
 
 def kernel_launch_count() -> int:

@@ -84,48 +84,73 @@ bool dims_valid(const laser_probe_dims* d) {
     return d && d->d > 0 && d->V > 0 && d->N >= 0 && d->R >= 0 && (d->d % 8) == 0;
 }
 
-// Choose (splits, tiles_per_split, tile_n): the vocabulary is cut into splits of T*BN rows, BN a
-// multiple of 16 and <= 256.  m_tiles*splits should fill the SMs in whole rounds; among such
-// choices minimise the busiest CTA's work, counted in W rows plus a charge per tile for re-streaming
-// the 128 hidden rows from L2.
-void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
-    const int m_tiles = dm.N > 0 ? ceil_div(dm.N, kTileM) : 1;
-    const int s_unit = num_sms / gcd_i(num_sms, m_tiles);
+// Choose (splits, tiles_per_split, tile_n) for one kernel variant.  A "unit" is what executes a work
+// item: a CTA (single mode, 128 token rows) or a CTA pair (pair mode, 256 token rows).  The
+// vocabulary is cut into splits of T*BN rows, BN a multiple of `bn_step` and <= 256.  m_tiles*splits
+// should fill the units in whole rounds; among such choices minimise the busiest unit's work, counted
+// in W rows plus a charge per tile for re-streaming the hidden rows from L2.
+double plan_variant(const laser_probe_dims& dm, int units, int tile_m, int bn_step, int* oS, int* oT,
+                    int* oBN) {
+    const int m_tiles = dm.N > 0 ? ceil_div(dm.N, tile_m) : 1;
+    const int s_unit = units / gcd_i(units, m_tiles);
     const double kTileCharge = 32.0;  // W-row equivalents per tile (hidden re-stream, pipeline bubble)
     double best = 1e300;
-    int bS = 1, bT = 1, bBN = 16;
+    int bS = 1, bT = 1, bBN = bn_step;
     for (int k = 1; k <= 4; ++k) {
         const int s_try = s_unit * k;
         const int L = ceil_div(dm.V, s_try);
         const int t_min = ceil_div(L, kMaxTileN);
         for (int T = t_min; T <= t_min + 3; ++T) {
-            const int BN = round_up(ceil_div(L, T), 16);
+            const int BN = round_up(ceil_div(L, T), bn_step);
             if (BN > kMaxTileN) continue;
             const int S = ceil_div(dm.V, T * BN);
             const long items = static_cast<long>(m_tiles) * S;
-            const long rounds = (items + num_sms - 1) / num_sms;
+            const long rounds = (items + units - 1) / units;
             const double cost = static_cast<double>(rounds) * T * (BN + kTileCharge);
             if (cost < best - 1e-9) { best = cost; bS = S; bT = T; bBN = BN; }
         }
     }
+    *oS = bS; *oT = bT; *oBN = bBN;
+    return best;
+}
+
+std::atomic<int> g_force_mode{LASER_MODE_AUTO};
+
+void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
+    // CTA pairs (tcgen05 cta_group::2, M = 256) when there is more than one 128-row token tile: each
+    // W tile then enters a pair's shared memory once instead of once per token tile and one issuing
+    // thread feeds two SMs' tensor cores (measured +10..17 % for N >= 256).  An odd count of 128-row
+    // tiles makes the pair kernel compute one padding tile; that costs more than the pair gains
+    // until there are about ten tiles (measured: N = 384 and 640 are faster on single CTAs).
+    const int mode = g_force_mode.load(std::memory_order_relaxed);
+    const int t128 = ceil_div(dm.N, kTileM);
+    const bool auto_pair = t128 >= 2 && ((t128 % 2) == 0 || t128 >= 10);
+    const bool pair = mode == LASER_MODE_PAIR || (mode == LASER_MODE_AUTO && auto_pair);
+    const int tile_m = pair ? 2 * kTileM : kTileM;
+    const int units = pair ? (num_sms / 2 > 0 ? num_sms / 2 : 1) : num_sms;
+    int S, T, BN;
+    plan_variant(dm, units, tile_m, pair ? 32 : 16, &S, &T, &BN);
     pl->num_sms = num_sms;
-    pl->m_tiles = m_tiles;
-    pl->splits = bS;
-    pl->tiles_per_split = bT;
-    pl->tile_n = bBN;
+    pl->m_tiles = dm.N > 0 ? ceil_div(dm.N, tile_m) : 1;
+    pl->splits = S;
+    pl->tiles_per_split = T;
+    pl->tile_n = BN;
     pl->k_blocks = ceil_div(dm.d, kBlockK);
-    const int stage_bytes = kABytes + bBN * 128;
+    const int stage_bytes = kABytes + (pair ? BN / 2 : BN) * 128;
     int stages = (kMaxDynSmem - kSmemSlack) / stage_bytes;
     if (stages > kMaxStages) stages = kMaxStages;
     pl->stages = stages;
-    pl->work_items = m_tiles * bS;
-    pl->grid = pl->work_items < num_sms ? pl->work_items : num_sms;
+    pl->work_items = pl->m_tiles * S;
+    const int busy = pl->work_items < units ? pl->work_items : units;
+    pl->grid = pair ? 2 * busy : busy;
     pl->smem_bytes = stages * stage_bytes + kSmemSlack;
     pl->kernel_launches = 2;
+    pl->tile_m = tile_m;
+    pl->cta_pair = pair ? 1 : 0;
 }
 
 size_t workspace_bytes_for(const laser_probe_plan& pl) {
-    size_t b = static_cast<size_t>(12) * pl.splits * pl.m_tiles * kTileM;
+    size_t b = static_cast<size_t>(12) * pl.splits * pl.m_tiles * pl.tile_m;
     return b < 16 ? 16 : b;
 }
 
@@ -275,7 +300,8 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         return LASER_E_WORKSPACE;
 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
-    const int n_pad = pl.m_tiles * kTileM;
+    const int n_pad = pl.m_tiles * pl.tile_m;
+    const bool pair = pl.cta_pair != 0;
     float* ws_m = static_cast<float*>(workspace);
     int32_t* ws_a = reinterpret_cast<int32_t*>(ws_m + static_cast<size_t>(pl.splits) * n_pad);
     float* ws_s = reinterpret_cast<float*>(ws_a + static_cast<size_t>(pl.splits) * n_pad);
@@ -286,15 +312,19 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
     const int prof_slot = g_prof.calls;
     if (run_fused) {
         if (!di->attr_set) {
-            cudaError_t e = cudaFuncSetAttribute(laser_probe_fused_kernel,
+            cudaError_t e = cudaFuncSetAttribute(laser_probe_fused_kernel<false>,
                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(laser_probe_fused_kernel<true>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
             if (e != cudaSuccess) return set_cuda_error("cudaFuncSetAttribute", e);
             di->attr_set = true;
         }
         CUtensorMap tm_h, tm_w;
         int rc = get_tensor_map(hidden, N, dims->d, kTileM, &tm_h);
         if (rc != LASER_OK) return rc;
-        rc = get_tensor_map(W, dims->V, dims->d, pl.tile_n, &tm_w);
+        const int b_rows = pair ? pl.tile_n / 2 : pl.tile_n;   // W rows one CTA stages per tile
+        rc = get_tensor_map(W, dims->V, dims->d, b_rows, &tm_w);
         if (rc != LASER_OK) return rc;
 
         FusedParams fp;
@@ -302,7 +332,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         fp.m_tiles = pl.m_tiles; fp.splits = pl.splits; fp.tiles_per_split = pl.tiles_per_split;
         fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
         fp.work_items = pl.work_items; fp.n_pad = n_pad;
-        fp.stage_bytes = static_cast<uint32_t>(kABytes + pl.tile_n * 128);
+        fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
         fp.tx_bytes = fp.stage_bytes;  // OOB rows are zero-filled and still counted
         // W is streamed once when a single token tile exists; with several token tiles the other
         // CTAs re-read the same rows from L2, so do not mark them evict-first.
@@ -318,14 +348,24 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         // Programmatic dependent launch: the prologue (barrier init, TMEM allocation, descriptor
         // prefetch) may overlap the tail of the previous kernel in the stream; the kernel executes
         // griddepcontrol.wait before its first global-memory access.
-        cudaLaunchAttribute fattr[1];
+        cudaLaunchAttribute fattr[2];
+        unsigned na = 0;
         if (use_pdl && !prof) {
-            fattr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-            fattr[0].val.programmaticStreamSerializationAllowed = 1;
-            cfg.attrs = fattr;
-            cfg.numAttrs = 1;
+            fattr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            fattr[na].val.programmaticStreamSerializationAllowed = 1;
+            ++na;
         }
-        cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel, tm_h, tm_w, fp);
+        if (pair) {   // the two CTAs of a pair form a cluster (same TPC)
+            fattr[na].id = cudaLaunchAttributeClusterDimension;
+            fattr[na].val.clusterDim.x = 2;
+            fattr[na].val.clusterDim.y = 1;
+            fattr[na].val.clusterDim.z = 1;
+            ++na;
+        }
+        cfg.attrs = fattr;
+        cfg.numAttrs = na;
+        cudaError_t e = pair ? cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<true>, tm_h, tm_w, fp)
+                             : cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<false>, tm_h, tm_w, fp);
         if (e != cudaSuccess) return set_cuda_error("launch laser_probe_fused_kernel", e);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
@@ -521,6 +561,12 @@ int laser_profile_read(float* ms_fused_sum, float* ms_finalize_sum, int32_t* cal
         *ms_fused_sum += a; *ms_finalize_sum += b;
     }
     g_prof.calls = 0;
+    return LASER_OK;
+}
+
+int laser_probe_set_mode(int mode) {
+    if (mode < LASER_MODE_AUTO || mode > LASER_MODE_PAIR) return LASER_E_MODE;
+    g_force_mode.store(mode, std::memory_order_relaxed);
     return LASER_OK;
 }
 

@@ -39,9 +39,9 @@ constexpr float kLog2e = 1.4426950408889634f;
 struct FusedParams {
     int32_t n_alloc, d, V;
     int32_t m_tiles, splits, tiles_per_split, tile_n, k_blocks, stages;
-    int32_t work_items, n_pad;
-    uint32_t tx_bytes;     // bytes TMA delivers per stage (hidden box + W box)
-    uint32_t stage_bytes;  // shared-memory stride of a stage: kABytes + tile_n * 128
+    int32_t work_items, n_pad;   // m_tiles counts items of 128 (single) / 256 (pair) token rows
+    uint32_t tx_bytes;     // bytes TMA delivers per stage and CTA (hidden box + W box)
+    uint32_t stage_bytes;  // shared-memory stride of a stage: kABytes + (W rows per CTA) * 128
     uint64_t w_policy;     // L2 eviction policy for the W stream
     float* ws_m;           // [splits, n_pad] running max per (split, row)
     int32_t* ws_a;         // [splits, n_pad] argmax
@@ -59,9 +59,10 @@ __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t smem_addr) {
     desc |= static_cast<uint64_t>(2) << 61;                       // SWIZZLE_128B   [61,64)
     return desc;
 }
-// Instruction descriptor for kind::f16: D fp32, A/B bf16, both K-major, M = 128, N = tile_n.
-__device__ __forceinline__ uint32_t make_idesc_bf16(uint32_t n) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((kTileM >> 4) << 24);
+// Instruction descriptor for kind::f16: D fp32, A/B bf16, both K-major, M = m (128, or 256 for a
+// cta_group::2 pair), N = tile_n.
+__device__ __forceinline__ uint32_t make_idesc_bf16(uint32_t n, uint32_t m) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((m >> 4) << 24);
 }
 
 // ---------------------------------------------------------------------------------- epilogue math
@@ -111,6 +112,17 @@ __device__ __forceinline__ void fold_columns(const uint32_t (&r)[NC], int vbase,
 }
 
 // ---------------------------------------------------------------------------------- fused kernel
+// kPair = false: one CTA per SM, tcgen05 cta_group::1, a work item is (128 token rows, vocab split).
+// kPair = true : clusters of two CTAs (the two SMs of a TPC), tcgen05 cta_group::2: one M = 256 MMA
+//                spans both CTAs.  A work item is (256 token rows, vocab split); CTA `rank` of the pair
+//                stages its own 128 token rows (A) and its own half of the vocabulary tile (B rows
+//                [rank*BN/2, +BN/2)), so each W byte enters the pair's shared memory once instead of
+//                once per 128-row token tile; the accumulator of CTA `rank` holds rows
+//                [rank*128, +128) x all BN columns, and the epilogue is the same as in single mode.
+//                Only the leader (rank 0) issues MMAs; its full barriers collect the TMA bytes of
+//                both CTAs, its commits are multicast to both CTAs' barriers, and the epilogue warps
+//                of both CTAs release the accumulator on the leader's tmem-empty barrier.
+template <bool kPair>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                          const __grid_constant__ CUtensorMap tmap_w, const FusedParams p) {
@@ -129,6 +141,11 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
+    const uint32_t rank = kPair ? ptx::cluster_ctarank() : 0u;   // 0 = leader
+    const int unit = kPair ? (blockIdx.x >> 1) : blockIdx.x;     // CTA (single) or CTA pair
+    const int units = kPair ? (gridDim.x >> 1) : gridDim.x;
+    constexpr int kRowsPerItem = kPair ? 2 * kTileM : kTileM;
+    constexpr int kEpiArrivals = kPair ? 8 : 4;                  // one per epilogue warp (of both CTAs)
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap_hidden);
@@ -139,16 +156,17 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         }
         for (int b = 0; b < 2; ++b) {
             ptx::mbar_init(tfull_bar(b), 1);
-            ptx::mbar_init(tempty_bar(b), kEpilogueThreads);
+            ptx::mbar_init(tempty_bar(b), kEpiArrivals);
         }
         ptx::fence_mbar_init();
     }
     if (warp == 1) {
-        ptx::tmem_alloc(tmem_slot, kTmemCols);
-        ptx::tmem_relinquish();
+        ptx::tmem_alloc_t<kPair>(tmem_slot, kTmemCols);
+        ptx::tmem_relinquish_t<kPair>();
     }
     ptx::tc_fence_before();
-    __syncthreads();
+    if constexpr (kPair) ptx::cluster_sync();   // the peer's barriers exist before anything remote
+    else __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
@@ -159,71 +177,97 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     ptx::pdl_launch_dependents();
 
     const int T = p.tiles_per_split, BN = p.tile_n;
+    const int b_rows = kPair ? (BN >> 1) : BN;   // W rows this CTA stages per tile
 
     if (warp == 0) {
         // ===================================================================== TMA producer
-        if (lane == 0) {
+        // Converged warp, one elected lane issues (see the MMA issuer).
+        {
+            const int k_blocks = p.k_blocks, stages = p.stages;
+            const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);  // leader's barriers
             int stage = 0;
             uint32_t phase = 0;
-            for (int w = blockIdx.x; w < p.work_items; w += gridDim.x) {
+            for (int w = unit; w < p.work_items; w += units) {
                 const int mt = w % p.m_tiles, sp = w / p.m_tiles;
                 const int v0 = sp * T * BN;
                 const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
+                const int a_row = mt * kRowsPerItem + static_cast<int>(rank) * kTileM;
                 for (int t = 0; t < ntiles; ++t) {
-                    for (int kb = 0; kb < p.k_blocks; ++kb) {
+                    const int b_row = v0 + t * BN + static_cast<int>(rank) * b_rows;
+                    for (int kb = 0; kb < k_blocks; ++kb) {
                         ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
-                        const uint32_t sa = smem + static_cast<uint32_t>(stage) * p.stage_bytes;
-                        ptx::mbar_arrive_expect_tx(full_bar(stage), p.tx_bytes);
-                        ptx::tma_load_2d(sa, &tmap_hidden, full_bar(stage), kb * kBlockK,
-                                         mt * kTileM, ptx::kEvictLast);
-                        ptx::tma_load_2d(sa + kABytes, &tmap_w, full_bar(stage), kb * kBlockK,
-                                         v0 + t * BN, p.w_policy);
-                        if (++stage == p.stages) { stage = 0; phase ^= 1u; }
+                        if (ptx::elect_one()) {
+                            const uint32_t sa = smem + static_cast<uint32_t>(stage) * p.stage_bytes;
+                            const uint32_t fb = full0 + 8u * stage;
+                            if constexpr (kPair) {
+                                // both CTAs' bytes complete on the leader's barrier
+                                if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2u * p.tx_bytes);
+                                ptx::tma_load_2d_pair(sa, &tmap_hidden, fb, kb * kBlockK, a_row, ptx::kEvictLast);
+                                ptx::tma_load_2d_pair(sa + kABytes, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
+                            } else {
+                                ptx::mbar_arrive_expect_tx(fb, p.tx_bytes);
+                                ptx::tma_load_2d(sa, &tmap_hidden, fb, kb * kBlockK, a_row, ptx::kEvictLast);
+                                ptx::tma_load_2d(sa + kABytes, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
+                            }
+                        }
+                        __syncwarp();
+                        if (++stage == stages) { stage = 0; phase ^= 1u; }
                     }
                 }
             }
         }
     } else if (warp == 1) {
         // ===================================================================== MMA issuer
-        if (lane == 0) {
-            const uint32_t idesc = make_idesc_bf16(static_cast<uint32_t>(BN));
+        // The whole warp walks the loop converged (every lane polls the barriers); one elected lane
+        // issues.  Descriptors advance by additions only: +2 per UMMA_K step inside the 128-byte
+        // swizzle row, +stage_bytes/16 per pipeline stage.
+        if (rank == 0) {
+            const uint32_t idesc = make_idesc_bf16(static_cast<uint32_t>(BN), kRowsPerItem);
+            const uint64_t a_desc0 = make_smem_desc_sw128(smem);
+            const uint64_t b_desc0 = make_smem_desc_sw128(smem + kABytes);
+            const uint32_t stage_step = p.stage_bytes >> 4;
+            const int k_blocks = p.k_blocks, stages = p.stages;
             int stage = 0;
-            uint32_t phase = 0, acc = 0;
-            for (int w = blockIdx.x; w < p.work_items; w += gridDim.x) {
+            uint32_t phase = 0, acc = 0, desc_off = 0;
+            for (int w = unit; w < p.work_items; w += units) {
                 const int sp = w / p.m_tiles;
                 const int v0 = sp * T * BN;
                 const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
                 for (int t = 0; t < ntiles; ++t, ++acc) {
                     const uint32_t buf = acc & 1u, aphase = (acc >> 1) & 1u;
-                    ptx::mbar_wait(tempty_bar(buf), aphase ^ 1u);  // epilogue drained this buffer
+                    // epilogue (of both CTAs in pair mode) drained this buffer
+                    if constexpr (kPair) ptx::mbar_wait_cluster(tempty_bar(buf), aphase ^ 1u);
+                    else ptx::mbar_wait(tempty_bar(buf), aphase ^ 1u);
                     ptx::tc_fence_after();
                     const uint32_t d_tmem = tmem_base + buf * kMaxTileN;
-                    for (int kb = 0; kb < p.k_blocks; ++kb) {
+                    for (int kb = 0; kb < k_blocks; ++kb) {
                         ptx::mbar_wait(full_bar(stage), phase);  // TMA bytes have landed
                         ptx::tc_fence_after();
-                        const uint32_t sa = smem + static_cast<uint32_t>(stage) * p.stage_bytes;
-                        const uint64_t a_desc = make_smem_desc_sw128(sa);
-                        const uint64_t b_desc = make_smem_desc_sw128(sa + kABytes);
-#pragma unroll
-                        for (int k = 0; k < kBlockK / kUmmaK; ++k) {
-                            // +32 bytes along K inside the swizzle row = +2 in the address field
-                            ptx::umma_bf16(d_tmem, a_desc + 2u * k, b_desc + 2u * k, idesc,
-                                           (kb | k) != 0);
+                        if (ptx::elect_one()) {
+                            const uint64_t a_desc = a_desc0 + desc_off;
+                            const uint64_t b_desc = b_desc0 + desc_off;
+                            ptx::umma_bf16_t<kPair>(d_tmem, a_desc, b_desc, idesc, kb != 0);
+                            ptx::umma_bf16_t<kPair>(d_tmem, a_desc + 2u, b_desc + 2u, idesc, 1u);
+                            ptx::umma_bf16_t<kPair>(d_tmem, a_desc + 4u, b_desc + 4u, idesc, 1u);
+                            ptx::umma_bf16_t<kPair>(d_tmem, a_desc + 6u, b_desc + 6u, idesc, 1u);
+                            ptx::umma_commit_t<kPair>(empty_bar(stage));  // frees the stage when the MMAs retire
+                            if (kb == k_blocks - 1)
+                                ptx::umma_commit_t<kPair>(tfull_bar(buf));  // accumulator complete -> epilogue
                         }
-                        ptx::umma_commit(empty_bar(stage));  // frees the stage when the MMAs retire
-                        if (++stage == p.stages) { stage = 0; phase ^= 1u; }
+                        __syncwarp();
+                        desc_off += stage_step;
+                        if (++stage == stages) { stage = 0; phase ^= 1u; desc_off = 0; }
                     }
-                    ptx::umma_commit(tfull_bar(buf));  // accumulator complete -> epilogue
                 }
             }
         }
     } else {
         // ===================================================================== epilogue (4 warps)
         const int q = warp & 3;  // a warp may only touch TMEM lanes [32*(warp%4), +32)
-        const int row = q * 32 + lane;
+        const int row = static_cast<int>(rank) * kTileM + q * 32 + lane;
         const uint32_t lane_addr = static_cast<uint32_t>(q * 32) << 16;
         uint32_t acc = 0;
-        for (int w = blockIdx.x; w < p.work_items; w += gridDim.x) {
+        for (int w = unit; w < p.work_items; w += units) {
             const int mt = w % p.m_tiles, sp = w / p.m_tiles;
             const int v0 = sp * T * BN;
             const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
@@ -249,10 +293,15 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                     ptx::tmem_wait_ld();
                     fold_columns<16>(r, vt + c, p.V, m, a, s);
                 }
+                // all of this warp's TMEM reads have completed (wait::ld): one arrival per warp
                 ptx::tc_fence_before();
-                ptx::mbar_arrive(tempty_bar(buf));
+                __syncwarp();
+                if (lane == 0) {
+                    if constexpr (kPair) ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(buf), 0u));
+                    else ptx::mbar_arrive(tempty_bar(buf));
+                }
             }
-            const size_t o = static_cast<size_t>(sp) * p.n_pad + static_cast<size_t>(mt) * kTileM + row;
+            const size_t o = static_cast<size_t>(sp) * p.n_pad + static_cast<size_t>(mt) * kRowsPerItem + row;
             p.ws_m[o] = m;
             p.ws_a[o] = a;
             p.ws_s[o] = s;
@@ -260,11 +309,13 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     }
 
     // ------------------------------------------------------------------------- teardown
+    __syncwarp();   // reconverge the warps whose lane 0 ran a role loop
     ptx::tc_fence_before();
-    __syncthreads();
+    if constexpr (kPair) ptx::cluster_sync();   // the peer may still read this CTA's shared memory / TMEM
+    else __syncthreads();
     if (warp == 1) {
         ptx::tc_fence_after();
-        ptx::tmem_dealloc(tmem_base, kTmemCols);
+        ptx::tmem_dealloc_t<kPair>(tmem_base, kTmemCols);
     }
 }
 

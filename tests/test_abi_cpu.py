@@ -47,21 +47,43 @@ def test_library_is_sm100a_with_tcgen05_and_tma():
 @pytest.mark.parametrize("dims", [(128, 1536, 151936, 16), (256, 3584, 152064, 32), (1024, 4096, 128256, 64),
                                   (32, 64, 1000, 8), (8, 1536, 151936, 1), (64, 1536, 151936, 8),
                                   (512, 1536, 151936, 64), (4096, 1536, 151936, 512),
-                                  (16384, 1536, 151936, 2048), (1, 8, 1, 1), (300, 72, 70001, 20)])
+                                  (16384, 1536, 151936, 2048), (1, 8, 1, 1), (300, 72, 70001, 20),
+                                  (640, 4096, 128256, 64), (1300, 1536, 151936, 100)])
 def test_plan_invariants(dims):
     N, d, V, R = dims
     p = B.plan_query(*dims)
     bn, T, S = p["tile_n"], p["tiles_per_split"], p["splits"]
-    assert bn % 16 == 0 and 16 <= bn <= 256
+    pair, tm = p["cta_pair"], p["tile_m"]
+    t128 = -(-N // 128)
+    assert pair == (1 if t128 >= 2 and (t128 % 2 == 0 or t128 >= 10) else 0) and tm == (256 if pair else 128)
+    assert bn % (32 if pair else 16) == 0 and 16 <= bn <= 256
     assert S * T * bn >= V and (S - 1) * T * bn < V          # splits tile the vocabulary exactly once
-    assert p["m_tiles"] == max(1, -(-N // 128)) and p["k_blocks"] == -(-d // 64)
-    assert p["work_items"] == p["m_tiles"] * S and 1 <= p["grid"] <= min(p["num_sms"], p["work_items"])
+    assert p["m_tiles"] == max(1, -(-N // tm)) and p["k_blocks"] == -(-d // 64)
+    units = p["num_sms"] // 2 if pair else p["num_sms"]
+    assert p["work_items"] == p["m_tiles"] * S
+    assert p["grid"] == (2 if pair else 1) * min(units, p["work_items"])
     assert 2 <= p["stages"] <= 8
-    assert p["stages"] * (16384 + bn * 128) + 1280 == p["smem_bytes"] <= 227 * 1024
-    assert B.workspace_bytes(*dims) == max(16, 12 * S * p["m_tiles"] * 128)
-    # the busiest CTA does at most ~8 % more than an even share of W rows (+ one tile of slack)
-    rounds = -(-p["work_items"] // p["grid"])
-    assert rounds * T * bn <= 1.08 * (p["m_tiles"] * V / p["grid"]) + bn
+    b_rows = bn // 2 if pair else bn                          # W rows one CTA stages per tile
+    assert p["stages"] * (16384 + b_rows * 128) + 1280 == p["smem_bytes"] <= 227 * 1024
+    assert B.workspace_bytes(*dims) == max(16, 12 * S * p["m_tiles"] * tm)
+    # the busiest unit does at most ~8 % more than an even share of W rows (+ one tile of slack)
+    busy = min(units, p["work_items"])
+    rounds = -(-p["work_items"] // busy)
+    assert rounds * T * bn <= 1.08 * (p["m_tiles"] * V / busy) + bn
+
+
+def test_forced_modes_plan():
+    try:
+        B.set_mode(B.MODE_PAIR)
+        p = B.plan_query(32, 64, 1000, 8)
+        assert p["cta_pair"] == 1 and p["tile_m"] == 256 and p["grid"] % 2 == 0 and p["tile_n"] % 32 == 0
+        B.set_mode(B.MODE_SINGLE)
+        p = B.plan_query(4096, 1536, 151936, 512)
+        assert p["cta_pair"] == 0 and p["tile_m"] == 128 and p["m_tiles"] == 32
+        with pytest.raises(B.LaserError):
+            B.set_mode(5)
+    finally:
+        B.set_mode(B.MODE_AUTO)
 
 
 def test_c2_plan_is_the_documented_one():

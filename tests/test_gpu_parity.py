@@ -117,6 +117,71 @@ def test_scaled_shapes(P, V, d, R, L, n_alloc, var_len):
     _log(w.name, st)
 
 
+# ------------------------------------------------------------------ both kernel variants on every shape class
+@pytest.fixture
+def force_mode():
+    """Force the single-CTA or the CTA-pair kernel (laser_probe_set_mode); restored afterwards."""
+    from paper_2606_31580_b200 import binding as B
+
+    def _set(mode):
+        B.set_mode(mode)
+    yield _set
+    B.set_mode(B.MODE_AUTO)
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
+    (5000, 256, 12, 8, None, None),        # N = 96: the pair's second CTA holds only padding rows
+    (33000, 512, 40, None, 400, (1, 16)),  # N = 400: two 256-row items, second one ragged
+    (70001, 128, 20, None, 300, (0, 24)),  # empty requests, odd V
+    (1000, 64, 3, 130, None, None),        # a request that straddles the two CTAs of a pair
+    (17, 8, 2, 3, None, None),             # V smaller than half a tile
+])
+def test_forced_variants(P, force_mode, mode, V, d, R, L, n_alloc, var_len):
+    force_mode(mode)
+    w = wl.scaled(f"mode{mode}-V{V}-d{d}", V, d, 0.05, R, L, seed=V + d + mode, N_alloc=n_alloc, var_len=var_len)
+    st = P.check(w)
+    assert st["plan"]["cta_pair"] == (1 if mode == 2 else 0)
+    _log(w.name, st)
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_forced_variants_c5_512(P, force_mode, c2_W_bits, mode):
+    force_mode(mode)
+    w = wl.config_c5(512, c2_W_bits)
+    g = P.run_gpu(w)
+    assert g.plan["cta_pair"] == (1 if mode == 2 else 0)
+    ora, rows, reqs = P.run_oracle(w, _pick_requests(w, 6, 512))
+    st = P.compare(w, g, ora, rows, reqs, f"C5:512/mode{mode}")
+    _log(f"C5:512/mode{mode}", st)
+    pl = w.planted >= 0
+    assert np.all(g.argmax[pl] == w.planted[pl])
+
+
+def test_ties_in_pair_mode(P, force_mode):
+    """Duplicate W rows across the two halves of a pair's vocabulary tile, across tiles and splits."""
+    from paper_2606_31580_b200 import binding as B
+    force_mode(2)
+    V, d, N = 20000, 128, 200
+    plan = B.plan_query(N, d, V, 2)
+    assert plan["cta_pair"] == 1
+    bn, T = plan["tile_n"], plan["tiles_per_split"]
+    rng = np.random.default_rng(9)
+    Wf = (rng.standard_normal((V, d)) * 0.05).astype(np.float32)
+    h = rng.standard_normal((N, d)).astype(np.float32)
+    for row in (0, 150):                            # a row of the leader CTA, a row of the peer CTA
+        big = (h[row] * 0.5).astype(np.float32)
+        for v1, v2 in [(bn // 2 - 1, bn // 2), (bn - 1, bn), (T * bn - 1, T * bn), (5, 3 * T * bn + 7)]:
+            W2 = Wf.copy(); W2[v1] = big; W2[v2] = big
+            w = wl.Workload("ties-pair", wl.bf16_bits(W2), wl.bf16_bits(h), wl.fixed_offsets(2, 100),
+                            np.array([0.3, 0.7], np.float32))
+            g = P.run_gpu(w)
+            assert g.argmax[row] == v1, (row, v1, v2, g.argmax[row], plan)
+            ora, rows, reqs = P.run_oracle(w)
+            assert ora.argmax[row] == v1 and ora.gap2[row] == 0.0
+            P.compare(w, g, ora, rows, reqs, "ties-pair")
+
+
 # ------------------------------------------------------------------ closed forms on the GPU
 def test_uniform_logits_gpu(P):
     """P1 on the device: hidden = 0 -> pmax = 1/V, argmax 0 (lowest index), conf = 1/V."""
