@@ -11,9 +11,12 @@ one laser_probe_confidence() call, two kernel launches.  Default workload: BASEL
 
 `value`    rows/s with every input already resident in HBM (device-timed, CUDA events on the launch
            stream, barrier + synchronize either side, max over ranks).
-`e2e`      rows/s through laser_probe_confidence_host(): per-step inputs (hidden, req_offsets, load)
-           in pinned HOST memory, H2D + kernels + D2H of conf/argmax/exit + sync inside the timed
-           region.  W, the model's LM-head weight, stays resident (it is not a per-step input).
+`e2e`      rows/s through laser_probe_confidence_host_async(): per-step inputs (hidden, req_offsets,
+           load) in pinned HOST memory, H2D + kernels + D2H of conf/argmax/exit inside the timed
+           region, every step's result read on the host; two batches in flight on two streams so the
+           copy of one overlaps the kernels of the other.  e2e.sync_value is the same through the
+           synchronous laser_probe_confidence_host() (one batch at a time).  W, the model's LM-head
+           weight, stays resident (it is not a per-step input).
 `roofline` for the dominant (fused) kernel: algorithmic bytes per launch / its own average duration
            (events recorded by the library either side of that kernel, second pass of K steps).
 `cpu_baseline` the fp64 oracle, as it stands, on this box's host cores (rank 0, N=1 only).
@@ -247,11 +250,11 @@ def run_ours(args):
             dist.barrier()
 
     peaks = measured_peaks()
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    sampler.start()                      # NVML initialises while the workload is generated
     W_cache: dict = {}
     w = make_workload(args.workload, rank, W_cache)
     case = GpuCase(w, device, two_w_copies=(w.V * w.d * 2 < 2_000_000_000))
-    sampler = ClockSampler(physical_gpu_index(local_rank))
-    sampler.start()
 
     for _ in range(args.warmup):
         case.step()
@@ -268,24 +271,61 @@ def run_ours(args):
     # dominant kernel on its own (second pass, same stream, library-recorded events)
     fused_us, fin_us = case.kernel_times(args.steps)
 
-    # end to end through the host-buffer entry point
-    hp = B.HostProbe(w.N_alloc, w.d, w.V, w.R, device=device)
+    # end to end through the host-buffer entry points: per-step inputs in pinned host memory, results
+    # read on the host every step.  Two batches in flight (laser_probe_confidence_host_async on two
+    # streams, one staging/workspace/output set each) so that the H2D copy of batch i+1 overlaps the
+    # kernels of batch i, as a serving loop would run it; the one-batch-at-a-time synchronous call
+    # (laser_probe_confidence_host) is timed as well and reported as e2e.sync_*.
+    depth = 2
+    slots = [B.HostProbe(w.N_alloc, w.d, w.V, w.R, device=device) for _ in range(depth)]
+    streams = [torch.cuda.Stream(device=device) for _ in range(depth)]
+    hp = slots[0]
     hh = B.bf16_tensor_from_bits(w.hidden_bits, pin=True)
     hoff = torch.from_numpy(w.req_offsets).pin_memory()
     hload = torch.from_numpy(w.load).pin_memory()
-    for _ in range(args.warmup):
-        hp(hh, case.Ws[0], hoff, hload, case.tp)
+
+    def e2e_pipelined(n):
+        """n steps, `depth` in flight; returns (ms, exits seen on the host)."""
+        pending = [False] * depth
+        seen = 0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for st in streams:
+            st.wait_event(e0)
+        tw0 = time.perf_counter()
+        for i in range(n):
+            k = i % depth
+            if pending[k]:
+                streams[k].synchronize()
+                seen += int(slots[k].exit.sum())          # the step's result, read on the host
+            slots[k].submit(hh, case.Ws[i % len(case.Ws)], hoff, hload, case.tp, streams[k])
+            pending[k] = True
+        for k in range(depth):
+            if pending[k]:
+                streams[k].synchronize()
+                seen += int(slots[k].exit.sum())
+        tw1 = time.perf_counter()
+        for st in streams:
+            torch.cuda.current_stream().wait_stream(st)
+        e1.record()
+        torch.cuda.synchronize()
+        return max(e0.elapsed_time(e1), (tw1 - tw0) * 1e3), seen
+
+    def e2e_sync(n):
+        torch.cuda.synchronize()
+        tw0 = time.perf_counter()
+        for i in range(n):
+            out = hp(hh, case.Ws[i % len(case.Ws)], hoff, hload, case.tp)
+            _ = int(out.exit.sum())
+        return (time.perf_counter() - tw0) * 1e3
+
+    e2e_pipelined(args.warmup)
+    e2e_sync(args.warmup)
     barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record()
-    te0 = time.perf_counter()
-    for i in range(args.steps):
-        hp(hh, case.Ws[i % len(case.Ws)], hoff, hload, case.tp)
-    te1 = time.perf_counter()
-    e1.record()
-    torch.cuda.synchronize()
-    e2e_ms = max(e0.elapsed_time(e1), (te1 - te0) * 1e3)   # host-synchronous: wall == device span
+    e2e_ms, _seen = e2e_pipelined(args.steps)
+    barrier()
+    e2e_sync_ms = e2e_sync(args.steps)
 
     if dist is not None:
         t = torch.tensor([ms, e2e_ms], device=device, dtype=torch.float64)
@@ -323,8 +363,13 @@ def run_ours(args):
             requests_per_sec=reqs_all / (ms_per_step * 1e-3),
             clocks=clocks,
             e2e=dict(value=rows_all / (e2e_ms / args.steps * 1e-3), unit=UNIT,
-                     h2d_bytes_per_step=hp.h2d_bytes, d2h_bytes_per_step=hp.d2h_bytes,
-                     ms_per_step=e2e_ms / args.steps),
+                     h2d_bytes_per_step=w.N_valid * w.d * 2 + (w.R + 1) * 4 + w.R * 4,
+                     d2h_bytes_per_step=hp.d2h_bytes,
+                     ms_per_step=e2e_ms / args.steps, batches_in_flight=depth,
+                     api="laser_probe_confidence_host_async, 2 streams; results read on the host every step",
+                     sync_value=float(w.N_valid) * world / (e2e_sync_ms / args.steps * 1e-3),
+                     sync_ms_per_step=e2e_sync_ms / args.steps,
+                     sync_api="laser_probe_confidence_host (one batch at a time, rank 0's figure x ranks)"),
             gpu_launches=int(launches),
             roofline=roof,
         )
@@ -422,8 +467,8 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2")
     ap.add_argument("--no-sweep", action="store_true")

@@ -140,7 +140,10 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
  * End-to-end form with HOST buffers for the per-step tensors (W stays resident on the device: it is
  * the model's weight, not a per-step input).  Copies hidden / req_offsets / load to the device
  * staging buffers, runs laser_probe_confidence, copies conf / argmax / exit back, and synchronises
- * `stream` before returning.  Host buffers should be pinned for the copies to be asynchronous.
+ * `stream` before returning.  Host buffers should be pinned for the copies to be asynchronous; when
+ * req_offsets, load and the three outputs are pinned AND device-mapped (cudaHostAlloc,
+ * cudaHostRegister, torch pin_memory) the kernels access them in place over PCIe and only `hidden`
+ * is copied (one transfer per call instead of six).  Pageable buffers take the staged path.
  *
  *   h_*          host pointers (same shapes and dtypes as above)
  *   d_staging    device scratch >= laser_probe_staging_bytes(dims), 256-byte aligned
@@ -153,6 +156,17 @@ int laser_probe_confidence_host(const void* h_hidden, const void* W, const int32
                                 const laser_probe_dims* dims, void* workspace,
                                 size_t workspace_bytes, void* d_staging, size_t staging_bytes,
                                 void* stream);
+/* Same without the final synchronisation: returns after enqueueing the copies and the kernels on
+ * `stream`; results are in the host buffers once `stream` has been synchronised by the caller.  With
+ * two (staging, workspace, output) sets on two streams a serving loop overlaps the host->device copy
+ * of batch i+1 with the kernels of batch i.  Host buffers must stay valid until then. */
+int laser_probe_confidence_host_async(const void* h_hidden, const void* W,
+                                      const int32_t* h_req_offsets, const float* h_load,
+                                      const laser_tau_params* tau_params, float* h_out_conf,
+                                      int32_t* h_out_argmax, uint8_t* h_out_exit,
+                                      const laser_probe_dims* dims, void* workspace,
+                                      size_t workspace_bytes, void* d_staging, size_t staging_bytes,
+                                      void* stream);
 
 /* Host, scalar-array version of a4 (Eq. 5 + clamp) in the same float arithmetic as the kernel. */
 int laser_tau_from_load(const float* load, int32_t R, const laser_tau_params* tau_params,

@@ -20,7 +20,7 @@ MODE_AUTO, MODE_SINGLE, MODE_PAIR = 0, 1, 2
 EXPORTS = [
     "laser_tau_params_default", "laser_probe_workspace_bytes", "laser_probe_plan_query",
     "laser_probe_confidence", "laser_probe_confidence_agg", "laser_probe_staging_bytes",
-    "laser_probe_confidence_host", "laser_tau_from_load", "laser_ema_update",
+    "laser_probe_confidence_host", "laser_probe_confidence_host_async", "laser_tau_from_load", "laser_ema_update",
     "laser_budget_params_default", "laser_allocate_budget", "laser_status_string",
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
     "laser_profile_read", "laser_probe_set_mode",
@@ -88,6 +88,7 @@ def lib():
         L.laser_probe_confidence_agg.argtypes = common + [C.c_int]
         L.laser_probe_confidence_host.argtypes = [vp, vp, i32p, fp, tp, fp, i32p, u8p, dp, vp,
                                                   C.c_size_t, vp, C.c_size_t, vp]
+        L.laser_probe_confidence_host_async.argtypes = L.laser_probe_confidence_host.argtypes
         L.laser_tau_from_load.argtypes = [fp, C.c_int32, tp, fp]
         L.laser_ema_update.argtypes = [fp, fp, C.c_int32, C.c_float]
         L.laser_budget_params_default.argtypes = [C.POINTER(BudgetParams)]
@@ -237,19 +238,29 @@ class HostProbe:
         self.conf = torch.empty(R, dtype=torch.float32).pin_memory()
         self.argmax = torch.empty(N, dtype=torch.int32).pin_memory()
         self.exit = torch.empty(R, dtype=torch.uint8).pin_memory()
-        self.h2d_bytes = N * d * 2 + (R + 1) * 4 + R * 4
+        self.h2d_bytes = N * d * 2 + (R + 1) * 4 + R * 4   # upper bound: only valid rows are copied
         self.d2h_bytes = R * 4 + N * 4 + R
 
-    def __call__(self, h_hidden, W, h_req_offsets, h_load, params: TauParams, stream=None):
+    def _call(self, fn, h_hidden, W, h_req_offsets, h_load, params, stream):
         torch = self.torch
         assert not h_hidden.is_cuda and W.is_cuda
         s = (stream or torch.cuda.current_stream(self.device)).cuda_stream
-        _check(lib().laser_probe_confidence_host(
+        _check(fn(
             h_hidden.data_ptr(), W.data_ptr(), h_req_offsets.data_ptr(), h_load.data_ptr(),
             C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(),
             C.byref(self.dims), self.workspace.data_ptr(), self.workspace.numel(),
             self.staging.data_ptr(), self.staging.numel(), s))
         return ProbeOutputs(self.conf, self.argmax, self.exit, None, None)
+
+    def __call__(self, h_hidden, W, h_req_offsets, h_load, params: TauParams, stream=None):
+        """Synchronous: results are in the returned host tensors on return."""
+        return self._call(lib().laser_probe_confidence_host, h_hidden, W, h_req_offsets, h_load, params, stream)
+
+    def submit(self, h_hidden, W, h_req_offsets, h_load, params: TauParams, stream):
+        """laser_probe_confidence_host_async: enqueue on `stream` and return; the outputs are valid
+        after stream.synchronize().  One HostProbe per in-flight batch."""
+        return self._call(lib().laser_probe_confidence_host_async, h_hidden, W, h_req_offsets, h_load,
+                          params, stream)
 
 
 def bf16_tensor_from_bits(bits, device=None, pin=False):

@@ -422,12 +422,12 @@ size_t laser_probe_staging_bytes(const laser_probe_dims* dims) {
     return staging_layout(*dims).total;
 }
 
-int laser_probe_confidence_host(const void* h_hidden, const void* W, const int32_t* h_req_offsets,
-                                const float* h_load, const laser_tau_params* tau_params,
-                                float* h_out_conf, int32_t* h_out_argmax, uint8_t* h_out_exit,
-                                const laser_probe_dims* dims, void* workspace,
-                                size_t workspace_bytes, void* d_staging, size_t staging_bytes,
-                                void* stream_v) {
+int laser_probe_confidence_host_async(const void* h_hidden, const void* W, const int32_t* h_req_offsets,
+                                      const float* h_load, const laser_tau_params* tau_params,
+                                      float* h_out_conf, int32_t* h_out_argmax, uint8_t* h_out_exit,
+                                      const laser_probe_dims* dims, void* workspace,
+                                      size_t workspace_bytes, void* d_staging, size_t staging_bytes,
+                                      void* stream_v) {
     if (!dims || !tau_params) return LASER_E_NULL;
     if (!dims_valid(dims)) return LASER_E_DIMS;
     const int N = dims->N, R = dims->R;
@@ -440,35 +440,79 @@ int laser_probe_confidence_host(const void* h_hidden, const void* W, const int32
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
     uint8_t* base = static_cast<uint8_t*>(d_staging);
     cudaError_t e;
-    if (N > 0) {
-        e = cudaMemcpyAsync(base + st.hidden, h_hidden, static_cast<size_t>(N) * dims->d * 2,
+    // Rows >= req_offsets[R] are padding and never aggregated: copy the valid rows only (the offsets
+    // are host memory here).  Out-of-range offsets fall back to all N rows.
+    int n_copy = N;
+    if (R > 0 && h_req_offsets[R] >= 0 && h_req_offsets[R] <= N) n_copy = h_req_offsets[R];
+    else if (R == 0) n_copy = 0;
+    if (n_copy > 0) {
+        e = cudaMemcpyAsync(base + st.hidden, h_hidden, static_cast<size_t>(n_copy) * dims->d * 2,
                             cudaMemcpyHostToDevice, stream);
         if (e != cudaSuccess) return set_cuda_error("H2D hidden", e);
     }
-    if (R > 0) {
-        e = cudaMemcpyAsync(base + st.offsets, h_req_offsets, static_cast<size_t>(R + 1) * 4,
-                            cudaMemcpyHostToDevice, stream);
-        if (e != cudaSuccess) return set_cuda_error("H2D req_offsets", e);
-        e = cudaMemcpyAsync(base + st.load, h_load, static_cast<size_t>(R) * 4, cudaMemcpyHostToDevice, stream);
-        if (e != cudaSuccess) return set_cuda_error("H2D load", e);
+    // Zero-copy for the small tensors: when req_offsets, load and the three outputs all live in
+    // pinned, device-mapped host memory (cudaHostAlloc / cudaHostRegister / torch pin_memory), the
+    // finalize kernel reads and writes them over PCIe directly — the reads overlap the fused kernel
+    // (they precede griddepcontrol.wait) — and the call issues one copy (hidden) instead of six.
+    auto mapped = [](const void* h) -> void* {
+        if (!h) return nullptr;
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, h) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+        return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
+    };
+    void* m_off = R > 0 ? mapped(h_req_offsets) : nullptr;
+    void* m_load = R > 0 ? mapped(h_load) : nullptr;
+    void* m_conf = R > 0 ? mapped(h_out_conf) : nullptr;
+    void* m_exit = R > 0 ? mapped(h_out_exit) : nullptr;
+    void* m_arg = N > 0 ? mapped(h_out_argmax) : nullptr;
+    const bool zero_copy = (R == 0 || (m_off && m_load && m_conf && m_exit)) && (N == 0 || m_arg);
+    if (zero_copy) {
+        int rc = laser_probe_confidence(base + st.hidden, W, static_cast<int32_t*>(m_off),
+                                        static_cast<float*>(m_load), tau_params,
+                                        static_cast<float*>(m_conf), static_cast<int32_t*>(m_arg),
+                                        static_cast<uint8_t*>(m_exit), dims, workspace, workspace_bytes,
+                                        stream_v, nullptr, nullptr);
+        if (rc != LASER_OK) return rc;
+    } else {
+        if (R > 0) {
+            e = cudaMemcpyAsync(base + st.offsets, h_req_offsets, static_cast<size_t>(R + 1) * 4,
+                                cudaMemcpyHostToDevice, stream);
+            if (e != cudaSuccess) return set_cuda_error("H2D req_offsets", e);
+            e = cudaMemcpyAsync(base + st.load, h_load, static_cast<size_t>(R) * 4, cudaMemcpyHostToDevice, stream);
+            if (e != cudaSuccess) return set_cuda_error("H2D load", e);
+        }
+        int rc = laser_probe_confidence(base + st.hidden, W, reinterpret_cast<int32_t*>(base + st.offsets),
+                                        reinterpret_cast<float*>(base + st.load), tau_params,
+                                        reinterpret_cast<float*>(base + st.conf),
+                                        reinterpret_cast<int32_t*>(base + st.argmax), base + st.exit_, dims,
+                                        workspace, workspace_bytes, stream_v, nullptr, nullptr);
+        if (rc != LASER_OK) return rc;
+        if (R > 0) {
+            e = cudaMemcpyAsync(h_out_conf, base + st.conf, static_cast<size_t>(R) * 4, cudaMemcpyDeviceToHost, stream);
+            if (e != cudaSuccess) return set_cuda_error("D2H conf", e);
+            e = cudaMemcpyAsync(h_out_exit, base + st.exit_, static_cast<size_t>(R), cudaMemcpyDeviceToHost, stream);
+            if (e != cudaSuccess) return set_cuda_error("D2H exit", e);
+        }
+        if (N > 0) {
+            e = cudaMemcpyAsync(h_out_argmax, base + st.argmax, static_cast<size_t>(N) * 4, cudaMemcpyDeviceToHost, stream);
+            if (e != cudaSuccess) return set_cuda_error("D2H argmax", e);
+        }
     }
-    int rc = laser_probe_confidence(base + st.hidden, W, reinterpret_cast<int32_t*>(base + st.offsets),
-                                    reinterpret_cast<float*>(base + st.load), tau_params,
-                                    reinterpret_cast<float*>(base + st.conf),
-                                    reinterpret_cast<int32_t*>(base + st.argmax), base + st.exit_, dims,
-                                    workspace, workspace_bytes, stream_v, nullptr, nullptr);
+    return LASER_OK;
+}
+
+int laser_probe_confidence_host(const void* h_hidden, const void* W, const int32_t* h_req_offsets,
+                                const float* h_load, const laser_tau_params* tau_params,
+                                float* h_out_conf, int32_t* h_out_argmax, uint8_t* h_out_exit,
+                                const laser_probe_dims* dims, void* workspace,
+                                size_t workspace_bytes, void* d_staging, size_t staging_bytes,
+                                void* stream_v) {
+    int rc = laser_probe_confidence_host_async(h_hidden, W, h_req_offsets, h_load, tau_params, h_out_conf,
+                                               h_out_argmax, h_out_exit, dims, workspace, workspace_bytes,
+                                               d_staging, staging_bytes, stream_v);
     if (rc != LASER_OK) return rc;
-    if (R > 0) {
-        e = cudaMemcpyAsync(h_out_conf, base + st.conf, static_cast<size_t>(R) * 4, cudaMemcpyDeviceToHost, stream);
-        if (e != cudaSuccess) return set_cuda_error("D2H conf", e);
-        e = cudaMemcpyAsync(h_out_exit, base + st.exit_, static_cast<size_t>(R), cudaMemcpyDeviceToHost, stream);
-        if (e != cudaSuccess) return set_cuda_error("D2H exit", e);
-    }
-    if (N > 0) {
-        e = cudaMemcpyAsync(h_out_argmax, base + st.argmax, static_cast<size_t>(N) * 4, cudaMemcpyDeviceToHost, stream);
-        if (e != cudaSuccess) return set_cuda_error("D2H argmax", e);
-    }
-    e = cudaStreamSynchronize(stream);
+    if (dims->N == 0 && dims->R == 0) return LASER_OK;
+    cudaError_t e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream_v));
     if (e != cudaSuccess) return set_cuda_error("cudaStreamSynchronize", e);
     return LASER_OK;
 }

@@ -319,6 +319,29 @@ def test_deterministic_and_host_entry(P, c2_W_bits):
              torch.from_numpy(w.load).pin_memory(), B.TauParams(**w.tau_params))
     assert np.array_equal(out.conf.numpy(), a.conf) and np.array_equal(out.argmax.numpy(), a.argmax)
     assert np.array_equal(out.exit.numpy(), a.exit)
+    # asynchronous form: two batches in flight on two streams, results valid after the stream sync
+    hps = [B.HostProbe(w.N_alloc, w.d, w.V, w.R) for _ in range(2)]
+    sts = [torch.cuda.Stream() for _ in range(2)]
+    w2 = wl.config_c5(64, c2_W_bits)
+    w2.load = (1.0 - w.load).astype(np.float32)                 # second batch: other thresholds
+    a2 = P.run_gpu(w2, dev=dict(dev, load=torch.from_numpy(w2.load).cuda()))
+    ins = [(hh, torch.from_numpy(w.req_offsets).pin_memory(), torch.from_numpy(w.load).pin_memory()),
+           (hh, torch.from_numpy(w2.req_offsets).pin_memory(), torch.from_numpy(w2.load).pin_memory())]
+    for rep in range(3):
+        for k in range(2):
+            hps[k].submit(ins[k][0], dev["W"], ins[k][1], ins[k][2], B.TauParams(**w.tau_params), sts[k])
+        for k, want in enumerate((a, a2)):
+            sts[k].synchronize()
+            assert np.array_equal(hps[k].conf.numpy(), want.conf) and np.array_equal(hps[k].exit.numpy(), want.exit)
+            assert np.array_equal(hps[k].argmax.numpy(), want.argmax)
+    # pageable host buffers take the staged-copy path; same results
+    hp2 = B.HostProbe(w.N_alloc, w.d, w.V, w.R)
+    hp2.conf, hp2.argmax, hp2.exit = (torch.full((w.R,), -7.0), torch.full((w.N_alloc,), -7, dtype=torch.int32),
+                                      torch.full((w.R,), 7, dtype=torch.uint8))
+    out2 = hp2(B.bf16_tensor_from_bits(w.hidden_bits), dev["W"], torch.from_numpy(w.req_offsets.copy()),
+               torch.from_numpy(w.load.copy()), B.TauParams(**w.tau_params))
+    assert np.array_equal(out2.conf.numpy(), a.conf) and np.array_equal(out2.argmax.numpy(), a.argmax)
+    assert np.array_equal(out2.exit.numpy(), a.exit)
 
 
 def test_error_codes_on_device(P):
