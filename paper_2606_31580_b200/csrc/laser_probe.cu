@@ -321,7 +321,12 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
             di->attr_set = true;
         }
         CUtensorMap tm_h, tm_w;
-        int rc = get_tensor_map(hidden, N, dims->d, kTileM, &tm_h);
+        // Fewer than 128 rows in total: stage only the 8-row groups that hold rows.  TMA's zero fill of
+        // out-of-range rows is slow (N = 8: 90 -> 75 us per step at the C2 shape without it).  The
+        // other rows of the A tile keep whatever shared memory held; they feed TMEM lanes whose
+        // statistics nobody reads (rows are independent).
+        const int a_rows = N < kTileM ? round_up(N, 8) : kTileM;
+        int rc = get_tensor_map(hidden, N, dims->d, a_rows, &tm_h);
         if (rc != LASER_OK) return rc;
         const int b_rows = pair ? pl.tile_n / 2 : pl.tile_n;   // W rows one CTA stages per tile
         rc = get_tensor_map(W, dims->V, dims->d, b_rows, &tm_w);
@@ -333,7 +338,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
         fp.work_items = pl.work_items; fp.n_pad = n_pad;
         fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
-        fp.tx_bytes = fp.stage_bytes;  // OOB rows are zero-filled and still counted
+        fp.tx_bytes = static_cast<uint32_t>((a_rows + b_rows) * 128);  // OOB rows are zero-filled and still counted
         // W is streamed once when a single token tile exists; with several token tiles the other
         // CTAs re-read the same rows from L2, so do not mark them evict-first.
         fp.w_policy = (pl.m_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
