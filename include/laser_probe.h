@@ -91,7 +91,7 @@ enum { LASER_AGG_MEAN = 0, LASER_AGG_GEOMEAN = 1, LASER_AGG_MIN = 2 };
 /* Writes the paper's defaults.  Host. */
 int laser_tau_params_default(laser_tau_params* out);
 
-/* Device scratch laser_probe_confidence needs for `dims`, in bytes (12 * splits * m_tiles * tile_m,
+/* Device scratch laser_probe_confidence needs for `dims`, in bytes (16 * splits * m_tiles * tile_m,
  * at least 16).  Returns 0 for invalid dims.  Host; needs no GPU. */
 size_t laser_probe_workspace_bytes(const laser_probe_dims* dims);
 

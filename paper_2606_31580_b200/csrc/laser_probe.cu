@@ -150,7 +150,7 @@ void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
 }
 
 size_t workspace_bytes_for(const laser_probe_plan& pl) {
-    size_t b = static_cast<size_t>(12) * pl.splits * pl.m_tiles * pl.tile_m;
+    size_t b = static_cast<size_t>(16) * pl.splits * pl.m_tiles * pl.tile_m;
     return b < 16 ? 16 : b;
 }
 
@@ -302,9 +302,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
     const int n_pad = pl.m_tiles * pl.tile_m;
     const bool pair = pl.cta_pair != 0;
-    float* ws_m = static_cast<float*>(workspace);
-    int32_t* ws_a = reinterpret_cast<int32_t*>(ws_m + static_cast<size_t>(pl.splits) * n_pad);
-    float* ws_s = reinterpret_cast<float*>(ws_a + static_cast<size_t>(pl.splits) * n_pad);
+    float4* ws = static_cast<float4*>(workspace);
 
     const bool run_fused = (N > 0 && R > 0);
     static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
@@ -342,7 +340,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         // W is streamed once when a single token tile exists; with several token tiles the other
         // CTAs re-read the same rows from L2, so do not mark them evict-first.
         fp.w_policy = (pl.m_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
-        fp.ws_m = ws_m; fp.ws_a = ws_a; fp.ws_s = ws_s;
+        fp.ws = ws;
 
         if (prof) cudaEventRecord(g_prof.ev[prof_slot][0], stream);
         cudaLaunchConfig_t cfg{};
@@ -378,7 +376,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
     FinalizeParams fz;
     fz.n_alloc = N; fz.R = run_fused ? R : 0; fz.splits = pl.splits; fz.n_pad = n_pad;
     fz.agg_mode = aggregate_mode;
-    fz.ws_m = ws_m; fz.ws_a = ws_a; fz.ws_s = ws_s;
+    fz.ws = ws;
     fz.req_offsets = req_offsets; fz.load = load;
     fz.out_conf = out_conf; fz.out_argmax = out_argmax; fz.out_exit = out_exit;
     fz.out_tau = out_tau_opt; fz.out_pmax = out_pmax_opt;

@@ -43,9 +43,7 @@ struct FusedParams {
     uint32_t tx_bytes;     // bytes TMA delivers per stage and CTA (hidden box + W box)
     uint32_t stage_bytes;  // shared-memory stride of a stage: kABytes + (W rows per CTA) * 128
     uint64_t w_policy;     // L2 eviction policy for the W stream
-    float* ws_m;           // [splits, n_pad] running max per (split, row)
-    int32_t* ws_a;         // [splits, n_pad] argmax
-    float* ws_s;           // [splits, n_pad] sum of exp(logit - max)
+    float4* ws;            // [n_pad, splits] per (row, split): {max, sum exp(logit - max), argmax bits, 0}
 };
 
 // ---------------------------------------------------------------------------------- descriptors
@@ -301,10 +299,10 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                     else ptx::mbar_arrive(tempty_bar(buf));
                 }
             }
-            const size_t o = static_cast<size_t>(sp) * p.n_pad + static_cast<size_t>(mt) * kRowsPerItem + row;
-            p.ws_m[o] = m;
-            p.ws_a[o] = a;
-            p.ws_s[o] = s;
+            // row-major over splits: the finalize kernel reads a row's partials as contiguous 16-byte
+            // records (coalesced); the scattered 16-byte stores here are fire-and-forget
+            const size_t o = (static_cast<size_t>(mt) * kRowsPerItem + row) * p.splits + sp;
+            p.ws[o] = make_float4(m, s, __int_as_float(a), 0.f);
         }
     }
 
@@ -334,9 +332,7 @@ __host__ __device__ __forceinline__ float tau_eval(float load, const TauParamsDe
 
 struct FinalizeParams {
     int32_t n_alloc, R, splits, n_pad, agg_mode;
-    const float* ws_m;
-    const int32_t* ws_a;
-    const float* ws_s;
+    const float4* ws;
     const int32_t* req_offsets;
     const float* load;
     float* out_conf;
@@ -360,7 +356,7 @@ __device__ __forceinline__ void merge_stats(float& m, int& a, float& s, float m2
 
 constexpr int kFinalizeThreads = 256;
 constexpr int kFinalizeWarps = kFinalizeThreads / 32;
-constexpr int kMergeBatch = 4;  // partials a lane loads before it starts merging
+constexpr int kMergeBatch = 5;  // partials a lane loads before it starts merging (148 splits: one batch)
 
 // Blocks [0, R): one request each.  A warp takes rows b+w, b+w+8, ...: its lanes stride over the
 // vocabulary splits of the row (loads issued in batches so that they overlap), fold their own
@@ -368,9 +364,13 @@ constexpr int kMergeBatch = 4;  // partials a lane loads before it starts mergin
 // Blocks [R, R + ceil(n_alloc/256)): mark padding rows (n >= req_offsets[R]).
 // Everything that does not depend on the fused kernel (offsets, load, threshold) is read before
 // griddepcontrol.wait so that under programmatic dependent launch it overlaps the fused kernel.
+// launch_dependents is issued first of all: the next call's fused kernel may then take every SM the
+// current fused kernel vacates and run its prologue there; it still blocks in its own
+// griddepcontrol.wait until this grid (hence, transitively, the current fused kernel) has completed.
 __global__ void __launch_bounds__(kFinalizeThreads)
 laser_probe_finalize_kernel(const FinalizeParams p) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    ptx::pdl_launch_dependents();
     if (static_cast<int>(blockIdx.x) >= p.R) {
         const int n = (blockIdx.x - p.R) * kFinalizeThreads + threadIdx.x;
         const int n_valid = (p.R > 0) ? __ldg(p.req_offsets + p.R) : 0;
@@ -387,7 +387,6 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
     if (threadIdx.x == 0) tau = tau_eval(__ldg(p.load + r), p.tau);   // a4
 
     ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
-    ptx::pdl_launch_dependents();  // the next kernel's prologue may overlap the rest of this one
 
     // running aggregate of this warp's rows: sum (mean), sum of logs (geomean), min
     float acc = (p.agg_mode == 2) ? CUDART_INF_F : 0.f;
@@ -395,20 +394,16 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
     for (int n = b + warp; n < e; n += kFinalizeWarps) {
         float m = -CUDART_INF_F, s = 0.f;
         int a = 0x7fffffff;
+        const float4* rec = p.ws + static_cast<size_t>(n) * p.splits;
         for (int sp0 = lane; sp0 < p.splits; sp0 += 32 * kMergeBatch) {
-            float pm[kMergeBatch], ps[kMergeBatch];
-            int pa[kMergeBatch];
+            float4 v[kMergeBatch];
 #pragma unroll
             for (int j = 0; j < kMergeBatch; ++j) {
                 const int sp = sp0 + 32 * j;
-                const bool ok = sp < p.splits;
-                const size_t o = static_cast<size_t>(ok ? sp : 0) * p.n_pad + n;
-                pm[j] = ok ? p.ws_m[o] : -CUDART_INF_F;
-                pa[j] = ok ? p.ws_a[o] : 0x7fffffff;
-                ps[j] = ok ? p.ws_s[o] : 0.f;
+                v[j] = sp < p.splits ? rec[sp] : make_float4(-CUDART_INF_F, 0.f, __int_as_float(0x7fffffff), 0.f);
             }
 #pragma unroll
-            for (int j = 0; j < kMergeBatch; ++j) merge_stats(m, a, s, pm[j], pa[j], ps[j]);
+            for (int j = 0; j < kMergeBatch; ++j) merge_stats(m, a, s, v[j].x, __float_as_int(v[j].z), v[j].y);
         }
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
