@@ -61,7 +61,10 @@ typedef struct {
     int32_t N, d, V, R;
 } laser_probe_dims;
 
-/* How a call is laid out on the GPU (informational; filled by laser_probe_plan_query). */
+/* How a call is laid out on the GPU (informational; filled by laser_probe_plan_query).  splits /
+ * tiles_per_split / work_items describe a batch whose N rows are all valid; when req_offsets[R] < N
+ * leaves whole token tiles of padding, the kernels skip them and re-deal the vocabulary tiles over the
+ * remaining token tiles on the device (same tile_n), so padding rows cost no tensor work. */
 typedef struct {
     int32_t num_sms;         /* SMs the plan was made for                                             */
     int32_t m_tiles;         /* ceil(N / tile_m) token tiles                                          */
@@ -76,6 +79,7 @@ typedef struct {
     int32_t kernel_launches; /* kernels one laser_probe_confidence call enqueues                      */
     int32_t tile_m;          /* token rows per work item: 128 (one CTA) or 256 (CTA pair)             */
     int32_t cta_pair;        /* 1: clusters of two CTAs, tcgen05 cta_group::2; 0: one CTA per item    */
+    int32_t ws_splits;       /* workspace records per row (>= splits: the most any re-plan can use)   */
 } laser_probe_plan;
 
 /* Kernel variant selection.  AUTO (default): one CTA per work item for N <= 128 rows and for small
@@ -91,7 +95,7 @@ enum { LASER_AGG_MEAN = 0, LASER_AGG_GEOMEAN = 1, LASER_AGG_MIN = 2 };
 /* Writes the paper's defaults.  Host. */
 int laser_tau_params_default(laser_tau_params* out);
 
-/* Device scratch laser_probe_confidence needs for `dims`, in bytes (16 * splits * m_tiles * tile_m,
+/* Device scratch laser_probe_confidence needs for `dims`, in bytes (16 * ws_splits * m_tiles * tile_m,
  * at least 16).  Returns 0 for invalid dims.  Host; needs no GPU. */
 size_t laser_probe_workspace_bytes(const laser_probe_dims* dims);
 

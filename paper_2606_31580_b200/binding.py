@@ -54,7 +54,7 @@ class Dims(C.Structure):
 class Plan(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("num_sms", "m_tiles", "splits", "tiles_per_split", "tile_n", "k_blocks", "stages",
-                 "grid", "work_items", "smem_bytes", "kernel_launches", "tile_m", "cta_pair")]
+                 "grid", "work_items", "smem_bytes", "kernel_launches", "tile_m", "cta_pair", "ws_splits")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}

@@ -129,9 +129,20 @@ void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
     const int tile_m = pair ? 2 * kTileM : kTileM;
     const int units = pair ? (num_sms / 2 > 0 ? num_sms / 2 : 1) : num_sms;
     int S, T, BN;
-    plan_variant(dm, units, tile_m, pair ? 32 : 16, &S, &T, &BN);
+    plan_variant(dm, units, tile_m, pair ? 32 : 16, &S, &T, &BN);   // fixes the tile height BN
     pl->num_sms = num_sms;
     pl->m_tiles = dm.N > 0 ? ceil_div(dm.N, tile_m) : 1;
+    // The deal of tiles to units comes from the function the kernels also use: with padding rows in
+    // the batch they re-plan on the device for the token items that hold rows (same BN).
+    const int total_tiles = ceil_div(dm.V, BN);
+    const SplitPlan sp = plan_splits(total_tiles, pl->m_tiles, units);
+    S = sp.splits; T = sp.T;
+    int ws_splits = S;
+    for (int m = 1; m < pl->m_tiles; ++m) {
+        const int sm = plan_splits(total_tiles, m, units).splits;
+        if (sm > ws_splits) ws_splits = sm;
+    }
+    pl->ws_splits = ws_splits;
     pl->splits = S;
     pl->tiles_per_split = T;
     pl->tile_n = BN;
@@ -150,7 +161,7 @@ void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
 }
 
 size_t workspace_bytes_for(const laser_probe_plan& pl) {
-    size_t b = static_cast<size_t>(16) * pl.splits * pl.m_tiles * pl.tile_m;
+    size_t b = static_cast<size_t>(16) * pl.ws_splits * pl.m_tiles * pl.tile_m;
     return b < 16 ? 16 : b;
 }
 
@@ -332,7 +343,11 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
 
         FusedParams fp;
         fp.n_alloc = N; fp.d = dims->d; fp.V = dims->V;
-        fp.m_tiles = pl.m_tiles; fp.splits = pl.splits; fp.tiles_per_split = pl.tiles_per_split;
+        fp.m_tiles = pl.m_tiles; fp.splits = pl.ws_splits; fp.tiles_per_split = pl.tiles_per_split;
+        fp.req_offsets = req_offsets; fp.R = R;
+        fp.total_tiles = ceil_div(dims->V, pl.tile_n);
+        fp.units = pair ? (di->sms / 2 > 0 ? di->sms / 2 : 1) : di->sms;
+        fp.replan = pl.m_tiles > 1 ? 1 : 0;
         fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
         fp.work_items = pl.work_items; fp.n_pad = n_pad;
         fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
@@ -374,7 +389,11 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
     }
 
     FinalizeParams fz;
-    fz.n_alloc = N; fz.R = run_fused ? R : 0; fz.splits = pl.splits; fz.n_pad = n_pad;
+    fz.n_alloc = N; fz.R = run_fused ? R : 0; fz.splits = pl.ws_splits; fz.n_pad = n_pad;
+    fz.m_tiles = pl.m_tiles; fz.rows_per_item = pl.tile_m;
+    fz.total_tiles = ceil_div(dims->V, pl.tile_n);
+    fz.units = pair ? (di->sms / 2 > 0 ? di->sms / 2 : 1) : di->sms;
+    fz.replan = (run_fused && pl.m_tiles > 1) ? 1 : 0;
     fz.agg_mode = aggregate_mode;
     fz.ws = ws;
     fz.req_offsets = req_offsets; fz.load = load;

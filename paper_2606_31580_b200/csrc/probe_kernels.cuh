@@ -36,6 +36,31 @@ constexpr int kFusedThreads = 192;  // warp 0 TMA, warp 1 MMA + TMEM alloc, warp
 constexpr int kEpilogueThreads = 128;
 constexpr float kLog2e = 1.4426950408889634f;
 
+// How the vocabulary tiles are dealt to the execution units (CTAs, or CTA pairs) for `m_items` token
+// items: cut the `total_tiles` tiles of tile_n rows into `splits` contiguous ranges of `T` tiles such
+// that m_items * splits fills the units in whole rounds with the least work on the busiest unit.
+// Shared by the host planner and both kernels: when a batch carries padding rows (req_offsets[R] <
+// N) the kernels re-plan on the device for the token items that actually hold rows.
+struct SplitPlan {
+    int T, splits;
+};
+__host__ __device__ inline SplitPlan plan_splits(int total_tiles, int m_items, int units) {
+    int a = units, b = m_items;
+    while (b) { const int t = a % b; a = b; b = t; }
+    const int s_unit = units / a;   // smallest split count that fills whole rounds
+    SplitPlan best{total_tiles, 1};
+    long best_cost = -1;
+    for (int k = 1; k <= 4; ++k) {
+        const int s_try = s_unit * k;
+        const int T = (total_tiles + s_try - 1) / s_try;
+        const int S = (total_tiles + T - 1) / T;
+        const long rounds = (static_cast<long>(m_items) * S + units - 1) / units;
+        const long cost = rounds * (T * 8 + 1);   // a small charge per round for the item switch
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best.T = T; best.splits = S; }
+    }
+    return best;
+}
+
 struct FusedParams {
     int32_t n_alloc, d, V;
     int32_t m_tiles, splits, tiles_per_split, tile_n, k_blocks, stages;
@@ -44,6 +69,11 @@ struct FusedParams {
     uint32_t stage_bytes;  // shared-memory stride of a stage: kABytes + (W rows per CTA) * 128
     uint64_t w_policy;     // L2 eviction policy for the W stream
     float4* ws;            // [n_pad, splits] per (row, split): {max, sum exp(logit - max), argmax bits, 0}
+    // Padding-aware re-planning (m_tiles > 1 only): token items at or beyond req_offsets[R] are
+    // skipped and the vocabulary tiles are re-dealt over the remaining items; `splits` above stays
+    // the record stride (the largest split count any item count can produce).
+    const int32_t* req_offsets;
+    int32_t R, total_tiles, units, replan;
 };
 
 // ---------------------------------------------------------------------------------- descriptors
@@ -174,8 +204,22 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     // Let the finalize kernel's CTAs become resident now (they block in griddepcontrol.wait).
     ptx::pdl_launch_dependents();
 
-    const int T = p.tiles_per_split, BN = p.tile_n;
+    int T = p.tiles_per_split, m_items = p.m_tiles, work_items = p.work_items;
+    const int BN = p.tile_n;
     const int b_rows = kPair ? (BN >> 1) : BN;   // W rows this CTA stages per tile
+    if (p.replan) {   // uniform across the grid: every thread reads the same word
+        const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
+        m_items = (n_valid + kRowsPerItem - 1) / kRowsPerItem;
+        if (m_items < p.m_tiles) {
+            if (m_items > 0) {
+                const SplitPlan sp = plan_splits(p.total_tiles, m_items, p.units);
+                T = sp.T;
+                work_items = m_items * sp.splits;
+            } else {
+                work_items = 0;
+            }
+        }
+    }
 
     if (warp == 0) {
         // ===================================================================== TMA producer
@@ -185,8 +229,8 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);  // leader's barriers
             int stage = 0;
             uint32_t phase = 0;
-            for (int w = unit; w < p.work_items; w += units) {
-                const int mt = w % p.m_tiles, sp = w / p.m_tiles;
+            for (int w = unit; w < work_items; w += units) {
+                const int mt = w % m_items, sp = w / m_items;
                 const int v0 = sp * T * BN;
                 const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
                 const int a_row = mt * kRowsPerItem + static_cast<int>(rank) * kTileM;
@@ -227,8 +271,8 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             const int k_blocks = p.k_blocks, stages = p.stages;
             int stage = 0;
             uint32_t phase = 0, acc = 0, desc_off = 0;
-            for (int w = unit; w < p.work_items; w += units) {
-                const int sp = w / p.m_tiles;
+            for (int w = unit; w < work_items; w += units) {
+                const int sp = w / m_items;
                 const int v0 = sp * T * BN;
                 const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
                 for (int t = 0; t < ntiles; ++t, ++acc) {
@@ -265,8 +309,8 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         const int row = static_cast<int>(rank) * kTileM + q * 32 + lane;
         const uint32_t lane_addr = static_cast<uint32_t>(q * 32) << 16;
         uint32_t acc = 0;
-        for (int w = unit; w < p.work_items; w += units) {
-            const int mt = w % p.m_tiles, sp = w / p.m_tiles;
+        for (int w = unit; w < work_items; w += units) {
+            const int mt = w % m_items, sp = w / m_items;
             const int v0 = sp * T * BN;
             const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
             float m = -CUDART_INF_F, s = 0.f;
@@ -332,6 +376,7 @@ __host__ __device__ __forceinline__ float tau_eval(float load, const TauParamsDe
 
 struct FinalizeParams {
     int32_t n_alloc, R, splits, n_pad, agg_mode;
+    int32_t m_tiles, rows_per_item, total_tiles, units, replan;   // see FusedParams
     const float4* ws;
     const int32_t* req_offsets;
     const float* load;
@@ -385,6 +430,12 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
     const int b = __ldg(p.req_offsets + r), e = __ldg(p.req_offsets + r + 1);
     float tau = 0.f;
     if (threadIdx.x == 0) tau = tau_eval(__ldg(p.load + r), p.tau);   // a4
+    int nsplit = p.splits;   // records per row the fused kernel wrote
+    if (p.replan) {
+        const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
+        const int m_items = (n_valid + p.rows_per_item - 1) / p.rows_per_item;
+        if (m_items > 0) nsplit = plan_splits(p.total_tiles, min(m_items, p.m_tiles), p.units).splits;
+    }
 
     ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
 
@@ -395,12 +446,12 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
         float m = -CUDART_INF_F, s = 0.f;
         int a = 0x7fffffff;
         const float4* rec = p.ws + static_cast<size_t>(n) * p.splits;
-        for (int sp0 = lane; sp0 < p.splits; sp0 += 32 * kMergeBatch) {
+        for (int sp0 = lane; sp0 < nsplit; sp0 += 32 * kMergeBatch) {
             float4 v[kMergeBatch];
 #pragma unroll
             for (int j = 0; j < kMergeBatch; ++j) {
                 const int sp = sp0 + 32 * j;
-                v[j] = sp < p.splits ? rec[sp] : make_float4(-CUDART_INF_F, 0.f, __int_as_float(0x7fffffff), 0.f);
+                v[j] = sp < nsplit ? rec[sp] : make_float4(-CUDART_INF_F, 0.f, __int_as_float(0x7fffffff), 0.f);
             }
 #pragma unroll
             for (int j = 0; j < kMergeBatch; ++j) merge_stats(m, a, s, v[j].x, __float_as_int(v[j].z), v[j].y);

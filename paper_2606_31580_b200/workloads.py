@@ -69,10 +69,11 @@ class Workload:
 
     def algorithmic_bytes(self) -> int:
         """W once + hidden + argmax out + (load in, conf + exit out)."""
-        return 2 * self.V * self.d + 2 * self.N_alloc * self.d + 4 * self.N_alloc + 9 * self.R + 4 * (self.R + 1)
+        return 2 * self.V * self.d + 2 * self.N_valid * self.d + 4 * self.N_alloc + 9 * self.R + 4 * (self.R + 1)
 
     def flops(self) -> int:
-        return 2 * self.N_alloc * self.V * self.d
+        """Algorithmic flops: the valid rows only (padding rows need no projection)."""
+        return 2 * self.N_valid * self.V * self.d
 
 
 # ------------------------------------------------------------------------------------ pieces

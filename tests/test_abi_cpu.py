@@ -65,7 +65,8 @@ def test_plan_invariants(dims):
     assert 2 <= p["stages"] <= 8
     b_rows = bn // 2 if pair else bn                          # W rows one CTA stages per tile
     assert p["stages"] * (16384 + b_rows * 128) + 1280 == p["smem_bytes"] <= 227 * 1024
-    assert B.workspace_bytes(*dims) == max(16, 16 * S * p["m_tiles"] * tm)
+    assert B.workspace_bytes(*dims) == max(16, 16 * p["ws_splits"] * p["m_tiles"] * tm)
+    assert p["ws_splits"] >= S and (p["ws_splits"] == S or p["m_tiles"] > 1)
     # the busiest unit does at most ~8 % more than an even share of W rows (+ one tile of slack)
     busy = min(units, p["work_items"])
     rounds = -(-p["work_items"] // busy)

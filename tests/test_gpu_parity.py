@@ -158,6 +158,24 @@ def test_forced_variants_c5_512(P, force_mode, c2_W_bits, mode):
     assert np.all(g.argmax[pl] == w.planted[pl])
 
 
+@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("R,L,var_len,n_alloc", [
+    (20, None, (1, 16), 1000),   # ~170 valid rows of 1000: most token tiles are padding
+    (32, 8, None, 1024),         # exactly 256 valid rows: boundary of a pair item
+    (33, 8, None, 1024),         # 264 valid rows: one row group into the next item
+    (5, 0, None, 700),           # every request empty, several token tiles allocated
+])
+def test_padding_tiles_are_skipped_and_replanned(P, force_mode, mode, R, L, var_len, n_alloc):
+    """req_offsets[R] < N leaves whole token tiles of padding: the kernels skip them and re-deal the
+    vocabulary over the tiles that hold rows (device-side plan_splits); results must not change."""
+    force_mode(mode)
+    w = wl.scaled(f"pad-m{mode}-R{R}", 33000, 512, 0.05, R, L, seed=R + 17, N_alloc=n_alloc, var_len=var_len)
+    assert w.N_valid < w.N_alloc
+    st = P.check(w)
+    assert st["plan"]["m_tiles"] > 1
+    _log(w.name, st)
+
+
 def test_ties_in_pair_mode(P, force_mode):
     """Duplicate W rows across the two halves of a pair's vocabulary tile, across tiles and splits."""
     from paper_2606_31580_b200 import binding as B
