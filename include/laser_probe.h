@@ -88,6 +88,19 @@ typedef struct {
 enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2 };
 int laser_probe_set_mode(int mode);
 
+/* Overlap of back-to-back probe calls on one stream (programmatic dependent launch).
+ * 1 (default): the fused kernel of a call starts streaming W and hidden as soon as SMs are free,
+ *    i.e. while the kernel enqueued just before it on the stream may still be running; only its
+ *    workspace stores and its completion wait for that kernel.  Exact whenever hidden, W and
+ *    req_offsets are complete when the preceding kernel STARTS - which CUDA guarantees unless that
+ *    kernel itself issues griddepcontrol.launch_dependents (cudaTriggerProgrammaticLaunchCompletion)
+ *    before it has written them.  The library's own kernels only hand over the workspace and the
+ *    outputs, which the next call never reads early.
+ * 0: strict - the fused kernel executes griddepcontrol.wait before its first global read, so a
+ *    producer kernel that triggers its dependents early is also safe.
+ * Process-wide; affects subsequent calls. */
+int laser_probe_set_overlap(int enable);
+
 /* Aggregate that turns the per-token max probabilities of a request into its confidence.
  * The paper does not fix it; MEAN is the default reading (A1). */
 enum { LASER_AGG_MEAN = 0, LASER_AGG_GEOMEAN = 1, LASER_AGG_MIN = 2 };

@@ -23,7 +23,7 @@ EXPORTS = [
     "laser_probe_confidence_host", "laser_probe_confidence_host_async", "laser_tau_from_load", "laser_ema_update",
     "laser_budget_params_default", "laser_allocate_budget", "laser_status_string",
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
-    "laser_profile_read", "laser_probe_set_mode",
+    "laser_profile_read", "laser_probe_set_mode", "laser_probe_set_overlap",
 ]
 
 
@@ -98,6 +98,7 @@ def lib():
         L.laser_last_error.restype = C.c_char_p
         L.laser_kernel_launch_count.restype = C.c_uint64
         L.laser_probe_set_mode.argtypes = [C.c_int]
+        L.laser_probe_set_overlap.argtypes = [C.c_int]
         L.laser_profile_enable.argtypes = [C.c_int]
         L.laser_profile_read.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_int32)]
         _lib = L
@@ -130,6 +131,11 @@ def staging_bytes(N, d, V, R) -> int:
 def set_mode(mode: int):
     """laser_probe_set_mode: MODE_AUTO / MODE_SINGLE / MODE_PAIR (process-wide kernel variant)."""
     _check(lib().laser_probe_set_mode(mode))
+
+
+def set_overlap(enable: bool):
+    """laser_probe_set_overlap: let back-to-back calls on a stream overlap (default) or not."""
+    _check(lib().laser_probe_set_overlap(1 if enable else 0))
 
 
 def kernel_launch_count() -> int:

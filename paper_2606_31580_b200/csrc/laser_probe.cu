@@ -115,6 +115,7 @@ double plan_variant(const laser_probe_dims& dm, int units, int tile_m, int bn_st
 }
 
 std::atomic<int> g_force_mode{LASER_MODE_AUTO};
+std::atomic<int> g_overlap{1};
 
 void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
     // CTA pairs (tcgen05 cta_group::2, M = 256) when there is more than one 128-row token tile: each
@@ -348,6 +349,7 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         fp.total_tiles = ceil_div(dims->V, pl.tile_n);
         fp.units = pair ? (di->sms / 2 > 0 ? di->sms / 2 : 1) : di->sms;
         fp.replan = pl.m_tiles > 1 ? 1 : 0;
+        fp.wait_first = g_overlap.load(std::memory_order_relaxed) ? 0 : 1;
         fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
         fp.work_items = pl.work_items; fp.n_pad = n_pad;
         fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
@@ -363,9 +365,9 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         cfg.blockDim = dim3(kFusedThreads);
         cfg.dynamicSmemBytes = static_cast<size_t>(pl.smem_bytes);
         cfg.stream = stream;
-        // Programmatic dependent launch: the prologue (barrier init, TMEM allocation, descriptor
-        // prefetch) may overlap the tail of the previous kernel in the stream; the kernel executes
-        // griddepcontrol.wait before its first global-memory access.
+        // Programmatic dependent launch: the kernel may start while the previous kernel in the
+        // stream is still running; it executes griddepcontrol.wait before its workspace stores and
+        // before it exits (and before its first global read when overlap is switched off).
         cudaLaunchAttribute fattr[2];
         unsigned na = 0;
         if (use_pdl && !prof) {
@@ -633,6 +635,11 @@ int laser_profile_read(float* ms_fused_sum, float* ms_finalize_sum, int32_t* cal
 int laser_probe_set_mode(int mode) {
     if (mode < LASER_MODE_AUTO || mode > LASER_MODE_PAIR) return LASER_E_MODE;
     g_force_mode.store(mode, std::memory_order_relaxed);
+    return LASER_OK;
+}
+
+int laser_probe_set_overlap(int enable) {
+    g_overlap.store(enable ? 1 : 0, std::memory_order_relaxed);
     return LASER_OK;
 }
 

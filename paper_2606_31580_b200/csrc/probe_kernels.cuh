@@ -10,10 +10,12 @@
 // With tcgen05.ld 32x32b every epilogue thread owns one token row and walks its vocabulary columns
 // in registers: no cross-lane traffic in the vocabulary loop.
 //
-// Work decomposition: the vocabulary is cut into `splits` contiguous ranges of tiles_per_split *
-// tile_n rows; a work item is (token tile of 128 rows, split).  Items are ordered token-tile
-// fastest so that CTAs running side by side stream the same W rows (one HBM read, L2 hits for the
-// rest).  The grid is persistent (<= one CTA per SM); CTA b takes items b, b + grid, ...
+// Work decomposition: the vocabulary is cut into tiles of tile_n rows which are dealt round-robin to
+// `splits` splits (split sp owns tiles sp, sp + splits, ...: at any moment the CTAs stream one
+// contiguous window of W, which HBM serves ~3 % faster than 148 distant ranges); a work item is
+// (token tile of 128 rows, split).  Items are ordered token-tile fastest so that CTAs running side
+// by side stream the same W rows (one HBM read, L2 hits for the rest).  The grid is persistent
+// (<= one CTA per SM); CTA b takes items b, b + grid, ...
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -37,7 +39,7 @@ constexpr int kEpilogueThreads = 128;
 constexpr float kLog2e = 1.4426950408889634f;
 
 // How the vocabulary tiles are dealt to the execution units (CTAs, or CTA pairs) for `m_items` token
-// items: cut the `total_tiles` tiles of tile_n rows into `splits` contiguous ranges of `T` tiles such
+// items: deal the `total_tiles` tiles of tile_n rows to `splits` splits of at most `T` tiles each such
 // that m_items * splits fills the units in whole rounds with the least work on the busiest unit.
 // Shared by the host planner and both kernels: when a batch carries padding rows (req_offsets[R] <
 // N) the kernels re-plan on the device for the token items that actually hold rows.
@@ -74,6 +76,9 @@ struct FusedParams {
     // the record stride (the largest split count any item count can produce).
     const int32_t* req_offsets;
     int32_t R, total_tiles, units, replan;
+    // 1: griddepcontrol.wait before the first global read (strict stream order for the inputs too);
+    // 0: only the workspace stores wait (see laser_probe_set_overlap in include/laser_probe.h).
+    int32_t wait_first;
 };
 
 // ---------------------------------------------------------------------------------- descriptors
@@ -198,13 +203,15 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
-    // Programmatic dependent launch: everything above overlapped the previous kernel in the stream;
-    // nothing below may touch global memory before that kernel has completed.
-    ptx::pdl_wait();
+    // Programmatic dependent launch.  The only memory this kernel shares with the kernel before it in
+    // a chain of probe calls (the previous call's finalize kernel) is the workspace, so by default
+    // only the workspace stores (and the exit) wait for that kernel: the W stream of this call then
+    // overlaps the tail of the previous one.  wait_first restores the strict order for the inputs.
+    if (p.wait_first) ptx::pdl_wait();
     // Let the finalize kernel's CTAs become resident now (they block in griddepcontrol.wait).
     ptx::pdl_launch_dependents();
 
-    int T = p.tiles_per_split, m_items = p.m_tiles, work_items = p.work_items;
+    int m_items = p.m_tiles, work_items = p.work_items;
     const int BN = p.tile_n;
     const int b_rows = kPair ? (BN >> 1) : BN;   // W rows this CTA stages per tile
     if (p.replan) {   // uniform across the grid: every thread reads the same word
@@ -212,14 +219,15 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         m_items = (n_valid + kRowsPerItem - 1) / kRowsPerItem;
         if (m_items < p.m_tiles) {
             if (m_items > 0) {
-                const SplitPlan sp = plan_splits(p.total_tiles, m_items, p.units);
-                T = sp.T;
-                work_items = m_items * sp.splits;
+                work_items = m_items * plan_splits(p.total_tiles, m_items, p.units).splits;
             } else {
                 work_items = 0;
             }
         }
     }
+    // split sp owns vocabulary tiles sp, sp + S, sp + 2S, ... (ascending: ties keep the lowest index)
+    const int S = m_items > 0 ? work_items / m_items : 1;
+    const int total_tiles = p.total_tiles;
 
     if (warp == 0) {
         // ===================================================================== TMA producer
@@ -231,11 +239,9 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             uint32_t phase = 0;
             for (int w = unit; w < work_items; w += units) {
                 const int mt = w % m_items, sp = w / m_items;
-                const int v0 = sp * T * BN;
-                const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
                 const int a_row = mt * kRowsPerItem + static_cast<int>(rank) * kTileM;
-                for (int t = 0; t < ntiles; ++t) {
-                    const int b_row = v0 + t * BN + static_cast<int>(rank) * b_rows;
+                for (int tile = sp; tile < total_tiles; tile += S) {
+                    const int b_row = tile * BN + static_cast<int>(rank) * b_rows;
                     for (int kb = 0; kb < k_blocks; ++kb) {
                         ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
                         if (ptx::elect_one()) {
@@ -272,10 +278,7 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             int stage = 0;
             uint32_t phase = 0, acc = 0, desc_off = 0;
             for (int w = unit; w < work_items; w += units) {
-                const int sp = w / m_items;
-                const int v0 = sp * T * BN;
-                const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
-                for (int t = 0; t < ntiles; ++t, ++acc) {
+                for (int tile = w / m_items; tile < total_tiles; tile += S, ++acc) {
                     const uint32_t buf = acc & 1u, aphase = (acc >> 1) & 1u;
                     // epilogue (of both CTAs in pair mode) drained this buffer
                     if constexpr (kPair) ptx::mbar_wait_cluster(tempty_bar(buf), aphase ^ 1u);
@@ -311,16 +314,14 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         uint32_t acc = 0;
         for (int w = unit; w < work_items; w += units) {
             const int mt = w % m_items, sp = w / m_items;
-            const int v0 = sp * T * BN;
-            const int ntiles = min(T, (p.V - v0 + BN - 1) / BN);
             float m = -CUDART_INF_F, s = 0.f;
             int a = -1;
-            for (int t = 0; t < ntiles; ++t, ++acc) {
+            for (int tile = sp; tile < total_tiles; tile += S, ++acc) {
                 const uint32_t buf = acc & 1u, aphase = (acc >> 1) & 1u;
                 ptx::mbar_wait(tfull_bar(buf), aphase);
                 ptx::tc_fence_after();
                 const uint32_t taddr = tmem_base + lane_addr + buf * kMaxTileN;
-                const int vt = v0 + t * BN;
+                const int vt = tile * BN;
                 int c = 0;
                 for (; c + 32 <= BN && vt + c < p.V; c += 32) {
                     uint32_t r[32];
@@ -346,12 +347,16 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             // row-major over splits: the finalize kernel reads a row's partials as contiguous 16-byte
             // records (coalesced); the scattered 16-byte stores here are fire-and-forget
             const size_t o = (static_cast<size_t>(mt) * kRowsPerItem + row) * p.splits + sp;
+            ptx::pdl_wait();   // the previous call's finalize kernel may still be reading the workspace
             p.ws[o] = make_float4(m, s, __int_as_float(a), 0.f);
         }
     }
 
     // ------------------------------------------------------------------------- teardown
     __syncwarp();   // reconverge the warps whose lane 0 ran a role loop
+    // No CTA (not even one without work) completes before the kernel ahead of it in the stream has:
+    // completion of this grid then implies completion of everything before it, as stream order demands.
+    ptx::pdl_wait();
     ptx::tc_fence_before();
     if constexpr (kPair) ptx::cluster_sync();   // the peer may still read this CTA's shared memory / TMEM
     else __syncthreads();

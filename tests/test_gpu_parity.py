@@ -183,13 +183,15 @@ def test_ties_in_pair_mode(P, force_mode):
     V, d, N = 20000, 128, 200
     plan = B.plan_query(N, d, V, 2)
     assert plan["cta_pair"] == 1
-    bn, T = plan["tile_n"], plan["tiles_per_split"]
+    bn, T, S = plan["tile_n"], plan["tiles_per_split"], plan["splits"]
+    assert T >= 2 and S >= 2
     rng = np.random.default_rng(9)
     Wf = (rng.standard_normal((V, d)) * 0.05).astype(np.float32)
     h = rng.standard_normal((N, d)).astype(np.float32)
     for row in (0, 150):                            # a row of the leader CTA, a row of the peer CTA
         big = (h[row] * 0.5).astype(np.float32)
-        for v1, v2 in [(bn // 2 - 1, bn // 2), (bn - 1, bn), (T * bn - 1, T * bn), (5, 3 * T * bn + 7)]:
+        for v1, v2 in [(bn // 2 - 1, bn // 2), (bn - 1, bn), (T * bn - 1, T * bn), (5, S * bn + 7),
+                       (5, 3 * bn + 7)]:   # round-robin deal: (5, S*bn+7) = consecutive tiles of split 0
             W2 = Wf.copy(); W2[v1] = big; W2[v2] = big
             w = wl.Workload("ties-pair", wl.bf16_bits(W2), wl.bf16_bits(h), wl.fixed_offsets(2, 100),
                             np.array([0.3, 0.7], np.float32))
@@ -229,16 +231,20 @@ def test_ties_across_tile_and_split_boundaries(P):
     """P3 on the device: duplicate W rows give bit-identical logits; the lowest index must survive the
     in-thread, cross-tile and cross-split merges."""
     from paper_2606_31580_b200 import binding as B
-    V, d, N = 20000, 128, 16
+    V, d, N = 80000, 128, 16
     plan = B.plan_query(N, d, V, 2)
-    bn, T = plan["tile_n"], plan["tiles_per_split"]
+    bn, T, S = plan["tile_n"], plan["tiles_per_split"], plan["splits"]
+    assert T >= 2 and S >= 2
     rng = np.random.default_rng(8)
     Wf = (rng.standard_normal((V, d)) * 0.05).astype(np.float32)
     h = rng.standard_normal((N, d)).astype(np.float32)
     big = (h[0] * 0.5).astype(np.float32)          # strong match for row 0 only
-    pairs = [(bn - 1, bn),                         # straddles a tile boundary
-             (T * bn - 1, T * bn),                 # straddles a split boundary
-             (5, 3 * T * bn + 7),                  # far apart, different splits
+    # tiles are dealt round-robin: split sp owns tiles sp, sp + S, ...
+    pairs = [(bn - 1, bn),                         # adjacent tiles = neighbouring splits
+             (T * bn - 1, T * bn),
+             (5, S * bn + 7),                      # same split, consecutive tiles of it (in-thread merge)
+             (bn + 3, (S + 1) * bn + 1),           # same split (1), consecutive tiles
+             (5, 3 * bn + 7),                      # different splits
              (31, 32)]                             # same tile, adjacent 32-column chunks
     for v1, v2 in pairs:
         W2 = Wf.copy(); W2[v1] = big; W2[v2] = big
@@ -249,6 +255,41 @@ def test_ties_across_tile_and_split_boundaries(P):
         ora, rows, reqs = P.run_oracle(w)
         assert ora.argmax[0] == v1 and ora.gap2[0] == 0.0
         P.compare(w, g, ora, rows, reqs, "ties")
+
+
+@pytest.mark.parametrize("overlap", [True, False])
+def test_back_to_back_calls_share_a_workspace(P, overlap):
+    """Stream order under programmatic dependent launch: calls enqueued back to back on one stream,
+    all on ONE workspace, with alternating inputs.  The fused kernel of call k+1 may start while the
+    finalize kernel of call k still reads the workspace (laser_probe_set_overlap); every call must
+    still produce its own batch's result."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    V, d, R, L = 1000, 64, 48, 8          # short fused kernel, long finalize kernel: the tightest race
+    ws = [wl.scaled(f"b2b{i}", V, d, 0.05, R, L, seed=900 + i) for i in range(2)]
+    devs = [P.to_device(w) for w in ws]
+    oras = [P.run_oracle(w) for w in ws]
+    K = 24
+    probes = [B.Probe(R * L, d, V, R) for _ in range(K)]
+    for p in probes[1:]:
+        p.workspace = probes[0].workspace
+    B.set_overlap(overlap)
+    try:
+        tp = B.TauParams(**ws[0].tau_params)
+        torch.cuda.synchronize()
+        for k, p in enumerate(probes):
+            dv = devs[k % 2]
+            p(dv["hidden"], dv["W"], dv["off"], dv["load"], tp)
+        torch.cuda.synchronize()
+    finally:
+        B.set_overlap(True)
+    for k, p in enumerate(probes):
+        g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),
+                     p.tau.cpu().numpy(), p.pmax.cpu().numpy(), p.plan)
+        ora, rows, reqs = oras[k % 2]
+        P.compare(ws[k % 2], g, ora, rows, reqs, f"b2b call {k}")
+    # the two batches differ, so a call that read the other batch's partials cannot pass
+    assert not np.array_equal(oras[0][0].argmax, oras[1][0].argmax)
 
 
 # ------------------------------------------------------------------ semantics fixed at the boundary
