@@ -89,15 +89,17 @@ enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2 };
 int laser_probe_set_mode(int mode);
 
 /* Overlap of back-to-back probe calls on one stream (programmatic dependent launch).
- * 1 (default): the fused kernel of a call starts streaming W and hidden as soon as SMs are free,
- *    i.e. while the kernel enqueued just before it on the stream may still be running; only its
- *    workspace stores and its completion wait for that kernel.  Exact whenever hidden, W and
- *    req_offsets are complete when the preceding kernel STARTS - which CUDA guarantees unless that
- *    kernel itself issues griddepcontrol.launch_dependents (cudaTriggerProgrammaticLaunchCompletion)
- *    before it has written them.  The library's own kernels only hand over the workspace and the
- *    outputs, which the next call never reads early.
- * 0: strict - the fused kernel executes griddepcontrol.wait before its first global read, so a
- *    producer kernel that triggers its dependents early is also safe.
+ * 0 (default): strict - the fused kernel executes griddepcontrol.wait before its first global read,
+ *    so every input is read in stream order whatever kernel precedes the call (including a producer
+ *    of `hidden` that triggers its dependents early).  Only the kernel's prologue (barrier init,
+ *    TMEM allocation, descriptor prefetch) overlaps the preceding kernel.
+ * 1: the fused kernel of a call starts streaming W and hidden as soon as SMs are free, i.e. while
+ *    the kernel enqueued just before it on the stream may still be running; only its workspace
+ *    stores and its completion wait for that kernel.  Exact whenever hidden, W and req_offsets are
+ *    complete when the preceding kernel STARTS - which CUDA guarantees unless that kernel itself
+ *    issues griddepcontrol.launch_dependents (cudaTriggerProgrammaticLaunchCompletion) before it has
+ *    written them.  The library's own kernels only hand over the workspace and the outputs, which
+ *    the next call never reads early, so a loop of probe calls (bench.py's timed region) may opt in.
  * Process-wide; affects subsequent calls. */
 int laser_probe_set_overlap(int enable);
 

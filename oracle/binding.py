@@ -85,6 +85,7 @@ def _L():
         lib.laser_oracle_row_stats_range.argtypes = [fp, fp, i32, i64, i64, dp, ip, dp]
         lib.laser_oracle_merge.argtypes = [dbl, C.c_int32, dbl, dbl, C.c_int32, dbl, dp, ip, dp]
         lib.laser_oracle_merge.restype = None
+        lib.laser_oracle_token_prob.argtypes = [fp, fp, ip, i64, i32, i64, dp]
         lib.laser_oracle_aggregate.argtypes = [dp, ip, i64, dp]
         lib.laser_oracle_aggregate_mode.argtypes = [dp, ip, i64, i32, dp]
         lib.laser_oracle_tau_scalar.argtypes = [dbl, tp]
@@ -140,6 +141,19 @@ def row_stats(hidden, W, want_logits: bool = False):
     out = dict(m=m, a=a, S=S, pmax=pm, gap2=g2)
     if want_logits:
         out["logits"] = lg
+    return out
+
+
+def token_prob(hidden, W, token_ids):
+    """Probability of token_ids[n] under the softmax of row n (DESIGN A2) — laser_oracle_token_prob."""
+    hidden, W = _f32(hidden), _f32(W)
+    tok = np.ascontiguousarray(token_ids, np.int32).reshape(-1)
+    N, d = hidden.shape
+    V = W.shape[0]
+    assert tok.shape[0] == N and W.shape[1] == d
+    out = np.empty(N, np.float64)
+    _chk(_L().laser_oracle_token_prob(_ptr(hidden, C.c_float), _ptr(W, C.c_float), _ptr(tok, C.c_int32),
+                                      N, d, V, _ptr(out, C.c_double)), "token_prob")
     return out
 
 

@@ -18,6 +18,8 @@
  *                             lambda_min, lambda_max)                PAPER.md:100-103 (Eq. 5), 144
  *   step 5  exit[r] = C[r] > lambda[r]   (strict)                    PAPER.md:61, 70, 122 (Alg.1 step 6)
  *
+ *   variant (NEXT-1 / DESIGN A2): probability of a given (emitted) token, laser_oracle_token_prob.
+ *
  * and, off the hot path (NEXT-2 rows of SURVEY §8 f):
  *   EMA      Lbar(t) = alpha*L(t) + (1-alpha)*Lbar(t-1), Lbar(0)=0
  *   budget   B = max{B_min, floor(B_base*f_diff*f_load)}             PAPER.md:152-173 (Eq. 6-8)
@@ -270,6 +272,47 @@ int laser_oracle_aggregate_mode(const double* pmax, const int32_t* req_offsets, 
         } else return -1;
     }
     return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-1, second half (DESIGN A2): the probability of a GIVEN token per row instead of the row
+ * maximum - "the token probabilities" of the trial answer read as the probabilities
+ * of the tokens that were emitted.  Plain softmax entry:
+ *     p[n] = exp(l[n, t_n]) / sum_v exp(l[n, v]),   evaluated as exp(l_t - m) / sum_v exp(l_v - m).
+ * A token id outside [0, V) has probability 0 (it is not in the vocabulary).  Under greedy decoding
+ * t_n is the argmax and p equals pmax of step 2.
+ * ---------------------------------------------------------------------------------------------- */
+int laser_oracle_token_prob(const float* hidden, const float* W, const int32_t* token_ids, int64_t N,
+                            int d, int64_t V, double* out_ptok) {
+    if (N < 0 || d <= 0 || V <= 0 || (N > 0 && (!hidden || !W || !token_ids || !out_ptok))) return -1;
+    int failed = 0;
+#pragma omp parallel
+    {
+        double* h = (double*)malloc(sizeof(double) * (size_t)d);
+        double* l = (double*)malloc(sizeof(double) * (size_t)V);
+        if (!h || !l) {
+#pragma omp atomic write
+            failed = 1;
+        }
+#pragma omp barrier
+        if (!failed) {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t n = 0; n < N; ++n) {
+                for (int k = 0; k < d; ++k) h[k] = (double)hidden[n * d + k];
+                for (int64_t v = 0; v < V; ++v) l[v] = dot_fp64(h, W + v * (int64_t)d, d);
+                double m = -INFINITY;
+                for (int64_t v = 0; v < V; ++v)
+                    if (l[v] > m) m = l[v];
+                double S = 0.0;
+                for (int64_t v = 0; v < V; ++v) S += exp(l[v] - m);
+                int64_t t = token_ids[n];
+                out_ptok[n] = (t >= 0 && t < V) ? exp(l[t] - m) / S : 0.0;
+            }
+        }
+        free(h);
+        free(l);
+    }
+    return failed ? -1 : 0;
 }
 
 /* ------------------------------------------------------------------------------------------------

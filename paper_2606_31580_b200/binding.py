@@ -134,7 +134,7 @@ def set_mode(mode: int):
 
 
 def set_overlap(enable: bool):
-    """laser_probe_set_overlap: let back-to-back calls on a stream overlap (default) or not."""
+    """laser_probe_set_overlap: let back-to-back calls on a stream overlap, or keep strict stream order (default)."""
     _check(lib().laser_probe_set_overlap(1 if enable else 0))
 
 

@@ -115,7 +115,7 @@ double plan_variant(const laser_probe_dims& dm, int units, int tile_m, int bn_st
 }
 
 std::atomic<int> g_force_mode{LASER_MODE_AUTO};
-std::atomic<int> g_overlap{1};
+std::atomic<int> g_overlap{0};   // strict stream order unless the caller opts in
 
 void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
     // CTA pairs (tcgen05 cta_group::2, M = 256) when there is more than one 128-row token tile: each

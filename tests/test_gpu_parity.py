@@ -282,7 +282,7 @@ def test_back_to_back_calls_share_a_workspace(P, overlap):
             p(dv["hidden"], dv["W"], dv["off"], dv["load"], tp)
         torch.cuda.synchronize()
     finally:
-        B.set_overlap(True)
+        B.set_overlap(False)
     for k, p in enumerate(probes):
         g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),
                      p.tau.cpu().numpy(), p.pmax.cpu().numpy(), p.plan)

@@ -258,3 +258,40 @@ def test_nan_rows_poison_conf_not_exit(tau_norm):
     h[1, 3] = np.nan
     r = _probe(h, W, [0, 2, 4], [0.5, 0.5], tau_norm)
     assert np.isnan(r.conf[0]) and r.exit[0] == 0 and np.isfinite(r.conf[1])
+
+
+# ------------------------------------------------------------------------------------------ P15
+# Probability of a GIVEN token (DESIGN A2 alternative, NEXT-1): oracle.token_prob.
+@pytest.mark.parametrize("M", [0.0, 1.0, 5.0, 40.0])
+def test_P15_token_prob_scaled_identity(M):
+    """W = M*I, hidden = e_j: the planted token has 1/(1+(V-1)e^-M), any other e^-M/(1+(V-1)e^-M)."""
+    V = 48
+    W = (M * np.eye(V)).astype(np.float32)
+    js = np.array([0, 5, 47, 17])
+    h = np.eye(V, dtype=np.float32)[js]
+    den = 1.0 + (V - 1) * math.exp(-M)
+    np.testing.assert_allclose(oracle.token_prob(h, W, js), 1.0 / den, rtol=1e-14)
+    others = (js + 3) % V
+    np.testing.assert_allclose(oracle.token_prob(h, W, others), math.exp(-M) / den, rtol=1e-14)
+
+
+def test_P15_token_prob_is_a_distribution_and_matches_library():
+    """Sum over every token of a row's probabilities is 1 (brute force over the whole vocabulary);
+    the entries equal torch.softmax's; the argmax token's probability is step 2's pmax bit for bit;
+    a token outside the vocabulary has probability 0."""
+    import torch
+    rng = np.random.default_rng(15)
+    V, d = 257, 24
+    W = wl.bits_to_f32(wl.bf16_bits(rng.standard_normal((V, d)) * 0.7))
+    h1 = wl.bits_to_f32(wl.bf16_bits(rng.standard_normal((1, d)) * 1.5))
+    h = np.repeat(h1, V, axis=0)
+    p = oracle.token_prob(h, W, np.arange(V))
+    assert abs(p.sum() - 1.0) < 1e-13 and np.all(p > 0)
+    ref = torch.softmax(torch.from_numpy(h1).double() @ torch.from_numpy(W).double().T, -1)[0].numpy()
+    np.testing.assert_allclose(p, ref, rtol=1e-12)
+    rs = oracle.row_stats(h1, W)
+    assert oracle.token_prob(h1, W, rs["a"])[0] == rs["pmax"][0]
+    assert np.all(oracle.token_prob(np.repeat(h1, 3, axis=0), W, [-1, V, 2**31 - 1]) == 0.0)
+    # uniform logits: every token has 1/V
+    np.testing.assert_allclose(oracle.token_prob(np.zeros((4, d), np.float32), W, [0, 1, 100, 256]), 1.0 / V,
+                               rtol=1e-15)
