@@ -41,7 +41,7 @@ enum {
     LASER_E_WORKSPACE = -5, /* workspace NULL or smaller than laser_probe_workspace_bytes()           */
     LASER_E_ARCH = -6,      /* current device is not compute capability 10.0 (B200)                   */
     LASER_E_CUDA = -7,      /* a CUDA runtime / driver call failed; see laser_last_error()            */
-    LASER_E_MODE = -8       /* unknown aggregate mode                                                 */
+    LASER_E_MODE = -8       /* unknown aggregate / probability / kernel mode                          */
 };
 
 /* Hyper-parameters of Eq. 5; defaults are the paper's.  `l_target` and load[] share
@@ -154,6 +154,87 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
                                const laser_probe_dims* dims, void* workspace,
                                size_t workspace_bytes, void* stream, float* out_tau_opt,
                                float* out_pmax_opt, int aggregate_mode);
+
+/* Which probability of a trial-answer token enters the aggregate.  PAPER.md:61 says the confidence
+ * is "computed from the token probabilities" and does not say which (A2):
+ *   LASER_PROB_MAX    the row maximum max_v softmax(logits[n,:]) (default; equals the emitted token's
+ *                     probability under greedy decoding)
+ *   LASER_PROB_TOKEN  the probability of a given token, softmax(logits[n,:])[token_ids[n]] - the token
+ *                     the engine actually emitted at that position.  A token id outside [0, V) has
+ *                     probability 0.  out_argmax is still the row argmax. */
+enum { LASER_PROB_MAX = 0, LASER_PROB_TOKEN = 1 };
+
+/* Options of laser_probe_confidence_opt / laser_probe_combine (HOST struct, copied by value). */
+typedef struct {
+    int32_t aggregate_mode;    /* LASER_AGG_*                                                        */
+    int32_t prob_mode;         /* LASER_PROB_*                                                       */
+    const int32_t* token_ids;  /* device, int32 [N]; required for LASER_PROB_TOKEN, else may be NULL */
+} laser_probe_options;
+
+/* laser_probe_confidence with options (NULL options = defaults: mean of the row maxima).  With
+ * LASER_PROB_TOKEN, out_pmax_opt receives the token probabilities.  Costs no extra HBM traffic: the
+ * token's logit rides in the spare word of the 16-byte statistics record. */
+int laser_probe_confidence_opt(const void* hidden, const void* W, const int32_t* req_offsets,
+                               const float* load, const laser_tau_params* tau_params,
+                               float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+                               const laser_probe_dims* dims, void* workspace,
+                               size_t workspace_bytes, void* stream, float* out_tau_opt,
+                               float* out_pmax_opt, const laser_probe_options* options);
+
+/*
+ * Vocabulary-parallel probe (SURVEY.md §8 e: the LM head's tensor-parallel layout).  GPU g holds the
+ * rows [v_offset_g, v_offset_g + V_g) of W and the whole batch; the path becomes
+ *
+ *   every GPU:  laser_probe_partial  a1 + a2 over its shard -> one 16-byte record per row
+ *   exchange :  the records of all G shards meet on every GPU, laid out [G, N]
+ *   every GPU:  laser_probe_combine  merge of the G records per row, then a3, a4, a5 as above
+ *
+ * The merge is the associative operator the split-V path already uses, so the result equals the
+ * single-GPU call up to the rounding order of the sum of exponentials.  The exchange is either a
+ * collective of the caller (NCCL all-gather of N*16 bytes per GPU), or done by the producer itself:
+ * with `peers`, laser_probe_partial stores each record straight into every GPU's gathered buffer
+ * through peer-mapped pointers (NVLink) and then raises a flag there; laser_probe_combine waits for
+ * the G flags.  No collective call, no host synchronisation.
+ */
+typedef struct {
+    float m;       /* max logit over the shard (-inf: empty / padding row)                            */
+    float s;       /* sum_v exp(logit - m) over the shard                                            */
+    int32_t a;     /* GLOBAL vocabulary index of the lowest-index maximum (INT32_MAX: none)          */
+    float l_tok;   /* logit of the row's token if the shard holds it, else -inf (LASER_PROB_TOKEN)   */
+} laser_row_stats;
+
+enum { LASER_MAX_PEERS = 16 };
+/* Peer-push exchange (HOST struct).  peer_stats[g] / peer_flags[g] are device pointers valid on THIS
+ * GPU that address GPU g's gathered buffer [world, N] and flag array [world] (peer-mapped, e.g.
+ * CUDA IPC or symmetric memory; entry [rank] is this GPU's own).  `epoch` must increase by one per
+ * exchange on every GPU and never be 0 (flags start at 0).  A gathered buffer may be rewritten two
+ * exchanges later: alternate two (stats, flags) sets by epoch parity. */
+typedef struct {
+    int32_t rank, world;                       /* 0 <= rank < world <= LASER_MAX_PEERS */
+    uint32_t epoch;
+    laser_row_stats* peer_stats[LASER_MAX_PEERS];
+    uint32_t* peer_flags[LASER_MAX_PEERS];
+} laser_probe_peers;
+
+/* a1 + a2 over one vocabulary shard.  dims->V = rows of W_shard; v_offset = global index of its row
+ * 0; token_ids_opt (device int32 [N], GLOBAL ids) or NULL.  out_stats: device [N] or NULL (rows >=
+ * req_offsets[R] get the neutral record {-inf, 0, INT32_MAX, -inf}).  peers_opt: see above; at least
+ * one of out_stats / peers_opt must be given.  workspace as for laser_probe_confidence with the same
+ * dims.  Asynchronous on `stream`; three kernels with peers (fused, reduce, signal), else two. */
+int laser_probe_partial(const void* hidden, const void* W_shard, const int32_t* req_offsets,
+                        const int32_t* token_ids_opt, const laser_probe_dims* dims, int32_t v_offset,
+                        laser_row_stats* out_stats, const laser_probe_peers* peers_opt,
+                        void* workspace, size_t workspace_bytes, void* stream);
+
+/* Merge + a3-a5 over gathered statistics.  stats: device [G, N] (shard-major).  dims->N and dims->R
+ * are used (d, V ignored but must be valid).  wait_flags_opt: device uint32 [G] or NULL; when given
+ * every block first waits until all G flags have reached `epoch` (peer-push exchange).  One kernel. */
+int laser_probe_combine(const laser_row_stats* stats, int32_t G, const int32_t* req_offsets,
+                        const float* load, const laser_tau_params* tau_params, float* out_conf,
+                        int32_t* out_argmax, uint8_t* out_exit, const laser_probe_dims* dims,
+                        void* stream, float* out_tau_opt, float* out_pmax_opt,
+                        const laser_probe_options* options, const uint32_t* wait_flags_opt,
+                        uint32_t epoch);
 
 /*
  * End-to-end form with HOST buffers for the per-step tensors (W stays resident on the device: it is

@@ -15,6 +15,7 @@ _SO = Path(__file__).resolve().parent / "liblaser_probe.so"
 _lib = None
 
 AGG_MEAN, AGG_GEOMEAN, AGG_MIN = 0, 1, 2
+PROB_MAX, PROB_TOKEN = 0, 1
 MODE_AUTO, MODE_SINGLE, MODE_PAIR = 0, 1, 2
 
 EXPORTS = [
@@ -24,6 +25,7 @@ EXPORTS = [
     "laser_budget_params_default", "laser_allocate_budget", "laser_status_string",
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
     "laser_profile_read", "laser_probe_set_mode", "laser_probe_set_overlap",
+    "laser_probe_confidence_opt", "laser_probe_partial", "laser_probe_combine",
 ]
 
 
@@ -60,6 +62,20 @@ class Plan(C.Structure):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
 
 
+class Options(C.Structure):
+    """laser_probe_options."""
+    _fields_ = [("aggregate_mode", C.c_int32), ("prob_mode", C.c_int32), ("token_ids", C.c_void_p)]
+
+
+MAX_PEERS = 16
+
+
+class Peers(C.Structure):
+    """laser_probe_peers (peer-push exchange of the vocabulary-parallel probe)."""
+    _fields_ = [("rank", C.c_int32), ("world", C.c_int32), ("epoch", C.c_uint32),
+                ("peer_stats", C.c_void_p * MAX_PEERS), ("peer_flags", C.c_void_p * MAX_PEERS)]
+
+
 class LaserError(RuntimeError):
     def __init__(self, status, text):
         super().__init__(f"laser_probe status {status}: {text}")
@@ -86,6 +102,11 @@ def lib():
         common = [vp, vp, i32p, fp, tp, fp, i32p, u8p, dp, vp, C.c_size_t, vp, fp, fp]
         L.laser_probe_confidence.argtypes = common
         L.laser_probe_confidence_agg.argtypes = common + [C.c_int]
+        L.laser_probe_confidence_opt.argtypes = common + [C.POINTER(Options)]
+        L.laser_probe_partial.argtypes = [vp, vp, i32p, i32p, dp, C.c_int32, vp, C.POINTER(Peers), vp,
+                                          C.c_size_t, vp]
+        L.laser_probe_combine.argtypes = [vp, C.c_int32, i32p, fp, tp, fp, i32p, u8p, dp, vp, fp, fp,
+                                          C.POINTER(Options), vp, C.c_uint32]
         L.laser_probe_confidence_host.argtypes = [vp, vp, i32p, fp, tp, fp, i32p, u8p, dp, vp,
                                                   C.c_size_t, vp, C.c_size_t, vp]
         L.laser_probe_confidence_host_async.argtypes = L.laser_probe_confidence_host.argtypes
@@ -211,9 +232,12 @@ class Probe:
         self.pmax = torch.empty(N, dtype=torch.float32, device=self.device) if debug_outputs else None
         self.plan = plan_query(N, d, V, R)
 
-    def __call__(self, hidden, W, req_offsets, load, params: TauParams, stream=None, agg=AGG_MEAN):
+    def __call__(self, hidden, W, req_offsets, load, params: TauParams, stream=None, agg=AGG_MEAN,
+                 token_ids=None):
         """hidden bf16 [N,d], W bf16 [V,d], req_offsets int32 [R+1], load float32 [R] — device
-        tensors.  Enqueues on `stream` (default: torch's current stream); does not synchronise."""
+        tensors.  Enqueues on `stream` (default: torch's current stream); does not synchronise.
+        token_ids (device int32 [N]) selects LASER_PROB_TOKEN: the aggregate runs over the
+        probabilities of those tokens instead of the row maxima."""
         torch = self.torch
         d = self.dims
         assert hidden.dtype == torch.bfloat16 and W.dtype == torch.bfloat16
@@ -222,12 +246,85 @@ class Probe:
         assert req_offsets.dtype == torch.int32 and req_offsets.numel() == d.R + 1
         assert load.dtype == torch.float32 and load.numel() == d.R
         s = (stream or torch.cuda.current_stream(self.device)).cuda_stream
-        _check(lib().laser_probe_confidence_agg(
+        opt = _options(torch, agg, token_ids, d.N)
+        _check(lib().laser_probe_confidence_opt(
             hidden.data_ptr(), W.data_ptr(), req_offsets.data_ptr(), load.data_ptr(),
             C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(),
             C.byref(d), self.workspace.data_ptr(), self.workspace.numel(), s,
             self.tau.data_ptr() if self.tau is not None else None,
-            self.pmax.data_ptr() if self.pmax is not None else None, agg))
+            self.pmax.data_ptr() if self.pmax is not None else None, C.byref(opt)))
+        return ProbeOutputs(self.conf, self.argmax, self.exit, self.tau, self.pmax)
+
+
+def _options(torch, agg, token_ids, N) -> Options:
+    if token_ids is None:
+        return Options(agg, PROB_MAX, None)
+    assert token_ids.dtype == torch.int32 and token_ids.numel() == N and token_ids.is_contiguous()
+    return Options(agg, PROB_TOKEN, token_ids.data_ptr())
+
+
+class VocabShardProbe:
+    """Vocabulary-parallel probe, one instance per GPU (rank g of G): laser_probe_partial over this
+    GPU's rows of W, exchange of the 16-byte row records, laser_probe_combine.
+
+    stats_all is the gathered buffer [G, N, 4] (float32 view of laser_row_stats).  `partial` writes
+    this rank's records to stats_local [N, 4]; the caller all-gathers them into stats_all (see
+    parallel.VocabParallelProbe) and calls `combine`.  With `peers` (parallel.PeerExchange) partial
+    pushes the records into every rank's gathered buffer itself and combine waits for the flags."""
+
+    def __init__(self, N, d, V_shard, R, v_offset, world, device="cuda", debug_outputs=True):
+        import torch
+        self.torch = torch
+        self.dims = Dims(N, d, V_shard, R)
+        self.v_offset, self.world = int(v_offset), int(world)
+        self.device = torch.device(device)
+        wb = workspace_bytes(N, d, V_shard, R)
+        if wb == 0:
+            raise LaserError(-2, "invalid dimensions")
+        self.workspace = torch.empty(wb, dtype=torch.uint8, device=self.device)
+        self.stats_local = torch.empty((N, 4), dtype=torch.float32, device=self.device)
+        self.stats_all = torch.empty((world, N, 4), dtype=torch.float32, device=self.device)
+        self.conf = torch.empty(R, dtype=torch.float32, device=self.device)
+        self.argmax = torch.empty(N, dtype=torch.int32, device=self.device)
+        self.exit = torch.empty(R, dtype=torch.uint8, device=self.device)
+        self.tau = torch.empty(R, dtype=torch.float32, device=self.device) if debug_outputs else None
+        self.pmax = torch.empty(N, dtype=torch.float32, device=self.device) if debug_outputs else None
+        self.plan = plan_query(N, d, V_shard, R)
+
+    def _stream(self, stream):
+        return (stream or self.torch.cuda.current_stream(self.device)).cuda_stream
+
+    def partial(self, hidden, W_shard, req_offsets, token_ids=None, stream=None, out=None, peers: Peers | None = None):
+        """a1 + a2 over this shard -> stats_local (or `out`, a [N, 4] float32 tensor)."""
+        torch, d = self.torch, self.dims
+        assert hidden.dtype == torch.bfloat16 and W_shard.dtype == torch.bfloat16
+        assert hidden.is_contiguous() and W_shard.is_contiguous()
+        assert tuple(hidden.shape) == (d.N, d.d) and tuple(W_shard.shape) == (d.V, d.d)
+        assert req_offsets.dtype == torch.int32 and req_offsets.numel() == d.R + 1
+        if token_ids is not None:
+            assert token_ids.dtype == torch.int32 and token_ids.numel() == d.N
+        out = self.stats_local if out is None else out
+        assert out.dtype == torch.float32 and out.numel() == d.N * 4 and out.is_contiguous()
+        _check(lib().laser_probe_partial(
+            hidden.data_ptr(), W_shard.data_ptr(), req_offsets.data_ptr(),
+            token_ids.data_ptr() if token_ids is not None else None, C.byref(d), self.v_offset,
+            out.data_ptr(), C.byref(peers) if peers is not None else None,
+            self.workspace.data_ptr(), self.workspace.numel(), self._stream(stream)))
+        return out
+
+    def combine(self, req_offsets, load, params: TauParams, stats_all=None, agg=AGG_MEAN, token_prob=False,
+                stream=None, wait_flags=None, epoch=0):
+        """Merge of the G records per row + a3-a5 -> ProbeOutputs."""
+        torch, d = self.torch, self.dims
+        st = self.stats_all if stats_all is None else stats_all
+        assert st.dtype == torch.float32 and st.numel() == self.world * d.N * 4 and st.is_contiguous()
+        opt = Options(agg, PROB_TOKEN if token_prob else PROB_MAX, None)
+        _check(lib().laser_probe_combine(
+            st.data_ptr(), self.world, req_offsets.data_ptr(), load.data_ptr(), C.byref(params),
+            self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(), C.byref(d),
+            self._stream(stream), self.tau.data_ptr() if self.tau is not None else None,
+            self.pmax.data_ptr() if self.pmax is not None else None, C.byref(opt),
+            wait_flags.data_ptr() if wait_flags is not None else None, epoch))
         return ProbeOutputs(self.conf, self.argmax, self.exit, self.tau, self.pmax)
 
 

@@ -257,6 +257,140 @@ Staging staging_layout(const laser_probe_dims& d) {
     return s;
 }
 
+int options_valid(const laser_probe_options& o, int N) {
+    if (o.aggregate_mode < LASER_AGG_MEAN || o.aggregate_mode > LASER_AGG_MIN) return LASER_E_MODE;
+    if (o.prob_mode < LASER_PROB_MAX || o.prob_mode > LASER_PROB_TOKEN) return LASER_E_MODE;
+    if (o.prob_mode == LASER_PROB_TOKEN && N > 0 && !o.token_ids) return LASER_E_NULL;
+    return LASER_OK;
+}
+
+// sm_100 only, no fallback.
+int require_b200(DeviceInfo** out) {
+    bool ok = false;
+    DeviceInfo* di = current_device(&ok);
+    if (!ok || !di) { g_last_error = "no usable CUDA device"; return LASER_E_CUDA; }
+    if (di->cc_major != 10 || di->cc_minor != 0) return LASER_E_ARCH;
+    *out = di;
+    return LASER_OK;
+}
+
+int units_for(const DeviceInfo* di, bool pair) { return pair ? (di->sms / 2 > 0 ? di->sms / 2 : 1) : di->sms; }
+
+// Enqueue laser_probe_fused_kernel for `dims` (W has dims.V rows; v_offset localises token_ids).
+int launch_fused(DeviceInfo* di, const laser_probe_plan& pl, const void* hidden, const void* W,
+                 const int32_t* req_offsets, const laser_probe_dims& dims, const int32_t* token_ids,
+                 int v_offset, float4* ws, cudaStream_t stream, bool allow_pdl) {
+    const int N = dims.N;
+    const bool pair = pl.cta_pair != 0;
+    static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
+    if (!di->attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(laser_probe_fused_kernel<false>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(laser_probe_fused_kernel<true>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
+        if (e != cudaSuccess) return set_cuda_error("cudaFuncSetAttribute", e);
+        di->attr_set = true;
+    }
+    CUtensorMap tm_h, tm_w;
+    // Fewer than 128 rows in total: stage only the 8-row groups that hold rows.  TMA's zero fill of
+    // out-of-range rows is slow (N = 8: 90 -> 75 us per step at the C2 shape without it).  The
+    // other rows of the A tile keep whatever shared memory held; they feed TMEM lanes whose
+    // statistics nobody reads (rows are independent).
+    const int a_rows = N < kTileM ? round_up(N, 8) : kTileM;
+    int rc = get_tensor_map(hidden, N, dims.d, a_rows, &tm_h);
+    if (rc != LASER_OK) return rc;
+    const int b_rows = pair ? pl.tile_n / 2 : pl.tile_n;   // W rows one CTA stages per tile
+    rc = get_tensor_map(W, dims.V, dims.d, b_rows, &tm_w);
+    if (rc != LASER_OK) return rc;
+
+    FusedParams fp;
+    fp.n_alloc = N; fp.d = dims.d; fp.V = dims.V;
+    fp.m_tiles = pl.m_tiles; fp.splits = pl.ws_splits; fp.tiles_per_split = pl.tiles_per_split;
+    fp.req_offsets = req_offsets; fp.R = dims.R;
+    fp.total_tiles = ceil_div(dims.V, pl.tile_n);
+    fp.units = units_for(di, pair);
+    fp.replan = pl.m_tiles > 1 ? 1 : 0;
+    fp.wait_first = g_overlap.load(std::memory_order_relaxed) ? 0 : 1;
+    fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
+    fp.work_items = pl.work_items; fp.n_pad = pl.m_tiles * pl.tile_m;
+    fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
+    fp.tx_bytes = static_cast<uint32_t>((a_rows + b_rows) * 128);  // OOB rows are zero-filled and still counted
+    // W is streamed once when a single token tile exists; with several token tiles the other
+    // CTAs re-read the same rows from L2, so do not mark them evict-first.
+    fp.w_policy = (pl.m_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
+    fp.ws = ws;
+    fp.token_ids = token_ids;
+    fp.v_offset = v_offset;
+
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(pl.grid);
+    cfg.blockDim = dim3(kFusedThreads);
+    cfg.dynamicSmemBytes = static_cast<size_t>(pl.smem_bytes);
+    cfg.stream = stream;
+    // Programmatic dependent launch: the kernel may start while the previous kernel in the
+    // stream is still running; it executes griddepcontrol.wait before its workspace stores and
+    // before it exits (and before its first global read unless overlap is switched on).
+    cudaLaunchAttribute fattr[2];
+    unsigned na = 0;
+    if (use_pdl && allow_pdl) {
+        fattr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        fattr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (pair) {   // the two CTAs of a pair form a cluster (same TPC)
+        fattr[na].id = cudaLaunchAttributeClusterDimension;
+        fattr[na].val.clusterDim.x = 2;
+        fattr[na].val.clusterDim.y = 1;
+        fattr[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    cfg.attrs = fattr;
+    cfg.numAttrs = na;
+    cudaError_t e = pair ? cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<true>, tm_h, tm_w, fp)
+                         : cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<false>, tm_h, tm_w, fp);
+    if (e != cudaSuccess) return set_cuda_error("launch laser_probe_fused_kernel", e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return LASER_OK;
+}
+
+// The fields of FinalizeParams that describe the fused kernel's workspace for `dims`.
+FinalizeParams finalize_params(const DeviceInfo* di, const laser_probe_plan& pl, const laser_probe_dims& dims,
+                               bool run_fused, const int32_t* req_offsets) {
+    FinalizeParams fz{};
+    fz.n_alloc = dims.N; fz.R = dims.R; fz.splits = pl.ws_splits; fz.n_pad = pl.m_tiles * pl.tile_m;
+    fz.m_tiles = pl.m_tiles; fz.rows_per_item = pl.tile_m;
+    fz.total_tiles = ceil_div(dims.V, pl.tile_n);
+    fz.units = units_for(di, pl.cta_pair != 0);
+    fz.replan = (run_fused && pl.m_tiles > 1) ? 1 : 0;
+    fz.req_offsets = req_offsets;
+    fz.wait_flags = nullptr; fz.epoch = 0; fz.a_offset = 0; fz.prob_mode = 0; fz.agg_mode = 0;
+    return fz;
+}
+
+// Enqueue laser_probe_finalize_kernel: blocks [0, R) aggregate, the rest mark padding rows.
+int launch_finalize(const FinalizeParams& fz, cudaStream_t stream, bool pdl) {
+    const int grid = fz.R + ceil_div(fz.n_alloc, kFinalizeThreads);
+    if (grid <= 0) return LASER_OK;
+    static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kFinalizeThreads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    if (pdl && use_pdl) {
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+    }
+    cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_finalize_kernel, fz);
+    if (e != cudaSuccess) return set_cuda_error("launch laser_probe_finalize_kernel", e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return LASER_OK;
+}
+
 }  // namespace
 
 // ============================================================================================ ABI
@@ -283,16 +417,19 @@ size_t laser_probe_workspace_bytes(const laser_probe_dims* dims) {
     return workspace_bytes_for(pl);
 }
 
-int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t* req_offsets,
+int laser_probe_confidence_opt(const void* hidden, const void* W, const int32_t* req_offsets,
                                const float* load, const laser_tau_params* tau_params,
                                float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
                                const laser_probe_dims* dims, void* workspace,
                                size_t workspace_bytes, void* stream_v, float* out_tau_opt,
-                               float* out_pmax_opt, int aggregate_mode) {
+                               float* out_pmax_opt, const laser_probe_options* options) {
     if (!dims || !tau_params) return LASER_E_NULL;
     if (!dims_valid(dims)) return LASER_E_DIMS;
     if (!params_valid(tau_params)) return LASER_E_PARAMS;
-    if (aggregate_mode < LASER_AGG_MEAN || aggregate_mode > LASER_AGG_MIN) return LASER_E_MODE;
+    laser_probe_options opt{LASER_AGG_MEAN, LASER_PROB_MAX, nullptr};
+    if (options) opt = *options;
+    int rc = options_valid(opt, dims->N);
+    if (rc != LASER_OK) return rc;
     const int N = dims->N, R = dims->R;
     if (N == 0 && R == 0) return LASER_OK;
     if (N > 0 && (!hidden || !W || !out_argmax)) return LASER_E_NULL;
@@ -300,11 +437,9 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
     if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(W) & 15))
         return LASER_E_ALIGN;
 
-    bool ok = false;
-    DeviceInfo* di = current_device(&ok);
-    if (!ok || !di) { g_last_error = "no usable CUDA device"; return LASER_E_CUDA; }
-    if (di->cc_major != 10 || di->cc_minor != 0) return LASER_E_ARCH;  // sm_100a only, no fallback
-
+    DeviceInfo* di = nullptr;
+    rc = require_b200(&di);
+    if (rc != LASER_OK) return rc;
     laser_probe_plan pl;
     make_plan(*dims, di->sms, &pl);
     if (!workspace || workspace_bytes < workspace_bytes_for(pl) ||
@@ -312,123 +447,47 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
         return LASER_E_WORKSPACE;
 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
-    const int n_pad = pl.m_tiles * pl.tile_m;
-    const bool pair = pl.cta_pair != 0;
-    float4* ws = static_cast<float4*>(workspace);
-
     const bool run_fused = (N > 0 && R > 0);
-    static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
     const bool prof = g_prof.on && g_prof.created && run_fused && g_prof.calls < kProfRing;
     const int prof_slot = g_prof.calls;
     if (run_fused) {
-        if (!di->attr_set) {
-            cudaError_t e = cudaFuncSetAttribute(laser_probe_fused_kernel<false>,
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
-            if (e == cudaSuccess)
-                e = cudaFuncSetAttribute(laser_probe_fused_kernel<true>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
-            if (e != cudaSuccess) return set_cuda_error("cudaFuncSetAttribute", e);
-            di->attr_set = true;
-        }
-        CUtensorMap tm_h, tm_w;
-        // Fewer than 128 rows in total: stage only the 8-row groups that hold rows.  TMA's zero fill of
-        // out-of-range rows is slow (N = 8: 90 -> 75 us per step at the C2 shape without it).  The
-        // other rows of the A tile keep whatever shared memory held; they feed TMEM lanes whose
-        // statistics nobody reads (rows are independent).
-        const int a_rows = N < kTileM ? round_up(N, 8) : kTileM;
-        int rc = get_tensor_map(hidden, N, dims->d, a_rows, &tm_h);
-        if (rc != LASER_OK) return rc;
-        const int b_rows = pair ? pl.tile_n / 2 : pl.tile_n;   // W rows one CTA stages per tile
-        rc = get_tensor_map(W, dims->V, dims->d, b_rows, &tm_w);
-        if (rc != LASER_OK) return rc;
-
-        FusedParams fp;
-        fp.n_alloc = N; fp.d = dims->d; fp.V = dims->V;
-        fp.m_tiles = pl.m_tiles; fp.splits = pl.ws_splits; fp.tiles_per_split = pl.tiles_per_split;
-        fp.req_offsets = req_offsets; fp.R = R;
-        fp.total_tiles = ceil_div(dims->V, pl.tile_n);
-        fp.units = pair ? (di->sms / 2 > 0 ? di->sms / 2 : 1) : di->sms;
-        fp.replan = pl.m_tiles > 1 ? 1 : 0;
-        fp.wait_first = g_overlap.load(std::memory_order_relaxed) ? 0 : 1;
-        fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
-        fp.work_items = pl.work_items; fp.n_pad = n_pad;
-        fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
-        fp.tx_bytes = static_cast<uint32_t>((a_rows + b_rows) * 128);  // OOB rows are zero-filled and still counted
-        // W is streamed once when a single token tile exists; with several token tiles the other
-        // CTAs re-read the same rows from L2, so do not mark them evict-first.
-        fp.w_policy = (pl.m_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
-        fp.ws = ws;
-
         if (prof) cudaEventRecord(g_prof.ev[prof_slot][0], stream);
-        cudaLaunchConfig_t cfg{};
-        cfg.gridDim = dim3(pl.grid);
-        cfg.blockDim = dim3(kFusedThreads);
-        cfg.dynamicSmemBytes = static_cast<size_t>(pl.smem_bytes);
-        cfg.stream = stream;
-        // Programmatic dependent launch: the kernel may start while the previous kernel in the
-        // stream is still running; it executes griddepcontrol.wait before its workspace stores and
-        // before it exits (and before its first global read when overlap is switched off).
-        cudaLaunchAttribute fattr[2];
-        unsigned na = 0;
-        if (use_pdl && !prof) {
-            fattr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-            fattr[na].val.programmaticStreamSerializationAllowed = 1;
-            ++na;
-        }
-        if (pair) {   // the two CTAs of a pair form a cluster (same TPC)
-            fattr[na].id = cudaLaunchAttributeClusterDimension;
-            fattr[na].val.clusterDim.x = 2;
-            fattr[na].val.clusterDim.y = 1;
-            fattr[na].val.clusterDim.z = 1;
-            ++na;
-        }
-        cfg.attrs = fattr;
-        cfg.numAttrs = na;
-        cudaError_t e = pair ? cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<true>, tm_h, tm_w, fp)
-                             : cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<false>, tm_h, tm_w, fp);
-        if (e != cudaSuccess) return set_cuda_error("launch laser_probe_fused_kernel", e);
-        g_launches.fetch_add(1, std::memory_order_relaxed);
+        rc = launch_fused(di, pl, hidden, W, req_offsets, *dims,
+                          opt.prob_mode == LASER_PROB_TOKEN ? opt.token_ids : nullptr, 0,
+                          static_cast<float4*>(workspace), stream, !prof);
+        if (rc != LASER_OK) return rc;
     }
 
-    FinalizeParams fz;
-    fz.n_alloc = N; fz.R = run_fused ? R : 0; fz.splits = pl.ws_splits; fz.n_pad = n_pad;
-    fz.m_tiles = pl.m_tiles; fz.rows_per_item = pl.tile_m;
-    fz.total_tiles = ceil_div(dims->V, pl.tile_n);
-    fz.units = pair ? (di->sms / 2 > 0 ? di->sms / 2 : 1) : di->sms;
-    fz.replan = (run_fused && pl.m_tiles > 1) ? 1 : 0;
-    fz.agg_mode = aggregate_mode;
-    fz.ws = ws;
-    fz.req_offsets = req_offsets; fz.load = load;
+    FinalizeParams fz = finalize_params(di, pl, *dims, run_fused, req_offsets);
+    fz.agg_mode = opt.aggregate_mode;
+    fz.prob_mode = opt.prob_mode;
+    fz.ws = static_cast<const float4*>(workspace);
+    fz.row_stride = pl.ws_splits; fz.split_stride = 1;
+    fz.load = load;
     fz.out_conf = out_conf; fz.out_argmax = out_argmax; fz.out_exit = out_exit;
     fz.out_tau = out_tau_opt; fz.out_pmax = out_pmax_opt;
     fz.tau = to_dev(tau_params);
-    const int pad_blocks = ceil_div(N, kFinalizeThreads);
-    if (!run_fused && R > 0) {
-        // N == 0 with R > 0: every request is empty -> conf 0, exit 0, tau still defined.
-        // Handled by the same kernel: req_offsets are all 0, no partials are read.
-        fz.R = R;
-    }
-    const int grid = fz.R + pad_blocks;
-    if (grid > 0) {
-        cudaLaunchConfig_t cfg{};
-        cfg.gridDim = dim3(grid);
-        cfg.blockDim = dim3(kFinalizeThreads);
-        cfg.dynamicSmemBytes = 0;
-        cfg.stream = stream;
-        cudaLaunchAttribute attr[1];
-        if (prof) cudaEventRecord(g_prof.ev[prof_slot][1], stream);
-        if (run_fused && use_pdl && !prof) {
-            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-            attr[0].val.programmaticStreamSerializationAllowed = 1;
-            cfg.attrs = attr;
-            cfg.numAttrs = 1;
-        }
-        cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_finalize_kernel, fz);
-        if (e != cudaSuccess) return set_cuda_error("launch laser_probe_finalize_kernel", e);
-        g_launches.fetch_add(1, std::memory_order_relaxed);
-        if (prof) { cudaEventRecord(g_prof.ev[prof_slot][2], stream); g_prof.calls++; }
-    }
+    // N == 0 with R > 0: every request is empty -> conf 0, exit 0, tau still defined.  Handled by the
+    // same kernel: req_offsets are all 0, no partials are read.
+    fz.R = R;
+    if (!run_fused && R == 0) fz.R = 0;
+    if (prof) cudaEventRecord(g_prof.ev[prof_slot][1], stream);
+    rc = launch_finalize(fz, stream, run_fused && !prof);
+    if (rc != LASER_OK) return rc;
+    if (prof) { cudaEventRecord(g_prof.ev[prof_slot][2], stream); g_prof.calls++; }
     return LASER_OK;
+}
+
+int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t* req_offsets,
+                               const float* load, const laser_tau_params* tau_params,
+                               float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+                               const laser_probe_dims* dims, void* workspace,
+                               size_t workspace_bytes, void* stream, float* out_tau_opt,
+                               float* out_pmax_opt, int aggregate_mode) {
+    const laser_probe_options opt{aggregate_mode, LASER_PROB_MAX, nullptr};
+    return laser_probe_confidence_opt(hidden, W, req_offsets, load, tau_params, out_conf, out_argmax,
+                                      out_exit, dims, workspace, workspace_bytes, stream, out_tau_opt,
+                                      out_pmax_opt, &opt);
 }
 
 int laser_probe_confidence(const void* hidden, const void* W, const int32_t* req_offsets,
@@ -436,9 +495,125 @@ int laser_probe_confidence(const void* hidden, const void* W, const int32_t* req
                            int32_t* out_argmax, uint8_t* out_exit, const laser_probe_dims* dims,
                            void* workspace, size_t workspace_bytes, void* stream,
                            float* out_tau_opt, float* out_pmax_opt) {
-    return laser_probe_confidence_agg(hidden, W, req_offsets, load, tau_params, out_conf, out_argmax,
-                                      out_exit, dims, workspace, workspace_bytes, stream,
-                                      out_tau_opt, out_pmax_opt, LASER_AGG_MEAN);
+    return laser_probe_confidence_opt(hidden, W, req_offsets, load, tau_params, out_conf, out_argmax,
+                                      out_exit, dims, workspace, workspace_bytes, stream, out_tau_opt,
+                                      out_pmax_opt, nullptr);
+}
+
+// ------------------------------------------------------------------------------ vocabulary-parallel
+int laser_probe_partial(const void* hidden, const void* W_shard, const int32_t* req_offsets,
+                        const int32_t* token_ids_opt, const laser_probe_dims* dims, int32_t v_offset,
+                        laser_row_stats* out_stats, const laser_probe_peers* peers_opt,
+                        void* workspace, size_t workspace_bytes, void* stream_v) {
+    if (!dims) return LASER_E_NULL;
+    if (!dims_valid(dims) || v_offset < 0) return LASER_E_DIMS;
+    if (!out_stats && !peers_opt) return LASER_E_NULL;
+    if (peers_opt) {
+        const laser_probe_peers& pe = *peers_opt;
+        if (pe.world < 1 || pe.world > LASER_MAX_PEERS || pe.rank < 0 || pe.rank >= pe.world || pe.epoch == 0)
+            return LASER_E_PARAMS;
+        for (int g = 0; g < pe.world; ++g)
+            if (!pe.peer_stats[g] || !pe.peer_flags[g]) return LASER_E_NULL;
+    }
+    const int N = dims->N, R = dims->R;
+    if (N > 0 && (!hidden || !W_shard)) return LASER_E_NULL;
+    if (R > 0 && !req_offsets) return LASER_E_NULL;
+    if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(W_shard) & 15) ||
+        (reinterpret_cast<uintptr_t>(out_stats) & 15))
+        return LASER_E_ALIGN;
+    DeviceInfo* di = nullptr;
+    int rc = require_b200(&di);
+    if (rc != LASER_OK) return rc;
+    laser_probe_plan pl;
+    make_plan(*dims, di->sms, &pl);
+    if (!workspace || workspace_bytes < workspace_bytes_for(pl) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 15))
+        return LASER_E_WORKSPACE;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+    const bool run_fused = (N > 0 && R > 0);
+    if (run_fused) {
+        rc = launch_fused(di, pl, hidden, W_shard, req_offsets, *dims, token_ids_opt, v_offset,
+                          static_cast<float4*>(workspace), stream, true);
+        if (rc != LASER_OK) return rc;
+    }
+    if (N > 0) {
+        ReduceParams rq{};
+        rq.f = finalize_params(di, pl, *dims, run_fused, req_offsets);
+        rq.f.R = run_fused ? R : 0;            // R == 0: every row is padding -> neutral records
+        rq.f.ws = static_cast<const float4*>(workspace);
+        rq.f.row_stride = pl.ws_splits; rq.f.split_stride = 1;
+        rq.f.a_offset = v_offset;
+        rq.out_stats = reinterpret_cast<float4*>(out_stats);
+        rq.rank = peers_opt ? peers_opt->rank : 0;
+        rq.world = peers_opt ? peers_opt->world : 0;
+        for (int g = 0; g < rq.world; ++g) rq.peer_stats[g] = reinterpret_cast<float4*>(peers_opt->peer_stats[g]);
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(ceil_div(N, kFinalizeWarps));
+        cfg.blockDim = dim3(kFinalizeThreads);
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
+        if (run_fused && use_pdl) {
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+        }
+        cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_reduce_kernel, rq);
+        if (e != cudaSuccess) return set_cuda_error("launch laser_probe_reduce_kernel", e);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    if (peers_opt) {
+        // Plain launch (full stream order): the reduce kernel's stores, remote ones included, have
+        // been performed when this kernel starts; it publishes the epoch on every GPU.
+        SignalParams sg{};
+        sg.rank = peers_opt->rank; sg.world = peers_opt->world; sg.epoch = peers_opt->epoch;
+        for (int g = 0; g < sg.world; ++g) sg.peer_flags[g] = peers_opt->peer_flags[g];
+        laser_probe_signal_kernel<<<1, 32, 0, stream>>>(sg);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return set_cuda_error("launch laser_probe_signal_kernel", e);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+    }
+    return LASER_OK;
+}
+
+int laser_probe_combine(const laser_row_stats* stats, int32_t G, const int32_t* req_offsets,
+                        const float* load, const laser_tau_params* tau_params, float* out_conf,
+                        int32_t* out_argmax, uint8_t* out_exit, const laser_probe_dims* dims,
+                        void* stream_v, float* out_tau_opt, float* out_pmax_opt,
+                        const laser_probe_options* options, const uint32_t* wait_flags_opt,
+                        uint32_t epoch) {
+    if (!dims || !tau_params) return LASER_E_NULL;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
+    if (G < 1 || G > LASER_MAX_PEERS) return LASER_E_DIMS;
+    if (!params_valid(tau_params)) return LASER_E_PARAMS;
+    laser_probe_options opt{LASER_AGG_MEAN, LASER_PROB_MAX, nullptr};
+    if (options) opt = *options;
+    if (opt.aggregate_mode < LASER_AGG_MEAN || opt.aggregate_mode > LASER_AGG_MIN ||
+        opt.prob_mode < LASER_PROB_MAX || opt.prob_mode > LASER_PROB_TOKEN)
+        return LASER_E_MODE;
+    const int N = dims->N, R = dims->R;
+    if (N == 0 && R == 0) return LASER_OK;
+    if (N > 0 && (!stats || !out_argmax)) return LASER_E_NULL;
+    if (R > 0 && (!req_offsets || !load || !out_conf || !out_exit)) return LASER_E_NULL;
+    if (reinterpret_cast<uintptr_t>(stats) & 15) return LASER_E_ALIGN;
+    DeviceInfo* di = nullptr;
+    int rc = require_b200(&di);
+    if (rc != LASER_OK) return rc;
+    FinalizeParams fz{};
+    fz.n_alloc = N; fz.R = R; fz.splits = G; fz.n_pad = N;
+    fz.m_tiles = 1; fz.rows_per_item = kTileM; fz.total_tiles = 1; fz.units = 1; fz.replan = 0;
+    fz.agg_mode = opt.aggregate_mode;
+    fz.prob_mode = opt.prob_mode;
+    fz.a_offset = 0;
+    fz.ws = reinterpret_cast<const float4*>(stats);
+    fz.row_stride = 1; fz.split_stride = N;
+    fz.wait_flags = wait_flags_opt; fz.epoch = epoch;
+    fz.req_offsets = req_offsets; fz.load = load;
+    fz.out_conf = out_conf; fz.out_argmax = out_argmax; fz.out_exit = out_exit;
+    fz.out_tau = out_tau_opt; fz.out_pmax = out_pmax_opt;
+    fz.tau = to_dev(tau_params);
+    return launch_finalize(fz, static_cast<cudaStream_t>(stream_v), false);
 }
 
 size_t laser_probe_staging_bytes(const laser_probe_dims* dims) {

@@ -70,7 +70,11 @@ struct FusedParams {
     uint32_t tx_bytes;     // bytes TMA delivers per stage and CTA (hidden box + W box)
     uint32_t stage_bytes;  // shared-memory stride of a stage: kABytes + (W rows per CTA) * 128
     uint64_t w_policy;     // L2 eviction policy for the W stream
-    float4* ws;            // [n_pad, splits] per (row, split): {max, sum exp(logit - max), argmax bits, 0}
+    float4* ws;            // [n_pad, splits] per (row, split): {max, sum exp(logit - max), argmax bits, token logit}
+    // LASER_PROB_TOKEN: token_ids[n] - v_offset is the column of W whose logit is kept for row n
+    // (nullptr: no token logit is tracked; v_offset = global vocabulary index of W's row 0).
+    const int32_t* token_ids;
+    int32_t v_offset;
     // Padding-aware re-planning (m_tiles > 1 only): token items at or beyond req_offsets[R] are
     // skipped and the vocabulary tiles are re-dealt over the remaining items; `splits` above stays
     // the record stride (the largest split count any item count can produce).
@@ -103,9 +107,11 @@ __device__ __forceinline__ uint32_t make_idesc_bf16(uint32_t n, uint32_t m) {
 // the running statistics (m, a, s):  m = max, a = lowest index attaining it, s = sum 2^{(x-m)log2e}.
 // Columns are visited in ascending vocabulary order and the update is strict (>), so ties keep the
 // lowest index.  Columns v >= V (TMA zero fill past the end of W) are masked out.
+// tok is the row's token column (LASER_PROB_TOKEN; negative = none): its logit is copied to lt when
+// this chunk holds it (once per row and vocabulary sweep).
 template <int NC>
 __device__ __forceinline__ void fold_columns(const uint32_t (&r)[NC], int vbase, int V, float& m,
-                                             int& a, float& s) {
+                                             int& a, float& s, int tok, float& lt) {
     float x[NC];
 #pragma unroll
     for (int j = 0; j < NC; ++j) x[j] = __uint_as_float(r[j]);
@@ -113,6 +119,12 @@ __device__ __forceinline__ void fold_columns(const uint32_t (&r)[NC], int vbase,
 #pragma unroll
         for (int j = 0; j < NC; ++j)
             if (vbase + j >= V) x[j] = -CUDART_INF_F;
+    }
+    const unsigned dt = static_cast<unsigned>(tok - vbase);
+    if (dt < static_cast<unsigned>(NC)) {
+#pragma unroll
+        for (int j = 0; j < NC; ++j)
+            if (static_cast<unsigned>(j) == dt) lt = x[j];
     }
     float c0 = x[0], c1 = x[1], c2 = x[2], c3 = x[3];
 #pragma unroll
@@ -314,8 +326,15 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         uint32_t acc = 0;
         for (int w = unit; w < work_items; w += units) {
             const int mt = w % m_items, sp = w / m_items;
-            float m = -CUDART_INF_F, s = 0.f;
-            int a = -1;
+            float m = -CUDART_INF_F, s = 0.f, lt = -CUDART_INF_F;
+            int a = -1, tok = -1;
+            if (p.token_ids != nullptr) {
+                const int n = mt * kRowsPerItem + row;
+                if (n < p.n_alloc) {
+                    const int t = __ldg(p.token_ids + n) - p.v_offset;
+                    tok = (t >= 0 && t < p.V) ? t : -1;   // not in this (shard of the) vocabulary
+                }
+            }
             for (int tile = sp; tile < total_tiles; tile += S, ++acc) {
                 const uint32_t buf = acc & 1u, aphase = (acc >> 1) & 1u;
                 ptx::mbar_wait(tfull_bar(buf), aphase);
@@ -327,14 +346,14 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                     uint32_t r[32];
                     ptx::tmem_ld_x32(taddr + c, r);
                     ptx::tmem_wait_ld();
-                    fold_columns<32>(r, vt + c, p.V, m, a, s);
+                    fold_columns<32>(r, vt + c, p.V, m, a, s, tok, lt);
                 }
                 // tile_n is a multiple of 16: at most one 16-column tail chunk
                 if (c + 16 == BN && vt + c < p.V) {
                     uint32_t r[16];
                     ptx::tmem_ld_x16(taddr + c, r);
                     ptx::tmem_wait_ld();
-                    fold_columns<16>(r, vt + c, p.V, m, a, s);
+                    fold_columns<16>(r, vt + c, p.V, m, a, s, tok, lt);
                 }
                 // all of this warp's TMEM reads have completed (wait::ld): one arrival per warp
                 ptx::tc_fence_before();
@@ -348,7 +367,7 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             // records (coalesced); the scattered 16-byte stores here are fire-and-forget
             const size_t o = (static_cast<size_t>(mt) * kRowsPerItem + row) * p.splits + sp;
             ptx::pdl_wait();   // the previous call's finalize kernel may still be reading the workspace
-            p.ws[o] = make_float4(m, s, __int_as_float(a), 0.f);
+            p.ws[o] = make_float4(m, s, __int_as_float(a), lt);
         }
     }
 
@@ -379,9 +398,23 @@ __host__ __device__ __forceinline__ float tau_eval(float load, const TauParamsDe
     return lam;
 }
 
+// One 16-byte record of online-softmax statistics: what the fused kernel leaves per (row, split) in
+// the workspace, what laser_probe_partial leaves per row of a vocabulary shard, and what
+// laser_probe_combine merges.  Same layout as laser_row_stats in include/laser_probe.h.
+//   x = max logit, y = sum exp(logit - max), z = argmax (int bits), w = logit of the row's token
 struct FinalizeParams {
     int32_t n_alloc, R, splits, n_pad, agg_mode;
     int32_t m_tiles, rows_per_item, total_tiles, units, replan;   // see FusedParams
+    // record (n, sp) lives at ws[n * row_stride + sp * split_stride]:
+    //   fused workspace [n_pad, splits]: row_stride = splits, split_stride = 1
+    //   gathered shard statistics [G, N]: row_stride = 1, split_stride = N  (laser_probe_combine)
+    int64_t row_stride, split_stride;
+    int32_t prob_mode;            // 0: row maximum 1/S; 1: the row's token exp(l_tok - m)/S
+    int32_t a_offset;             // added to every argmax (vocabulary shard offset; reduce kernel)
+    // laser_probe_combine over peer-pushed statistics: wait until flags[g] has reached `epoch` for
+    // every g < splits before reading (nullptr: the records are already complete in stream order).
+    const uint32_t* wait_flags;
+    uint32_t epoch;
     const float4* ws;
     const int32_t* req_offsets;
     const float* load;
@@ -393,8 +426,10 @@ struct FinalizeParams {
     TauParamsDev tau;
 };
 
-// (m,a,s) (+) (m',a',s'): commutative form — on equal maxima the smaller vocabulary index wins.
-__device__ __forceinline__ void merge_stats(float& m, int& a, float& s, float m2, int a2, float s2) {
+// (m,a,s,lt) (+) (m',a',s',lt'): commutative form - on equal maxima the smaller vocabulary index
+// wins; at most one operand carries a finite token logit.
+__device__ __forceinline__ void merge_stats(float& m, int& a, float& s, float& lt, float m2, int a2,
+                                            float s2, float lt2) {
     const float M = fmaxf(m, m2);
     const int an = (m > m2) ? a : ((m2 > m) ? a2 : min(a, a2));
     const float e1 = (m == M) ? 1.f : ptx::ex2_approx((m - M) * kLog2e);
@@ -402,15 +437,63 @@ __device__ __forceinline__ void merge_stats(float& m, int& a, float& s, float m2
     s = s * e1 + s2 * e2;
     m = M;
     a = an;
+    lt = fmaxf(lt, lt2);
 }
 
 constexpr int kFinalizeThreads = 256;
 constexpr int kFinalizeWarps = kFinalizeThreads / 32;
 constexpr int kMergeBatch = 5;  // partials a lane loads before it starts merging (148 splits: one batch)
 
+// Merge the nsplit records of one row across a warp (lanes stride over the records, loads issued in
+// batches so that they overlap; then shuffles).  Every lane returns the merged statistics.
+__device__ __forceinline__ void merge_row(const float4* rec, int64_t split_stride, int nsplit, int lane,
+                                          float& m, int& a, float& s, float& lt) {
+    m = -CUDART_INF_F; s = 0.f; lt = -CUDART_INF_F;
+    a = 0x7fffffff;
+    for (int sp0 = lane; sp0 < nsplit; sp0 += 32 * kMergeBatch) {
+        float4 v[kMergeBatch];
+#pragma unroll
+        for (int j = 0; j < kMergeBatch; ++j) {
+            const int sp = sp0 + 32 * j;
+            v[j] = sp < nsplit ? rec[sp * split_stride]
+                               : make_float4(-CUDART_INF_F, 0.f, __int_as_float(0x7fffffff), -CUDART_INF_F);
+        }
+#pragma unroll
+        for (int j = 0; j < kMergeBatch; ++j)
+            merge_stats(m, a, s, lt, v[j].x, __float_as_int(v[j].z), v[j].y, v[j].w);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const float m2 = __shfl_xor_sync(0xffffffffu, m, off);
+        const int a2 = __shfl_xor_sync(0xffffffffu, a, off);
+        const float s2 = __shfl_xor_sync(0xffffffffu, s, off);
+        const float l2 = __shfl_xor_sync(0xffffffffu, lt, off);
+        merge_stats(m, a, s, lt, m2, a2, s2, l2);
+    }
+}
+
+// Records per row the fused kernel wrote for this batch (device-side re-plan, see FusedParams).
+__device__ __forceinline__ int records_per_row(const FinalizeParams& p) {
+    int nsplit = p.splits;
+    if (p.replan) {
+        const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
+        const int m_items = (n_valid + p.rows_per_item - 1) / p.rows_per_item;
+        if (m_items > 0) nsplit = plan_splits(p.total_tiles, min(m_items, p.m_tiles), p.units).splits;
+    }
+    return nsplit;
+}
+
+// Spin until every peer's flag has reached `epoch` (peer GPUs store them with system scope after
+// their statistics have landed here).  One thread per flag, then a block barrier.
+__device__ __forceinline__ void wait_peer_flags(const uint32_t* flags, int G, uint32_t epoch) {
+    if (static_cast<int>(threadIdx.x) < G) {
+        while (static_cast<int32_t>(ptx::ld_acquire_sys_u32(flags + threadIdx.x) - epoch) < 0) __nanosleep(64);
+    }
+    __syncthreads();
+}
+
 // Blocks [0, R): one request each.  A warp takes rows b+w, b+w+8, ...: its lanes stride over the
-// vocabulary splits of the row (loads issued in batches so that they overlap), fold their own
-// partials, then merge across the warp with shuffles.
+// records of the row, fold their own, then merge across the warp with shuffles.
 // Blocks [R, R + ceil(n_alloc/256)): mark padding rows (n >= req_offsets[R]).
 // Everything that does not depend on the fused kernel (offsets, load, threshold) is read before
 // griddepcontrol.wait so that under programmatic dependent launch it overlaps the fused kernel.
@@ -435,49 +518,33 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
     const int b = __ldg(p.req_offsets + r), e = __ldg(p.req_offsets + r + 1);
     float tau = 0.f;
     if (threadIdx.x == 0) tau = tau_eval(__ldg(p.load + r), p.tau);   // a4
-    int nsplit = p.splits;   // records per row the fused kernel wrote
-    if (p.replan) {
-        const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
-        const int m_items = (n_valid + p.rows_per_item - 1) / p.rows_per_item;
-        if (m_items > 0) nsplit = plan_splits(p.total_tiles, min(m_items, p.m_tiles), p.units).splits;
-    }
+    const int nsplit = records_per_row(p);
 
     ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
+    if (p.wait_flags != nullptr) wait_peer_flags(p.wait_flags, nsplit, p.epoch);
 
     // running aggregate of this warp's rows: sum (mean), sum of logs (geomean), min
     float acc = (p.agg_mode == 2) ? CUDART_INF_F : 0.f;
     bool any_nan = false;
     for (int n = b + warp; n < e; n += kFinalizeWarps) {
-        float m = -CUDART_INF_F, s = 0.f;
-        int a = 0x7fffffff;
-        const float4* rec = p.ws + static_cast<size_t>(n) * p.splits;
-        for (int sp0 = lane; sp0 < nsplit; sp0 += 32 * kMergeBatch) {
-            float4 v[kMergeBatch];
-#pragma unroll
-            for (int j = 0; j < kMergeBatch; ++j) {
-                const int sp = sp0 + 32 * j;
-                v[j] = sp < nsplit ? rec[sp] : make_float4(-CUDART_INF_F, 0.f, __int_as_float(0x7fffffff), 0.f);
-            }
-#pragma unroll
-            for (int j = 0; j < kMergeBatch; ++j) merge_stats(m, a, s, v[j].x, __float_as_int(v[j].z), v[j].y);
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            const float m2 = __shfl_xor_sync(0xffffffffu, m, off);
-            const int a2 = __shfl_xor_sync(0xffffffffu, a, off);
-            const float s2 = __shfl_xor_sync(0xffffffffu, s, off);
-            merge_stats(m, a, s, m2, a2, s2);
-        }
+        float m, s, lt;
+        int a;
+        merge_row(p.ws + static_cast<int64_t>(n) * p.row_stride, p.split_stride, nsplit, lane, m, a, s, lt);
         // s >= 1 up to the rounding of ex2.approx; a probability does not exceed 1.  NaN stays NaN.
-        const float pmax = (s == s) ? fminf(1.0f / s, 1.0f) : CUDART_NAN_F;
+        float prob;
+        if (p.prob_mode == 0) {
+            prob = (s == s) ? fminf(1.0f / s, 1.0f) : CUDART_NAN_F;
+        } else {   // the row's token: exp(l_tok - m) / S; a token outside the vocabulary has l_tok = -inf -> 0
+            prob = (s == s) ? fminf(ptx::ex2_approx((lt - m) * kLog2e) / s, 1.0f) : CUDART_NAN_F;
+        }
         if (lane == 0) {
             p.out_argmax[n] = a;
-            if (p.out_pmax) p.out_pmax[n] = pmax;
+            if (p.out_pmax) p.out_pmax[n] = prob;
         }
-        any_nan |= (pmax != pmax);
-        if (p.agg_mode == 0) acc += pmax;
-        else if (p.agg_mode == 1) acc += logf(pmax);
-        else acc = fminf(acc, pmax);
+        any_nan |= (prob != prob);
+        if (p.agg_mode == 0) acc += prob;
+        else if (p.agg_mode == 1) acc += logf(prob);
+        else acc = fminf(acc, prob);
     }
     if (p.agg_mode == 2 && any_nan) acc = CUDART_NAN_F;
     if (lane == 0) warp_acc[warp] = acc;
@@ -504,6 +571,58 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
         p.out_conf[r] = conf;                  // a3
         p.out_exit[r] = (conf > tau) ? 1 : 0;  // a5: strict; NaN > tau is false
         if (p.out_tau) p.out_tau[r] = tau;
+    }
+}
+
+// ---------------------------------------------------------------------------------- vocab-parallel
+// laser_probe_partial: the fused kernel over one vocabulary SHARD, then this kernel: one warp per row
+// merges the row's split records into a single record {m, S, argmax + v_offset, l_tok} and stores it
+//   * to out_stats[n] (local), and
+//   * when peers are given, to slot [rank, n] of every GPU's gathered buffer [G, N] through
+//     peer-mapped pointers (NVLink stores; 16 bytes per row and peer) - the all-gather of the
+//     statistics is done by the producer, no collective call.
+// Rows n >= req_offsets[R] (padding) get the neutral record.
+constexpr int kMaxPeers = 16;
+struct ReduceParams {
+    FinalizeParams f;          // ws, strides, replan fields, req_offsets, R, n_alloc, a_offset
+    float4* out_stats;         // [n_alloc] or nullptr
+    int32_t rank, world;       // world = 0: no peers
+    float4* peer_stats[kMaxPeers];   // peer_stats[g] = base of GPU g's gathered buffer [world, n_alloc]
+};
+
+__global__ void __launch_bounds__(kFinalizeThreads)
+laser_probe_reduce_kernel(const ReduceParams q) {
+    const FinalizeParams& p = q.f;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    ptx::pdl_launch_dependents();
+    const int n = blockIdx.x * kFinalizeWarps + warp;
+    const int n_valid = (p.R > 0) ? min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc) : 0;
+    const int nsplit = records_per_row(p);
+    ptx::pdl_wait();
+    if (n >= p.n_alloc) return;
+    float m = -CUDART_INF_F, s = 0.f, lt = -CUDART_INF_F;
+    int a = 0x7fffffff;
+    if (n < n_valid) {
+        merge_row(p.ws + static_cast<int64_t>(n) * p.row_stride, p.split_stride, nsplit, lane, m, a, s, lt);
+        a += p.a_offset;
+    }
+    const float4 rec = make_float4(m, s, __int_as_float(a), lt);
+    if (lane == 0 && q.out_stats) q.out_stats[n] = rec;
+    if (lane < q.world) q.peer_stats[lane][static_cast<int64_t>(q.rank) * p.n_alloc + n] = rec;
+}
+
+// After the reduce kernel (stream order: its stores, remote ones included, have been performed):
+// publish `epoch` in slot [rank] of every GPU's flag array with a system-scope release store.
+struct SignalParams {
+    int32_t rank, world;
+    uint32_t epoch;
+    uint32_t* peer_flags[kMaxPeers];   // peer_flags[g] = GPU g's flag array [world]
+};
+__global__ void laser_probe_signal_kernel(const SignalParams q) {
+    const int g = threadIdx.x;
+    if (g < q.world) {
+        __threadfence_system();
+        ptx::st_release_sys_u32(q.peer_flags[g] + q.rank, q.epoch);
     }
 }
 

@@ -162,3 +162,19 @@ def test_ema_and_budget_match_oracle():
     want = oracle.budget(pt.astype(np.float64), Lr.astype(np.float64), q)
     assert np.array_equal(got, want)
     assert got.min() >= 2 and got.max() <= 15
+
+
+def test_partial_combine_validation_needs_no_gpu():
+    import ctypes as C
+    from paper_2606_31580_b200 import binding as B
+    L = B.lib()
+    d = B.Dims(8, 64, 100, 1)
+    tp = B.TauParams()
+    assert L.laser_probe_partial(None, None, None, None, C.byref(d), 0, None, None, None, 0, None) == -1
+    assert L.laser_probe_partial(None, None, None, None, C.byref(d), -1, None, None, None, 0, None) == -2
+    assert L.laser_probe_combine(None, 0, None, None, C.byref(tp), None, None, None, C.byref(d), None, None,
+                                 None, None, None, 0) == -2
+    assert L.laser_probe_combine(None, 17, None, None, C.byref(tp), None, None, None, C.byref(d), None, None,
+                                 None, None, None, 0) == -2
+    assert L.laser_probe_combine(None, 2, None, None, C.byref(tp), None, None, None, C.byref(d), None, None,
+                                 None, None, None, 0) == -1

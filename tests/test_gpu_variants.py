@@ -1,0 +1,229 @@
+"""GPU parity of the widened rows (SURVEY §8 f): LASER_PROB_TOKEN (probability of the emitted token,
+DESIGN A2) and the vocabulary-parallel probe (laser_probe_partial / laser_probe_combine, §8 e), each
+against the fp64 oracle on the same seeded inputs.  All tests need a B200 (`-m gpu`).
+
+The vocabulary-parallel path is exercised on ONE GPU by running the G shards' partial calls one
+after the other on one stream (no kernel waits for another): what is tested is every byte of the data
+path - shard-local statistics, global argmax offsets, token localisation, record layout [G, N], the
+merge - not cross-GPU memory visibility, which needs more than one GPU."""
+import numpy as np
+import pytest
+
+from paper_2606_31580_b200 import parallel as par, workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import _parity as p
+    return p
+
+
+def _token_ids(w, ora, seed):
+    """A mix per row: the oracle's argmax (greedy decoding), the planted token, a random token, and
+    ids outside the vocabulary."""
+    rng = np.random.default_rng(seed)
+    N = w.N_alloc
+    tok = rng.integers(0, w.V, size=N).astype(np.int64)
+    kind = rng.integers(0, 4, size=N)
+    am = np.where(ora.argmax >= 0, ora.argmax, 0)
+    tok = np.where(kind == 0, am, tok)
+    if w.planted is not None:
+        tok = np.where((kind == 1) & (w.planted >= 0), w.planted, tok)
+    oov = rng.random(N) < 0.05
+    tok = np.where(oov, rng.choice([-1, -7, w.V, w.V + 5, 2**31 - 1], size=N), tok)
+    return tok.astype(np.int32)
+
+
+def _oracle_token_mode(w, ora, tok, agg):
+    """Oracle result for LASER_PROB_TOKEN: token probabilities -> aggregate -> exit (tau unchanged)."""
+    import oracle
+    nv = w.N_valid
+    pt = np.full(w.N_alloc, np.nan)
+    if nv:
+        pt[:nv] = oracle.token_prob(w.hidden_f32()[:nv], w.W_f32(), tok[:nv])
+    conf = oracle.aggregate(np.nan_to_num(pt, nan=0.0), w.req_offsets, mode=agg)
+    ex, margin = oracle.exit_mask(conf, ora.tau)
+    return pt, conf, ex, margin
+
+
+def _compare_token_mode(P, w, g, ora, pt, conf, ex, margin, label):
+    nv = w.N_valid
+    # argmax is still the row argmax
+    mism = g.argmax[:nv] != ora.argmax[:nv]
+    assert not (mism & ~(ora.gap2[:nv] < P.GAP_EXEMPT)).any(), f"{label}: argmax"
+    assert np.all(g.argmax[nv:] == -1)
+    dp = np.abs(g.pmax[:nv].astype(np.float64) - pt[:nv])
+    assert np.all(dp <= P.PMAX_TOL), f"{label}: token prob error {dp.max():.3e} at row {dp.argmax()}"
+    dc = np.abs(g.conf.astype(np.float64) - conf)
+    assert np.all(dc <= P.CONF_TOL), f"{label}: conf error {dc.max():.3e}"
+    bad = (g.exit != ex) & ~(margin <= P.MARGIN_EXEMPT)
+    assert not bad.any(), f"{label}: exit mismatch on {np.nonzero(bad)[0][:8]}"
+    return dict(max_ptok_err=float(dp.max()) if dp.size else 0.0, max_conf_err=float(dc.max()) if dc.size else 0.0,
+                exits=int(ex.sum()), requests_exempt=int((margin <= P.MARGIN_EXEMPT).sum()))
+
+
+@pytest.mark.parametrize("agg", [0, 1])
+@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
+    (33000, 512, 12, 8, None, None),          # one token tile, several vocabulary tiles, ragged V
+    (9000, 256, 40, None, 400, (1, 16)),      # several token tiles (pair variant), padding rows
+    (1000, 64, 8, 4, None, None),             # C1 shape
+])
+def test_token_prob_mode(P, V, d, R, L, n_alloc, var_len, agg):
+    """LASER_PROB_TOKEN: conf aggregates softmax(logits)[token_ids[n]] instead of the row maximum."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    w = wl.scaled(f"tok-V{V}", V, d, 0.05, R, L, seed=77, N_alloc=n_alloc, var_len=var_len)
+    ora, rows, reqs = P.run_oracle(w)
+    tok = _token_ids(w, ora, seed=5)
+    pt, conf, ex, margin = _oracle_token_mode(w, ora, tok, agg)
+    dev = P.to_device(w)
+    probe = B.Probe(w.N_alloc, w.d, w.V, w.R)
+    probe.conf.fill_(-7.0); probe.argmax.fill_(-7); probe.exit.fill_(7); probe.pmax.fill_(-7.0)
+    out = probe(dev["hidden"], dev["W"], dev["off"], dev["load"], B.TauParams(**w.tau_params), agg=agg,
+                token_ids=torch.from_numpy(tok).cuda())
+    torch.cuda.synchronize()
+    g = P.GpuRun(out.conf.cpu().numpy(), out.argmax.cpu().numpy(), out.exit.cpu().numpy(),
+                 out.tau.cpu().numpy(), out.pmax.cpu().numpy(), probe.plan)
+    st = _compare_token_mode(P, w, g, ora, pt, conf, ex, margin, w.name)
+    print(w.name, agg, st)
+    # greedy decoding: token = argmax => identical to the default mode
+    out2 = probe(dev["hidden"], dev["W"], dev["off"], dev["load"], B.TauParams(**w.tau_params), agg=agg,
+                 token_ids=out.argmax.clone())
+    torch.cuda.synchronize()
+    pm_tok = out2.pmax.cpu().numpy().copy()
+    out3 = probe(dev["hidden"], dev["W"], dev["off"], dev["load"], B.TauParams(**w.tau_params), agg=agg)
+    torch.cuda.synchronize()
+    nv = w.N_valid
+    np.testing.assert_allclose(pm_tok[:nv], out3.pmax.cpu().numpy()[:nv], rtol=2e-6, atol=0)
+
+
+def test_token_prob_c2_shape(P, c2_W_bits):
+    """Full C2 shape, the launch configuration bench.py times: token mode on planted / random tokens."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    w = wl.config_c2(c2_W_bits)
+    ora, rows, reqs = P.run_oracle(w)
+    tok = _token_ids(w, ora, seed=6)
+    pt, conf, ex, margin = _oracle_token_mode(w, ora, tok, 0)
+    dev = P.to_device(w)
+    probe = B.Probe(w.N_alloc, w.d, w.V, w.R)
+    out = probe(dev["hidden"], dev["W"], dev["off"], dev["load"], B.TauParams(**w.tau_params),
+                token_ids=torch.from_numpy(tok).cuda())
+    torch.cuda.synchronize()
+    g = P.GpuRun(out.conf.cpu().numpy(), out.argmax.cpu().numpy(), out.exit.cpu().numpy(),
+                 out.tau.cpu().numpy(), out.pmax.cpu().numpy(), probe.plan)
+    print("tok-c2", _compare_token_mode(P, w, g, ora, pt, conf, ex, margin, "tok-c2"))
+
+
+def test_token_mode_needs_token_ids(P):
+    import ctypes as C
+    from paper_2606_31580_b200 import binding as B
+    w = wl.config_c1()
+    dev = P.to_device(w)
+    probe = B.Probe(w.N_alloc, w.d, w.V, w.R)
+    opt = B.Options(0, B.PROB_TOKEN, None)
+    tp = B.TauParams(**w.tau_params)
+    rc = B.lib().laser_probe_confidence_opt(
+        dev["hidden"].data_ptr(), dev["W"].data_ptr(), dev["off"].data_ptr(), dev["load"].data_ptr(),
+        C.byref(tp), probe.conf.data_ptr(), probe.argmax.data_ptr(), probe.exit.data_ptr(),
+        C.byref(probe.dims), probe.workspace.data_ptr(), probe.workspace.numel(), None, None, None, C.byref(opt))
+    assert rc == -1
+    opt = B.Options(0, 5, None)
+    rc = B.lib().laser_probe_confidence_opt(
+        dev["hidden"].data_ptr(), dev["W"].data_ptr(), dev["off"].data_ptr(), dev["load"].data_ptr(),
+        C.byref(tp), probe.conf.data_ptr(), probe.argmax.data_ptr(), probe.exit.data_ptr(),
+        C.byref(probe.dims), probe.workspace.data_ptr(), probe.workspace.numel(), None, None, None, C.byref(opt))
+    assert rc == -8
+
+
+# ------------------------------------------------------------------------------- vocabulary-parallel
+def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False):
+    """G virtual ranks on one GPU, one after the other on one stream."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    dev = P.to_device(w)
+    tok_d = torch.from_numpy(tok).cuda() if tok is not None else None
+    tp = B.TauParams(**w.tau_params)
+    N = w.N_alloc
+    stats_all = torch.full((G, N, 4), 123.0, dtype=torch.float32, device="cuda")   # poisoned
+    flags = torch.zeros(G, dtype=torch.int32, device="cuda")
+    shards = []
+    for g in range(G):
+        v0, v1 = par.shard_vocab(w.V, G, g)
+        sh = B.VocabShardProbe(N, w.d, v1 - v0, w.R, v0, G)
+        Wg = dev["W"][v0:v1].contiguous()
+        if peer:
+            pe = B.Peers()
+            pe.rank, pe.world, pe.epoch = g, G, 3
+            for k in range(G):           # one GPU: every "peer" buffer is the same buffer
+                pe.peer_stats[k] = stats_all.data_ptr()
+                pe.peer_flags[k] = flags.data_ptr()
+            sh.partial(dev["hidden"], Wg, dev["off"], token_ids=tok_d, peers=pe)
+        else:
+            sh.partial(dev["hidden"], Wg, dev["off"], token_ids=tok_d, out=stats_all[g])
+        shards.append((sh, Wg))
+    sh = shards[0][0]
+    sh.conf.fill_(-7.0); sh.argmax.fill_(-7); sh.exit.fill_(7); sh.pmax.fill_(-7.0)
+    out = sh.combine(dev["off"], dev["load"], tp, stats_all=stats_all, agg=agg, token_prob=tok is not None,
+                     wait_flags=flags if peer else None, epoch=3 if peer else 0)
+    torch.cuda.synchronize()
+    if peer:
+        assert np.all(flags.cpu().numpy() == 3)
+    return P.GpuRun(out.conf.cpu().numpy(), out.argmax.cpu().numpy(), out.exit.cpu().numpy(),
+                    out.tau.cpu().numpy(), out.pmax.cpu().numpy(), sh.plan), stats_all.cpu().numpy()
+
+
+@pytest.mark.parametrize("peer", [False, True])
+@pytest.mark.parametrize("G", [1, 2, 3, 8])
+@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
+    (33000, 512, 12, 8, None, None),
+    (9001, 256, 40, None, 400, (1, 16)),     # V not divisible by G, several token tiles, padding rows
+])
+def test_vocab_parallel_matches_oracle(P, G, peer, V, d, R, L, n_alloc, var_len):
+    w = wl.scaled(f"vp-V{V}-G{G}", V, d, 0.05, R, L, seed=88, N_alloc=n_alloc, var_len=var_len)
+    g, stats = _run_vocab_parallel(P, w, G, peer=peer)
+    ora, rows, reqs = P.run_oracle(w)
+    st = P.compare(w, g, ora, rows, reqs, w.name)
+    print(w.name, "peer" if peer else "collective", {k: v for k, v in st.items() if k != "plan"})
+    # the shard records themselves: global argmax inside the shard's range, neutral padding rows
+    nv = w.N_valid
+    for k in range(G):
+        v0, v1 = par.shard_vocab(V, G, k)
+        a = stats[k, :, 2].view(np.int32)
+        assert np.all((a[:nv] >= v0) & (a[:nv] < v1))
+        assert np.all(a[nv:] == 2**31 - 1) and np.all(np.isneginf(stats[k, nv:, 0])) and np.all(stats[k, nv:, 1] == 0)
+
+
+def test_vocab_parallel_token_mode_and_ties(P):
+    """Token mode across shards (the token's logit lives in exactly one shard) and a tie between two
+    shards (duplicate winning rows of W in different shards: the lower global index wins)."""
+    G = 4
+    w = wl.scaled("vp-tok", 20000, 256, 0.05, 10, 8, seed=89)
+    ora, rows, reqs = P.run_oracle(w)
+    tok = _token_ids(w, ora, seed=9)
+    g, _ = _run_vocab_parallel(P, w, G, tok=tok, agg=1)
+    pt, conf, ex, margin = _oracle_token_mode(w, ora, tok, 1)
+    print("vp-tok", _compare_token_mode(P, w, g, ora, pt, conf, ex, margin, "vp-tok"))
+    # tie across shards: copy the winning row of request 0's first token into a later shard
+    Wb = w.W_bits.copy()
+    v1 = int(ora.argmax[0])
+    v2 = (v1 + 3 * (w.V // G)) % w.V
+    lo, hi = min(v1, v2), max(v1, v2)
+    Wb[hi] = Wb[lo] = w.W_bits[v1]
+    w2 = wl.Workload("vp-tie", Wb, w.hidden_bits, w.req_offsets, w.load, w.tau_params)
+    g2, _ = _run_vocab_parallel(P, w2, G)
+    ora2, rows2, reqs2 = P.run_oracle(w2)
+    assert ora2.argmax[0] == lo and ora2.gap2[0] == 0.0
+    assert g2.argmax[0] == lo            # bit-identical logits in both shards: exact tie on the GPU too
+    P.compare(w2, g2, ora2, rows2, reqs2, "vp-tie")
+
+
+def test_vocab_parallel_c2_shape(P, c2_W_bits):
+    """C2 at G = 8: each virtual rank streams 1/8 of the LM head (the tensor-parallel layout)."""
+    w = wl.config_c2(c2_W_bits)
+    g, _ = _run_vocab_parallel(P, w, 8, peer=True)
+    ora, rows, reqs = P.run_oracle(w)
+    st = P.compare(w, g, ora, rows, reqs, "vp-c2-G8")
+    print("vp-c2-G8", {k: v for k, v in st.items() if k != "plan"})
