@@ -259,6 +259,27 @@ class GpuCase:
         return fused / n * 1e3, fin / n * 1e3
 
 
+def realised_distribution(w: wl.Workload, case) -> dict:
+    """One untimed call with the debug outputs on: the realised shares of rows / requests per
+    confidence band (SURVEY §8 d: polarisation must be visible next to every number)."""
+    import torch
+    B = case.B
+    probe = B.Probe(w.N_alloc, w.d, w.V, w.R, device=case.hidden.device, debug_outputs=True)
+    out = probe(case.hidden, case.Ws[0], case.off, case.load, case.tp)
+    torch.cuda.synchronize()
+    nv = w.N_valid
+    pm = out.pmax[:nv].float().cpu().numpy()
+    conf, tau, ex = out.conf.cpu().numpy(), out.tau.cpu().numpy(), out.exit.cpu().numpy()
+
+    def bands(x):
+        n = max(len(x), 1)
+        return {"lt_0.5": float((x < 0.5).sum()) / n, "0.5_0.88": float(((x >= 0.5) & (x < 0.88)).sum()) / n,
+                "0.88_0.97": float(((x >= 0.88) & (x <= 0.97)).sum()) / n, "gt_0.97": float((x > 0.97).sum()) / n}
+    return dict(rows=bands(pm), requests=bands(conf), exits=int(ex.sum()), requests_total=int(w.R),
+                requests_within_0p05_of_tau=int((np.abs(conf - tau) < 0.05).sum()),
+                tau_min=float(tau.min()) if len(tau) else None, tau_max=float(tau.max()) if len(tau) else None)
+
+
 def run_ours(args):
     import torch
     from paper_2606_31580_b200 import binding as B
@@ -444,6 +465,7 @@ def run_ours(args):
                      sync_api="laser_probe_confidence_host (one batch at a time, rank 0's figure x ranks)"),
             gpu_launches=int(launches),
             roofline=roof,
+            realised=realised_distribution(w, case),
         )
 
     # heavy-load sweep (configs[4]) — rank 0, single GPU only; W shared with C2
@@ -464,6 +486,38 @@ def run_ours(args):
                               frac=r["frac"], frac_of_nominal=r["frac_of_nominal"], plan=c.probe.plan))
             del c
         out["sweep"] = sweep
+
+    # vocabulary-parallel layout (laser_probe_partial + laser_probe_combine): what ONE rank of G would
+    # execute per step - its 1/G slice of W, then the merge of G records per row.  The exchange itself
+    # needs G GPUs and is not part of this figure.
+    if rank == 0 and world == 1 and not args.no_sweep and args.workload == "C2":
+        from paper_2606_31580_b200 import parallel as par
+        vp = []
+        for G in (2, 4, 8):
+            v0, v1 = par.shard_vocab(w.V, G, 0)
+            sh = B.VocabShardProbe(w.N_alloc, w.d, v1 - v0, w.R, v0, G, device=device, debug_outputs=False)
+            sh.stats_all.fill_(float("-inf"))
+            Wg = [Wc[v0:v1] for Wc in case.Ws]       # contiguous row slices of the resident copies
+            def vp_step(i, sh=sh, Wg=Wg):
+                sh.partial(case.hidden, Wg[i % len(Wg)], case.off, out=sh.stats_all[0])
+                sh.combine(case.off, case.load, case.tp)
+            for i in range(5):
+                vp_step(i)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            k = min(args.steps, 500)
+            e0.record()
+            for i in range(k):
+                vp_step(i)
+            e1.record()
+            torch.cuda.synchronize()
+            us = e0.elapsed_time(e1) / k * 1e3
+            vp.append(dict(G=G, shard_rows=v1 - v0, us_per_step_per_rank=us, kernels_per_step=3,
+                           shard_gb_per_s=(v1 - v0) * w.d * 2 / (us * 1e-6) / 1e9, plan=sh.plan))
+        out["vocab_parallel_per_rank"] = dict(
+            note="one rank's work at G-way vocabulary sharding, measured on one GPU: partial over the "
+                 "first 1/G of W + combine of G records per row; the N*16-byte exchange is not included",
+            points=vp)
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, target_s=10.0)
