@@ -227,3 +227,37 @@ def test_vocab_parallel_c2_shape(P, c2_W_bits):
     ora, rows, reqs = P.run_oracle(w)
     st = P.compare(w, g, ora, rows, reqs, "vp-c2-G8")
     print("vp-c2-G8", {k: v for k, v in st.items() if k != "plan"})
+
+
+@pytest.mark.parametrize("exchange", ["collective", "peer"])
+def test_vocab_parallel_process_group_world1(P, exchange):
+    """parallel.VocabParallelProbe end to end inside a real torch.distributed NCCL group (world size 1,
+    the only size one GPU allows): all-gather exchange, and the peer-push exchange over
+    torch symmetric memory (peer-mapped buffers, epoch flags, two buffer sets alternating)."""
+    import socket
+    import os
+    import torch
+    import torch.distributed as dist
+    from paper_2606_31580_b200 import binding as B
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dev0 = torch.device("cuda", torch.cuda.current_device())
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev0)
+    try:
+        w = wl.scaled("vp-pg", 9001, 256, 0.05, 40, None, seed=88, N_alloc=400, var_len=(1, 16))
+        dev = P.to_device(w)
+        ora, rows, reqs = P.run_oracle(w)
+        vp = par.VocabParallelProbe(dist, w.N_alloc, w.d, w.V, w.R, dev0, exchange=exchange, debug_outputs=True)
+        Wg = dev["W"][vp.v0:vp.v1].contiguous()
+        for it in range(5):      # several epochs: both buffer sets are reused
+            vp.shard.conf.fill_(-7.0); vp.shard.argmax.fill_(-7); vp.shard.exit.fill_(7)
+            out = vp(dev["hidden"], Wg, dev["off"], dev["load"], B.TauParams(**w.tau_params))
+            torch.cuda.synchronize()
+            g = P.GpuRun(out.conf.cpu().numpy(), out.argmax.cpu().numpy(), out.exit.cpu().numpy(),
+                         out.tau.cpu().numpy(), out.pmax.cpu().numpy(), vp.shard.plan)
+            P.compare(w, g, ora, rows, reqs, f"vp-pg-{exchange}-{it}")
+        if exchange == "peer":
+            assert vp.peers.epoch == 5
+    finally:
+        dist.destroy_process_group()
