@@ -468,9 +468,7 @@ int laser_probe_confidence_opt(const void* hidden, const void* W, const int32_t*
     fz.out_tau = out_tau_opt; fz.out_pmax = out_pmax_opt;
     fz.tau = to_dev(tau_params);
     // N == 0 with R > 0: every request is empty -> conf 0, exit 0, tau still defined.  Handled by the
-    // same kernel: req_offsets are all 0, no partials are read.
-    fz.R = R;
-    if (!run_fused && R == 0) fz.R = 0;
+    // same kernel (fz.R = R): req_offsets are all 0, no partials are read.
     if (prof) cudaEventRecord(g_prof.ev[prof_slot][1], stream);
     rc = launch_finalize(fz, stream, run_fused && !prof);
     if (rc != LASER_OK) return rc;

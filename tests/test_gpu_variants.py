@@ -261,3 +261,36 @@ def test_vocab_parallel_process_group_world1(P, exchange):
             assert vp.peers.epoch == 5
     finally:
         dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------- seeded shape fuzz
+def _fuzz_case(i):
+    rng = np.random.default_rng(4242 + i)
+    V = int(rng.choice([rng.integers(1, 300), rng.integers(300, 5000), rng.integers(5000, 40000)]))
+    d = 8 * int(rng.integers(1, 65))
+    R = int(rng.integers(1, 41))
+    lo = int(rng.integers(0, 3))
+    hi = lo + int(rng.integers(0, 20))
+    pad = int(rng.choice([0, 0, 1, 7, 130, 300]))
+    mode = int(rng.integers(0, 3))
+    agg = int(rng.integers(0, 3))
+    return V, d, R, (lo, hi), pad, mode, agg
+
+
+@pytest.mark.parametrize("i", range(32))
+def test_fuzz_shapes_modes_aggregates(P, i):
+    """32 seeded random shapes (V 1..40000, d 8..512, ragged requests incl. empty ones, padding rows)
+    x kernel variant (auto / single / pair) x aggregate, each against the oracle."""
+    from paper_2606_31580_b200 import binding as B
+    V, d, R, var_len, pad, mode, agg = _fuzz_case(i)
+    w0 = wl.scaled(f"fuzz{i}", V, d, 0.05, R, None, seed=9000 + i, var_len=var_len)
+    w = wl.scaled(f"fuzz{i}-V{V}-d{d}-R{R}-m{mode}-a{agg}", V, d, 0.05, R, None, seed=9000 + i, var_len=var_len,
+                  N_alloc=w0.N_valid + pad)
+    if w.N_alloc == 0:
+        pytest.skip("empty batch (covered by test_empty_batches_and_requests)")
+    B.set_mode(mode)
+    try:
+        st = P.check(w, agg=agg)
+    finally:
+        B.set_mode(B.MODE_AUTO)
+    print(w.name, {k: v for k, v in st.items() if k != "plan"}, "pair" if st["plan"]["cta_pair"] else "single")
