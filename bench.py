@@ -2,7 +2,7 @@
 """bench.py — throughput of the LASER confidence probe on B200 (one JSON line on stdout).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--workload C2|C3|C4|C5:<N>] [--no-sweep] [--no-cpu-baseline]
+                    [--workload C2|C3|C4|C5:<N>|shape:d=<d>,V=<V>,N=<N>] [--no-sweep] [--no-cpu-baseline]
 
 A "step" is one pass of the whole hot path (a1-a5 of include/laser_probe.h: projection, online
 softmax, per-request confidence, threshold, exit mask) over one batch of seeded synthetic input —

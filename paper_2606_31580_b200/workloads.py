@@ -249,7 +249,8 @@ def tau_band_stress(W_bits, sigma, R=256, L=8, seed: int = SEED_BASE + 6) -> Wor
 
 
 def by_name(name: str, W_cache: dict | None = None) -> Workload:
-    """'C1' | 'C2' | 'C3' | 'C4' | 'C5:<N>' ; W_cache lets C2/C5 share the 467 MB matrix."""
+    """'C1' | 'C2' | 'C3' | 'C4' | 'C5:<N>' | 'shape:d=<d>,V=<V>,N=<N>[,sigma=<s>]' (any LM-head shape:
+    N/8 requests of 8 rows, the polarised generator); W_cache lets C2/C5 share the 467 MB matrix."""
     W_cache = {} if W_cache is None else W_cache
     if name == "C1":
         return config_c1()
@@ -261,4 +262,13 @@ def by_name(name: str, W_cache: dict | None = None) -> Workload:
         return config_c3()
     if name == "C4":
         return config_c4()
+    if name.startswith("shape:"):
+        kv = dict(t.split("=") for t in name[len("shape:"):].split(","))
+        d, V, N = int(kv["d"]), int(kv["V"]), int(kv["N"])
+        sigma = float(kv.get("sigma", 0.02))
+        key = f"shape-W-{d}-{V}-{sigma}"
+        if key not in W_cache:
+            W_cache[key] = make_W(V, d, sigma, SEED_BASE + 9 + W_SEED_OFFSET + d + V)
+        return _qwen_like(f"shape-d{d}-V{V}-N{N}", V, d, sigma, max(N // 8, 1), 8 if N >= 8 else N, 0.95,
+                          SEED_BASE + 9 + N, "uniform", W_bits=W_cache[key])
     raise KeyError(name)
