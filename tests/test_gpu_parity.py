@@ -292,6 +292,38 @@ def test_back_to_back_calls_share_a_workspace(P, overlap):
     assert not np.array_equal(oras[0][0].argmax, oras[1][0].argmax)
 
 
+def test_c2_in_the_configuration_bench_times(P, c2_W_bits):
+    """The launch configuration of bench.py's timed region at full C2 size: laser_probe_set_overlap(1),
+    calls enqueued back to back on one stream, two resident copies of W alternating between calls,
+    one workspace.  Every call's outputs (kept in separate buffers) are compared with the oracle."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    w = wl.config_c2(c2_W_bits)
+    dev = P.to_device(w)
+    Ws = [dev["W"], dev["W"].clone()]
+    ora, rows, reqs = P.run_oracle(w)
+    K = 6
+    probes = [B.Probe(w.N_alloc, w.d, w.V, w.R) for _ in range(K)]
+    for p in probes[1:]:
+        p.workspace = probes[0].workspace
+    for p in probes:
+        p.conf.fill_(-7.0); p.argmax.fill_(-7); p.exit.fill_(7); p.pmax.fill_(-7.0)
+    tp = B.TauParams(**w.tau_params)
+    B.set_overlap(True)
+    try:
+        torch.cuda.synchronize()
+        for k, p in enumerate(probes):
+            p(dev["hidden"], Ws[k % 2], dev["off"], dev["load"], tp)
+        torch.cuda.synchronize()
+    finally:
+        B.set_overlap(False)
+    for k, p in enumerate(probes):
+        g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),
+                     p.tau.cpu().numpy(), p.pmax.cpu().numpy(), p.plan)
+        st = P.compare(w, g, ora, rows, reqs, f"c2 bench configuration, call {k}")
+    _log("c2-bench-config", st)
+
+
 # ------------------------------------------------------------------ semantics fixed at the boundary
 def test_nan_row_poisons_only_its_request(P):
     w = wl.scaled("nan", 3000, 64, 0.05, 3, 4, seed=11)
