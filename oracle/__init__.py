@@ -9,6 +9,6 @@ Citations are to /root/reference/PAPER.md (line numbers) — see the header of l
 """
 from .binding import (  # noqa: F401
     TauParams, BudgetParams, build, num_threads, row_stats, row_stats_range, merge, aggregate,
-    token_prob,
+    token_prob, SimPolicy, sim_queue, sim_summary,
     tau, tau_scalar, tau_unclamped, exit_mask, probe, ema, budget, f_diff, f_load, ProbeResult,
 )

@@ -15,6 +15,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "laser_oracle.c"
+_SRCS = [_SRC, _HERE / "laser_sim_oracle.c"]
 _SO = _HERE / "liblaser_oracle.so"
 _lib = None
 
@@ -22,6 +23,13 @@ _lib = None
 class _TauParamsC(C.Structure):
     _fields_ = [(n, C.c_double) for n in
                 ("lambda_base", "beta", "gamma", "l_target", "lambda_min", "lambda_max")]
+
+
+class _SimPolicyC(C.Structure):
+    _fields_ = ([(n, C.c_double) for n in
+                 ("lambda_base", "beta", "gamma", "l_target", "lambda_min", "lambda_max", "alpha",
+                  "b_base", "b_min", "f_min", "f_max", "p_min", "p_max", "budget_l_target")] +
+                [(n, C.c_int32) for n in ("early_exit", "adaptive_budget", "fixed_budget", "pad_")])
 
 
 class _BudgetParamsC(C.Structure):
@@ -60,12 +68,41 @@ class BudgetParams:
                               self.p_max, self.l_target)
 
 
+@dataclass
+class SimPolicy:
+    """One serving policy of the simulation.  Defaults = LASER with the paper's parameters
+    (PAPER.md:166, 195): adaptive threshold (Eq. 5) + budget pre-allocation (Eq. 6-8)."""
+    lambda_base: float = 0.95
+    beta: float = 0.04
+    gamma: float = 1.0
+    l_target: float = 10.0
+    lambda_min: float = 0.88
+    lambda_max: float = 0.97
+    alpha: float = 0.3
+    b_base: float = 10.0
+    b_min: float = 2.0
+    f_min: float = 0.6
+    f_max: float = 1.5
+    p_min: float = 50.0
+    p_max: float = 275.0
+    budget_l_target: float = 10.0
+    early_exit: int = 1
+    adaptive_budget: int = 1
+    fixed_budget: int = 10
+
+    def _c(self):
+        return _SimPolicyC(self.lambda_base, self.beta, self.gamma, self.l_target, self.lambda_min,
+                           self.lambda_max, self.alpha, self.b_base, self.b_min, self.f_min, self.f_max,
+                           self.p_min, self.p_max, self.budget_l_target, self.early_exit,
+                           self.adaptive_budget, self.fixed_budget, 0)
+
+
 def build(force: bool = False) -> Path:
     """Compile laser_oracle.c -> liblaser_oracle.so with gcc (-O2, OpenMP, no fast-math)."""
-    if force or not _SO.exists() or _SO.stat().st_mtime < _SRC.stat().st_mtime:
+    if force or not _SO.exists() or _SO.stat().st_mtime < max(f.stat().st_mtime for f in _SRCS):
         tmp = _SO.with_suffix(f".so.tmp{os.getpid()}")
         cmd = ["gcc", "-O3", "-fopenmp", "-fno-fast-math", "-ffp-contract=off",
-               "-shared", "-fPIC", "-o", str(tmp), str(_SRC), "-lm"]
+               "-shared", "-fPIC", "-o", str(tmp), *map(str, _SRCS), "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _SO)
     return _SO
@@ -102,6 +139,9 @@ def _L():
         lib.laser_oracle_f_load.argtypes = [dbl, qp]
         lib.laser_oracle_f_load.restype = dbl
         lib.laser_oracle_budget.argtypes = [dp, dp, i64, qp, ip]
+        lib.laser_sim_oracle_queue.argtypes = [dp, ip, i64, fp, fp, ip, fp, fp, i64, C.c_int32,
+                                               C.POINTER(_SimPolicyC), dp, ip, bp, ip, dp]
+        lib.laser_sim_oracle_summary.argtypes = [dp, dp, ip, i64, dbl, dp]
         _lib = lib
     return _lib
 
@@ -268,4 +308,40 @@ def budget(prompt_tokens, L, q: BudgetParams):
     out = np.empty(pt.shape[0], np.int32)
     _chk(_L().laser_oracle_budget(_ptr(pt, C.c_double), _ptr(L, C.c_double), pt.shape[0],
                                   C.byref(q._c()), _ptr(out, C.c_int32)), "budget")
+    return out
+
+
+def sim_queue(arrival, sample_id, pool, policy: SimPolicy):
+    """Algorithm 1 over one single-server FIFO queue - laser_sim_oracle_queue.
+    pool = dict(chunk_time [S,K] f32, conf [S,K] f32, prompt_tokens [S] i32, t_prefill [S] f32,
+    t_conclusion [S] f32).  Returns dict(finish, chunks, exited, budget, margin)."""
+    arrival = np.ascontiguousarray(arrival, np.float64).reshape(-1)
+    sid = np.ascontiguousarray(sample_id, np.int32).reshape(-1)
+    ct, cf = _f32(pool["chunk_time"]), _f32(pool["conf"])
+    pt = np.ascontiguousarray(pool["prompt_tokens"], np.int32)
+    tp_, tc = _f32(pool["t_prefill"]), _f32(pool["t_conclusion"])
+    S, K = ct.shape
+    n = arrival.shape[0]
+    assert sid.shape[0] == n and cf.shape == (S, K) and pt.shape[0] == S
+    fin, mg = np.empty(n, np.float64), np.empty(n, np.float64)
+    ch, bd = np.empty(n, np.int32), np.empty(n, np.int32)
+    ex = np.empty(n, np.uint8)
+    _chk(_L().laser_sim_oracle_queue(_ptr(arrival, C.c_double), _ptr(sid, C.c_int32), n,
+                                     _ptr(ct, C.c_float), _ptr(cf, C.c_float), _ptr(pt, C.c_int32),
+                                     _ptr(tp_, C.c_float), _ptr(tc, C.c_float), S, K,
+                                     C.byref(policy._c()), _ptr(fin, C.c_double), _ptr(ch, C.c_int32),
+                                     _ptr(ex, C.c_uint8), _ptr(bd, C.c_int32), _ptr(mg, C.c_double)),
+         "sim_queue")
+    return dict(finish=fin, chunks=ch, exited=ex, budget=bd, margin=mg)
+
+
+def sim_summary(arrival, finish, chunks, deadline: float = 30.0):
+    """[mean latency, P95 latency (nearest rank), throughput, SLO share, mean chunks]."""
+    arrival = np.ascontiguousarray(arrival, np.float64)
+    finish = np.ascontiguousarray(finish, np.float64)
+    chunks = np.ascontiguousarray(chunks, np.int32)
+    out = np.empty(5, np.float64)
+    _chk(_L().laser_sim_oracle_summary(_ptr(arrival, C.c_double), _ptr(finish, C.c_double),
+                                       _ptr(chunks, C.c_int32), arrival.shape[0], deadline,
+                                       _ptr(out, C.c_double)), "sim_summary")
     return out

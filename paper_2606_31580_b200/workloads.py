@@ -272,3 +272,59 @@ def by_name(name: str, W_cache: dict | None = None) -> Workload:
         return _qwen_like(f"shape-d{d}-V{V}-N{N}", V, d, sigma, max(N // 8, 1), 8 if N >= 8 else N, 0.95,
                           SEED_BASE + 9 + N, "uniform", W_bits=W_cache[key])
     raise KeyError(name)
+
+
+# ------------------------------------------------------------------------------------ serving simulation
+# Inputs of the serving simulation (SURVEY §8 f NEXT-4).  The paper feeds its
+# discrete-event simulation with per-sample inference times and confidences measured on MATH-500 with
+# an RTX 4090; neither the benchmark nor the weights exist here, so a seeded synthetic POOL of samples
+# stands in for them: per sample a prompt length, prefill / conclusion times, and per
+# reasoning chunk a duration and the confidence at the ATP that ends it.  Inputs only - none of the
+# method's arithmetic (no threshold, budget, EMA or queue) lives here.
+def sim_pool(S: int = 500, K: int = 15, seed: int = SEED_BASE + 40) -> dict:
+    """S samples x K chunks.  Confidence trajectories are polarised: low until the
+    sample's solve chunk, high afterwards, with some ATPs in the band where the threshold decides."""
+    rng = np.random.default_rng(seed)
+    prompt = rng.integers(30, 321, size=S).astype(np.int32)
+    hard = (prompt.astype(np.float64) - 30.0) / 290.0                       # longer prompt = harder
+    solve = 1 + rng.geometric(0.35 - 0.2 * hard, size=S)                    # chunk index (1-based) that solves
+    k = np.arange(1, K + 1)[None, :]
+    low = rng.uniform(0.30, 0.90, size=(S, K))
+    high = rng.uniform(0.955, 0.9995, size=(S, K))
+    band = rng.uniform(0.90, 0.972, size=(S, K))
+    conf = np.where(k >= solve[:, None], high, low)
+    in_band = rng.random((S, K)) < 0.18
+    near = (k >= solve[:, None] - 1) & (k <= solve[:, None] + 1)
+    conf = np.where(in_band & near, band, conf)
+    return dict(
+        chunk_time=rng.uniform(0.15, 0.55, size=(S, K)).astype(np.float32),
+        conf=conf.astype(np.float32),
+        prompt_tokens=prompt,
+        t_prefill=(0.03 + 0.0002 * prompt + rng.uniform(0, 0.02, S)).astype(np.float32),
+        t_conclusion=rng.uniform(0.3, 0.8, size=S).astype(np.float32),
+    )
+
+
+def sim_arrivals_poisson(n_rep: int, n_req: int, qps: float, seed: int):
+    """Poisson arrivals at rate qps: float64 [n_req, n_rep] (replication fastest), ascending per column."""
+    rng = np.random.default_rng(seed)
+    gaps = rng.exponential(1.0 / qps, size=(n_req, n_rep))
+    return np.cumsum(gaps, axis=0)
+
+
+def sim_arrivals_burst(n_rep: int, seed: int, phases=((600.0, 1.0), (600.0, 5.0), (600.0, 1.0))):
+    """The paper's three-phase burst (10 min at 1 QPS, 10 at 5, 10 at 1): a Poisson
+    process conditioned on each phase holding its expected number of arrivals (uniform order
+    statistics inside the phase), so that every replication has the same request count."""
+    rng = np.random.default_rng(seed)
+    cols, t0 = [], 0.0
+    for dur, rate in phases:
+        m = int(round(dur * rate))
+        cols.append(t0 + np.sort(rng.uniform(0.0, dur, size=(m, n_rep)), axis=0))
+        t0 += dur
+    return np.concatenate(cols, axis=0)
+
+
+def sim_sample_ids(n_rep: int, n_req: int, S: int, seed: int):
+    """Which pool sample each request is: int32 [n_req, n_rep]."""
+    return np.random.default_rng(seed).integers(0, S, size=(n_req, n_rep)).astype(np.int32)
