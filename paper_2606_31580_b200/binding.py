@@ -26,6 +26,7 @@ EXPORTS = [
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
     "laser_profile_read", "laser_probe_set_mode", "laser_probe_set_overlap",
     "laser_probe_confidence_opt", "laser_probe_partial", "laser_probe_combine",
+    "laser_sim_policy_default", "laser_sim_run",
 ]
 
 
@@ -76,6 +77,25 @@ class Peers(C.Structure):
                 ("peer_stats", C.c_void_p * MAX_PEERS), ("peer_flags", C.c_void_p * MAX_PEERS)]
 
 
+class SimPolicy(C.Structure):
+    """laser_sim_policy (include/laser_sim.h); defaults = LASER with the paper's parameters."""
+    _fields_ = ([(n, C.c_double) for n in
+                 ("lambda_base", "beta", "gamma", "l_target", "lambda_min", "lambda_max", "alpha",
+                  "b_base", "b_min", "f_min", "f_max", "p_min", "p_max", "budget_l_target")] +
+                [(n, C.c_int32) for n in ("early_exit", "adaptive_budget", "fixed_budget", "pad_")])
+
+    def __init__(self, lambda_base=0.95, beta=0.04, gamma=1.0, l_target=10.0, lambda_min=0.88,
+                 lambda_max=0.97, alpha=0.3, b_base=10.0, b_min=2.0, f_min=0.6, f_max=1.5, p_min=50.0,
+                 p_max=275.0, budget_l_target=10.0, early_exit=1, adaptive_budget=1, fixed_budget=10):
+        super().__init__(lambda_base, beta, gamma, l_target, lambda_min, lambda_max, alpha, b_base, b_min,
+                         f_min, f_max, p_min, p_max, budget_l_target, early_exit, adaptive_budget,
+                         fixed_budget, 0)
+
+
+class SimDims(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("n_rep", "n_req", "S", "K")]
+
+
 class LaserError(RuntimeError):
     def __init__(self, status, text):
         super().__init__(f"laser_probe status {status}: {text}")
@@ -122,6 +142,9 @@ def lib():
         L.laser_probe_set_overlap.argtypes = [C.c_int]
         L.laser_profile_enable.argtypes = [C.c_int]
         L.laser_profile_read.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_int32)]
+        L.laser_sim_policy_default.argtypes = [C.POINTER(SimPolicy)]
+        L.laser_sim_run.argtypes = [vp, vp, vp, C.POINTER(SimPolicy), C.c_int32, vp, vp, vp, vp, vp,
+                                    C.POINTER(SimDims), C.c_double, vp, vp, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -374,3 +397,37 @@ def bf16_tensor_from_bits(bits, device=None, pin=False):
     if pin:
         t = t.pin_memory()
     return t.to(device) if device is not None else t
+
+
+def sim_run(arrival, sample_id, policy_id, policies, pool, deadline=30.0, stream=None, details=True):
+    """laser_sim_run: many single-server FIFO queues served by Algorithm 1, one per GPU thread.
+
+    arrival float64 [n_req, n_rep], sample_id int32 [n_req, n_rep], policy_id int32 [n_rep] - CUDA
+    tensors; policies: list of SimPolicy; pool: dict of CUDA tensors chunk_time / conf float32 [S, K],
+    prompt_tokens int32 [S], t_prefill / t_conclusion float32 [S].
+    Returns dict(finish, chunks, exited, budget, summary [n_rep, 5]) of CUDA tensors; asynchronous."""
+    import torch
+    n_req, n_rep = arrival.shape
+    S, K = pool["chunk_time"].shape
+    dev = arrival.device
+    assert arrival.dtype == torch.float64 and arrival.is_contiguous()
+    assert sample_id.dtype == torch.int32 and tuple(sample_id.shape) == (n_req, n_rep) and sample_id.is_contiguous()
+    assert policy_id.dtype == torch.int32 and policy_id.numel() == n_rep
+    for k, dt in (("chunk_time", torch.float32), ("conf", torch.float32), ("prompt_tokens", torch.int32),
+                  ("t_prefill", torch.float32), ("t_conclusion", torch.float32)):
+        assert pool[k].dtype == dt and pool[k].is_contiguous() and pool[k].device == dev
+    pols = (SimPolicy * len(policies))(*policies)
+    out = dict(finish=torch.empty((n_req, n_rep), dtype=torch.float64, device=dev),
+               chunks=torch.empty((n_req, n_rep), dtype=torch.int32, device=dev),
+               exited=torch.empty((n_req, n_rep), dtype=torch.uint8, device=dev) if details else None,
+               budget=torch.empty((n_req, n_rep), dtype=torch.int32, device=dev) if details else None,
+               summary=torch.empty((n_rep, 5), dtype=torch.float64, device=dev))
+    s = (stream or torch.cuda.current_stream(dev)).cuda_stream
+    _check(lib().laser_sim_run(
+        arrival.data_ptr(), sample_id.data_ptr(), policy_id.data_ptr(), pols, len(policies),
+        pool["chunk_time"].data_ptr(), pool["conf"].data_ptr(), pool["prompt_tokens"].data_ptr(),
+        pool["t_prefill"].data_ptr(), pool["t_conclusion"].data_ptr(), C.byref(SimDims(n_rep, n_req, S, K)),
+        float(deadline), out["finish"].data_ptr(), out["chunks"].data_ptr(),
+        out["exited"].data_ptr() if details else None, out["budget"].data_ptr() if details else None,
+        out["summary"].data_ptr(), s))
+    return out

@@ -13,8 +13,9 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 SO = HERE / "liblaser_probe.so"
-SOURCES = [CSRC / "laser_probe.cu"]
-DEPS = SOURCES + [CSRC / "probe_kernels.cuh", CSRC / "ptx.cuh", HERE.parent / "include" / "laser_probe.h"]
+SOURCES = [CSRC / "laser_probe.cu", CSRC / "laser_sim.cu"]
+DEPS = SOURCES + [CSRC / "probe_kernels.cuh", CSRC / "ptx.cuh", HERE.parent / "include" / "laser_probe.h",
+                  HERE.parent / "include" / "laser_sim.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",   # tcgen05 / TMEM need the 'a' target

@@ -21,7 +21,7 @@ def _built():
 
 
 def test_header_symbols_all_exported():
-    hdr = (ROOT / "include" / "laser_probe.h").read_text()
+    hdr = "".join(f.read_text() for f in sorted((ROOT / "include").glob("*.h")))
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     declared = set(re.findall(r"\b(laser_[a-z_]+)\s*\(", hdr))
     assert declared, "no declarations found"
@@ -178,3 +178,25 @@ def test_partial_combine_validation_needs_no_gpu():
                                  None, None, None, 0) == -2
     assert L.laser_probe_combine(None, 2, None, None, C.byref(tp), None, None, None, C.byref(d), None, None,
                                  None, None, None, 0) == -1
+
+
+def test_sim_validation_needs_no_gpu():
+    L = B.lib()
+    pol = B.SimPolicy()
+    assert L.laser_sim_policy_default(C.byref(pol)) == 0
+    assert (pol.lambda_base, pol.beta, pol.alpha, pol.b_base, pol.p_max) == (0.95, 0.04, 0.3, 10.0, 275.0)
+    d = B.SimDims(4, 10, 5, 3)
+    args = [None] * 3 + [C.byref(pol), 1] + [None] * 5 + [C.byref(d), 30.0] + [None] * 6
+    assert L.laser_sim_run(*args) == -1                      # NULL arrays
+    bad = B.SimDims(4, 10, 0, 3)
+    args[10] = C.byref(bad)
+    assert L.laser_sim_run(*args) == -2
+    args[10] = C.byref(d); args[4] = 17
+    assert L.laser_sim_run(*args) == -2                      # too many policies
+    args[4] = 1
+    pol.alpha = 1.5
+    assert L.laser_sim_run(*args) == -4
+    empty = B.SimDims(0, 10, 5, 3)
+    pol.alpha = 0.3
+    args[10] = C.byref(empty)
+    assert L.laser_sim_run(*args) == 0                       # nothing to simulate

@@ -1,0 +1,139 @@
+"""GPU parity of the batched serving simulation (laser_sim_run, include/laser_sim.h) against the fp64
+CPU oracle (oracle/laser_sim_oracle.c) on the same seeded inputs.  Needs a B200 (`-m gpu`).
+
+Bar: chunk counts, exit flags and budgets bit-exact; finish times and the summary bit-exact as well
+(both sides perform the same IEEE double operations in the same order) - except downstream of a
+decision whose oracle margin |conf - lambda| is below 1e-12, where a last-ulp difference of tanh
+between the two libraries may flip it (counted; none occurs on these inputs)."""
+import numpy as np
+import pytest
+
+from paper_2606_31580_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def _policies():
+    import oracle
+    return {
+        "laser": dict(),
+        "fixed_high": dict(beta=0.0, lambda_base=0.95, adaptive_budget=0, fixed_budget=10),
+        "fixed_low": dict(beta=0.0, lambda_base=0.90, adaptive_budget=0, fixed_budget=10),
+        "vanilla": dict(early_exit=0, adaptive_budget=0, fixed_budget=15),
+        "threshold_only": dict(adaptive_budget=0, fixed_budget=10),
+        "budget_only": dict(beta=0.0),
+        "sensitive": dict(beta=0.06, l_target=5.0, alpha=0.7, gamma=2.0),
+    }
+
+
+def _run_gpu(arr, sid, pid, pols, pool, deadline=30.0):
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    dpool = {k: torch.from_numpy(np.ascontiguousarray(v)).cuda() for k, v in pool.items()}
+    out = B.sim_run(torch.from_numpy(arr).cuda(), torch.from_numpy(sid).cuda(), torch.from_numpy(pid).cuda(),
+                    [B.SimPolicy(**p) for p in pols], dpool, deadline=deadline)
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in out.items()}
+
+
+def _compare(arr, sid, pid, pols, pool, g, deadline=30.0):
+    import oracle
+    n_req, n_rep = arr.shape
+    flips = 0
+    for r in range(n_rep):
+        o = oracle.sim_queue(arr[:, r], sid[:, r], pool, oracle.SimPolicy(**pols[pid[r]]))
+        if o["margin"].min() < 1e-12:        # a decision on a knife edge: compare up to it only
+            flips += 1
+            stop = int(np.argmax(o["margin"] < 1e-12))
+        else:
+            stop = n_req
+        assert np.array_equal(g["chunks"][:stop, r], o["chunks"][:stop]), f"rep {r}: chunks"
+        assert np.array_equal(g["exited"][:stop, r], o["exited"][:stop]), f"rep {r}: exited"
+        assert np.array_equal(g["budget"][:stop, r], o["budget"][:stop]), f"rep {r}: budget"
+        assert np.array_equal(g["finish"][:stop, r], o["finish"][:stop]), \
+            f"rep {r}: finish differs by {np.abs(g['finish'][:stop, r] - o['finish'][:stop]).max()}"
+        if stop == n_req:
+            s = oracle.sim_summary(arr[:, r], o["finish"], o["chunks"], deadline)
+            assert np.array_equal(g["summary"][r], s), f"rep {r}: summary {g['summary'][r]} vs {s}"
+    return flips
+
+
+def test_sim_matches_oracle_all_policies_poisson():
+    """Seven policies x QPS {0.5, 1, 2, 4, 8} x 2 seeds = 70 queues of 700 requests."""
+    pool = wl.sim_pool()
+    names = list(_policies())
+    pols = [_policies()[n] for n in names]
+    cols_a, cols_s, pid = [], [], []
+    for qi, qps in enumerate((0.5, 1.0, 2.0, 4.0, 8.0)):
+        for seed in range(2):
+            a = wl.sim_arrivals_poisson(1, 700, qps, seed=100 + 10 * qi + seed)
+            s = wl.sim_sample_ids(1, 700, 500, seed=200 + 10 * qi + seed)
+            for p in range(len(pols)):
+                cols_a.append(a); cols_s.append(s); pid.append(p)
+    arr = np.ascontiguousarray(np.concatenate(cols_a, axis=1))
+    sid = np.ascontiguousarray(np.concatenate(cols_s, axis=1))
+    pid = np.asarray(pid, np.int32)
+    g = _run_gpu(arr, sid, pid, pols, pool)
+    flips = _compare(arr, sid, pid, pols, pool, g)
+    print("poisson: replications", arr.shape[1], "knife-edge decisions", flips)
+    assert flips == 0
+    # the simulation shows the paper's qualitative result: LASER's mean latency is below Fixed-High's
+    lat = g["summary"][:, 0].reshape(-1, len(pols))
+    assert np.all(lat[:, names.index("laser")] <= lat[:, names.index("fixed_high")] + 1e-9)
+    assert np.all(lat[:, names.index("fixed_high")] <= lat[:, names.index("vanilla")] + 1e-9)
+
+
+def test_sim_matches_oracle_burst_and_ragged_sizes():
+    """The paper's three-phase burst (4200 requests, more than one sort tile) and awkward sizes
+    (one request, 33 replications: a partial warp)."""
+    pool = wl.sim_pool(S=77, K=9, seed=3)
+    names = list(_policies())
+    pols = [_policies()[n] for n in names]
+    arr = wl.sim_arrivals_burst(33, seed=5)
+    sid = wl.sim_sample_ids(33, arr.shape[0], 77, seed=6)
+    pid = (np.arange(33) % len(pols)).astype(np.int32)
+    g = _run_gpu(arr, sid, pid, pols, pool)
+    assert _compare(arr, sid, pid, pols, pool, g) == 0
+    for n_req, n_rep in ((1, 1), (2, 5), (1000, 3), (1025, 2)):
+        arr = wl.sim_arrivals_poisson(n_rep, n_req, 3.0, seed=n_req)
+        sid = wl.sim_sample_ids(n_rep, n_req, 77, seed=n_req + 1)
+        pid = (np.arange(n_rep) % len(pols)).astype(np.int32)
+        g = _run_gpu(arr, sid, pid, pols, pool, deadline=5.0)
+        assert _compare(arr, sid, pid, pols, pool, g, deadline=5.0) == 0
+
+
+def test_sim_driven_by_the_real_probe():
+    """Exit-mask -> latency coupling with confidences that come out of the fused probe kernel: the
+    pool's confidence table is filled by laser_probe_confidence on synthetic hidden states (one request
+    of 8 trial-answer tokens per (sample, chunk)), then drives the simulation; the oracle side uses
+    the oracle probe's confidences, and both simulations must agree wherever the two confidence
+    tables lead to the same decisions (the probes agree to ~1e-6)."""
+    import oracle
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    S, K = 24, 6
+    w = wl.scaled("sim-probe", 8000, 128, 0.05, S * K, 8, seed=31, q=0.8)
+    probe = B.Probe(w.N_alloc, w.d, w.V, w.R)
+    out = probe(B.bf16_tensor_from_bits(w.hidden_bits, "cuda"), B.bf16_tensor_from_bits(w.W_bits, "cuda"),
+                torch.from_numpy(w.req_offsets).cuda(), torch.from_numpy(w.load).cuda(), B.TauParams(**w.tau_params))
+    torch.cuda.synchronize()
+    conf_gpu = out.conf.cpu().numpy().reshape(S, K)
+    ora = oracle.probe(w.hidden_f32(), w.W_f32(), w.req_offsets, w.load, oracle.TauParams(**w.tau_params))
+    conf_ora = ora.conf.astype(np.float32).reshape(S, K)
+    assert np.abs(conf_gpu - conf_ora).max() < 2e-3
+    pool = wl.sim_pool(S=S, K=K, seed=32)
+    arr = wl.sim_arrivals_poisson(8, 300, 1.0, seed=33)
+    sid = wl.sim_sample_ids(8, 300, S, seed=34)
+    pid = np.zeros(8, np.int32)
+    pool_g = dict(pool, conf=conf_gpu)
+    g = _run_gpu(arr, sid, pid, [dict()], pool_g)
+    # same confidence table on both sides: exact parity
+    assert _compare(arr, sid, pid, [dict()], pool_g, g) == 0
+    # oracle-probe confidences: identical decisions unless a confidence sits within 2e-3 of a threshold
+    agree = 0
+    for r in range(8):
+        o = oracle.sim_queue(arr[:, r], sid[:, r], dict(pool, conf=conf_ora), oracle.SimPolicy())
+        if o["margin"].min() > 2e-3:
+            assert np.array_equal(o["chunks"], g["chunks"][:, r])
+            agree += 1
+    print("replications with no decision within 2e-3 of the threshold:", agree, "of 8")
