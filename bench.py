@@ -280,6 +280,78 @@ def realised_distribution(w: wl.Workload, case) -> dict:
                 tau_min=float(tau.min()) if len(tau) else None, tau_max=float(tau.max()) if len(tau) else None)
 
 
+SIM_POLICIES = {
+    "laser": dict(),
+    "fixed_high": dict(beta=0.0, lambda_base=0.95, adaptive_budget=0, fixed_budget=10),
+    "fixed_low": dict(beta=0.0, lambda_base=0.90, adaptive_budget=0, fixed_budget=10),
+    "vanilla": dict(early_exit=0, adaptive_budget=0, fixed_budget=15),
+    "threshold_only": dict(adaptive_budget=0, fixed_budget=10),
+    "budget_only": dict(beta=0.0),
+}
+SIM_QPS = (0.5, 1.0, 2.0, 4.0, 8.0)
+
+
+def serving_sim_bench(device, seeds: int = 128, n_req: int = 1000, with_cpu: bool = True) -> dict:
+    """Secondary measurement (SURVEY §8 f NEXT-4): laser_sim_run over policies x arrival rates x seeds
+    of synthetic single-server FIFO queues (one GPU thread each), next to the oracle's loop on the host.
+    The latency table is illustrative only: the sample pool is synthetic."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    names = list(SIM_POLICIES)
+    pool = wl.sim_pool()
+    cols_a, cols_s, pid, key = [], [], [], []
+    for qi, qps in enumerate(SIM_QPS):
+        a = wl.sim_arrivals_poisson(seeds, n_req, qps, seed=wl.SEED_BASE + 50 + qi)
+        sid = wl.sim_sample_ids(seeds, n_req, pool["conf"].shape[0], seed=wl.SEED_BASE + 60 + qi)
+        for pi in range(len(names)):
+            cols_a.append(a); cols_s.append(sid)
+            pid += [pi] * seeds; key += [(pi, qi)] * seeds
+    arr = np.ascontiguousarray(np.concatenate(cols_a, axis=1))
+    sid = np.ascontiguousarray(np.concatenate(cols_s, axis=1))
+    pid = np.asarray(pid, np.int32)
+    n_rep = arr.shape[1]
+    d_arr, d_sid, d_pid = (torch.from_numpy(x).to(device) for x in (arr, sid, pid))
+    d_pool = {k: torch.from_numpy(np.ascontiguousarray(v)).to(device) for k, v in pool.items()}
+    pols = [B.SimPolicy(**SIM_POLICIES[n]) for n in names]
+    for _ in range(3):
+        out = B.sim_run(d_arr, d_sid, d_pid, pols, d_pool, details=False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    reps = 5
+    e0.record()
+    for _ in range(reps):
+        out = B.sim_run(d_arr, d_sid, d_pid, pols, d_pool, details=False)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    summ = out["summary"].cpu().numpy()
+    key = np.asarray(key)
+    table = {}
+    for pi, name in enumerate(names):
+        table[name] = {}
+        for qi, qps in enumerate(SIM_QPS):
+            m = (key[:, 0] == pi) & (key[:, 1] == qi)
+            table[name][str(qps)] = dict(mean_latency_s=float(summ[m, 0].mean()), p95_latency_s=float(summ[m, 1].mean()),
+                                         throughput_qps=float(summ[m, 2].mean()), slo_share=float(summ[m, 3].mean()),
+                                         mean_chunks=float(summ[m, 4].mean()))
+    res = dict(value=n_rep * n_req / (ms * 1e-3), unit="simulated requests/s", ms_per_run=ms, n_rep=n_rep,
+               n_req=n_req, gpu_launches_per_run=2, policies=names, qps=list(SIM_QPS), seeds=seeds,
+               data="synthetic sample pool (500 samples x 15 chunks) and Poisson arrivals, DESIGN.md §10",
+               table=table)
+    if with_cpu:
+        import oracle
+        k = min(n_rep, 60)
+        pick = np.linspace(0, n_rep - 1, k).astype(int)
+        t0 = time.perf_counter()
+        for r in pick:
+            o = oracle.sim_queue(arr[:, r], sid[:, r], pool, oracle.SimPolicy(**SIM_POLICIES[names[pid[r]]]))
+            oracle.sim_summary(arr[:, r], o["finish"], o["chunks"], 30.0)
+        dt = time.perf_counter() - t0
+        res["cpu_oracle"] = dict(value=k * n_req / dt, unit="simulated requests/s", cores=1, kind="oracle",
+                                 sample=f"{k} of the {n_rep} replications, one after the other")
+    return res
+
+
 def run_ours(args):
     import torch
     from paper_2606_31580_b200 import binding as B
@@ -518,6 +590,9 @@ def run_ours(args):
             note="one rank's work at G-way vocabulary sharding, measured on one GPU: partial over the "
                  "first 1/G of W + combine of G records per row; the N*16-byte exchange is not included",
             points=vp)
+
+    if rank == 0 and world == 1 and not args.no_sweep and args.workload == "C2":
+        out["serving_sim"] = serving_sim_bench(device, with_cpu=not args.no_cpu_baseline)
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, target_s=10.0)
