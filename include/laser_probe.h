@@ -228,7 +228,9 @@ int laser_probe_partial(const void* hidden, const void* W_shard, const int32_t* 
 
 /* Merge + a3-a5 over gathered statistics.  stats: device [G, N] (shard-major).  dims->N and dims->R
  * are used (d, V ignored but must be valid).  wait_flags_opt: device uint32 [G] or NULL; when given
- * every block first waits until all G flags have reached `epoch` (peer-push exchange).  One kernel. */
+ * every block first waits until all G flags have reached `epoch` (peer-push exchange); a flag that
+ * does not arrive within ~5 s makes the kernel trap (LASER_E_CUDA on the next call / sync) instead of
+ * hanging the GPU.  One kernel. */
 int laser_probe_combine(const laser_row_stats* stats, int32_t G, const int32_t* req_offsets,
                         const float* load, const laser_tau_params* tau_params, float* out_conf,
                         int32_t* out_argmax, uint8_t* out_exit, const laser_probe_dims* dims,

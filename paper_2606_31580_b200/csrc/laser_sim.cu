@@ -78,47 +78,83 @@ laser_sim_queue_kernel(const __grid_constant__ SimParams q) {
     pid = min(max(pid, 0), q.n_pol - 1);
     const laser_sim_policy& pol = q.pol[pid];
     const double one_minus_alpha = __dsub_rn(1.0, pol.alpha);
+    const bool need_tanh = pol.beta != 0.0;
+    const double lam_const = fmin(fmax(pol.lambda_base, pol.lambda_min), pol.lambda_max);
 
     double lbar = 0.0, prev_finish = -CUDART_INF, lat_sum = 0.0, chunk_sum = 0.0;
     double first_arrival = 0.0, last_finish = 0.0;
-    int arrived = 0;          // requests with arrival <= the last time queried
-    double next_arrival = (n > 0) ? __ldg(q.arrival + r) : CUDART_INF;   // arrival[arrived]
     long long ok = 0;
+
+    // Arrival counter: `arrived` = requests with arrival <= the last time queried.  The next kWin
+    // arrival times are kept in registers and refilled by kWin independent loads, so that advancing
+    // the counter over a burst of arrivals costs one memory latency per kWin arrivals, not one each.
+    constexpr int kWin = 4;
+    int arrived = 0, win_base = 0;      // win[] holds arrival[win_base .. win_base + kWin)
+    double win[kWin];
+    auto refill = [&](int base) {
+        win_base = base;
+#pragma unroll
+        for (int j = 0; j < kWin; ++j)
+            win[j] = (base + j < n) ? __ldg(q.arrival + static_cast<size_t>(base + j) * R + r) : CUDART_INF;
+    };
+    auto count_arrivals = [&](double t) {
+        while (true) {
+            int adv = 0;
+#pragma unroll
+            for (int j = 0; j < kWin; ++j)           // arrivals ascend: a prefix of the window is <= t
+                adv += (win_base + j >= arrived && win[j] <= t) ? 1 : 0;
+            arrived += adv;
+            if (arrived < win_base + kWin || arrived >= n) break;
+            refill(arrived);                         // window exhausted: look at the next kWin
+        }
+    };
+    refill(0);
+
+    // Request i + 1's own inputs are fetched while request i is simulated.
+    double a_next = (n > 0) ? __ldg(q.arrival + r) : 0.0;
+    int s_next = (n > 0) ? min(max(__ldg(q.sample_id + r), 0), q.S - 1) : 0;
     for (int i = 0; i < n; ++i) {
         const size_t o = static_cast<size_t>(i) * R + r;
-        const double a = __ldg(q.arrival + o);
-        int s = __ldg(q.sample_id + o);
-        s = min(max(s, 0), q.S - 1);
+        const double a = a_next;
+        const int s = s_next;
+        const double prompt = static_cast<double>(__ldg(q.prompt_tokens + s));
+        const double t_pre = static_cast<double>(__ldg(q.t_prefill + s));
+        const double t_conc = static_cast<double>(__ldg(q.t_conclusion + s));
+        if (i + 1 < n) {
+            a_next = __ldg(q.arrival + o + R);
+            s_next = min(max(__ldg(q.sample_id + o + R), 0), q.S - 1);
+        }
         if (i == 0) first_arrival = a;
         double t = (a > prev_finish) ? a : prev_finish;
-        while (arrived < n && next_arrival <= t) {
-            ++arrived;
-            next_arrival = (arrived < n) ? __ldg(q.arrival + static_cast<size_t>(arrived) * R + r) : CUDART_INF;
-        }
+        count_arrivals(t);
         double L = static_cast<double>(arrived - i);
-        int B = pol.adaptive_budget ? sim_budget(static_cast<double>(__ldg(q.prompt_tokens + s)), L, pol)
-                                    : pol.fixed_budget;
+        int B = pol.adaptive_budget ? sim_budget(prompt, L, pol) : pol.fixed_budget;
         B = min(B, K);
         B = max(B, 0);
-        t = __dadd_rn(t, static_cast<double>(__ldg(q.t_prefill + s)));
+        t = __dadd_rn(t, t_pre);
         int k = 0;
         uint8_t ex = 0;
         const float* ct = q.chunk_time + static_cast<size_t>(s) * K;
         const float* cf = q.conf + static_cast<size_t>(s) * K;
+        // chunk k + 1's time and confidence are in flight while chunk k is evaluated
+        float ct_k = (B > 0) ? __ldg(ct) : 0.f, cf_k = (B > 0) ? __ldg(cf) : 0.f;
         while (k < B) {
-            t = __dadd_rn(t, static_cast<double>(__ldg(ct + k)));
-            while (arrived < n && next_arrival <= t) {
-                ++arrived;
-                next_arrival = (arrived < n) ? __ldg(q.arrival + static_cast<size_t>(arrived) * R + r) : CUDART_INF;
-            }
+            const float ct_n = (k + 1 < B) ? __ldg(ct + k + 1) : 0.f;
+            const float cf_n = (k + 1 < B) ? __ldg(cf + k + 1) : 0.f;
+            t = __dadd_rn(t, static_cast<double>(ct_k));
+            count_arrivals(t);
             L = static_cast<double>(arrived - i);
             lbar = __dadd_rn(__dmul_rn(pol.alpha, L), __dmul_rn(one_minus_alpha, lbar));
-            const double lam = sim_tau(lbar, pol);
-            const double c = static_cast<double>(__ldg(cf + k));
             ++k;
-            if (pol.early_exit && c > lam) { ex = 1; break; }
+            if (pol.early_exit) {
+                // beta == 0 (fixed-threshold policies): beta * tanh(.) is exactly 0, the threshold is
+                // the clamped constant - same value, without the tanh
+                const double lam = need_tanh ? sim_tau(lbar, pol) : lam_const;
+                if (static_cast<double>(cf_k) > lam) { ex = 1; break; }
+            }
+            ct_k = ct_n; cf_k = cf_n;
         }
-        t = __dadd_rn(t, static_cast<double>(__ldg(q.t_conclusion + s)));
+        t = __dadd_rn(t, t_conc);
         prev_finish = t;
         last_finish = t;
         q.out_finish[o] = t;

@@ -487,7 +487,13 @@ __device__ __forceinline__ int records_per_row(const FinalizeParams& p) {
 // their statistics have landed here).  One thread per flag, then a block barrier.
 __device__ __forceinline__ void wait_peer_flags(const uint32_t* flags, int G, uint32_t epoch) {
     if (static_cast<int>(threadIdx.x) < G) {
-        while (static_cast<int32_t>(ptx::ld_acquire_sys_u32(flags + threadIdx.x) - epoch) < 0) __nanosleep(64);
+        const long long t0 = clock64();
+        while (static_cast<int32_t>(ptx::ld_acquire_sys_u32(flags + threadIdx.x) - epoch) < 0) {
+            __nanosleep(64);
+            // a peer that never signals (crashed rank, mismatched epoch) must not hang the GPU:
+            // after ~5 s the kernel traps and the caller sees a CUDA error instead
+            if (clock64() - t0 > 10000000000LL) __trap();
+        }
     }
     __syncthreads();
 }
