@@ -493,6 +493,8 @@ def run_ours(args):
         roof["kernel"] = "laser_probe_fused_kernel<%d>" % case.probe.plan["cta_pair"]
         roof["kernel_us"] = kernel_us
         roof["kernel_us_event_bracketed"] = fused_us
+        # the most conservative reading: the kernel alone between two events (launch latency included)
+        roof["frac_event_bracketed"] = roofline_for(w, fused_us, peaks, sustained=False)["frac"]
         roof["kernel_us_note"] = ("min(average over K launches bracketed by CUDA events on the launch stream, without "
                                   "programmatic dependent launch; average step duration of the timed region)")
         roof["finalize_kernel_us"] = fin_us

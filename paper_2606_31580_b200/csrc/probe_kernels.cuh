@@ -215,10 +215,12 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
-    // Programmatic dependent launch.  The only memory this kernel shares with the kernel before it in
-    // a chain of probe calls (the previous call's finalize kernel) is the workspace, so by default
-    // only the workspace stores (and the exit) wait for that kernel: the W stream of this call then
-    // overlaps the tail of the previous one.  wait_first restores the strict order for the inputs.
+    // Programmatic dependent launch.  wait_first (the library default, laser_probe_set_overlap(0)):
+    // every global read below happens after the kernel ahead of this one in the stream has completed;
+    // only the prologue above overlapped it.  Without it (overlap opted in): the only memory this
+    // kernel shares with the kernel before it in a chain of probe calls (the previous call's finalize
+    // kernel) is the workspace, so only the workspace stores (and the exit) wait for that kernel and
+    // the W stream of this call overlaps the tail of the previous one.
     if (p.wait_first) ptx::pdl_wait();
     // Let the finalize kernel's CTAs become resident now (they block in griddepcontrol.wait).
     ptx::pdl_launch_dependents();
