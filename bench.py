@@ -621,7 +621,7 @@ def cpu_baseline(w: wl.Workload, target_s: float):
     hid, off, load = w.hidden_f32()[:rows], w.req_offsets[:reqs + 1], w.load[:reqs]
     Wf = w.W_f32()
     best, spent, reps = None, 0.0, 0
-    while spent < target_s and reps < 5:
+    while spent < target_s and reps < 20:        # about target_s (10 s) of CPU work
         r = oracle.probe(hid, Wf, off, load, tp)
         best = r.seconds if best is None else min(best, r.seconds)
         spent += r.seconds
