@@ -240,6 +240,30 @@ class GpuCase:
         ts.sort()
         return ts[len(ts) // 2]
 
+    def graph_replay_us(self, calls: int, reps: int = 20):
+        """Median duration (us) of replaying a CUDA graph that holds `calls` back-to-back probe calls,
+        captured under the current overlap setting - how a serving engine that captures its step
+        would run the probe (no per-launch host work)."""
+        torch = self.torch
+        side = torch.cuda.Stream(device=self.hidden.device)
+        g = torch.cuda.CUDAGraph()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                for i in range(calls):
+                    self.probe(self.hidden, self.Ws[i % len(self.Ws)], self.off, self.load, self.tp, stream=side)
+        ts = []
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            e0.record()
+            g.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        ts.sort()
+        return ts[len(ts) // 2]
+
     def kernel_times(self, steps: int):
         """Average duration (us) of the fused and the finalize kernel over `steps` calls."""
         B = self.B
@@ -400,7 +424,12 @@ def run_ours(args):
     for _ in range(3):
         case.step()
     strict_ms = case.time_steps(args.steps, barrier)
+
+    # CUDA-graph replay under the strict default: one call, and ten calls in one graph
+    graph_one_us = case.graph_replay_us(1)
+    graph_ten_us = case.graph_replay_us(10) / 10.0
     B.set_overlap(True)
+    graph_ten_overlap_us = case.graph_replay_us(10) / 10.0
 
     # dominant kernel on its own (second pass, same stream, library-recorded events)
     fused_us, fin_us = case.kernel_times(args.steps)
@@ -523,6 +552,10 @@ def run_ours(args):
                         ms_per_step=strict_ms / args.steps,
                         note="the same K steps with laser_probe_set_overlap(0), the library default: every "
                              "input read waits for the preceding kernel (griddepcontrol.wait first)"),
+            cuda_graph=dict(one_call_us=graph_one_us, per_call_us_ten_calls_strict=graph_ten_us,
+                            per_call_us_ten_calls_overlap=graph_ten_overlap_us,
+                            note="median replay time of a captured CUDA graph holding 1 / 10 probe calls "
+                                 "(rank 0); a call is capturable: no sync, no allocation, no host read"),
             sustained=dict(value=rows_all / (sustained_ms / args.steps * 1e-3), unit=UNIT,
                            ms_per_step=sustained_ms / args.steps, clocks=sustained_clocks,
                            note=f"the same K steps timed again after {SETTLE_S} s of continuous probing "

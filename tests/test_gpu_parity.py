@@ -454,3 +454,41 @@ def test_error_codes_on_device(P):
     with pytest.raises(B.LaserError) as e:
         pr(dev["hidden"], mis, dev["off"], dev["load"], tp)
     assert e.value.status == -3
+
+
+def test_cuda_graph_capture_and_replay(P, c2_W_bits):
+    """A serving engine captures its decode step in a CUDA graph: the probe call (two kernel launches
+    with programmatic-dependent-launch attributes, no synchronisation, no allocation) must be
+    capturable, and a replay must read the CURRENT contents of the input buffers."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    w1 = wl.config_c2(c2_W_bits)
+    w2 = wl.config_c2(c2_W_bits, seed=wl.SEED_BASE + 2 + 7919)          # another batch, same shapes
+    d1, d2 = P.to_device(w1), P.to_device(w2)
+    hidden, off, load = d1["hidden"].clone(), d1["off"].clone(), d1["load"].clone()
+    probe = B.Probe(w1.N_alloc, w1.d, w1.V, w1.R)
+    tp = B.TauParams(**w1.tau_params)
+    probe(hidden, d1["W"], off, load, tp)                               # warm-up outside capture
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            probe(hidden, d1["W"], off, load, tp, stream=side)
+    for w, d in ((w1, d1), (w2, d2), (w1, d1)):
+        hidden.copy_(d["hidden"]); off.copy_(d["off"]); load.copy_(d["load"])
+        probe.conf.fill_(-7.0); probe.argmax.fill_(-7); probe.exit.fill_(7)
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        run = P.GpuRun(probe.conf.cpu().numpy(), probe.argmax.cpu().numpy(), probe.exit.cpu().numpy(),
+                       probe.tau.cpu().numpy(), probe.pmax.cpu().numpy(), probe.plan)
+        ora, rows, reqs = P.run_oracle(w)
+        P.compare(w, run, ora, rows, reqs, f"graph replay {w.name}")
+    # replay latency of one captured call (both kernels), for the record
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ts = []
+    for _ in range(20):
+        torch.cuda.synchronize(); e0.record(); g.replay(); e1.record(); torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1) * 1e3)
+    print("graph replay, one call: median %.1f us" % sorted(ts)[len(ts) // 2])
