@@ -137,3 +137,42 @@ def test_sim_driven_by_the_real_probe():
             assert np.array_equal(o["chunks"], g["chunks"][:, r])
             agree += 1
     print("replications with no decision within 2e-3 of the threshold:", agree, "of 8")
+
+
+def test_sim_fuzz_random_policies():
+    """64 replications with randomly drawn policy parameters (all of Eq. 5-8, alpha, switches), pool
+    sizes and arrival rates: every integer output and every double must equal the oracle's."""
+    rng = np.random.default_rng(777)
+    for trial in range(4):
+        S, K = int(rng.integers(1, 40)), int(rng.integers(1, 20))
+        pool = wl.sim_pool(S=S, K=K, seed=900 + trial)
+        pols = []
+        for _ in range(16):
+            lo, hi = sorted(rng.uniform(0.80, 0.99, size=2))
+            pols.append(dict(lambda_base=float(rng.uniform(0.85, 0.99)), beta=float(rng.choice([0.0, rng.uniform(0.0, 0.1)])),
+                             gamma=float(rng.uniform(0.3, 3.0)), l_target=float(rng.uniform(1.0, 20.0)),
+                             lambda_min=float(lo), lambda_max=float(hi), alpha=float(rng.uniform(0.0, 1.0)),
+                             b_base=float(rng.integers(1, 20)), b_min=float(rng.integers(1, 4)),
+                             f_min=float(rng.uniform(0.3, 1.0)), f_max=float(rng.uniform(1.0, 2.0)),
+                             p_min=float(rng.integers(10, 100)), p_max=float(rng.integers(150, 400)),
+                             budget_l_target=float(rng.uniform(1.0, 20.0)), early_exit=int(rng.integers(0, 2)),
+                             adaptive_budget=int(rng.integers(0, 2)), fixed_budget=int(rng.integers(0, 25))))
+        n_req = int(rng.integers(1, 400))
+        cols = [wl.sim_arrivals_poisson(1, n_req, float(rng.uniform(0.1, 10.0)), seed=1000 + 64 * trial + r) for r in range(64)]
+        arr = np.ascontiguousarray(np.concatenate(cols, axis=1))
+        sid = wl.sim_sample_ids(64, n_req, S, seed=2000 + trial)
+        pid = rng.integers(0, 16, size=64).astype(np.int32)
+        g = _run_gpu(arr, sid, pid, pols, pool, deadline=float(rng.uniform(1.0, 60.0)))
+        # _compare uses the default deadline for the summary; recompute with the one used
+        import oracle
+        flips = 0
+        for r in range(64):
+            o = oracle.sim_queue(arr[:, r], sid[:, r], pool, oracle.SimPolicy(**pols[pid[r]]))
+            if o["margin"].min() < 1e-12:
+                flips += 1
+                continue
+            assert np.array_equal(g["chunks"][:, r], o["chunks"]) and np.array_equal(g["budget"][:, r], o["budget"])
+            assert np.array_equal(g["exited"][:, r], o["exited"]) and np.array_equal(g["finish"][:, r], o["finish"])
+            s = oracle.sim_summary(arr[:, r], o["finish"], o["chunks"], 30.0)
+            assert np.array_equal(g["summary"][r, [0, 1, 2, 4]], s[[0, 1, 2, 4]])
+        assert flips <= 1
