@@ -570,7 +570,7 @@ def run_ours(args):
                      sync_value=float(w.N_valid) * world / (e2e_sync_ms / args.steps * 1e-3),
                      sync_ms_per_step=e2e_sync_ms / args.steps,
                      sync_api="laser_probe_confidence_host (one batch at a time, rank 0's figure x ranks)"),
-            gpu_launches=int(launches),
+            gpu_launches=int(launches) * world,      # every rank enqueues the same calls
             roofline=roof,
             realised=realised_distribution(w, case),
         )
