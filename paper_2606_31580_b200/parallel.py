@@ -98,7 +98,13 @@ class VocabParallelProbe:
             return sh.combine(req_offsets, load, params, stats_all=stats_all, agg=agg,
                               token_prob=token_ids is not None, stream=stream, wait_flags=flags, epoch=epoch)
         sh.partial(hidden, W_shard, req_offsets, token_ids=token_ids, stream=stream)
-        gather_row_stats(self.dist, sh.stats_local, sh.stats_all, self.group)
+        if stream is not None:
+            # the collective is ordered against torch's CURRENT stream: make that the caller's stream
+            import torch
+            with torch.cuda.stream(stream):
+                gather_row_stats(self.dist, sh.stats_local, sh.stats_all, self.group)
+        else:
+            gather_row_stats(self.dist, sh.stats_local, sh.stats_all, self.group)
         return sh.combine(req_offsets, load, params, agg=agg, token_prob=token_ids is not None, stream=stream)
 
 
