@@ -250,9 +250,12 @@ def test_vocab_parallel_process_group_world1(P, exchange):
         ora, rows, reqs = P.run_oracle(w)
         vp = par.VocabParallelProbe(dist, w.N_alloc, w.d, w.V, w.R, dev0, exchange=exchange, debug_outputs=True)
         Wg = dev["W"][vp.v0:vp.v1].contiguous()
-        for it in range(5):      # several epochs: both buffer sets are reused
+        side = torch.cuda.Stream()
+        for it in range(5):      # several epochs: both buffer sets are reused; odd ones on a side stream
             vp.shard.conf.fill_(-7.0); vp.shard.argmax.fill_(-7); vp.shard.exit.fill_(7)
-            out = vp(dev["hidden"], Wg, dev["off"], dev["load"], B.TauParams(**w.tau_params))
+            torch.cuda.synchronize()
+            out = vp(dev["hidden"], Wg, dev["off"], dev["load"], B.TauParams(**w.tau_params),
+                     stream=side if it % 2 else None)
             torch.cuda.synchronize()
             g = P.GpuRun(out.conf.cpu().numpy(), out.argmax.cpu().numpy(), out.exit.cpu().numpy(),
                          out.tau.cpu().numpy(), out.pmax.cpu().numpy(), vp.shard.plan)
