@@ -272,7 +272,8 @@ int laser_sim_run(const double* arrival, const int32_t* sample_id, const int32_t
         int n_pow2 = 1;
         while (n_pow2 < dims->n_req) n_pow2 <<= 1;
         const size_t smem = static_cast<size_t>(n_pow2) * sizeof(double);
-        static bool attr_set = false;
+        static bool attr_set_dev[64] = {};    // the attribute is per device
+        bool& attr_set = attr_set_dev[dev & 63];
         if (!attr_set) {
             if (cudaFuncSetAttribute(laser_sim_p95_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      LASER_SIM_MAX_P95_REQUESTS * static_cast<int>(sizeof(double))) != cudaSuccess) {
