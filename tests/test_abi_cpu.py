@@ -200,3 +200,33 @@ def test_sim_validation_needs_no_gpu():
     pol.alpha = 0.3
     args[10] = C.byref(empty)
     assert L.laser_sim_run(*args) == 0                       # nothing to simulate
+
+
+def test_headers_are_plain_c_and_link(tmp_path):
+    """include/*.h compile as C99 (no C++-isms, no torch types) and a C program links against the
+    library and calls host-only entry points."""
+    import shutil, subprocess
+    if not shutil.which("gcc"):
+        pytest.skip("gcc not on PATH")
+    src = tmp_path / "abi.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include "laser_probe.h"
+#include "laser_sim.h"
+int main(void) {
+    laser_tau_params t; laser_sim_policy sp; laser_probe_dims d = {128, 1536, 151936, 16}; laser_probe_plan pl;
+    float load[3] = {0.0f, 10.0f, 20.0f}, tau[3];
+    if (laser_tau_params_default(&t) != LASER_OK || laser_sim_policy_default(&sp) != LASER_OK) return 1;
+    if (laser_tau_from_load(load, 3, &t, tau) != LASER_OK) return 2;
+    if (laser_probe_plan_query(&d, &pl) != LASER_OK || laser_probe_workspace_bytes(&d) == 0) return 3;
+    if (laser_probe_confidence(0, 0, 0, 0, &t, 0, 0, 0, &d, 0, 0, 0, 0, 0) != LASER_E_NULL) return 4;
+    printf("%.6f %.6f %.6f %d %s\n", tau[0], tau[1], tau[2], pl.splits, laser_status_string(LASER_E_ARCH));
+    return 0;
+}
+''')
+    exe = tmp_path / "abi"
+    so_dir = ROOT / "paper_2606_31580_b200"
+    subprocess.run(["gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-I", str(ROOT / "include"), str(src),
+                    "-o", str(exe), f"-L{so_dir}", "-llaser_probe", f"-Wl,-rpath,{so_dir}"], check=True)
+    out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
+    assert out[:3] == ["0.970000", "0.950000", "0.919536"] and int(out[3]) == 147
