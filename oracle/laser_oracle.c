@@ -347,12 +347,17 @@ double laser_oracle_f_load(double L, const oracle_budget_params* q) {
     return (f < 1.0) ? f : 1.0;
 }
 
-/* Eq. 6: B = max{B_min, floor(B_base * f_diff * f_load)}; raw L(t) (DESIGN A14) */
+/* Eq. 6: B = max{B_min, floor(B_base * f_diff * f_load)}; raw L(t) (DESIGN A14).
+ * The floor is that of the real-number product.  Evaluated in binary the product can land one ulp
+ * below an integer that the exact value reaches (paper defaults, |p| = 100: f_diff = 0.6 + 50/225*0.9
+ * = 0.8 exactly and B = floor(10*0.8) = 8, while 0.6 + 50.0/225.0*0.9 = 0.7999999999999999), so the
+ * floor is taken of product + 1e-9 (DESIGN A19) - far above any rounding error of three
+ * multiplications (~1e-15) and far below the spacing of the exact values next to an integer. */
 int laser_oracle_budget(const double* prompt_tokens, const double* L, int64_t R,
                         const oracle_budget_params* q, int32_t* out_B) {
     if (R < 0 || !q || (R > 0 && (!prompt_tokens || !L || !out_B))) return -1;
     for (int64_t r = 0; r < R; ++r) {
-        double b = floor(q->b_base * laser_oracle_f_diff(prompt_tokens[r], q) * laser_oracle_f_load(L[r], q));
+        double b = floor(q->b_base * laser_oracle_f_diff(prompt_tokens[r], q) * laser_oracle_f_load(L[r], q) + 1e-9);
         if (b < q->b_min) b = q->b_min;
         out_B[r] = (int32_t)b;
     }

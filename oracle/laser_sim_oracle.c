@@ -6,9 +6,9 @@
  * path.  Citations are /root/reference/PAPER.md line numbers; "DESIGN S<n>" are the readings listed
  * in DESIGN.md §10 where the paper is silent.
  *
- * The paper (§5.1): "we employ discrete-event simulation.  We first run each method on
- * all benchmark samples to obtain per-sample inference times and accuracy, then simulate Poisson
- * arrivals ... using a single-server FIFO queue", SLO deadline d = 30 s; metrics: average latency, P95
+ * The paper's evaluation vehicle (§5.1) is a discrete-event simulation: per-sample
+ * inference times and accuracy are measured once, then Poisson arrivals are played into a
+ * single-server FIFO queue with an SLO deadline d = 30 s; the metrics are average latency, P95
  * latency, throughput, SLO satisfaction.  Here the per-sample data is a POOL of S
  * samples, each with its prompt length, prefill time, conclusion time and, per reasoning chunk k, the
  * chunk's duration and the confidence measured at the ATP that ends it (Eq. 2, PAPER.md:63-68:
@@ -68,7 +68,7 @@ static int32_t sim_budget(double prompt_tokens, double L, const sim_policy* p) {
     double den = (L > 1.0) ? L : 1.0;
     double f_load = p->budget_l_target / den;
     if (f_load > 1.0) f_load = 1.0;
-    double b = floor(p->b_base * f_diff * f_load);
+    double b = floor(p->b_base * f_diff * f_load + 1e-9);   /* floor of the real product, DESIGN A19 */
     if (b < p->b_min) b = p->b_min;
     return (int32_t)b;
 }

@@ -109,3 +109,24 @@ def test_budget_eq6_to_8_pins():
     B = oracle.budget([50, 275, 275, 162.5, 50, 275], [0, 0, 20, 30, 100, 1000], q)
     #   floor(10*.6*1)=6, floor(10*1.5)=15, floor(15*.5)=7, floor(10*1.05/3)=3, max(2, floor(.6))=2, 2
     assert list(B) == [6, 15, 7, 3, 2, 2]
+
+
+def test_budget_floor_is_that_of_the_exact_product():
+    """Eq. 6 floors a real-number product.  Exact rational arithmetic (a different
+    formulation from the oracle's doubles) over the whole grid |p| < 600, L <= 60 with the paper's
+    defaults: the oracle must agree everywhere, in particular at the points where
+    the exact product IS an integer and binary evaluation lands one ulp below it (DESIGN A19)."""
+    from fractions import Fraction as Fr
+    q = oracle.BudgetParams()
+    f_min, f_max, p_min, p_max, b_base, b_min, l_t = Fr(3, 5), Fr(3, 2), 50, 275, 10, 2, 10
+    ps, Ls = np.meshgrid(np.arange(1, 600), np.arange(0, 61), indexing="ij")
+    got = oracle.budget(ps.ravel().astype(np.float64), Ls.ravel().astype(np.float64), q)
+    want = []
+    for p_, L_ in zip(ps.ravel().tolist(), Ls.ravel().tolist()):
+        fd = min(max(f_min + Fr(p_ - p_min, p_max - p_min) * (f_max - f_min), f_min), f_max)
+        fl = min(Fr(1), Fr(l_t, max(1, L_)))
+        want.append(max(b_min, (b_base * fd * fl).__floor__()))
+    want = np.asarray(want)
+    assert np.array_equal(got, want), np.flatnonzero(got != want)[:10]
+    # the two interior exact-integer points named in the review of round 1
+    assert list(oracle.budget([100.0, 65.0], [5.0, 11.0], q)) == [8, 6]
