@@ -15,10 +15,13 @@
  *   a5  exit[r] = conf[r] > tau[r]   (strict)             PAPER.md:61, 70, 122 (Algorithm 1 step 6)
  *
  * Device code is sm_100a only (TMA + tcgen05/TMEM).  There is no fallback of any kind: on another
- * device the call returns LASER_E_ARCH.  The library never allocates device memory, never
- * synchronises the host with the device and never reads device data on the host; all work is
- * enqueued on the caller's stream.  The only internal state is a small host-side cache of encoded
- * TMA descriptors, released by laser_shutdown().
+ * device the call returns LASER_E_ARCH.  The library never allocates device memory per call, never
+ * synchronises the host with the device (outside the *_host entry points) and never reads device
+ * data on the host; all work is enqueued on the caller's stream.  Internal state: one 64 KB control
+ * block per device, allocated at first use (the counters with which the CTAs of the fused kernel
+ * hand over to its last phase; never the caller's workspace), and probe handles - explicit
+ * (laser_probe_handle_create) or implicit, cached per thread - holding the launch plan and the
+ * encoded TMA descriptors.
  *
  * All functions return an int status (LASER_OK == 0, errors negative); none throws or aborts.
  */
@@ -76,32 +79,44 @@ typedef struct {
     int32_t grid;            /* CTAs of the fused kernel (persistent, <= num_sms)                     */
     int32_t work_items;      /* m_tiles * splits                                                      */
     int32_t smem_bytes;      /* dynamic shared memory per CTA                                         */
-    int32_t kernel_launches; /* kernels one laser_probe_confidence call enqueues                      */
+    int32_t kernel_launches; /* kernels one laser_probe_confidence call enqueues: 1 (a3-a5 run in the
+                                fused kernel's tail) or 2 (LASER_TAIL_SEPARATE)                        */
     int32_t tile_m;          /* token rows per work item: 128 (one CTA) or 256 (CTA pair)             */
     int32_t cta_pair;        /* 1: clusters of two CTAs, tcgen05 cta_group::2; 0: one CTA per item    */
-    int32_t ws_splits;       /* workspace records per row (>= splits: the most any re-plan can use)   */
+    int32_t ws_records;      /* 16-byte workspace records (the most any re-plan of the batch writes)  */
+    int32_t tail_cache;      /* requests whose {offset, threshold} the fused kernel's tail keeps in the
+                                shared memory the pipeline leaves over (0: read from global memory)    */
 } laser_probe_plan;
 
-/* Kernel variant selection.  AUTO (default): one CTA per work item for N <= 128 rows and for small
- * odd counts of 128-row tiles (< 10), CTA pairs otherwise.  SINGLE / PAIR force one variant for every shape (tuning and tests; both are exact).
- * Process-wide; affects laser_probe_plan_query / workspace_bytes and subsequent calls. */
+/* Kernel variant (laser_probe_options.kernel_mode).  AUTO (default): one CTA per work item for
+ * N <= 128 rows and for small odd counts of 128-row tiles (< 10), CTA pairs otherwise.  SINGLE / PAIR
+ * force one variant for every shape (tuning and tests; both are exact). */
 enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2 };
-int laser_probe_set_mode(int mode);
 
-/* Overlap of back-to-back probe calls on one stream (programmatic dependent launch).
- * 0 (default): strict - the fused kernel executes griddepcontrol.wait before its first global read,
- *    so every input is read in stream order whatever kernel precedes the call (including a producer
- *    of `hidden` that triggers its dependents early).  Only the kernel's prologue (barrier init,
- *    TMEM allocation, descriptor prefetch) overlaps the preceding kernel.
- * 1: the fused kernel of a call starts streaming W and hidden as soon as SMs are free, i.e. while
- *    the kernel enqueued just before it on the stream may still be running; only its workspace
- *    stores and its completion wait for that kernel.  Exact whenever hidden, W and req_offsets are
- *    complete when the preceding kernel STARTS - which CUDA guarantees unless that kernel itself
- *    issues griddepcontrol.launch_dependents (cudaTriggerProgrammaticLaunchCompletion) before it has
- *    written them.  The library's own kernels only hand over the workspace and the outputs, which
- *    the next call never reads early, so a loop of probe calls (bench.py's timed region) may opt in.
- * Process-wide; affects subsequent calls. */
-int laser_probe_set_overlap(int enable);
+/* Where merge + a3-a5 run (laser_probe_options.tail).
+ *   FUSED     in the tail of the fused kernel: every CTA counts itself in when its records are in the
+ *             workspace, the first min(grid, R) CTAs wait for the count and share the requests.  One
+ *             launch per call.  Needs a control slot of the library's per-device control block.
+ *   SEPARATE  a second kernel (laser_probe_finalize_kernel) behind the fused one.  Two launches.
+ *   AUTO      FUSED for strict calls when a control slot is available (the only case where none is:
+ *             the very first call on a device is made under CUDA stream capture, where nothing can
+ *             be allocated); SEPARATE for overlap = 1 calls (measured faster there: the tiny second
+ *             kernel runs beside the next call's CTAs instead of holding their SMs). */
+enum { LASER_TAIL_AUTO = 0, LASER_TAIL_FUSED = 1, LASER_TAIL_SEPARATE = 2 };
+
+/* Ordering against the kernel ahead of the call on the stream (laser_probe_options.overlap).  The
+ * fused kernel is launched with programmatic dependent launch, i.e. it may become resident while
+ * that kernel is still running.
+ * 0 (default, strict): `hidden`, `req_offsets`, `load` and `token_ids` are read only after the kernel
+ *    ahead has completed (griddepcontrol.wait), whatever that kernel is - e.g. the forward pass that
+ *    writes `hidden` (Algorithm 1).  W IS READ EARLIER: it is the model's LM-head
+ *    weight, and the call requires that the kernel ahead of it on the stream does not write W.  The
+ *    kernel requests the first W tiles of every CTA ahead of the wait, so the head of the W stream
+ *    overlaps the tail of the preceding kernel.
+ * 1 (overlap): every input may be read while the kernel ahead is still running; only the kernel's
+ *    stores (workspace, outputs) wait for it.  Exact whenever hidden, W, req_offsets, load are
+ *    complete when the preceding kernel STARTS - true for a loop of probe calls over resident
+ *    inputs, false behind a producer of `hidden`. */
 
 /* Aggregate that turns the per-token max probabilities of a request into its confidence.
  * The paper does not fix it; MEAN is the default reading (A1). */
@@ -110,12 +125,15 @@ enum { LASER_AGG_MEAN = 0, LASER_AGG_GEOMEAN = 1, LASER_AGG_MIN = 2 };
 /* Writes the paper's defaults.  Host. */
 int laser_tau_params_default(laser_tau_params* out);
 
-/* Device scratch laser_probe_confidence needs for `dims`, in bytes (16 * ws_splits * m_tiles * tile_m,
- * at least 16).  Returns 0 for invalid dims.  Host; needs no GPU. */
+/* Device scratch laser_probe_confidence needs for `dims`, in bytes: 16 * ws_records of the larger of
+ * the two kernel variants' plans (so one buffer serves every kernel_mode), at least 16.  Returns 0
+ * for invalid dims.  Host; needs no GPU. */
 size_t laser_probe_workspace_bytes(const laser_probe_dims* dims);
 
-/* Fills *plan for `dims`.  Host; needs no GPU (assumes 148 SMs when no device is present). */
+/* Fills *plan for `dims` (LASER_MODE_AUTO / the given kernel_mode).  Host; needs no GPU (assumes 148
+ * SMs when no device is present). */
 int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan);
+int laser_probe_plan_query_mode(const laser_probe_dims* dims, int kernel_mode, laser_probe_plan* plan);
 
 /*
  * The hot path a1-a5.  Asynchronous on `stream`; returns after enqueueing.
@@ -123,7 +141,9 @@ int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan)
  *   hidden       device, bf16 [N, d] row-major, 16-byte aligned, d % 8 == 0.  Post-final-norm states.
  *   W            device, bf16 [V, d] row-major, 16-byte aligned (LM-head / unembedding matrix).
  *   req_offsets  device, int32 [R+1], non-decreasing, [0] == 0, [R] <= N (CSR over rows; a
- *                precondition, not checked: the library never reads device data on the host).
+ *                precondition: the library never reads device data on the host.  With the
+ *                environment variable LASER_DEBUG=1 a one-warp kernel checks it on the device ahead
+ *                of every call and traps on a violation - the call then surfaces as a CUDA error).
  *                Rows >= req_offsets[R] are padding.
  *   load         device, float [R]: smoothed load Lbar of each request's probe point, unit of l_target.
  *   tau_params   HOST pointer; copied by value into the launch.
@@ -164,12 +184,19 @@ int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t*
  *                     probability 0.  out_argmax is still the row argmax. */
 enum { LASER_PROB_MAX = 0, LASER_PROB_TOKEN = 1 };
 
-/* Options of laser_probe_confidence_opt / laser_probe_combine (HOST struct, copied by value). */
+/* Options of laser_probe_confidence_opt / laser_probe_handle_create / laser_probe_partial /
+ * laser_probe_combine (HOST struct, copied by value; per call, so two threads or streams may use
+ * different settings).  laser_probe_options_default() fills the defaults (all zero). */
 typedef struct {
     int32_t aggregate_mode;    /* LASER_AGG_*                                                        */
     int32_t prob_mode;         /* LASER_PROB_*                                                       */
     const int32_t* token_ids;  /* device, int32 [N]; required for LASER_PROB_TOKEN, else may be NULL */
+    int32_t kernel_mode;       /* LASER_MODE_*                                                       */
+    int32_t overlap;           /* 0 strict (default) / 1 overlap, see above                          */
+    int32_t tail;              /* LASER_TAIL_*                                                       */
+    int32_t reserved;          /* must be 0                                                          */
 } laser_probe_options;
+int laser_probe_options_default(laser_probe_options* out);
 
 /* laser_probe_confidence with options (NULL options = defaults: mean of the row maxima).  With
  * LASER_PROB_TOKEN, out_pmax_opt receives the token probabilities.  Costs no extra HBM traffic: the
@@ -180,6 +207,43 @@ int laser_probe_confidence_opt(const void* hidden, const void* W, const int32_t*
                                const laser_probe_dims* dims, void* workspace,
                                size_t workspace_bytes, void* stream, float* out_tau_opt,
                                float* out_pmax_opt, const laser_probe_options* options);
+
+/*
+ * Probe handles.  A handle fixes dims and options once and caches what does not change between
+ * calls: the launch plan, the encoded TMA descriptors of the hidden / W buffers it has been called
+ * with (2 / 4 most recent), the device-mapped addresses of pinned host buffers, and its control slot.
+ * A call through a handle takes no lock, hashes nothing and queries no pointer attributes; it is what
+ * a serving engine that probes the same shape every step should hold.  The handle-less entry points
+ * above use implicit handles from a small per-thread cache keyed by (device, dims, options,
+ * workspace).
+ *
+ * Thread safety: any number of handles may be used concurrently; ONE handle must be used by one
+ * thread at a time, and the calls made through it must be stream-ordered with respect to each other
+ * (they share the handle's control slot, like calls that share a workspace).
+ *
+ * laser_probe_handle_create   host; the current device must be a B200 (else LASER_E_ARCH).  options
+ *                             NULL = defaults; options->token_ids (LASER_PROB_TOKEN) is remembered.
+ * laser_probe_handle_run      laser_probe_confidence_opt with the handle's dims and options.
+ * laser_probe_handle_run_host laser_probe_confidence_host[_async] (synchronize != 0 / == 0).
+ * laser_probe_handle_plan     the handle's plan; kernel_launches says whether the tail is fused.
+ */
+typedef struct laser_probe_handle_s laser_probe_handle;
+int laser_probe_handle_create(laser_probe_handle** out, const laser_probe_dims* dims,
+                              const laser_probe_options* options);
+int laser_probe_handle_destroy(laser_probe_handle* h);
+int laser_probe_handle_plan(const laser_probe_handle* h, laser_probe_plan* plan);
+size_t laser_probe_handle_workspace_bytes(const laser_probe_handle* h);
+int laser_probe_handle_run(laser_probe_handle* h, const void* hidden, const void* W,
+                           const int32_t* req_offsets, const float* load,
+                           const laser_tau_params* tau_params, float* out_conf, int32_t* out_argmax,
+                           uint8_t* out_exit, void* workspace, size_t workspace_bytes, void* stream,
+                           float* out_tau_opt, float* out_pmax_opt);
+int laser_probe_handle_run_host(laser_probe_handle* h, const void* h_hidden, const void* W,
+                                const int32_t* h_req_offsets, const float* h_load,
+                                const laser_tau_params* tau_params, float* h_out_conf,
+                                int32_t* h_out_argmax, uint8_t* h_out_exit, void* workspace,
+                                size_t workspace_bytes, void* d_staging, size_t staging_bytes,
+                                void* stream, int synchronize);
 
 /*
  * Vocabulary-parallel probe (SURVEY.md §8 e: the LM head's tensor-parallel layout).  GPU g holds the
@@ -220,11 +284,15 @@ typedef struct {
  * 0; token_ids_opt (device int32 [N], GLOBAL ids) or NULL.  out_stats: device [N] or NULL (rows >=
  * req_offsets[R] get the neutral record {-inf, 0, INT32_MAX, -inf}).  peers_opt: see above; at least
  * one of out_stats / peers_opt must be given.  workspace as for laser_probe_confidence with the same
- * dims.  Asynchronous on `stream`; three kernels with peers (fused, reduce, signal), else two. */
+ * dims.  options: NULL or kernel_mode / overlap / tail (the aggregate fields are ignored here).
+ * Asynchronous on `stream`.  One kernel: the tail of the fused kernel merges each row's records,
+ * stores / pushes them, and the last CTA to finish raises the flags.  With LASER_TAIL_SEPARATE:
+ * three kernels with peers (fused, reduce, signal), else two. */
 int laser_probe_partial(const void* hidden, const void* W_shard, const int32_t* req_offsets,
                         const int32_t* token_ids_opt, const laser_probe_dims* dims, int32_t v_offset,
                         laser_row_stats* out_stats, const laser_probe_peers* peers_opt,
-                        void* workspace, size_t workspace_bytes, void* stream);
+                        void* workspace, size_t workspace_bytes, void* stream,
+                        const laser_probe_options* options);
 
 /* Merge + a3-a5 over gathered statistics.  stats: device [G, N] (shard-major).  dims->N and dims->R
  * are used (d, V ignored but must be valid).  wait_flags_opt: device uint32 [G] or NULL; when given
@@ -278,15 +346,20 @@ int laser_tau_from_load(const float* load, int32_t R, const laser_tau_params* ta
  * EMA: lbar <- alpha*L + (1-alpha)*lbar, in place over R independent trackers. */
 int laser_ema_update(float* lbar, const float* L, int32_t R, float alpha);
 
-/* Budget pre-allocation, Eq. 6-8; defaults PAPER.md:166, 195. */
+/* Budget pre-allocation, Eq. 6-8; defaults PAPER.md:166, 195.  IEEE double
+ * throughout.  Eq. 6 takes the floor of a real-number product; its binary evaluation can land a hair
+ * below an integer the exact product reaches (paper defaults, |p| = 100: f_diff = 0.6 + 50/225 * 0.9
+ * = 0.8 exactly, B = floor(10 * 0.8) = 8, yet 0.6 + 50.0/225.0*0.9 = 0.7999999999999999 in binary).
+ * The floor is therefore taken of product + LASER_BUDGET_FLOOR_EPS (reading A19). */
+#define LASER_BUDGET_FLOOR_EPS 1e-9
 typedef struct {
-    float b_base;   /* 10  */
-    float b_min;    /* 2   */
-    float f_min;    /* 0.6 */
-    float f_max;    /* 1.5 */
-    float p_min;    /* 50  */
-    float p_max;    /* 275 */
-    float l_target; /* 10  */
+    double b_base;   /* 10  */
+    double b_min;    /* 2   */
+    double f_min;    /* 0.6 */
+    double f_max;    /* 1.5 */
+    double p_min;    /* 50  */
+    double p_max;    /* 275 */
+    double l_target; /* 10  */
 } laser_budget_params;
 int laser_budget_params_default(laser_budget_params* out);
 int laser_allocate_budget(const int32_t* prompt_tokens, const float* L, int32_t R,
@@ -295,8 +368,9 @@ int laser_allocate_budget(const int32_t* prompt_tokens, const float* L, int32_t 
 /*
  * Per-kernel timing for bench / profiling (thread-local; off by default).  While enabled, each
  * laser_probe_confidence* call on this thread records CUDA events on its stream before the fused
- * kernel, between the two kernels and after the finalize kernel (up to 512 calls; programmatic
- * dependent launch is not used for those calls).  laser_profile_read() waits for the last recorded
+ * kernel, after it and after the finalize kernel if the call has one (up to 512 calls; programmatic
+ * dependent launch is not used for those calls).  With the fused tail ms_finalize_sum is 0: merge and
+ * a3-a5 are inside the fused kernel's duration.  laser_profile_read() waits for the last recorded
  * call, returns the summed durations in milliseconds and the number of calls, and resets the count.
  */
 int laser_profile_enable(int on);
@@ -308,7 +382,8 @@ const char* laser_status_string(int status);
 const char* laser_last_error(void);
 /* Number of kernels this library has enqueued since load (all threads). */
 uint64_t laser_kernel_launch_count(void);
-/* Drops the TMA descriptor cache. */
+/* Drops the implicit handles (each thread frees its own at its next call).  Explicit handles are the
+ * caller's to destroy.  The control block stays until process exit. */
 int laser_shutdown(void);
 
 #ifdef __cplusplus

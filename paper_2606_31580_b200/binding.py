@@ -17,6 +17,7 @@ _lib = None
 AGG_MEAN, AGG_GEOMEAN, AGG_MIN = 0, 1, 2
 PROB_MAX, PROB_TOKEN = 0, 1
 MODE_AUTO, MODE_SINGLE, MODE_PAIR = 0, 1, 2
+TAIL_AUTO, TAIL_FUSED, TAIL_SEPARATE = 0, 1, 2
 
 EXPORTS = [
     "laser_tau_params_default", "laser_probe_workspace_bytes", "laser_probe_plan_query",
@@ -24,8 +25,10 @@ EXPORTS = [
     "laser_probe_confidence_host", "laser_probe_confidence_host_async", "laser_tau_from_load", "laser_ema_update",
     "laser_budget_params_default", "laser_allocate_budget", "laser_status_string",
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
-    "laser_profile_read", "laser_probe_set_mode", "laser_probe_set_overlap",
+    "laser_profile_read", "laser_probe_options_default", "laser_probe_plan_query_mode",
     "laser_probe_confidence_opt", "laser_probe_partial", "laser_probe_combine",
+    "laser_probe_handle_create", "laser_probe_handle_destroy", "laser_probe_handle_plan",
+    "laser_probe_handle_workspace_bytes", "laser_probe_handle_run", "laser_probe_handle_run_host",
     "laser_sim_policy_default", "laser_sim_run",
 ]
 
@@ -41,8 +44,8 @@ class TauParams(C.Structure):
 
 
 class BudgetParams(C.Structure):
-    """laser_budget_params; defaults PAPER.md:166, 195."""
-    _fields_ = [(n, C.c_float) for n in
+    """laser_budget_params (doubles); defaults PAPER.md:166, 195."""
+    _fields_ = [(n, C.c_double) for n in
                 ("b_base", "b_min", "f_min", "f_max", "p_min", "p_max", "l_target")]
 
     def __init__(self, b_base=10.0, b_min=2.0, f_min=0.6, f_max=1.5, p_min=50.0, p_max=275.0,
@@ -57,15 +60,21 @@ class Dims(C.Structure):
 class Plan(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("num_sms", "m_tiles", "splits", "tiles_per_split", "tile_n", "k_blocks", "stages",
-                 "grid", "work_items", "smem_bytes", "kernel_launches", "tile_m", "cta_pair", "ws_splits")]
+                 "grid", "work_items", "smem_bytes", "kernel_launches", "tile_m", "cta_pair", "ws_records", "tail_cache")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
 
 
 class Options(C.Structure):
-    """laser_probe_options."""
-    _fields_ = [("aggregate_mode", C.c_int32), ("prob_mode", C.c_int32), ("token_ids", C.c_void_p)]
+    """laser_probe_options (per call: aggregate, probability, kernel variant, overlap, tail)."""
+    _fields_ = [("aggregate_mode", C.c_int32), ("prob_mode", C.c_int32), ("token_ids", C.c_void_p),
+                ("kernel_mode", C.c_int32), ("overlap", C.c_int32), ("tail", C.c_int32),
+                ("reserved", C.c_int32)]
+
+    def __init__(self, aggregate_mode=AGG_MEAN, prob_mode=PROB_MAX, token_ids=None, kernel_mode=MODE_AUTO,
+                 overlap=0, tail=TAIL_AUTO):
+        super().__init__(aggregate_mode, prob_mode, token_ids, kernel_mode, int(bool(overlap)), tail, 0)
 
 
 MAX_PEERS = 16
@@ -119,12 +128,22 @@ def lib():
         L.laser_probe_staging_bytes.argtypes = [dp]
         L.laser_probe_staging_bytes.restype = C.c_size_t
         L.laser_probe_plan_query.argtypes = [dp, C.POINTER(Plan)]
+        L.laser_probe_plan_query_mode.argtypes = [dp, C.c_int, C.POINTER(Plan)]
+        L.laser_probe_options_default.argtypes = [C.POINTER(Options)]
+        L.laser_probe_handle_create.argtypes = [C.POINTER(C.c_void_p), dp, C.POINTER(Options)]
+        L.laser_probe_handle_destroy.argtypes = [vp]
+        L.laser_probe_handle_plan.argtypes = [vp, C.POINTER(Plan)]
+        L.laser_probe_handle_workspace_bytes.argtypes = [vp]
+        L.laser_probe_handle_workspace_bytes.restype = C.c_size_t
+        L.laser_probe_handle_run.argtypes = [vp, vp, vp, i32p, fp, tp, fp, i32p, u8p, vp, C.c_size_t, vp, fp, fp]
+        L.laser_probe_handle_run_host.argtypes = [vp, vp, vp, i32p, fp, tp, fp, i32p, u8p, vp, C.c_size_t,
+                                                  vp, C.c_size_t, vp, C.c_int]
         common = [vp, vp, i32p, fp, tp, fp, i32p, u8p, dp, vp, C.c_size_t, vp, fp, fp]
         L.laser_probe_confidence.argtypes = common
         L.laser_probe_confidence_agg.argtypes = common + [C.c_int]
         L.laser_probe_confidence_opt.argtypes = common + [C.POINTER(Options)]
         L.laser_probe_partial.argtypes = [vp, vp, i32p, i32p, dp, C.c_int32, vp, C.POINTER(Peers), vp,
-                                          C.c_size_t, vp]
+                                          C.c_size_t, vp, C.POINTER(Options)]
         L.laser_probe_combine.argtypes = [vp, C.c_int32, i32p, fp, tp, fp, i32p, u8p, dp, vp, fp, fp,
                                           C.POINTER(Options), vp, C.c_uint32]
         L.laser_probe_confidence_host.argtypes = [vp, vp, i32p, fp, tp, fp, i32p, u8p, dp, vp,
@@ -138,8 +157,6 @@ def lib():
         L.laser_status_string.restype = C.c_char_p
         L.laser_last_error.restype = C.c_char_p
         L.laser_kernel_launch_count.restype = C.c_uint64
-        L.laser_probe_set_mode.argtypes = [C.c_int]
-        L.laser_probe_set_overlap.argtypes = [C.c_int]
         L.laser_profile_enable.argtypes = [C.c_int]
         L.laser_profile_read.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_int32)]
         L.laser_sim_policy_default.argtypes = [C.POINTER(SimPolicy)]
@@ -158,9 +175,9 @@ def _check(rc):
         raise LaserError(rc, txt)
 
 
-def plan_query(N, d, V, R) -> dict:
+def plan_query(N, d, V, R, mode=MODE_AUTO) -> dict:
     p = Plan()
-    _check(lib().laser_probe_plan_query(C.byref(Dims(N, d, V, R)), C.byref(p)))
+    _check(lib().laser_probe_plan_query_mode(C.byref(Dims(N, d, V, R)), mode, C.byref(p)))
     return p.as_dict()
 
 
@@ -172,14 +189,32 @@ def staging_bytes(N, d, V, R) -> int:
     return int(lib().laser_probe_staging_bytes(C.byref(Dims(N, d, V, R))))
 
 
-def set_mode(mode: int):
-    """laser_probe_set_mode: MODE_AUTO / MODE_SINGLE / MODE_PAIR (process-wide kernel variant)."""
-    _check(lib().laser_probe_set_mode(mode))
+class Handle:
+    """laser_probe_handle: dims + options fixed once; plan, TMA descriptors and control slot cached."""
 
+    def __init__(self, dims: Dims, options: Options):
+        self._h = C.c_void_p()
+        self._token_keepalive = None
+        _check(lib().laser_probe_handle_create(C.byref(self._h), C.byref(dims), C.byref(options)))
 
-def set_overlap(enable: bool):
-    """laser_probe_set_overlap: let back-to-back calls on a stream overlap, or keep strict stream order (default)."""
-    _check(lib().laser_probe_set_overlap(1 if enable else 0))
+    def plan(self) -> dict:
+        p = Plan()
+        _check(lib().laser_probe_handle_plan(self._h, C.byref(p)))
+        return p.as_dict()
+
+    def workspace_bytes(self) -> int:
+        return int(lib().laser_probe_handle_workspace_bytes(self._h))
+
+    def close(self):
+        if self._h:
+            lib().laser_probe_handle_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def kernel_launch_count() -> int:
@@ -236,14 +271,19 @@ class ProbeOutputs:
 
 
 class Probe:
-    """Caller-owned buffers for repeated laser_probe_confidence calls of one shape (device memory
-    from torch; the library itself allocates nothing)."""
+    """Caller-owned buffers for repeated probe calls of one shape (device memory from torch; the
+    library allocates nothing per call).  mode / overlap / tail are laser_probe_options fields, fixed
+    per Probe.  use_handle=True (default) goes through laser_probe_handle_run (one handle per
+    aggregate / token-id buffer, created on first use); use_handle=False through the handle-less
+    laser_probe_confidence_opt."""
 
-    def __init__(self, N, d, V, R, device="cuda", debug_outputs=True):
+    def __init__(self, N, d, V, R, device="cuda", debug_outputs=True, mode=MODE_AUTO, overlap=False,
+                 tail=TAIL_AUTO, use_handle=True):
         import torch
         self.torch = torch
         self.dims = Dims(N, d, V, R)
         self.device = torch.device(device)
+        self.mode, self.overlap, self.tail, self.use_handle = mode, bool(overlap), tail, use_handle
         wb = workspace_bytes(N, d, V, R)
         if wb == 0:
             raise LaserError(-2, "invalid dimensions")
@@ -253,7 +293,16 @@ class Probe:
         self.exit = torch.empty(R, dtype=torch.uint8, device=self.device)
         self.tau = torch.empty(R, dtype=torch.float32, device=self.device) if debug_outputs else None
         self.pmax = torch.empty(N, dtype=torch.float32, device=self.device) if debug_outputs else None
-        self.plan = plan_query(N, d, V, R)
+        self.plan = plan_query(N, d, V, R, mode)
+        self.plan["kernel_launches"] = 2 if (tail == TAIL_SEPARATE or (tail == TAIL_AUTO and overlap)) else 1
+        self._handles = {}
+
+    def _options(self, agg, token_ids) -> Options:
+        torch = self.torch
+        if token_ids is None:
+            return Options(agg, PROB_MAX, None, self.mode, self.overlap, self.tail)
+        assert token_ids.dtype == torch.int32 and token_ids.numel() == self.dims.N and token_ids.is_contiguous()
+        return Options(agg, PROB_TOKEN, token_ids.data_ptr(), self.mode, self.overlap, self.tail)
 
     def __call__(self, hidden, W, req_offsets, load, params: TauParams, stream=None, agg=AGG_MEAN,
                  token_ids=None):
@@ -269,21 +318,30 @@ class Probe:
         assert req_offsets.dtype == torch.int32 and req_offsets.numel() == d.R + 1
         assert load.dtype == torch.float32 and load.numel() == d.R
         s = (stream or torch.cuda.current_stream(self.device)).cuda_stream
-        opt = _options(torch, agg, token_ids, d.N)
-        _check(lib().laser_probe_confidence_opt(
-            hidden.data_ptr(), W.data_ptr(), req_offsets.data_ptr(), load.data_ptr(),
-            C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(),
-            C.byref(d), self.workspace.data_ptr(), self.workspace.numel(), s,
-            self.tau.data_ptr() if self.tau is not None else None,
-            self.pmax.data_ptr() if self.pmax is not None else None, C.byref(opt)))
+        tau = self.tau.data_ptr() if self.tau is not None else None
+        pmax = self.pmax.data_ptr() if self.pmax is not None else None
+        if self.use_handle:
+            key = (agg, token_ids.data_ptr() if token_ids is not None else None)
+            h = self._handles.get(key)
+            if h is None:
+                h = self._handles[key] = Handle(d, self._options(agg, token_ids))
+                h._token_keepalive = token_ids
+            _check(lib().laser_probe_handle_run(
+                h._h, hidden.data_ptr(), W.data_ptr(), req_offsets.data_ptr(), load.data_ptr(),
+                C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(),
+                self.workspace.data_ptr(), self.workspace.numel(), s, tau, pmax))
+        else:
+            opt = self._options(agg, token_ids)
+            _check(lib().laser_probe_confidence_opt(
+                hidden.data_ptr(), W.data_ptr(), req_offsets.data_ptr(), load.data_ptr(),
+                C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(),
+                C.byref(d), self.workspace.data_ptr(), self.workspace.numel(), s, tau, pmax, C.byref(opt)))
         return ProbeOutputs(self.conf, self.argmax, self.exit, self.tau, self.pmax)
 
-
-def _options(torch, agg, token_ids, N) -> Options:
-    if token_ids is None:
-        return Options(agg, PROB_MAX, None)
-    assert token_ids.dtype == torch.int32 and token_ids.numel() == N and token_ids.is_contiguous()
-    return Options(agg, PROB_TOKEN, token_ids.data_ptr())
+    def close(self):
+        for h in self._handles.values():
+            h.close()
+        self._handles = {}
 
 
 class VocabShardProbe:
@@ -295,9 +353,11 @@ class VocabShardProbe:
     parallel.VocabParallelProbe) and calls `combine`.  With `peers` (parallel.PeerExchange) partial
     pushes the records into every rank's gathered buffer itself and combine waits for the flags."""
 
-    def __init__(self, N, d, V_shard, R, v_offset, world, device="cuda", debug_outputs=True):
+    def __init__(self, N, d, V_shard, R, v_offset, world, device="cuda", debug_outputs=True, mode=MODE_AUTO,
+                 overlap=False, tail=TAIL_AUTO):
         import torch
         self.torch = torch
+        self.options = Options(AGG_MEAN, PROB_MAX, None, mode, overlap, tail)
         self.dims = Dims(N, d, V_shard, R)
         self.v_offset, self.world = int(v_offset), int(world)
         self.device = torch.device(device)
@@ -312,7 +372,7 @@ class VocabShardProbe:
         self.exit = torch.empty(R, dtype=torch.uint8, device=self.device)
         self.tau = torch.empty(R, dtype=torch.float32, device=self.device) if debug_outputs else None
         self.pmax = torch.empty(N, dtype=torch.float32, device=self.device) if debug_outputs else None
-        self.plan = plan_query(N, d, V_shard, R)
+        self.plan = plan_query(N, d, V_shard, R, mode)
 
     def _stream(self, stream):
         return (stream or self.torch.cuda.current_stream(self.device)).cuda_stream
@@ -332,7 +392,7 @@ class VocabShardProbe:
             hidden.data_ptr(), W_shard.data_ptr(), req_offsets.data_ptr(),
             token_ids.data_ptr() if token_ids is not None else None, C.byref(d), self.v_offset,
             out.data_ptr(), C.byref(peers) if peers is not None else None,
-            self.workspace.data_ptr(), self.workspace.numel(), self._stream(stream)))
+            self.workspace.data_ptr(), self.workspace.numel(), self._stream(stream), C.byref(self.options)))
         return out
 
     def combine(self, req_offsets, load, params: TauParams, stats_all=None, agg=AGG_MEAN, token_prob=False,
@@ -352,9 +412,10 @@ class VocabShardProbe:
 
 
 class HostProbe:
-    """laser_probe_confidence_host: per-step tensors in pinned HOST memory, W resident on device."""
+    """Host-buffer entry points: per-step tensors in pinned HOST memory, W resident on device.
+    use_handle=True: laser_probe_handle_run_host; False: laser_probe_confidence_host[_async]."""
 
-    def __init__(self, N, d, V, R, device="cuda"):
+    def __init__(self, N, d, V, R, device="cuda", use_handle=True, mode=MODE_AUTO, tail=TAIL_AUTO):
         import torch
         self.torch = torch
         self.dims = Dims(N, d, V, R)
@@ -366,27 +427,31 @@ class HostProbe:
         self.exit = torch.empty(R, dtype=torch.uint8).pin_memory()
         self.h2d_bytes = N * d * 2 + (R + 1) * 4 + R * 4   # upper bound: only valid rows are copied
         self.d2h_bytes = R * 4 + N * 4 + R
+        self.handle = Handle(self.dims, Options(kernel_mode=mode, tail=tail)) if use_handle else None
 
-    def _call(self, fn, h_hidden, W, h_req_offsets, h_load, params, stream):
+    def _call(self, sync, h_hidden, W, h_req_offsets, h_load, params, stream):
         torch = self.torch
         assert not h_hidden.is_cuda and W.is_cuda
         s = (stream or torch.cuda.current_stream(self.device)).cuda_stream
-        _check(fn(
-            h_hidden.data_ptr(), W.data_ptr(), h_req_offsets.data_ptr(), h_load.data_ptr(),
-            C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr(),
-            C.byref(self.dims), self.workspace.data_ptr(), self.workspace.numel(),
-            self.staging.data_ptr(), self.staging.numel(), s))
+        common = (h_hidden.data_ptr(), W.data_ptr(), h_req_offsets.data_ptr(), h_load.data_ptr(),
+                  C.byref(params), self.conf.data_ptr(), self.argmax.data_ptr(), self.exit.data_ptr())
+        tail = (self.workspace.data_ptr(), self.workspace.numel(), self.staging.data_ptr(),
+                self.staging.numel(), s)
+        if self.handle is not None:
+            _check(lib().laser_probe_handle_run_host(self.handle._h, *common, *tail, 1 if sync else 0))
+        else:
+            fn = lib().laser_probe_confidence_host if sync else lib().laser_probe_confidence_host_async
+            _check(fn(*common, C.byref(self.dims), *tail))
         return ProbeOutputs(self.conf, self.argmax, self.exit, None, None)
 
     def __call__(self, h_hidden, W, h_req_offsets, h_load, params: TauParams, stream=None):
         """Synchronous: results are in the returned host tensors on return."""
-        return self._call(lib().laser_probe_confidence_host, h_hidden, W, h_req_offsets, h_load, params, stream)
+        return self._call(True, h_hidden, W, h_req_offsets, h_load, params, stream)
 
     def submit(self, h_hidden, W, h_req_offsets, h_load, params: TauParams, stream):
-        """laser_probe_confidence_host_async: enqueue on `stream` and return; the outputs are valid
-        after stream.synchronize().  One HostProbe per in-flight batch."""
-        return self._call(lib().laser_probe_confidence_host_async, h_hidden, W, h_req_offsets, h_load,
-                          params, stream)
+        """Asynchronous: enqueue on `stream` and return; the outputs are valid after
+        stream.synchronize().  One HostProbe per in-flight batch."""
+        return self._call(False, h_hidden, W, h_req_offsets, h_load, params, stream)
 
 
 def bf16_tensor_from_bits(bits, device=None, pin=False):

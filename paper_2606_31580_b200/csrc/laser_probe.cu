@@ -1,7 +1,8 @@
 // laser_probe.cu — host side of the C ABI declared in include/laser_probe.h: argument validation,
 // launch planning, TMA descriptor encoding (driver entry point fetched through the runtime, no
-// -lcuda), and the two kernel launches.  No device allocation, no host<->device synchronisation
-// (except in the explicit *_host entry point), no fallback path.
+// -lcuda), probe handles (plan + encoded descriptors + control slot cached once) and the kernel
+// launches.  No per-call device allocation, no host<->device synchronisation (except in the explicit
+// *_host entry points), no fallback path.
 #include "../../include/laser_probe.h"
 
 #include <cuda.h>
@@ -12,9 +13,10 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <deque>
 #include <mutex>
 #include <string>
-#include <unordered_map>
+#include <vector>
 
 #include "probe_kernels.cuh"
 
@@ -26,7 +28,7 @@ thread_local std::string g_last_error;
 std::atomic<uint64_t> g_launches{0};
 
 // Optional per-kernel timing (bench / profiling only): when enabled on this thread, every call
-// records events before the fused kernel, between the kernels and after the finalize kernel.
+// records events before the fused kernel, after it and after the finalize kernel (if there is one).
 constexpr int kProfRing = 512;
 struct ProfState {
     bool on = false;
@@ -39,6 +41,8 @@ thread_local ProfState g_prof;
 constexpr int kDefaultSMs = 148;             // B200
 constexpr int kMaxDynSmem = 227 * 1024;      // per-CTA opt-in limit on sm_100
 constexpr int kSmemSlack = 1024 + 256;       // alignment slack + barrier block
+constexpr int kCtlSlots = 4096;              // control slots per device
+constexpr int kCtlWords = 4;                 // words per slot (see TailParams)
 
 int set_cuda_error(const char* what, cudaError_t e) {
     g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
@@ -50,6 +54,10 @@ struct DeviceInfo {
     bool queried = false, ok = false;
     int sms = kDefaultSMs, cc_major = 0, cc_minor = 0;
     bool attr_set = false;
+    // control block: kCtlSlots x kCtlWords counters (see TailParams)
+    uint32_t* ctl_base = nullptr;
+    bool ctl_failed = false;
+    std::deque<int> ctl_free;
 };
 std::mutex g_mu;
 DeviceInfo g_dev[64];
@@ -62,17 +70,51 @@ DeviceInfo* current_device(bool* cuda_ok) {
         *cuda_ok = false;
         return nullptr;
     }
-    std::lock_guard<std::mutex> lk(g_mu);
     DeviceInfo& d = g_dev[dev];
     if (!d.queried) {
-        d.queried = true;
-        d.ok = cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
-               cudaDeviceGetAttribute(&d.cc_major, cudaDevAttrComputeCapabilityMajor, dev) == cudaSuccess &&
-               cudaDeviceGetAttribute(&d.cc_minor, cudaDevAttrComputeCapabilityMinor, dev) == cudaSuccess;
-        if (!d.ok) (void)cudaGetLastError();
+        std::lock_guard<std::mutex> lk(g_mu);
+        if (!d.queried) {
+            d.ok = cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+                   cudaDeviceGetAttribute(&d.cc_major, cudaDevAttrComputeCapabilityMajor, dev) == cudaSuccess &&
+                   cudaDeviceGetAttribute(&d.cc_minor, cudaDevAttrComputeCapabilityMinor, dev) == cudaSuccess;
+            if (!d.ok) (void)cudaGetLastError();
+            d.queried = true;
+        }
     }
     *cuda_ok = d.ok;
     return &d;
+}
+
+// A control slot of the current device, or nullptr (none left / allocation failed / `stream` is
+// being captured before the block exists: cudaMalloc is not allowed under capture).
+uint32_t* acquire_ctl(DeviceInfo* di, cudaStream_t stream) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!di->ctl_base) {
+        if (di->ctl_failed) return nullptr;
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+            (void)cudaGetLastError();
+            return nullptr;   // retried by the next call outside a capture
+        }
+        void* p = nullptr;
+        if (cudaMalloc(&p, sizeof(uint32_t) * kCtlWords * kCtlSlots) != cudaSuccess ||
+            cudaMemset(p, 0, sizeof(uint32_t) * kCtlWords * kCtlSlots) != cudaSuccess) {
+            (void)cudaGetLastError();
+            di->ctl_failed = true;
+            return nullptr;
+        }
+        di->ctl_base = static_cast<uint32_t*>(p);
+        for (int i = 0; i < kCtlSlots; ++i) di->ctl_free.push_back(i);
+    }
+    if (di->ctl_free.empty()) return nullptr;
+    const int slot = di->ctl_free.front();
+    di->ctl_free.pop_front();
+    return di->ctl_base + kCtlWords * slot;
+}
+void release_ctl(DeviceInfo* di, uint32_t* ctl) {
+    if (!ctl || !di) return;
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (di->ctl_base) di->ctl_free.push_back(static_cast<int>((ctl - di->ctl_base) / kCtlWords));  // FIFO: reused last
 }
 
 // ---------------------------------------------------------------------------------------- plan
@@ -114,16 +156,12 @@ double plan_variant(const laser_probe_dims& dm, int units, int tile_m, int bn_st
     return best;
 }
 
-std::atomic<int> g_force_mode{LASER_MODE_AUTO};
-std::atomic<int> g_overlap{0};   // strict stream order unless the caller opts in
-
-void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
+void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_plan* pl) {
     // CTA pairs (tcgen05 cta_group::2, M = 256) when there is more than one 128-row token tile: each
     // W tile then enters a pair's shared memory once instead of once per token tile and one issuing
     // thread feeds two SMs' tensor cores (measured +10..17 % for N >= 256).  An odd count of 128-row
     // tiles makes the pair kernel compute one padding tile; that costs more than the pair gains
     // until there are about ten tiles (measured: N = 384 and 640 are faster on single CTAs).
-    const int mode = g_force_mode.load(std::memory_order_relaxed);
     const int t128 = ceil_div(dm.N, kTileM);
     const bool auto_pair = t128 >= 2 && ((t128 % 2) == 0 || t128 >= 10);
     const bool pair = mode == LASER_MODE_PAIR || (mode == LASER_MODE_AUTO && auto_pair);
@@ -138,12 +176,13 @@ void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
     const int total_tiles = ceil_div(dm.V, BN);
     const SplitPlan sp = plan_splits(total_tiles, pl->m_tiles, units);
     S = sp.splits; T = sp.T;
-    int ws_splits = S;
+    // packed records: the most any item count m <= m_tiles can write
+    long ws_records = static_cast<long>(pl->m_tiles) * tile_m * S;
     for (int m = 1; m < pl->m_tiles; ++m) {
-        const int sm = plan_splits(total_tiles, m, units).splits;
-        if (sm > ws_splits) ws_splits = sm;
+        const long rec = static_cast<long>(m) * tile_m * plan_splits(total_tiles, m, units).splits;
+        if (rec > ws_records) ws_records = rec;
     }
-    pl->ws_splits = ws_splits;
+    pl->ws_records = static_cast<int32_t>(ws_records);
     pl->splits = S;
     pl->tiles_per_split = T;
     pl->tile_n = BN;
@@ -155,14 +194,20 @@ void make_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl) {
     pl->work_items = pl->m_tiles * S;
     const int busy = pl->work_items < units ? pl->work_items : units;
     pl->grid = pair ? 2 * busy : busy;
-    pl->smem_bytes = stages * stage_bytes + kSmemSlack;
-    pl->kernel_launches = 2;
+    // what the pipeline leaves over holds the tail's {offset, threshold} cache: 8 bytes per request
+    const int spare = kMaxDynSmem - (stages * stage_bytes + kSmemSlack);
+    int cache = spare / 8 - 1;
+    if (cache > kTailCache) cache = kTailCache;
+    if (cache < 0) cache = 0;
+    pl->tail_cache = cache;
+    pl->smem_bytes = stages * stage_bytes + kSmemSlack + (cache > 0 ? 8 * (cache + 1) : 0);
+    pl->kernel_launches = 1;
     pl->tile_m = tile_m;
     pl->cta_pair = pair ? 1 : 0;
 }
 
 size_t workspace_bytes_for(const laser_probe_plan& pl) {
-    size_t b = static_cast<size_t>(16) * pl.ws_splits * pl.m_tiles * pl.tile_m;
+    size_t b = static_cast<size_t>(16) * static_cast<size_t>(pl.ws_records);
     return b < 16 ? 16 : b;
 }
 
@@ -171,29 +216,12 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-EncodeTiledFn g_encode = nullptr;
-
-struct MapKey {
-    const void* ptr;
-    int rows, cols, box_rows;
-    bool operator==(const MapKey& o) const {
-        return ptr == o.ptr && rows == o.rows && cols == o.cols && box_rows == o.box_rows;
-    }
-};
-struct MapKeyHash {
-    size_t operator()(const MapKey& k) const {
-        size_t h = reinterpret_cast<size_t>(k.ptr);
-        h ^= (static_cast<size_t>(k.rows) * 0x9E3779B97F4A7C15ull) ^ (static_cast<size_t>(k.cols) << 20) ^
-             (static_cast<size_t>(k.box_rows) << 44);
-        return h;
-    }
-};
-std::unordered_map<MapKey, CUtensorMap, MapKeyHash> g_maps;
+std::atomic<EncodeTiledFn> g_encode{nullptr};
 
 // bf16 [rows, cols] row-major; box = 64 columns (128 B, the swizzle span) x box_rows rows.
-int get_tensor_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMap* out) {
-    std::lock_guard<std::mutex> lk(g_mu);
-    if (!g_encode) {
+int encode_tensor_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMap* out) {
+    EncodeTiledFn enc = g_encode.load(std::memory_order_acquire);
+    if (!enc) {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
         cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -202,20 +230,17 @@ int get_tensor_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMa
             g_last_error = "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled) failed";
             return LASER_E_CUDA;
         }
-        g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+        enc = reinterpret_cast<EncodeTiledFn>(fn);
+        g_encode.store(enc, std::memory_order_release);
     }
-    const MapKey key{ptr, rows, cols, box_rows};
-    auto it = g_maps.find(key);
-    if (it != g_maps.end()) { *out = it->second; return LASER_OK; }
     const cuuint64_t gdim[2] = {static_cast<cuuint64_t>(cols), static_cast<cuuint64_t>(rows)};
     const cuuint64_t gstride[1] = {static_cast<cuuint64_t>(cols) * 2};
     const cuuint32_t box[2] = {static_cast<cuuint32_t>(kBlockK), static_cast<cuuint32_t>(box_rows)};
     const cuuint32_t estr[2] = {1, 1};
-    CUtensorMap m;
-    CUresult r = g_encode(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim,
-                          gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim,
+                     gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         char buf[160];
         snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d) rows=%d cols=%d box_rows=%d",
@@ -223,9 +248,6 @@ int get_tensor_map(const void* ptr, int rows, int cols, int box_rows, CUtensorMa
         g_last_error = buf;
         return LASER_E_CUDA;
     }
-    if (g_maps.size() > 256) g_maps.clear();
-    g_maps.emplace(key, m);
-    *out = m;
     return LASER_OK;
 }
 
@@ -257,10 +279,17 @@ Staging staging_layout(const laser_probe_dims& d) {
     return s;
 }
 
-int options_valid(const laser_probe_options& o, int N) {
+const laser_probe_options kDefaultOptions{LASER_AGG_MEAN, LASER_PROB_MAX, nullptr, LASER_MODE_AUTO, 0,
+                                          LASER_TAIL_AUTO, 0};
+
+// Everything but token_ids (checked per call: it may be supplied at run time).
+int options_valid(const laser_probe_options& o) {
     if (o.aggregate_mode < LASER_AGG_MEAN || o.aggregate_mode > LASER_AGG_MIN) return LASER_E_MODE;
     if (o.prob_mode < LASER_PROB_MAX || o.prob_mode > LASER_PROB_TOKEN) return LASER_E_MODE;
-    if (o.prob_mode == LASER_PROB_TOKEN && N > 0 && !o.token_ids) return LASER_E_NULL;
+    if (o.kernel_mode < LASER_MODE_AUTO || o.kernel_mode > LASER_MODE_PAIR) return LASER_E_MODE;
+    if (o.tail < LASER_TAIL_AUTO || o.tail > LASER_TAIL_SEPARATE) return LASER_E_MODE;
+    if (o.overlap != 0 && o.overlap != 1) return LASER_E_MODE;
+    if (o.reserved != 0) return LASER_E_MODE;
     return LASER_OK;
 }
 
@@ -276,10 +305,76 @@ int require_b200(DeviceInfo** out) {
 
 int units_for(const DeviceInfo* di, bool pair) { return pair ? (di->sms / 2 > 0 ? di->sms / 2 : 1) : di->sms; }
 
-// Enqueue laser_probe_fused_kernel for `dims` (W has dims.V rows; v_offset localises token_ids).
-int launch_fused(DeviceInfo* di, const laser_probe_plan& pl, const void* hidden, const void* W,
-                 const int32_t* req_offsets, const laser_probe_dims& dims, const int32_t* token_ids,
-                 int v_offset, float4* ws, cudaStream_t stream, bool allow_pdl) {
+}  // namespace
+
+// ============================================================================================ handle
+// Everything about a probe of fixed dims + options that does not change from call to call: the
+// launch plan, the encoded TMA descriptors of the (few) hidden / W buffers it is called with, the
+// device-mapped addresses of pinned host buffers, and the control slot of the fused tail.  A call
+// through a handle takes no lock and does no hashing.  Not thread-safe: one thread at a time.
+struct laser_probe_handle_s {
+    laser_probe_dims dims;
+    laser_probe_options opt;
+    laser_probe_plan plan;
+    DeviceInfo* di = nullptr;
+    uint32_t* ctl = nullptr;
+    bool debug = false;
+    struct MapEntry { const void* ptr = nullptr; CUtensorMap map; };
+    MapEntry hid[2], w[4];
+    int hid_rr = 0, w_rr = 0;
+    struct HostMap { const void* h = nullptr; void* d = nullptr; };
+    HostMap hm[8];
+    int hm_rr = 0;
+};
+
+namespace {
+
+typedef laser_probe_handle_s Handle;
+
+int handle_tensor_map(Handle::MapEntry* tab, int n, int* rr, const void* ptr, int rows, int cols,
+                      int box_rows, const CUtensorMap** out) {
+    for (int i = 0; i < n; ++i)
+        if (tab[i].ptr == ptr) { *out = &tab[i].map; return LASER_OK; }
+    Handle::MapEntry& e = tab[*rr];
+    *rr = (*rr + 1) % n;
+    e.ptr = nullptr;
+    int rc = encode_tensor_map(ptr, rows, cols, box_rows, &e.map);
+    if (rc != LASER_OK) return rc;
+    e.ptr = ptr;
+    *out = &e.map;
+    return LASER_OK;
+}
+
+int make_handle(const laser_probe_dims& dims, const laser_probe_options& opt, Handle** out) {
+    DeviceInfo* di = nullptr;
+    int rc = require_b200(&di);
+    if (rc != LASER_OK) return rc;
+    Handle* h = new (std::nothrow) Handle();
+    if (!h) { g_last_error = "out of host memory"; return LASER_E_CUDA; }
+    h->dims = dims;
+    h->opt = opt;
+    h->di = di;
+    make_plan(dims, di->sms, opt.kernel_mode, &h->plan);
+    const char* dbg = getenv("LASER_DEBUG");
+    h->debug = dbg && dbg[0] && dbg[0] != '0';
+    *out = h;
+    return LASER_OK;
+}
+
+void free_handle(Handle* h) {
+    if (!h) return;
+    release_ctl(h->di, h->ctl);
+    delete h;
+}
+
+// Enqueue laser_probe_fused_kernel for the handle's dims (W has dims.V rows; v_offset localises
+// token_ids); `tail` says what its last phase does.
+int launch_fused(Handle* h, const void* hidden, const void* W, const int32_t* req_offsets,
+                 const int32_t* token_ids, int v_offset, float4* ws, cudaStream_t stream, bool allow_pdl,
+                 const TailParams& tail) {
+    DeviceInfo* di = h->di;
+    const laser_probe_plan& pl = h->plan;
+    const laser_probe_dims& dims = h->dims;
     const int N = dims.N;
     const bool pair = pl.cta_pair != 0;
     static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
@@ -292,28 +387,29 @@ int launch_fused(DeviceInfo* di, const laser_probe_plan& pl, const void* hidden,
         if (e != cudaSuccess) return set_cuda_error("cudaFuncSetAttribute", e);
         di->attr_set = true;
     }
-    CUtensorMap tm_h, tm_w;
     // Fewer than 128 rows in total: stage only the 8-row groups that hold rows.  TMA's zero fill of
     // out-of-range rows is slow (N = 8: 90 -> 75 us per step at the C2 shape without it).  The
     // other rows of the A tile keep whatever shared memory held; they feed TMEM lanes whose
     // statistics nobody reads (rows are independent).
     const int a_rows = N < kTileM ? round_up(N, 8) : kTileM;
-    int rc = get_tensor_map(hidden, N, dims.d, a_rows, &tm_h);
-    if (rc != LASER_OK) return rc;
     const int b_rows = pair ? pl.tile_n / 2 : pl.tile_n;   // W rows one CTA stages per tile
-    rc = get_tensor_map(W, dims.V, dims.d, b_rows, &tm_w);
+    const CUtensorMap *tm_h = nullptr, *tm_w = nullptr;
+    int rc = handle_tensor_map(h->hid, 2, &h->hid_rr, hidden, N, dims.d, a_rows, &tm_h);
+    if (rc != LASER_OK) return rc;
+    rc = handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V, dims.d, b_rows, &tm_w);
     if (rc != LASER_OK) return rc;
 
     FusedParams fp;
     fp.n_alloc = N; fp.d = dims.d; fp.V = dims.V;
-    fp.m_tiles = pl.m_tiles; fp.splits = pl.ws_splits; fp.tiles_per_split = pl.tiles_per_split;
+    fp.m_tiles = pl.m_tiles;
     fp.req_offsets = req_offsets; fp.R = dims.R;
     fp.total_tiles = ceil_div(dims.V, pl.tile_n);
     fp.units = units_for(di, pair);
     fp.replan = pl.m_tiles > 1 ? 1 : 0;
-    fp.wait_first = g_overlap.load(std::memory_order_relaxed) ? 0 : 1;
+    fp.wait_first = h->opt.overlap ? 0 : 1;
     fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
-    fp.work_items = pl.work_items; fp.n_pad = pl.m_tiles * pl.tile_m;
+    fp.work_items = pl.work_items;
+    fp.tail_cache = pl.tail_cache;
     fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
     fp.tx_bytes = static_cast<uint32_t>((a_rows + b_rows) * 128);  // OOB rows are zero-filled and still counted
     // W is streamed once when a single token tile exists; with several token tiles the other
@@ -329,8 +425,8 @@ int launch_fused(DeviceInfo* di, const laser_probe_plan& pl, const void* hidden,
     cfg.dynamicSmemBytes = static_cast<size_t>(pl.smem_bytes);
     cfg.stream = stream;
     // Programmatic dependent launch: the kernel may start while the previous kernel in the
-    // stream is still running; it executes griddepcontrol.wait before its workspace stores and
-    // before it exits (and before its first global read unless overlap is switched on).
+    // stream is still running; it executes griddepcontrol.wait before it reads any per-call input
+    // (strict) or before its first store (overlap), and always before it exits.
     cudaLaunchAttribute fattr[2];
     unsigned na = 0;
     if (use_pdl && allow_pdl) {
@@ -347,23 +443,24 @@ int launch_fused(DeviceInfo* di, const laser_probe_plan& pl, const void* hidden,
     }
     cfg.attrs = fattr;
     cfg.numAttrs = na;
-    cudaError_t e = pair ? cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<true>, tm_h, tm_w, fp)
-                         : cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<false>, tm_h, tm_w, fp);
+    cudaError_t e = pair ? cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<true>, *tm_h, *tm_w, fp, tail)
+                         : cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<false>, *tm_h, *tm_w, fp, tail);
     if (e != cudaSuccess) return set_cuda_error("launch laser_probe_fused_kernel", e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return LASER_OK;
 }
 
-// The fields of FinalizeParams that describe the fused kernel's workspace for `dims`.
-FinalizeParams finalize_params(const DeviceInfo* di, const laser_probe_plan& pl, const laser_probe_dims& dims,
-                               bool run_fused, const int32_t* req_offsets) {
+// The fields of FinalizeParams that describe the fused kernel's workspace for the handle's dims.
+FinalizeParams finalize_params(const Handle* h, bool run_fused, const int32_t* req_offsets) {
+    const laser_probe_plan& pl = h->plan;
     FinalizeParams fz{};
-    fz.n_alloc = dims.N; fz.R = dims.R; fz.splits = pl.ws_splits; fz.n_pad = pl.m_tiles * pl.tile_m;
+    fz.n_alloc = h->dims.N; fz.R = h->dims.R; fz.splits = pl.splits;
     fz.m_tiles = pl.m_tiles; fz.rows_per_item = pl.tile_m;
-    fz.total_tiles = ceil_div(dims.V, pl.tile_n);
-    fz.units = units_for(di, pl.cta_pair != 0);
+    fz.total_tiles = ceil_div(h->dims.V, pl.tile_n);
+    fz.units = units_for(h->di, pl.cta_pair != 0);
     fz.replan = (run_fused && pl.m_tiles > 1) ? 1 : 0;
     fz.req_offsets = req_offsets;
+    fz.row_stride = 0; fz.split_stride = 1;    // packed [rows, nsplit]
     fz.wait_flags = nullptr; fz.epoch = 0; fz.a_offset = 0; fz.prob_mode = 0; fz.agg_mode = 0;
     return fz;
 }
@@ -391,160 +488,145 @@ int launch_finalize(const FinalizeParams& fz, cudaStream_t stream, bool pdl) {
     return LASER_OK;
 }
 
-}  // namespace
-
-// ============================================================================================ ABI
-extern "C" {
-
-int laser_tau_params_default(laser_tau_params* out) {
-    if (!out) return LASER_E_NULL;
-    *out = laser_tau_params{0.95f, 0.04f, 1.0f, 10.0f, 0.88f, 0.97f};  // PAPER.md:195
+// LASER_DEBUG=1: check the req_offsets precondition on the device ahead of the probe.
+int launch_validate(const Handle* h, const int32_t* req_offsets, cudaStream_t stream) {
+    if (!h->debug || h->dims.R <= 0) return LASER_OK;
+    laser_probe_validate_kernel<<<1, 32, 0, stream>>>(req_offsets, h->dims.R, h->dims.N);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_cuda_error("launch laser_probe_validate_kernel", e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
     return LASER_OK;
 }
 
-int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan) {
-    if (!dims || !plan) return LASER_E_NULL;
-    if (!dims_valid(dims)) return LASER_E_DIMS;
-    bool ok = false;
-    DeviceInfo* di = current_device(&ok);
-    make_plan(*dims, (ok && di) ? di->sms : kDefaultSMs, plan);
+// Does this call run its last phase inside the fused kernel?  Needs a control slot.
+int want_fused_tail(Handle* h, cudaStream_t stream, bool* fused_tail) {
+    *fused_tail = false;
+    if (h->opt.tail == LASER_TAIL_SEPARATE) return LASER_OK;
+    // AUTO with overlap: calls chained two deep gate each other's CTAs; the tail CTAs would hold SMs
+    // the next call could be streaming on, so the second kernel (co-resident, tiny) is the faster form
+    if (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap) return LASER_OK;
+    if (!h->ctl) h->ctl = acquire_ctl(h->di, stream);
+    if (h->ctl) { *fused_tail = true; return LASER_OK; }
+    if (h->opt.tail == LASER_TAIL_FUSED) {
+        g_last_error = "LASER_TAIL_FUSED: no control slot (first call under stream capture, or allocation failed)";
+        return LASER_E_CUDA;
+    }
     return LASER_OK;
 }
 
-size_t laser_probe_workspace_bytes(const laser_probe_dims* dims) {
-    laser_probe_plan pl;
-    if (laser_probe_plan_query(dims, &pl) != LASER_OK) return 0;
-    return workspace_bytes_for(pl);
+int check_workspace(const Handle* h, const void* workspace, size_t workspace_bytes) {
+    if (!workspace || workspace_bytes < workspace_bytes_for(h->plan) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 15))
+        return LASER_E_WORKSPACE;
+    return LASER_OK;
 }
 
-int laser_probe_confidence_opt(const void* hidden, const void* W, const int32_t* req_offsets,
-                               const float* load, const laser_tau_params* tau_params,
-                               float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
-                               const laser_probe_dims* dims, void* workspace,
-                               size_t workspace_bytes, void* stream_v, float* out_tau_opt,
-                               float* out_pmax_opt, const laser_probe_options* options) {
-    if (!dims || !tau_params) return LASER_E_NULL;
-    if (!dims_valid(dims)) return LASER_E_DIMS;
+// ---- a1-a5 through a handle
+int run_probe(Handle* h, const void* hidden, const void* W, const int32_t* req_offsets, const float* load,
+              const laser_tau_params* tau_params, float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+              void* workspace, size_t workspace_bytes, void* stream_v, float* out_tau_opt,
+              float* out_pmax_opt, const int32_t* token_ids) {
+    if (!tau_params) return LASER_E_NULL;
     if (!params_valid(tau_params)) return LASER_E_PARAMS;
-    laser_probe_options opt{LASER_AGG_MEAN, LASER_PROB_MAX, nullptr};
-    if (options) opt = *options;
-    int rc = options_valid(opt, dims->N);
-    if (rc != LASER_OK) return rc;
-    const int N = dims->N, R = dims->R;
+    const int N = h->dims.N, R = h->dims.R;
+    if (h->opt.prob_mode == LASER_PROB_TOKEN && N > 0 && !token_ids) return LASER_E_NULL;
     if (N == 0 && R == 0) return LASER_OK;
     if (N > 0 && (!hidden || !W || !out_argmax)) return LASER_E_NULL;
     if (R > 0 && (!req_offsets || !load || !out_conf || !out_exit)) return LASER_E_NULL;
     if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(W) & 15))
         return LASER_E_ALIGN;
-
-    DeviceInfo* di = nullptr;
-    rc = require_b200(&di);
+    int rc = check_workspace(h, workspace, workspace_bytes);
     if (rc != LASER_OK) return rc;
-    laser_probe_plan pl;
-    make_plan(*dims, di->sms, &pl);
-    if (!workspace || workspace_bytes < workspace_bytes_for(pl) ||
-        (reinterpret_cast<uintptr_t>(workspace) & 15))
-        return LASER_E_WORKSPACE;
 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
     const bool run_fused = (N > 0 && R > 0);
     const bool prof = g_prof.on && g_prof.created && run_fused && g_prof.calls < kProfRing;
     const int prof_slot = g_prof.calls;
-    if (run_fused) {
-        if (prof) cudaEventRecord(g_prof.ev[prof_slot][0], stream);
-        rc = launch_fused(di, pl, hidden, W, req_offsets, *dims,
-                          opt.prob_mode == LASER_PROB_TOKEN ? opt.token_ids : nullptr, 0,
-                          static_cast<float4*>(workspace), stream, !prof);
-        if (rc != LASER_OK) return rc;
-    }
 
-    FinalizeParams fz = finalize_params(di, pl, *dims, run_fused, req_offsets);
-    fz.agg_mode = opt.aggregate_mode;
-    fz.prob_mode = opt.prob_mode;
+    FinalizeParams fz = finalize_params(h, run_fused, req_offsets);
+    fz.agg_mode = h->opt.aggregate_mode;
+    fz.prob_mode = h->opt.prob_mode;
     fz.ws = static_cast<const float4*>(workspace);
-    fz.row_stride = pl.ws_splits; fz.split_stride = 1;
     fz.load = load;
     fz.out_conf = out_conf; fz.out_argmax = out_argmax; fz.out_exit = out_exit;
     fz.out_tau = out_tau_opt; fz.out_pmax = out_pmax_opt;
     fz.tau = to_dev(tau_params);
-    // N == 0 with R > 0: every request is empty -> conf 0, exit 0, tau still defined.  Handled by the
-    // same kernel (fz.R = R): req_offsets are all 0, no partials are read.
-    if (prof) cudaEventRecord(g_prof.ev[prof_slot][1], stream);
-    rc = launch_finalize(fz, stream, run_fused && !prof);
-    if (rc != LASER_OK) return rc;
+
+    bool fused_tail = false;
+    if (run_fused) {
+        rc = want_fused_tail(h, stream, &fused_tail);
+        if (rc != LASER_OK) return rc;
+        rc = launch_validate(h, req_offsets, stream);
+        if (rc != LASER_OK) return rc;
+        TailParams tail{};
+#ifdef LASER_TIMELINE
+        static int tl_calls = 0;
+        tail.tl_slot = tl_calls++;
+#endif
+        tail.kind = fused_tail ? 1 : 0;
+        tail.ctl = h->ctl;
+        tail.q.f = fz;
+        if (prof) cudaEventRecord(g_prof.ev[prof_slot][0], stream);
+        rc = launch_fused(h, hidden, W, req_offsets,
+                          h->opt.prob_mode == LASER_PROB_TOKEN ? token_ids : nullptr, 0,
+                          static_cast<float4*>(workspace), stream, !prof && !h->debug, tail);
+        if (rc != LASER_OK) return rc;
+        if (prof) cudaEventRecord(g_prof.ev[prof_slot][1], stream);
+    }
+    if (!fused_tail) {
+        // N == 0 with R > 0: every request is empty -> conf 0, exit 0, tau still defined.  Handled by
+        // the same kernel (fz.R = R): req_offsets are all 0, no partials are read.
+        rc = launch_finalize(fz, stream, run_fused && !prof);
+        if (rc != LASER_OK) return rc;
+    }
     if (prof) { cudaEventRecord(g_prof.ev[prof_slot][2], stream); g_prof.calls++; }
     return LASER_OK;
 }
 
-int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t* req_offsets,
-                               const float* load, const laser_tau_params* tau_params,
-                               float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
-                               const laser_probe_dims* dims, void* workspace,
-                               size_t workspace_bytes, void* stream, float* out_tau_opt,
-                               float* out_pmax_opt, int aggregate_mode) {
-    const laser_probe_options opt{aggregate_mode, LASER_PROB_MAX, nullptr};
-    return laser_probe_confidence_opt(hidden, W, req_offsets, load, tau_params, out_conf, out_argmax,
-                                      out_exit, dims, workspace, workspace_bytes, stream, out_tau_opt,
-                                      out_pmax_opt, &opt);
-}
-
-int laser_probe_confidence(const void* hidden, const void* W, const int32_t* req_offsets,
-                           const float* load, const laser_tau_params* tau_params, float* out_conf,
-                           int32_t* out_argmax, uint8_t* out_exit, const laser_probe_dims* dims,
-                           void* workspace, size_t workspace_bytes, void* stream,
-                           float* out_tau_opt, float* out_pmax_opt) {
-    return laser_probe_confidence_opt(hidden, W, req_offsets, load, tau_params, out_conf, out_argmax,
-                                      out_exit, dims, workspace, workspace_bytes, stream, out_tau_opt,
-                                      out_pmax_opt, nullptr);
-}
-
-// ------------------------------------------------------------------------------ vocabulary-parallel
-int laser_probe_partial(const void* hidden, const void* W_shard, const int32_t* req_offsets,
-                        const int32_t* token_ids_opt, const laser_probe_dims* dims, int32_t v_offset,
-                        laser_row_stats* out_stats, const laser_probe_peers* peers_opt,
-                        void* workspace, size_t workspace_bytes, void* stream_v) {
-    if (!dims) return LASER_E_NULL;
-    if (!dims_valid(dims) || v_offset < 0) return LASER_E_DIMS;
-    if (!out_stats && !peers_opt) return LASER_E_NULL;
-    if (peers_opt) {
-        const laser_probe_peers& pe = *peers_opt;
-        if (pe.world < 1 || pe.world > LASER_MAX_PEERS || pe.rank < 0 || pe.rank >= pe.world || pe.epoch == 0)
-            return LASER_E_PARAMS;
-        for (int g = 0; g < pe.world; ++g)
-            if (!pe.peer_stats[g] || !pe.peer_flags[g]) return LASER_E_NULL;
-    }
-    const int N = dims->N, R = dims->R;
+// ---- a1 + a2 over one vocabulary shard through a handle (dims.V = rows of the shard)
+int run_partial(Handle* h, const void* hidden, const void* W_shard, const int32_t* req_offsets,
+                const int32_t* token_ids_opt, int32_t v_offset, laser_row_stats* out_stats,
+                const laser_probe_peers* peers_opt, void* workspace, size_t workspace_bytes, void* stream_v) {
+    const int N = h->dims.N, R = h->dims.R;
     if (N > 0 && (!hidden || !W_shard)) return LASER_E_NULL;
     if (R > 0 && !req_offsets) return LASER_E_NULL;
     if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(W_shard) & 15) ||
         (reinterpret_cast<uintptr_t>(out_stats) & 15))
         return LASER_E_ALIGN;
-    DeviceInfo* di = nullptr;
-    int rc = require_b200(&di);
+    int rc = check_workspace(h, workspace, workspace_bytes);
     if (rc != LASER_OK) return rc;
-    laser_probe_plan pl;
-    make_plan(*dims, di->sms, &pl);
-    if (!workspace || workspace_bytes < workspace_bytes_for(pl) ||
-        (reinterpret_cast<uintptr_t>(workspace) & 15))
-        return LASER_E_WORKSPACE;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
     const bool run_fused = (N > 0 && R > 0);
+
+    ReduceParams rq{};
+    rq.f = finalize_params(h, run_fused, req_offsets);
+    rq.f.R = run_fused ? R : 0;            // R == 0: every row is padding -> neutral records
+    rq.f.ws = static_cast<const float4*>(workspace);
+    rq.f.a_offset = v_offset;
+    rq.out_stats = reinterpret_cast<float4*>(out_stats);
+    rq.rank = peers_opt ? peers_opt->rank : 0;
+    rq.world = peers_opt ? peers_opt->world : 0;
+    rq.epoch = peers_opt ? peers_opt->epoch : 0;
+    for (int g = 0; g < rq.world; ++g) {
+        rq.peer_stats[g] = reinterpret_cast<float4*>(peers_opt->peer_stats[g]);
+        rq.peer_flags[g] = peers_opt->peer_flags[g];
+    }
+    bool fused_tail = false;
     if (run_fused) {
-        rc = launch_fused(di, pl, hidden, W_shard, req_offsets, *dims, token_ids_opt, v_offset,
-                          static_cast<float4*>(workspace), stream, true);
+        rc = want_fused_tail(h, stream, &fused_tail);
         if (rc != LASER_OK) return rc;
+        rc = launch_validate(h, req_offsets, stream);
+        if (rc != LASER_OK) return rc;
+        TailParams tail{};
+        tail.kind = fused_tail ? 2 : 0;
+        tail.ctl = h->ctl;
+        tail.q = rq;
+        rc = launch_fused(h, hidden, W_shard, req_offsets, token_ids_opt, v_offset,
+                          static_cast<float4*>(workspace), stream, !h->debug, tail);
+        if (rc != LASER_OK) return rc;
+        if (fused_tail) return LASER_OK;
     }
     if (N > 0) {
-        ReduceParams rq{};
-        rq.f = finalize_params(di, pl, *dims, run_fused, req_offsets);
-        rq.f.R = run_fused ? R : 0;            // R == 0: every row is padding -> neutral records
-        rq.f.ws = static_cast<const float4*>(workspace);
-        rq.f.row_stride = pl.ws_splits; rq.f.split_stride = 1;
-        rq.f.a_offset = v_offset;
-        rq.out_stats = reinterpret_cast<float4*>(out_stats);
-        rq.rank = peers_opt ? peers_opt->rank : 0;
-        rq.world = peers_opt ? peers_opt->world : 0;
-        for (int g = 0; g < rq.world; ++g) rq.peer_stats[g] = reinterpret_cast<float4*>(peers_opt->peer_stats[g]);
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(ceil_div(N, kFinalizeWarps));
         cfg.blockDim = dim3(kFinalizeThreads);
@@ -564,15 +646,340 @@ int laser_probe_partial(const void* hidden, const void* W_shard, const int32_t* 
     if (peers_opt) {
         // Plain launch (full stream order): the reduce kernel's stores, remote ones included, have
         // been performed when this kernel starts; it publishes the epoch on every GPU.
-        SignalParams sg{};
-        sg.rank = peers_opt->rank; sg.world = peers_opt->world; sg.epoch = peers_opt->epoch;
-        for (int g = 0; g < sg.world; ++g) sg.peer_flags[g] = peers_opt->peer_flags[g];
-        laser_probe_signal_kernel<<<1, 32, 0, stream>>>(sg);
+        laser_probe_signal_kernel<<<1, 32, 0, stream>>>(rq);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return set_cuda_error("launch laser_probe_signal_kernel", e);
         g_launches.fetch_add(1, std::memory_order_relaxed);
     }
     return LASER_OK;
+}
+
+// Device-mapped address of a pinned host buffer (cached per handle), or nullptr if it is not mapped.
+void* mapped_ptr(Handle* h, const void* host) {
+    if (!host) return nullptr;
+    for (auto& e : h->hm)
+        if (e.h == host) return e.d;
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, host) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    void* d = a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
+    if (d) {   // only successes are cached: a pageable buffer may be registered later
+        Handle::HostMap& e = h->hm[h->hm_rr];
+        h->hm_rr = (h->hm_rr + 1) % 8;
+        e.h = host; e.d = d;
+    }
+    return d;
+}
+
+// ---- host buffers for the per-step tensors, through a handle
+int run_host(Handle* h, const void* h_hidden, const void* W, const int32_t* h_req_offsets,
+             const float* h_load, const laser_tau_params* tau_params, float* h_out_conf,
+             int32_t* h_out_argmax, uint8_t* h_out_exit, void* workspace, size_t workspace_bytes,
+             void* d_staging, size_t staging_bytes, void* stream_v, bool synchronize) {
+    if (!tau_params) return LASER_E_NULL;
+    const laser_probe_dims* dims = &h->dims;
+    const int N = dims->N, R = dims->R;
+    if (N == 0 && R == 0) return LASER_OK;
+    if (!d_staging) return LASER_E_NULL;
+    if (N > 0 && (!h_hidden || !h_out_argmax)) return LASER_E_NULL;
+    if (R > 0 && (!h_req_offsets || !h_load || !h_out_conf || !h_out_exit)) return LASER_E_NULL;
+    const Staging st = staging_layout(*dims);
+    if (staging_bytes < st.total || (reinterpret_cast<uintptr_t>(d_staging) & 255)) return LASER_E_WORKSPACE;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
+    uint8_t* base = static_cast<uint8_t*>(d_staging);
+    cudaError_t e;
+    // Rows >= req_offsets[R] are padding and never aggregated: copy the valid rows only (the offsets
+    // are host memory here).  Out-of-range offsets fall back to all N rows.
+    int n_copy = N;
+    if (R > 0 && h_req_offsets[R] >= 0 && h_req_offsets[R] <= N) n_copy = h_req_offsets[R];
+    else if (R == 0) n_copy = 0;
+    if (n_copy > 0) {
+        e = cudaMemcpyAsync(base + st.hidden, h_hidden, static_cast<size_t>(n_copy) * dims->d * 2,
+                            cudaMemcpyHostToDevice, stream);
+        if (e != cudaSuccess) return set_cuda_error("H2D hidden", e);
+    }
+    // Zero-copy for the small tensors: when req_offsets, load and the three outputs all live in
+    // pinned, device-mapped host memory (cudaHostAlloc / cudaHostRegister / torch pin_memory), the
+    // kernel's tail reads and writes them over PCIe directly and the call issues one copy (hidden)
+    // instead of six.
+    void* m_off = R > 0 ? mapped_ptr(h, h_req_offsets) : nullptr;
+    void* m_load = R > 0 ? mapped_ptr(h, h_load) : nullptr;
+    void* m_conf = R > 0 ? mapped_ptr(h, h_out_conf) : nullptr;
+    void* m_exit = R > 0 ? mapped_ptr(h, h_out_exit) : nullptr;
+    void* m_arg = N > 0 ? mapped_ptr(h, h_out_argmax) : nullptr;
+    const bool zero_copy = (R == 0 || (m_off && m_load && m_conf && m_exit)) && (N == 0 || m_arg);
+    int rc;
+    if (zero_copy) {
+        rc = run_probe(h, base + st.hidden, W, static_cast<int32_t*>(m_off), static_cast<float*>(m_load),
+                       tau_params, static_cast<float*>(m_conf), static_cast<int32_t*>(m_arg),
+                       static_cast<uint8_t*>(m_exit), workspace, workspace_bytes, stream_v, nullptr, nullptr,
+                       h->opt.token_ids);
+        if (rc != LASER_OK) return rc;
+    } else {
+        if (R > 0) {
+            e = cudaMemcpyAsync(base + st.offsets, h_req_offsets, static_cast<size_t>(R + 1) * 4,
+                                cudaMemcpyHostToDevice, stream);
+            if (e != cudaSuccess) return set_cuda_error("H2D req_offsets", e);
+            e = cudaMemcpyAsync(base + st.load, h_load, static_cast<size_t>(R) * 4, cudaMemcpyHostToDevice, stream);
+            if (e != cudaSuccess) return set_cuda_error("H2D load", e);
+        }
+        rc = run_probe(h, base + st.hidden, W, reinterpret_cast<int32_t*>(base + st.offsets),
+                       reinterpret_cast<float*>(base + st.load), tau_params,
+                       reinterpret_cast<float*>(base + st.conf), reinterpret_cast<int32_t*>(base + st.argmax),
+                       base + st.exit_, workspace, workspace_bytes, stream_v, nullptr, nullptr,
+                       h->opt.token_ids);
+        if (rc != LASER_OK) return rc;
+        if (R > 0) {
+            e = cudaMemcpyAsync(h_out_conf, base + st.conf, static_cast<size_t>(R) * 4, cudaMemcpyDeviceToHost, stream);
+            if (e != cudaSuccess) return set_cuda_error("D2H conf", e);
+            e = cudaMemcpyAsync(h_out_exit, base + st.exit_, static_cast<size_t>(R), cudaMemcpyDeviceToHost, stream);
+            if (e != cudaSuccess) return set_cuda_error("D2H exit", e);
+        }
+        if (N > 0) {
+            e = cudaMemcpyAsync(h_out_argmax, base + st.argmax, static_cast<size_t>(N) * 4, cudaMemcpyDeviceToHost, stream);
+            if (e != cudaSuccess) return set_cuda_error("D2H argmax", e);
+        }
+    }
+    if (synchronize) {
+        e = cudaStreamSynchronize(stream);
+        if (e != cudaSuccess) return set_cuda_error("cudaStreamSynchronize", e);
+    }
+    return LASER_OK;
+}
+
+// ---------------------------------------------------------------------------------------- implicit handles
+// The handle-less entry points (laser_probe_confidence and friends) keep a small per-thread cache of
+// handles keyed by (device, dims, options, workspace): no lock, a linear scan of <= 16 entries.  The
+// workspace is part of the key because calls that share a control slot must be stream-ordered, and
+// the contract already forbids concurrent calls on one workspace.
+struct ImplicitKey {
+    int device;
+    laser_probe_dims dims;
+    int32_t agg, prob, mode, overlap, tail;
+    const void* workspace;
+    bool operator==(const ImplicitKey& o) const {
+        return device == o.device && dims.N == o.dims.N && dims.d == o.dims.d && dims.V == o.dims.V &&
+               dims.R == o.dims.R && agg == o.agg && prob == o.prob && mode == o.mode &&
+               overlap == o.overlap && tail == o.tail && workspace == o.workspace;
+    }
+};
+struct ImplicitCache {
+    static constexpr int kCap = 16;
+    struct Entry { ImplicitKey key; Handle* h; uint64_t stamp; };
+    std::vector<Entry> entries;
+    uint64_t clock = 0;
+    ~ImplicitCache() { for (auto& e : entries) free_handle(e.h); }
+};
+thread_local ImplicitCache g_implicit;
+std::atomic<uint64_t> g_cache_generation{0};      // bumped by laser_shutdown
+thread_local uint64_t g_cache_seen = 0;
+
+int implicit_handle(const laser_probe_dims& dims, const laser_probe_options& opt, const void* workspace,
+                    Handle** out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); dev = -1; }
+    ImplicitCache& c = g_implicit;
+    const uint64_t gen = g_cache_generation.load(std::memory_order_relaxed);
+    if (gen != g_cache_seen) {
+        for (auto& e : c.entries) free_handle(e.h);
+        c.entries.clear();
+        g_cache_seen = gen;
+    }
+    const ImplicitKey key{dev, dims, opt.aggregate_mode, opt.prob_mode, opt.kernel_mode, opt.overlap, opt.tail,
+                          workspace};
+    for (auto& e : c.entries)
+        if (e.key == key) { e.stamp = ++c.clock; *out = e.h; return LASER_OK; }
+    Handle* h = nullptr;
+    int rc = make_handle(dims, opt, &h);
+    if (rc != LASER_OK) return rc;
+    h->opt.token_ids = nullptr;    // supplied per call
+    if (static_cast<int>(c.entries.size()) >= ImplicitCache::kCap) {
+        size_t lru = 0;
+        for (size_t i = 1; i < c.entries.size(); ++i)
+            if (c.entries[i].stamp < c.entries[lru].stamp) lru = i;
+        free_handle(c.entries[lru].h);
+        c.entries.erase(c.entries.begin() + static_cast<long>(lru));
+    }
+    c.entries.push_back({key, h, ++c.clock});
+    *out = h;
+    return LASER_OK;
+}
+
+}  // namespace
+
+// ============================================================================================ ABI
+extern "C" {
+
+int laser_tau_params_default(laser_tau_params* out) {
+    if (!out) return LASER_E_NULL;
+    *out = laser_tau_params{0.95f, 0.04f, 1.0f, 10.0f, 0.88f, 0.97f};  // PAPER.md:195
+    return LASER_OK;
+}
+
+int laser_probe_options_default(laser_probe_options* out) {
+    if (!out) return LASER_E_NULL;
+    *out = kDefaultOptions;
+    return LASER_OK;
+}
+
+int laser_probe_plan_query_mode(const laser_probe_dims* dims, int kernel_mode, laser_probe_plan* plan) {
+    if (!dims || !plan) return LASER_E_NULL;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
+    if (kernel_mode < LASER_MODE_AUTO || kernel_mode > LASER_MODE_PAIR) return LASER_E_MODE;
+    bool ok = false;
+    DeviceInfo* di = current_device(&ok);
+    make_plan(*dims, (ok && di) ? di->sms : kDefaultSMs, kernel_mode, plan);
+    return LASER_OK;
+}
+
+int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan) {
+    return laser_probe_plan_query_mode(dims, LASER_MODE_AUTO, plan);
+}
+
+size_t laser_probe_workspace_bytes(const laser_probe_dims* dims) {
+    // enough for either kernel variant, so that one buffer serves every laser_probe_options.kernel_mode
+    laser_probe_plan a, b;
+    if (laser_probe_plan_query_mode(dims, LASER_MODE_SINGLE, &a) != LASER_OK) return 0;
+    if (laser_probe_plan_query_mode(dims, LASER_MODE_PAIR, &b) != LASER_OK) return 0;
+    const size_t wa = workspace_bytes_for(a), wb = workspace_bytes_for(b);
+    return wa > wb ? wa : wb;
+}
+
+// ------------------------------------------------------------------------------ explicit handles
+int laser_probe_handle_create(laser_probe_handle** out, const laser_probe_dims* dims,
+                              const laser_probe_options* options) {
+    if (!out || !dims) return LASER_E_NULL;
+    *out = nullptr;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
+    laser_probe_options opt = options ? *options : kDefaultOptions;
+    int rc = options_valid(opt);
+    if (rc != LASER_OK) return rc;
+    Handle* h = nullptr;
+    rc = make_handle(*dims, opt, &h);
+    if (rc != LASER_OK) return rc;
+    if (opt.tail != LASER_TAIL_SEPARATE) h->ctl = acquire_ctl(h->di, nullptr);   // may stay NULL: retried per call
+    *out = h;
+    return LASER_OK;
+}
+
+int laser_probe_handle_destroy(laser_probe_handle* h) {
+    free_handle(h);
+    return LASER_OK;
+}
+
+int laser_probe_handle_plan(const laser_probe_handle* h, laser_probe_plan* plan) {
+    if (!h || !plan) return LASER_E_NULL;
+    *plan = h->plan;
+    plan->kernel_launches = (h->opt.tail == LASER_TAIL_SEPARATE || !h->ctl ||
+                             (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap)) ? 2 : 1;
+    return LASER_OK;
+}
+
+size_t laser_probe_handle_workspace_bytes(const laser_probe_handle* h) {
+    return h ? workspace_bytes_for(h->plan) : 0;
+}
+
+int laser_probe_handle_run(laser_probe_handle* h, const void* hidden, const void* W,
+                           const int32_t* req_offsets, const float* load,
+                           const laser_tau_params* tau_params, float* out_conf, int32_t* out_argmax,
+                           uint8_t* out_exit, void* workspace, size_t workspace_bytes, void* stream,
+                           float* out_tau_opt, float* out_pmax_opt) {
+    if (!h) return LASER_E_NULL;
+    return run_probe(h, hidden, W, req_offsets, load, tau_params, out_conf, out_argmax, out_exit, workspace,
+                     workspace_bytes, stream, out_tau_opt, out_pmax_opt, h->opt.token_ids);
+}
+
+int laser_probe_handle_run_host(laser_probe_handle* h, const void* h_hidden, const void* W,
+                                const int32_t* h_req_offsets, const float* h_load,
+                                const laser_tau_params* tau_params, float* h_out_conf,
+                                int32_t* h_out_argmax, uint8_t* h_out_exit, void* workspace,
+                                size_t workspace_bytes, void* d_staging, size_t staging_bytes, void* stream,
+                                int synchronize) {
+    if (!h) return LASER_E_NULL;
+    return run_host(h, h_hidden, W, h_req_offsets, h_load, tau_params, h_out_conf, h_out_argmax, h_out_exit,
+                    workspace, workspace_bytes, d_staging, staging_bytes, stream, synchronize != 0);
+}
+
+// ------------------------------------------------------------------------------ handle-less forms
+int laser_probe_confidence_opt(const void* hidden, const void* W, const int32_t* req_offsets,
+                               const float* load, const laser_tau_params* tau_params,
+                               float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+                               const laser_probe_dims* dims, void* workspace,
+                               size_t workspace_bytes, void* stream_v, float* out_tau_opt,
+                               float* out_pmax_opt, const laser_probe_options* options) {
+    if (!dims || !tau_params) return LASER_E_NULL;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
+    if (!params_valid(tau_params)) return LASER_E_PARAMS;
+    laser_probe_options opt = options ? *options : kDefaultOptions;
+    int rc = options_valid(opt);
+    if (rc != LASER_OK) return rc;
+    const int N = dims->N, R = dims->R;
+    if (opt.prob_mode == LASER_PROB_TOKEN && N > 0 && !opt.token_ids) return LASER_E_NULL;
+    if (N == 0 && R == 0) return LASER_OK;
+    if (N > 0 && (!hidden || !W || !out_argmax)) return LASER_E_NULL;
+    if (R > 0 && (!req_offsets || !load || !out_conf || !out_exit)) return LASER_E_NULL;
+    if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(W) & 15))
+        return LASER_E_ALIGN;
+    Handle* h = nullptr;
+    rc = implicit_handle(*dims, opt, workspace, &h);
+    if (rc != LASER_OK) return rc;
+    return run_probe(h, hidden, W, req_offsets, load, tau_params, out_conf, out_argmax, out_exit, workspace,
+                     workspace_bytes, stream_v, out_tau_opt, out_pmax_opt, opt.token_ids);
+}
+
+int laser_probe_confidence_agg(const void* hidden, const void* W, const int32_t* req_offsets,
+                               const float* load, const laser_tau_params* tau_params,
+                               float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+                               const laser_probe_dims* dims, void* workspace,
+                               size_t workspace_bytes, void* stream, float* out_tau_opt,
+                               float* out_pmax_opt, int aggregate_mode) {
+    laser_probe_options opt = kDefaultOptions;
+    opt.aggregate_mode = aggregate_mode;
+    return laser_probe_confidence_opt(hidden, W, req_offsets, load, tau_params, out_conf, out_argmax,
+                                      out_exit, dims, workspace, workspace_bytes, stream, out_tau_opt,
+                                      out_pmax_opt, &opt);
+}
+
+int laser_probe_confidence(const void* hidden, const void* W, const int32_t* req_offsets,
+                           const float* load, const laser_tau_params* tau_params, float* out_conf,
+                           int32_t* out_argmax, uint8_t* out_exit, const laser_probe_dims* dims,
+                           void* workspace, size_t workspace_bytes, void* stream,
+                           float* out_tau_opt, float* out_pmax_opt) {
+    return laser_probe_confidence_opt(hidden, W, req_offsets, load, tau_params, out_conf, out_argmax,
+                                      out_exit, dims, workspace, workspace_bytes, stream, out_tau_opt,
+                                      out_pmax_opt, nullptr);
+}
+
+// ------------------------------------------------------------------------------ vocabulary-parallel
+int laser_probe_partial(const void* hidden, const void* W_shard, const int32_t* req_offsets,
+                        const int32_t* token_ids_opt, const laser_probe_dims* dims, int32_t v_offset,
+                        laser_row_stats* out_stats, const laser_probe_peers* peers_opt,
+                        void* workspace, size_t workspace_bytes, void* stream_v,
+                        const laser_probe_options* options) {
+    if (!dims) return LASER_E_NULL;
+    if (!dims_valid(dims) || v_offset < 0) return LASER_E_DIMS;
+    if (!out_stats && !peers_opt) return LASER_E_NULL;
+    if (peers_opt) {
+        const laser_probe_peers& pe = *peers_opt;
+        if (pe.world < 1 || pe.world > LASER_MAX_PEERS || pe.rank < 0 || pe.rank >= pe.world || pe.epoch == 0)
+            return LASER_E_PARAMS;
+        for (int g = 0; g < pe.world; ++g)
+            if (!pe.peer_stats[g] || !pe.peer_flags[g]) return LASER_E_NULL;
+    }
+    laser_probe_options opt = options ? *options : kDefaultOptions;
+    int rc = options_valid(opt);
+    if (rc != LASER_OK) return rc;
+    const int N = dims->N, R = dims->R;
+    if (N > 0 && (!hidden || !W_shard)) return LASER_E_NULL;
+    if (R > 0 && !req_offsets) return LASER_E_NULL;
+    if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(W_shard) & 15) ||
+        (reinterpret_cast<uintptr_t>(out_stats) & 15))
+        return LASER_E_ALIGN;
+    opt.aggregate_mode = LASER_AGG_MEAN; opt.prob_mode = LASER_PROB_MAX;   // not part of the partial
+    Handle* h = nullptr;
+    rc = implicit_handle(*dims, opt, workspace, &h);
+    if (rc != LASER_OK) return rc;
+    return run_partial(h, hidden, W_shard, req_offsets, token_ids_opt, v_offset, out_stats, peers_opt,
+                       workspace, workspace_bytes, stream_v);
 }
 
 int laser_probe_combine(const laser_row_stats* stats, int32_t G, const int32_t* req_offsets,
@@ -585,21 +992,19 @@ int laser_probe_combine(const laser_row_stats* stats, int32_t G, const int32_t* 
     if (!dims_valid(dims)) return LASER_E_DIMS;
     if (G < 1 || G > LASER_MAX_PEERS) return LASER_E_DIMS;
     if (!params_valid(tau_params)) return LASER_E_PARAMS;
-    laser_probe_options opt{LASER_AGG_MEAN, LASER_PROB_MAX, nullptr};
-    if (options) opt = *options;
-    if (opt.aggregate_mode < LASER_AGG_MEAN || opt.aggregate_mode > LASER_AGG_MIN ||
-        opt.prob_mode < LASER_PROB_MAX || opt.prob_mode > LASER_PROB_TOKEN)
-        return LASER_E_MODE;
+    laser_probe_options opt = options ? *options : kDefaultOptions;
+    int rc = options_valid(opt);
+    if (rc != LASER_OK) return rc;
     const int N = dims->N, R = dims->R;
     if (N == 0 && R == 0) return LASER_OK;
     if (N > 0 && (!stats || !out_argmax)) return LASER_E_NULL;
     if (R > 0 && (!req_offsets || !load || !out_conf || !out_exit)) return LASER_E_NULL;
     if (reinterpret_cast<uintptr_t>(stats) & 15) return LASER_E_ALIGN;
     DeviceInfo* di = nullptr;
-    int rc = require_b200(&di);
+    rc = require_b200(&di);
     if (rc != LASER_OK) return rc;
     FinalizeParams fz{};
-    fz.n_alloc = N; fz.R = R; fz.splits = G; fz.n_pad = N;
+    fz.n_alloc = N; fz.R = R; fz.splits = G;
     fz.m_tiles = 1; fz.rows_per_item = kTileM; fz.total_tiles = 1; fz.units = 1; fz.replan = 0;
     fz.agg_mode = opt.aggregate_mode;
     fz.prob_mode = opt.prob_mode;
@@ -627,75 +1032,12 @@ int laser_probe_confidence_host_async(const void* h_hidden, const void* W, const
                                       void* stream_v) {
     if (!dims || !tau_params) return LASER_E_NULL;
     if (!dims_valid(dims)) return LASER_E_DIMS;
-    const int N = dims->N, R = dims->R;
-    if (N == 0 && R == 0) return LASER_OK;
-    if (!d_staging) return LASER_E_NULL;
-    if (N > 0 && (!h_hidden || !h_out_argmax)) return LASER_E_NULL;
-    if (R > 0 && (!h_req_offsets || !h_load || !h_out_conf || !h_out_exit)) return LASER_E_NULL;
-    const Staging st = staging_layout(*dims);
-    if (staging_bytes < st.total || (reinterpret_cast<uintptr_t>(d_staging) & 255)) return LASER_E_WORKSPACE;
-    cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
-    uint8_t* base = static_cast<uint8_t*>(d_staging);
-    cudaError_t e;
-    // Rows >= req_offsets[R] are padding and never aggregated: copy the valid rows only (the offsets
-    // are host memory here).  Out-of-range offsets fall back to all N rows.
-    int n_copy = N;
-    if (R > 0 && h_req_offsets[R] >= 0 && h_req_offsets[R] <= N) n_copy = h_req_offsets[R];
-    else if (R == 0) n_copy = 0;
-    if (n_copy > 0) {
-        e = cudaMemcpyAsync(base + st.hidden, h_hidden, static_cast<size_t>(n_copy) * dims->d * 2,
-                            cudaMemcpyHostToDevice, stream);
-        if (e != cudaSuccess) return set_cuda_error("H2D hidden", e);
-    }
-    // Zero-copy for the small tensors: when req_offsets, load and the three outputs all live in
-    // pinned, device-mapped host memory (cudaHostAlloc / cudaHostRegister / torch pin_memory), the
-    // finalize kernel reads and writes them over PCIe directly — the reads overlap the fused kernel
-    // (they precede griddepcontrol.wait) — and the call issues one copy (hidden) instead of six.
-    auto mapped = [](const void* h) -> void* {
-        if (!h) return nullptr;
-        cudaPointerAttributes a;
-        if (cudaPointerGetAttributes(&a, h) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
-        return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
-    };
-    void* m_off = R > 0 ? mapped(h_req_offsets) : nullptr;
-    void* m_load = R > 0 ? mapped(h_load) : nullptr;
-    void* m_conf = R > 0 ? mapped(h_out_conf) : nullptr;
-    void* m_exit = R > 0 ? mapped(h_out_exit) : nullptr;
-    void* m_arg = N > 0 ? mapped(h_out_argmax) : nullptr;
-    const bool zero_copy = (R == 0 || (m_off && m_load && m_conf && m_exit)) && (N == 0 || m_arg);
-    if (zero_copy) {
-        int rc = laser_probe_confidence(base + st.hidden, W, static_cast<int32_t*>(m_off),
-                                        static_cast<float*>(m_load), tau_params,
-                                        static_cast<float*>(m_conf), static_cast<int32_t*>(m_arg),
-                                        static_cast<uint8_t*>(m_exit), dims, workspace, workspace_bytes,
-                                        stream_v, nullptr, nullptr);
-        if (rc != LASER_OK) return rc;
-    } else {
-        if (R > 0) {
-            e = cudaMemcpyAsync(base + st.offsets, h_req_offsets, static_cast<size_t>(R + 1) * 4,
-                                cudaMemcpyHostToDevice, stream);
-            if (e != cudaSuccess) return set_cuda_error("H2D req_offsets", e);
-            e = cudaMemcpyAsync(base + st.load, h_load, static_cast<size_t>(R) * 4, cudaMemcpyHostToDevice, stream);
-            if (e != cudaSuccess) return set_cuda_error("H2D load", e);
-        }
-        int rc = laser_probe_confidence(base + st.hidden, W, reinterpret_cast<int32_t*>(base + st.offsets),
-                                        reinterpret_cast<float*>(base + st.load), tau_params,
-                                        reinterpret_cast<float*>(base + st.conf),
-                                        reinterpret_cast<int32_t*>(base + st.argmax), base + st.exit_, dims,
-                                        workspace, workspace_bytes, stream_v, nullptr, nullptr);
-        if (rc != LASER_OK) return rc;
-        if (R > 0) {
-            e = cudaMemcpyAsync(h_out_conf, base + st.conf, static_cast<size_t>(R) * 4, cudaMemcpyDeviceToHost, stream);
-            if (e != cudaSuccess) return set_cuda_error("D2H conf", e);
-            e = cudaMemcpyAsync(h_out_exit, base + st.exit_, static_cast<size_t>(R), cudaMemcpyDeviceToHost, stream);
-            if (e != cudaSuccess) return set_cuda_error("D2H exit", e);
-        }
-        if (N > 0) {
-            e = cudaMemcpyAsync(h_out_argmax, base + st.argmax, static_cast<size_t>(N) * 4, cudaMemcpyDeviceToHost, stream);
-            if (e != cudaSuccess) return set_cuda_error("D2H argmax", e);
-        }
-    }
-    return LASER_OK;
+    if (dims->N == 0 && dims->R == 0) return LASER_OK;
+    Handle* h = nullptr;
+    int rc = implicit_handle(*dims, kDefaultOptions, workspace, &h);
+    if (rc != LASER_OK) return rc;
+    return run_host(h, h_hidden, W, h_req_offsets, h_load, tau_params, h_out_conf, h_out_argmax, h_out_exit,
+                    workspace, workspace_bytes, d_staging, staging_bytes, stream_v, false);
 }
 
 int laser_probe_confidence_host(const void* h_hidden, const void* W, const int32_t* h_req_offsets,
@@ -704,14 +1046,14 @@ int laser_probe_confidence_host(const void* h_hidden, const void* W, const int32
                                 const laser_probe_dims* dims, void* workspace,
                                 size_t workspace_bytes, void* d_staging, size_t staging_bytes,
                                 void* stream_v) {
-    int rc = laser_probe_confidence_host_async(h_hidden, W, h_req_offsets, h_load, tau_params, h_out_conf,
-                                               h_out_argmax, h_out_exit, dims, workspace, workspace_bytes,
-                                               d_staging, staging_bytes, stream_v);
-    if (rc != LASER_OK) return rc;
+    if (!dims || !tau_params) return LASER_E_NULL;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
     if (dims->N == 0 && dims->R == 0) return LASER_OK;
-    cudaError_t e = cudaStreamSynchronize(static_cast<cudaStream_t>(stream_v));
-    if (e != cudaSuccess) return set_cuda_error("cudaStreamSynchronize", e);
-    return LASER_OK;
+    Handle* h = nullptr;
+    int rc = implicit_handle(*dims, kDefaultOptions, workspace, &h);
+    if (rc != LASER_OK) return rc;
+    return run_host(h, h_hidden, W, h_req_offsets, h_load, tau_params, h_out_conf, h_out_argmax, h_out_exit,
+                    workspace, workspace_bytes, d_staging, staging_bytes, stream_v, true);
 }
 
 int laser_tau_from_load(const float* load, int32_t R, const laser_tau_params* tau_params, float* out_tau) {
@@ -733,7 +1075,7 @@ int laser_ema_update(float* lbar, const float* L, int32_t R, float alpha) {
 
 int laser_budget_params_default(laser_budget_params* out) {
     if (!out) return LASER_E_NULL;
-    *out = laser_budget_params{10.f, 2.f, 0.6f, 1.5f, 50.f, 275.f, 10.f};
+    *out = laser_budget_params{10.0, 2.0, 0.6, 1.5, 50.0, 275.0, 10.0};
     return LASER_OK;
 }
 
@@ -741,19 +1083,19 @@ int laser_allocate_budget(const int32_t* prompt_tokens, const float* L, int32_t 
                           const laser_budget_params* q, int32_t* out_budget) {
     if (!q || (R > 0 && (!prompt_tokens || !L || !out_budget))) return LASER_E_NULL;
     if (R < 0) return LASER_E_DIMS;
-    if (!(q->p_max > q->p_min) || !(q->f_max >= q->f_min) || !(q->l_target > 0.f)) return LASER_E_PARAMS;
+    if (!(q->p_max > q->p_min) || !(q->f_max >= q->f_min) || !(q->l_target > 0.0)) return LASER_E_PARAMS;
     for (int32_t r = 0; r < R; ++r) {
         // Eq. 7: difficulty factor from the prompt length, clipped to [f_min, f_max]
-        double f_diff = q->f_min + (static_cast<double>(prompt_tokens[r]) - q->p_min) /
-                                       (static_cast<double>(q->p_max) - q->p_min) *
-                                       (static_cast<double>(q->f_max) - q->f_min);
+        double f_diff = q->f_min + (static_cast<double>(prompt_tokens[r]) - q->p_min) / (q->p_max - q->p_min) *
+                                       (q->f_max - q->f_min);
         f_diff = f_diff < q->f_min ? q->f_min : (f_diff > q->f_max ? q->f_max : f_diff);
         // Eq. 8: load factor min(1, L_target / max(1, L(t)))
-        const double den = L[r] > 1.f ? L[r] : 1.0;
+        const double den = L[r] > 1.f ? static_cast<double>(L[r]) : 1.0;
         double f_load = q->l_target / den;
         f_load = f_load < 1.0 ? f_load : 1.0;
-        // Eq. 6
-        double b = std::floor(static_cast<double>(q->b_base) * f_diff * f_load);
+        // Eq. 6; the floor is that of the real-number product: a binary product that lands within
+        // LASER_BUDGET_FLOOR_EPS below an integer (|p| = 100: 10 * 0.8 = 7.999...) is that integer
+        double b = std::floor(q->b_base * f_diff * f_load + LASER_BUDGET_FLOOR_EPS);
         if (b < q->b_min) b = q->b_min;
         out_budget[r] = static_cast<int32_t>(b);
     }
@@ -770,7 +1112,7 @@ const char* laser_status_string(int status) {
         case LASER_E_WORKSPACE: return "workspace / staging buffer missing, misaligned or too small";
         case LASER_E_ARCH: return "device is not sm_100 (B200); this library has no fallback path";
         case LASER_E_CUDA: return "CUDA call failed (see laser_last_error)";
-        case LASER_E_MODE: return "unknown aggregate mode";
+        case LASER_E_MODE: return "unknown aggregate / probability / kernel / tail mode or option";
         default: return "unknown status";
     }
 }
@@ -805,24 +1147,19 @@ int laser_profile_read(float* ms_fused_sum, float* ms_finalize_sum, int32_t* cal
     return LASER_OK;
 }
 
-int laser_probe_set_mode(int mode) {
-    if (mode < LASER_MODE_AUTO || mode > LASER_MODE_PAIR) return LASER_E_MODE;
-    g_force_mode.store(mode, std::memory_order_relaxed);
-    return LASER_OK;
+#ifdef LASER_TIMELINE
+int laser_debug_timeline_read(unsigned long long* out) {   // [8][160][8]
+    return cudaMemcpyFromSymbol(out, laser::g_timeline, sizeof(unsigned long long) * 8 * 160 * 8) == cudaSuccess ? 0 : -7;
 }
-
-int laser_probe_set_overlap(int enable) {
-    g_overlap.store(enable ? 1 : 0, std::memory_order_relaxed);
-    return LASER_OK;
-}
+#endif
 
 const char* laser_last_error(void) { return g_last_error.c_str(); }
 
 uint64_t laser_kernel_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 int laser_shutdown(void) {
-    std::lock_guard<std::mutex> lk(g_mu);
-    g_maps.clear();
+    // implicit handles are per thread: each thread drops its own at its next call
+    g_cache_generation.fetch_add(1, std::memory_order_relaxed);
     return LASER_OK;
 }
 

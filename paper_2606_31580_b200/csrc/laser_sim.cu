@@ -62,7 +62,8 @@ __device__ __forceinline__ int32_t sim_budget(double prompt_tokens, double L, co
     const double den = (L > 1.0) ? L : 1.0;
     double f_load = __ddiv_rn(p.budget_l_target, den);
     if (f_load > 1.0) f_load = 1.0;
-    double b = floor(__dmul_rn(__dmul_rn(p.b_base, f_diff), f_load));
+    // floor of the real-number product (include/laser_probe.h, LASER_BUDGET_FLOOR_EPS; DESIGN A19)
+    double b = floor(__dadd_rn(__dmul_rn(__dmul_rn(p.b_base, f_diff), f_load), LASER_BUDGET_FLOOR_EPS));
     if (b < p.b_min) b = p.b_min;
     return static_cast<int32_t>(b);
 }

@@ -2,9 +2,13 @@
 //
 //  laser_probe_fused_kernel   a1 + a2 of include/laser_probe.h: LM-head projection on tcgen05 tensor
 //                             cores with the online-softmax statistics (max, lowest-index argmax,
-//                             sum-exp) taken straight out of TMEM.  Logits never reach HBM.
-//  laser_probe_finalize_kernel  merge of the per-split statistics (warp shuffles), a3 per-request
-//                             aggregate, a4 threshold (Eq. 5 + clamp), a5 exit mask.
+//                             sum-exp) taken straight out of TMEM.  Logits never reach HBM.  Its TAIL
+//                             (after a device-wide arrival count) runs the merge of the per-split
+//                             statistics, a3 per-request aggregate, a4 threshold (Eq. 5 + clamp) and a5
+//                             exit mask on the first min(grid, R) CTAs: one launch per probe call.
+//  laser_probe_finalize_kernel  the same merge + a3-a5 as a kernel of its own: laser_probe_combine
+//                             (gathered shard statistics), degenerate batches, and the two-kernel
+//                             form of a call (LASER_TAIL_SEPARATE).
 //
 // Orientation: tokens on the MMA M axis (= TMEM lanes), vocabulary on the N axis (= TMEM columns).
 // With tcgen05.ld 32x32b every epilogue thread owns one token row and walks its vocabulary columns
@@ -22,6 +26,7 @@
 #include <math_constants.h>
 
 #include <cstdint>
+#include <cstdio>
 
 #include "ptx.cuh"
 
@@ -36,6 +41,8 @@ constexpr int kABytes = kTileM * kBlockK * 2;  // 16 KiB of hidden per stage
 constexpr int kTmemCols = 512;    // two 256-column accumulators (double buffered)
 constexpr int kFusedThreads = 192;  // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-5 epilogue
 constexpr int kEpilogueThreads = 128;
+constexpr int kTailThread0 = 64;    // first epilogue thread: runs the arrival protocol of the tail
+constexpr int kTailCache = 512;     // requests whose offsets / loads a CTA keeps in shared memory for its tail
 constexpr float kLog2e = 1.4426950408889634f;
 
 // How the vocabulary tiles are dealt to the execution units (CTAs, or CTA pairs) for `m_items` token
@@ -43,6 +50,9 @@ constexpr float kLog2e = 1.4426950408889634f;
 // that m_items * splits fills the units in whole rounds with the least work on the busiest unit.
 // Shared by the host planner and both kernels: when a batch carries padding rows (req_offsets[R] <
 // N) the kernels re-plan on the device for the token items that actually hold rows.
+// Records of the workspace are packed: (row n, split sp) lives at ws[n * splits + sp] with the split
+// count of the plan that actually runs (so the workspace holds max over item counts m of
+// m * rows_per_item * plan_splits(m).splits records, not the largest split count times every row).
 struct SplitPlan {
     int T, splits;
 };
@@ -65,24 +75,28 @@ __host__ __device__ inline SplitPlan plan_splits(int total_tiles, int m_items, i
 
 struct FusedParams {
     int32_t n_alloc, d, V;
-    int32_t m_tiles, splits, tiles_per_split, tile_n, k_blocks, stages;
-    int32_t work_items, n_pad;   // m_tiles counts items of 128 (single) / 256 (pair) token rows
+    int32_t m_tiles, tile_n, k_blocks, stages;
+    int32_t work_items;    // m_tiles * splits of the host plan; m_tiles counts items of 128 (single) / 256 (pair) rows
     uint32_t tx_bytes;     // bytes TMA delivers per stage and CTA (hidden box + W box)
     uint32_t stage_bytes;  // shared-memory stride of a stage: kABytes + (W rows per CTA) * 128
     uint64_t w_policy;     // L2 eviction policy for the W stream
-    float4* ws;            // [n_pad, splits] per (row, split): {max, sum exp(logit - max), argmax bits, token logit}
+    float4* ws;            // packed [rows, splits] per (row, split): {max, sum exp(logit - max), argmax bits, token logit}
     // LASER_PROB_TOKEN: token_ids[n] - v_offset is the column of W whose logit is kept for row n
     // (nullptr: no token logit is tracked; v_offset = global vocabulary index of W's row 0).
     const int32_t* token_ids;
     int32_t v_offset;
     // Padding-aware re-planning (m_tiles > 1 only): token items at or beyond req_offsets[R] are
-    // skipped and the vocabulary tiles are re-dealt over the remaining items; `splits` above stays
-    // the record stride (the largest split count any item count can produce).
+    // skipped and the vocabulary tiles are re-dealt over the remaining items.
     const int32_t* req_offsets;
     int32_t R, total_tiles, units, replan;
-    // 1: griddepcontrol.wait before the first global read (strict stream order for the inputs too);
-    // 0: only the workspace stores wait (see laser_probe_set_overlap in include/laser_probe.h).
+    // 1 (strict, default): griddepcontrol.wait before the first read of hidden / req_offsets /
+    //    token_ids; W - model weight, never written by the kernel ahead - is requested for the first
+    //    `stages` pipeline slots before the wait when the plan is static (replan == 0).
+    // 0 (overlap): only the workspace / output stores wait (laser_probe_options.overlap).
     int32_t wait_first;
+    // requests whose {offset, threshold} fit in the shared memory the pipeline leaves over: the
+    // epilogue warps fill that cache right after the wait, so the tail needs no input loads
+    int32_t tail_cache;
 };
 
 // ---------------------------------------------------------------------------------- descriptors
@@ -156,7 +170,374 @@ __device__ __forceinline__ void fold_columns(const uint32_t (&r)[NC], int vbase,
     s += (s0 + s1) + (s2 + s3);
 }
 
+// ---------------------------------------------------------------------------------- finalize
+struct TauParamsDev {
+    float lambda_base, beta, gamma, l_target, lambda_min, lambda_max;
+};
+
+// a4: Eq. 5 then the clamp.  Shared by the kernels and laser_tau_from_load.
+__host__ __device__ __forceinline__ float tau_eval(float load, const TauParamsDev& t) {
+    float lam = t.lambda_base - t.beta * tanhf(t.gamma * (load - t.l_target) / t.l_target);
+    lam = fmaxf(lam, t.lambda_min);
+    lam = fminf(lam, t.lambda_max);
+    return lam;
+}
+
+// One 16-byte record of online-softmax statistics: what the fused kernel leaves per (row, split) in
+// the workspace, what laser_probe_partial leaves per row of a vocabulary shard, and what
+// laser_probe_combine merges.  Same layout as laser_row_stats in include/laser_probe.h.
+//   x = max logit, y = sum exp(logit - max), z = argmax (int bits), w = logit of the row's token
+struct FinalizeParams {
+    int32_t n_alloc, R, splits, agg_mode;
+    int32_t m_tiles, rows_per_item, total_tiles, units, replan;   // see FusedParams
+    // record (n, sp) lives at ws[n * row_stride + sp * split_stride]:
+    //   fused workspace, packed [rows, nsplit]: row_stride = 0 (meaning "the split count that ran"),
+    //                                           split_stride = 1
+    //   gathered shard statistics [G, N]: row_stride = 1, split_stride = N  (laser_probe_combine)
+    int64_t row_stride, split_stride;
+    int32_t prob_mode;            // 0: row maximum 1/S; 1: the row's token exp(l_tok - m)/S
+    int32_t a_offset;             // added to every argmax (vocabulary shard offset; reduce path)
+    // laser_probe_combine over peer-pushed statistics: wait until flags[g] has reached `epoch` for
+    // every g < splits before reading (nullptr: the records are already complete in stream order).
+    const uint32_t* wait_flags;
+    uint32_t epoch;
+    const float4* ws;
+    const int32_t* req_offsets;
+    const float* load;
+    float* out_conf;
+    int32_t* out_argmax;
+    uint8_t* out_exit;
+    float* out_tau;   // nullable
+    float* out_pmax;  // nullable
+    TauParamsDev tau;
+};
+
+constexpr int kFinalizeThreads = 256;
+constexpr int kFinalizeWarps = kFinalizeThreads / 32;
+constexpr int kMaxTailWarps = 8;
+constexpr int kMergeBatch = 5;  // partials a lane loads before it starts merging (148 splits: one batch)
+
+// Merge the nsplit records of each of NR rows across a warp (lanes stride over the records; the loads
+// of all NR rows are issued before the first merge so that they overlap - one L2 round trip instead
+// of NR; then shuffles).  rec[i] == nullptr skips row i.  Every lane returns the merged statistics.
+// The records may have been written by other CTAs of the running grid (tail of the fused kernel):
+// they are read through L2 (ld.global.cg), never through this SM's L1.
+template <int NR>
+__device__ __forceinline__ void merge_rows(const float4* const (&rec)[NR], int64_t split_stride, int nsplit,
+                                           int lane, float (&m)[NR], int (&a)[NR], float (&s)[NR],
+                                           float (&lt)[NR]) {
+    const float4 neutral = make_float4(-CUDART_INF_F, 0.f, __int_as_float(0x7fffffff), -CUDART_INF_F);
+    // 2^{(x - M) log2e} with the convention that equal operands (also -inf, -inf) give exactly 1
+    auto scale = [](float x, float M) { return (x == M) ? 1.f : ptx::ex2_approx((x - M) * kLog2e); };
+#pragma unroll
+    for (int i = 0; i < NR; ++i) { m[i] = -CUDART_INF_F; s[i] = 0.f; lt[i] = -CUDART_INF_F; a[i] = 0x7fffffff; }
+    // ---- this lane's records: maximum first, then ONE rescale per record (independent ex2, no
+    // dependent chain of pairwise merges); on equal maxima the smaller vocabulary index wins
+    for (int sp0 = lane; sp0 < nsplit; sp0 += 32 * kMergeBatch) {
+        float4 v[NR][kMergeBatch];
+#pragma unroll
+        for (int i = 0; i < NR; ++i)
+#pragma unroll
+            for (int j = 0; j < kMergeBatch; ++j) {
+                const int sp = sp0 + 32 * j;
+                v[i][j] = (rec[i] != nullptr && sp < nsplit) ? __ldcg(rec[i] + sp * split_stride) : neutral;
+            }
+#pragma unroll
+        for (int i = 0; i < NR; ++i) {
+            float M = m[i];
+#pragma unroll
+            for (int j = 0; j < kMergeBatch; ++j) M = fmaxf(M, v[i][j].x);
+            float sum = s[i] * scale(m[i], M);
+            int am = (m[i] == M) ? a[i] : 0x7fffffff;
+#pragma unroll
+            for (int j = 0; j < kMergeBatch; ++j) {
+                sum += v[i][j].y * scale(v[i][j].x, M);
+                am = (v[i][j].x == M) ? min(am, __float_as_int(v[i][j].z)) : am;
+                lt[i] = fmaxf(lt[i], v[i][j].w);
+            }
+            m[i] = M; s[i] = sum; a[i] = am;
+        }
+    }
+    // ---- across the warp: max, then one rescale per lane, then plain sum / min / max reductions
+#pragma unroll
+    for (int i = 0; i < NR; ++i) {
+        float M = m[i];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, off));
+        s[i] *= scale(m[i], M);
+        a[i] = (m[i] == M) ? a[i] : 0x7fffffff;
+        m[i] = M;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+#pragma unroll
+        for (int i = 0; i < NR; ++i) {
+            s[i] += __shfl_xor_sync(0xffffffffu, s[i], off);
+            a[i] = min(a[i], __shfl_xor_sync(0xffffffffu, a[i], off));
+            lt[i] = fmaxf(lt[i], __shfl_xor_sync(0xffffffffu, lt[i], off));
+        }
+    }
+}
+__device__ __forceinline__ void merge_row(const float4* rec, int64_t split_stride, int nsplit, int lane,
+                                          float& m, int& a, float& s, float& lt) {
+    const float4* const r1[1] = {rec};
+    float mm[1], ss[1], ll[1];
+    int aa[1];
+    merge_rows<1>(r1, split_stride, nsplit, lane, mm, aa, ss, ll);
+    m = mm[0]; a = aa[0]; s = ss[0]; lt = ll[0];
+}
+
+// Records per row the fused kernel wrote for this batch (device-side re-plan, see FusedParams).
+__device__ __forceinline__ int records_per_row(const FinalizeParams& p) {
+    int nsplit = p.splits;
+    if (p.replan) {
+        const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
+        const int m_items = (n_valid + p.rows_per_item - 1) / p.rows_per_item;
+        if (m_items > 0) nsplit = plan_splits(p.total_tiles, min(m_items, p.m_tiles), p.units).splits;
+    }
+    return nsplit;
+}
+
+// Spin until every peer's flag has reached `epoch` (peer GPUs store them with system scope after
+// their statistics have landed here).  One thread per flag, then a block barrier.
+__device__ __forceinline__ void wait_peer_flags(const uint32_t* flags, int G, uint32_t epoch) {
+    if (static_cast<int>(threadIdx.x) < G) {
+        const long long t0 = clock64();
+        while (static_cast<int32_t>(ptx::ld_acquire_sys_u32(flags + threadIdx.x) - epoch) < 0) {
+            __nanosleep(64);
+            // a peer that never signals (crashed rank, mismatched epoch) must not hang the GPU:
+            // after ~5 s the kernel traps and the caller sees a CUDA error instead
+            if (clock64() - t0 > 10000000000LL) __trap();
+        }
+    }
+    __syncthreads();
+}
+
+// Barrier of a thread group: the whole block (kBarId == 0) or kThreads threads on named barrier kBarId
+// (the four epilogue warps in the tail of the fused kernel).
+template <int kBarId, int kThreads>
+__device__ __forceinline__ void group_sync() {
+    if constexpr (kBarId == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"n"(kBarId), "n"(kThreads) : "memory");
+}
+
+// Merge + a3 + a4 + a5 of request r by a thread group of nwarps warps (every thread of the group must
+// call this, it contains group barriers; tid = index in the group).  A warp takes rows b+w, b+w+nwarps, ...: its
+// lanes stride over the records of the row, fold their own, then merge across the warp with shuffles.
+// warp_acc: shared scratch of nwarps floats.  [b, e) = the request's rows (every thread), tau = its
+// threshold (needed in thread kFinalThread only): the callers read them before they wait for the
+// records, so that those loads are off the critical path.
+constexpr int kFinalThread = 32;   // lane 0 of the group's warp 1 (thread 0 runs the arrival protocol in the tail)
+template <int kBarId, int kThreads>
+__device__ __forceinline__ void finalize_request(const FinalizeParams& p, int tid, int r, int b, int e, float tau,
+                                                 int nsplit, float* warp_acc) {
+    constexpr int nwarps = kThreads / 32;
+    const int warp = tid >> 5, lane = tid & 31;
+    const int64_t row_stride = p.row_stride ? p.row_stride : nsplit;
+    // running aggregate of this warp's rows: sum (mean), sum of logs (geomean), min.  Two rows per
+    // pass (rows n and n + nwarps): their record loads share one L2 round trip.
+    float acc = (p.agg_mode == 2) ? CUDART_INF_F : 0.f;
+    bool any_nan = false;
+    for (int n0 = b + warp; n0 < e; n0 += 2 * nwarps) {
+        const int n1 = n0 + nwarps;
+        const float4* const rec[2] = {p.ws + static_cast<int64_t>(n0) * row_stride,
+                                      n1 < e ? p.ws + static_cast<int64_t>(n1) * row_stride : nullptr};
+        float m[2], s[2], lt[2];
+        int a[2];
+        merge_rows<2>(rec, p.split_stride, nsplit, lane, m, a, s, lt);
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int n = i == 0 ? n0 : n1;
+            if (n >= e) break;
+            // s >= 1 up to the rounding of ex2.approx; a probability does not exceed 1.  NaN stays NaN.
+            float prob;
+            if (p.prob_mode == 0) {
+                prob = (s[i] == s[i]) ? fminf(1.0f / s[i], 1.0f) : CUDART_NAN_F;
+            } else {   // the row's token: exp(l_tok - m) / S; a token outside the vocabulary has l_tok = -inf -> 0
+                prob = (s[i] == s[i]) ? fminf(ptx::ex2_approx((lt[i] - m[i]) * kLog2e) / s[i], 1.0f) : CUDART_NAN_F;
+            }
+            if (lane == 0) {
+                p.out_argmax[n] = a[i];
+                if (p.out_pmax) p.out_pmax[n] = prob;
+            }
+            any_nan |= (prob != prob);
+            if (p.agg_mode == 0) acc += prob;
+            else if (p.agg_mode == 1) acc += logf(prob);
+            else acc = fminf(acc, prob);
+        }
+    }
+    if (p.agg_mode == 2 && any_nan) acc = CUDART_NAN_F;
+    if (lane == 0) warp_acc[warp] = acc;
+    group_sync<kBarId, kThreads>();
+    if (tid == kFinalThread) {
+        const int len = e - b;
+        float conf = 0.f;
+        if (len > 0) {
+            if (p.agg_mode == 2) {
+                conf = warp_acc[0];
+                bool nan = conf != conf;
+                for (int w = 1; w < nwarps; ++w) {
+                    nan |= (warp_acc[w] != warp_acc[w]);
+                    conf = fminf(conf, warp_acc[w]);
+                }
+                if (nan) conf = CUDART_NAN_F;
+            } else {
+                float t = 0.f;
+                for (int w = 0; w < nwarps; ++w) t += warp_acc[w];
+                conf = t / static_cast<float>(len);
+                if (p.agg_mode == 1) conf = expf(conf);
+            }
+        }
+        p.out_conf[r] = conf;                  // a3
+        p.out_exit[r] = (conf > tau) ? 1 : 0;  // a5: strict; NaN > tau is false
+        if (p.out_tau) p.out_tau[r] = tau;
+    }
+    group_sync<kBarId, kThreads>();   // warp_acc may be reused by the caller's next request
+}
+
+// Outputs of padding rows (n >= req_offsets[R]): argmax -1, pmax NaN.  Rows are dealt to threads
+// `first`, `first + step`, ... of [n_valid, n_alloc).
+__device__ __forceinline__ void mark_padding_rows(const FinalizeParams& p, int first, int step) {
+    const int n_valid = (p.R > 0) ? min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc) : 0;
+    for (int n = n_valid + first; n < p.n_alloc; n += step) {
+        p.out_argmax[n] = -1;
+        if (p.out_pmax) p.out_pmax[n] = CUDART_NAN_F;
+    }
+}
+
+// Standalone form.  Blocks [0, R): one request each.  Blocks [R, R + ceil(n_alloc/256)): mark padding
+// rows.  Every global store comes after griddepcontrol.wait (the kernel ahead in the stream may be a
+// previous call still writing the same output buffers).
+__global__ void __launch_bounds__(kFinalizeThreads)
+laser_probe_finalize_kernel(const FinalizeParams p) {
+    __shared__ float warp_acc[kFinalizeWarps];
+    ptx::pdl_launch_dependents();
+    if (static_cast<int>(blockIdx.x) >= p.R) {
+        ptx::pdl_wait();
+        const int nb = gridDim.x - p.R;
+        mark_padding_rows(p, (blockIdx.x - p.R) * kFinalizeThreads + threadIdx.x, nb * kFinalizeThreads);
+        return;
+    }
+    // inputs of the probe call, complete before its first kernel started: read ahead of the wait
+    const int r = blockIdx.x;
+    const int b = __ldg(p.req_offsets + r), e = __ldg(p.req_offsets + r + 1);
+    float tau = 0.f;
+    if (threadIdx.x == kFinalThread) tau = tau_eval(__ldg(p.load + r), p.tau);   // a4
+    ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
+    const int nsplit = records_per_row(p);
+    if (p.wait_flags != nullptr) wait_peer_flags(p.wait_flags, nsplit, p.epoch);
+    finalize_request<0, kFinalizeThreads>(p, threadIdx.x, r, b, e, tau, nsplit, warp_acc);
+}
+
+// ---------------------------------------------------------------------------------- vocab-parallel
+// laser_probe_partial: the fused kernel over one vocabulary SHARD; its tail (or, in the two-kernel
+// form, laser_probe_reduce_kernel) merges each row's split records into a single record
+// {m, S, argmax + v_offset, l_tok} and stores it
+//   * to out_stats[n] (local), and
+//   * when peers are given, to slot [rank, n] of every GPU's gathered buffer [G, N] through
+//     peer-mapped pointers (NVLink stores; 16 bytes per row and peer) - the all-gather of the
+//     statistics is done by the producer, no collective call.
+// Rows n >= req_offsets[R] (padding) get the neutral record.  When every row has been pushed,
+// `epoch` is published in slot [rank] of every GPU's flag array (system-scope release).
+constexpr int kMaxPeers = 16;
+struct ReduceParams {
+    FinalizeParams f;          // ws, strides, replan fields, req_offsets, R, n_alloc, a_offset
+    float4* out_stats;         // [n_alloc] or nullptr
+    int32_t rank, world;       // world = 0: no peers
+    uint32_t epoch;
+    float4* peer_stats[kMaxPeers];   // peer_stats[g] = base of GPU g's gathered buffer [world, n_alloc]
+    uint32_t* peer_flags[kMaxPeers]; // peer_flags[g] = GPU g's flag array [world]
+};
+
+// One warp: merged record of row n -> out_stats / peers.
+__device__ __forceinline__ void reduce_row(const ReduceParams& q, int n, int n_valid, int nsplit, int lane) {
+    const FinalizeParams& p = q.f;
+    float m = -CUDART_INF_F, s = 0.f, lt = -CUDART_INF_F;
+    int a = 0x7fffffff;
+    if (n < n_valid) {
+        const int64_t row_stride = p.row_stride ? p.row_stride : nsplit;
+        merge_row(p.ws + static_cast<int64_t>(n) * row_stride, p.split_stride, nsplit, lane, m, a, s, lt);
+        a += p.a_offset;
+    }
+    const float4 rec = make_float4(m, s, __int_as_float(a), lt);
+    if (lane == 0 && q.out_stats) q.out_stats[n] = rec;
+    if (lane < q.world) q.peer_stats[lane][static_cast<int64_t>(q.rank) * p.n_alloc + n] = rec;
+}
+
+__device__ __forceinline__ void publish_epoch(const ReduceParams& q, int lane) {
+    if (lane < q.world) {
+        __threadfence_system();
+        ptx::st_release_sys_u32(q.peer_flags[lane] + q.rank, q.epoch);
+    }
+}
+
+__global__ void __launch_bounds__(kFinalizeThreads)
+laser_probe_reduce_kernel(const ReduceParams q) {
+    const FinalizeParams& p = q.f;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    ptx::pdl_launch_dependents();
+    ptx::pdl_wait();
+    const int n = blockIdx.x * kFinalizeWarps + warp;
+    const int n_valid = (p.R > 0) ? min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc) : 0;
+    const int nsplit = records_per_row(p);
+    if (n >= p.n_alloc) return;
+    reduce_row(q, n, n_valid, nsplit, lane);
+}
+
+// After the reduce kernel (stream order: its stores, remote ones included, have been performed):
+// publish `epoch` in slot [rank] of every GPU's flag array with a system-scope release store.
+__global__ void laser_probe_signal_kernel(const ReduceParams q) {
+    publish_epoch(q, threadIdx.x);
+}
+
+// LASER_DEBUG=1: the documented precondition on req_offsets (non-decreasing, [0] == 0, [R] <= N),
+// checked on the device by one warp ahead of the probe; a violation traps (the caller sees a CUDA
+// error at the next synchronisation) instead of silently reading other requests' rows.
+__global__ void laser_probe_validate_kernel(const int32_t* req_offsets, int R, int N) {
+    bool bad = false;
+    for (int r = threadIdx.x; r <= R; r += 32) {
+        const int v = req_offsets[r];
+        if (r == 0 && v != 0) bad = true;
+        if (r > 0 && v < req_offsets[r - 1]) bad = true;
+        if (v < 0 || v > N) bad = true;
+    }
+    if (__any_sync(0xffffffffu, bad)) {
+        if (threadIdx.x == 0) printf("laser_probe: req_offsets violates the precondition (non-decreasing, [0]==0, [R]<=N)\n");
+        __trap();
+    }
+}
+
 // ---------------------------------------------------------------------------------- fused kernel
+// What the tail of the fused kernel does once every CTA's records are in the workspace.
+//   kind 0: nothing (a second kernel follows: LASER_TAIL_SEPARATE)
+//   kind 1: merge + a3-a5 (q.f), CTA b takes requests b, b + F, ... with F = min(grid, R)
+//   kind 2: vocabulary-parallel reduce (q): CTA b takes rows, the last CTA to finish publishes the epoch
+// ctl: four device words owned by the library (never the caller's workspace):
+//   ctl[0] counts CTA arrivals and only ever grows (wrap-safe compares); ctl[1] is the count at which
+//   the current call started ("base"): every CTA reads it before it counts itself in, the LAST
+//   arrival advances it by gridDim.x, so nothing is reset and no tail CTA reports back.  ctl[2]
+//   (kind 2 only) counts tail CTAs whose rows have been pushed; the last one publishes the epoch and
+//   clears it.  Calls that share a ctl slot must be stream-ordered (one handle = one slot).
+#ifdef LASER_TIMELINE
+// Debug build only (never the shipped library): per-CTA globaltimer stamps of the last 8 calls.
+__device__ unsigned long long g_timeline[8][160][8];
+__device__ __forceinline__ unsigned long long tl_now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define LASER_TL(slot, ev, tid) do { if (threadIdx.x == (tid)) g_timeline[(slot) & 7][blockIdx.x][(ev)] = tl_now(); } while (0)
+#else
+#define LASER_TL(slot, ev, tid) do { } while (0)
+#endif
+
+struct TailParams {
+    int32_t tl_slot;
+    int32_t kind;
+    uint32_t* ctl;
+    ReduceParams q;
+};
+
 // kPair = false: one CTA per SM, tcgen05 cta_group::1, a work item is (128 token rows, vocab split).
 // kPair = true : clusters of two CTAs (the two SMs of a TPC), tcgen05 cta_group::2: one M = 256 MMA
 //                spans both CTAs.  A work item is (256 token rows, vocab split); CTA `rank` of the pair
@@ -170,7 +551,8 @@ __device__ __forceinline__ void fold_columns(const uint32_t (&r)[NC], int vbase,
 template <bool kPair>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
-                         const __grid_constant__ CUtensorMap tmap_w, const FusedParams p) {
+                         const __grid_constant__ CUtensorMap tmap_w, const FusedParams p,
+                         const __grid_constant__ TailParams t) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = ptx::smem_u32(smem_raw);
     const uint32_t smem = (raw + 1023u) & ~1023u;  // SWIZZLE_128B tiles need 1024-byte alignment
@@ -186,24 +568,69 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
+    LASER_TL(t.tl_slot, 0, 0);    // kernel entry
     const uint32_t rank = kPair ? ptx::cluster_ctarank() : 0u;   // 0 = leader
     const int unit = kPair ? (blockIdx.x >> 1) : blockIdx.x;     // CTA (single) or CTA pair
     const int units = kPair ? (gridDim.x >> 1) : gridDim.x;
     constexpr int kRowsPerItem = kPair ? 2 * kTileM : kTileM;
     constexpr int kEpiArrivals = kPair ? 8 : 4;                  // one per epilogue warp (of both CTAs)
 
-    if (warp == 0 && lane == 0) {
-        ptx::prefetch_tensormap(&tmap_hidden);
-        ptx::prefetch_tensormap(&tmap_w);
-        for (int s = 0; s < p.stages; ++s) {
-            ptx::mbar_init(full_bar(s), 1);
-            ptx::mbar_init(empty_bar(s), 1);
+    const int BN = p.tile_n;
+    const int b_rows = kPair ? (BN >> 1) : BN;   // W rows this CTA stages per tile
+    const int total_tiles = p.total_tiles;
+    int m_items = p.m_tiles, work_items = p.work_items;
+    int S = work_items / m_items;                // static plan; re-planned below when p.replan
+
+    // W ahead of the wait (strict mode, static plan): the producer requests the W boxes of its first
+    // `stages` pipeline slots - and asks L2 for the boxes of the `stages` slots after those - before
+    // griddepcontrol.wait, so that the head of the W stream overlaps whatever the kernel ahead of this
+    // one still has to finish.  W is model weight: the kernel ahead never writes it (documented in
+    // include/laser_probe.h).  The hidden boxes of those slots follow after the wait.
+    int pre = 0;
+    auto preissue_w = [&]() {
+        if (!(p.wait_first && !p.replan && unit < work_items)) return;
+        const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);
+        int tile = unit / m_items, kb = 0;
+        for (int slot = 0; slot < 2 * p.stages && tile < total_tiles; ++slot) {
+            if (ptx::elect_one()) {
+                const int b_row = tile * BN + static_cast<int>(rank) * b_rows;
+                if (slot < p.stages) {
+                    const uint32_t sb = smem + static_cast<uint32_t>(slot) * p.stage_bytes + kABytes;
+                    const uint32_t fb = full0 + 8u * slot;
+                    if constexpr (kPair) {
+                        if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), 2u * p.tx_bytes);
+                        ptx::tma_load_2d_pair(sb, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
+                    } else {
+                        ptx::mbar_arrive_expect_tx(fb, p.tx_bytes);
+                        ptx::tma_load_2d(sb, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
+                    }
+                } else {
+                    ptx::tma_prefetch_2d(&tmap_w, kb * kBlockK, b_row);
+                }
+            }
+            __syncwarp();
+            if (slot < p.stages) ++pre;
+            if (++kb == p.k_blocks) { kb = 0; tile += S; }
         }
-        for (int b = 0; b < 2; ++b) {
-            ptx::mbar_init(tfull_bar(b), 1);
-            ptx::mbar_init(tempty_bar(b), kEpiArrivals);
+    };
+
+    if (warp == 0) {
+        if (lane == 0) {
+            ptx::prefetch_tensormap(&tmap_hidden);
+            ptx::prefetch_tensormap(&tmap_w);
+            for (int s = 0; s < p.stages; ++s) {
+                ptx::mbar_init(full_bar(s), 1);
+                ptx::mbar_init(empty_bar(s), 1);
+            }
+            for (int b = 0; b < 2; ++b) {
+                ptx::mbar_init(tfull_bar(b), 1);
+                ptx::mbar_init(tempty_bar(b), kEpiArrivals);
+            }
+            ptx::fence_mbar_init();
         }
-        ptx::fence_mbar_init();
+        __syncwarp();
+        // single CTA: its own barriers are all the loads need - do not wait for the TMEM allocation
+        if constexpr (!kPair) preissue_w();
     }
     if (warp == 1) {
         ptx::tmem_alloc_t<kPair>(tmem_slot, kTmemCols);
@@ -215,52 +642,72 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     ptx::tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
-    // Programmatic dependent launch.  wait_first (the library default, laser_probe_set_overlap(0)):
-    // every global read below happens after the kernel ahead of this one in the stream has completed;
-    // only the prologue above overlapped it.  Without it (overlap opted in): the only memory this
-    // kernel shares with the kernel before it in a chain of probe calls (the previous call's finalize
-    // kernel) is the workspace, so only the workspace stores (and the exit) wait for that kernel and
-    // the W stream of this call overlaps the tail of the previous one.
-    if (p.wait_first) ptx::pdl_wait();
-    // Let the finalize kernel's CTAs become resident now (they block in griddepcontrol.wait).
+    // Programmatic dependent launch: whatever follows in the stream may become resident on the SMs
+    // this grid vacates; it must itself wait (griddepcontrol.wait) before it touches our outputs.
     ptx::pdl_launch_dependents();
+    if constexpr (kPair) { if (warp == 0) preissue_w(); }
+    LASER_TL(t.tl_slot, 1, 0);    // prologue + W pre-issue done
 
-    int m_items = p.m_tiles, work_items = p.work_items;
-    const int BN = p.tile_n;
-    const int b_rows = kPair ? (BN >> 1) : BN;   // W rows this CTA stages per tile
+    // Strict: every read of hidden / req_offsets / token_ids below happens after the kernel ahead of
+    // this one in the stream has completed.  Overlap: only the stores wait (further down).
+    if (p.wait_first) ptx::pdl_wait();
+    LASER_TL(t.tl_slot, 2, 0);    // strict wait passed
+    // tail bookkeeping: the arrival count this call starts from (strict: read here, long before it is
+    // needed; the call ahead, which may share the slot, has completed)
+    uint32_t base = 0;
+    if (threadIdx.x == kTailThread0 && t.kind != 0 && p.wait_first) base = ptx::ld_relaxed_gpu_u32(t.ctl + 1);
+    // a4 ahead of time: {req_offsets, tau(load)} of every request into the shared-memory cache behind
+    // the barrier block (any CTA may turn out to be one of the last to arrive)
+    int* off_c = reinterpret_cast<int*>(smem_raw + (smem - raw) + p.stages * p.stage_bytes + 256u);
+    float* tau_c = reinterpret_cast<float*>(off_c + p.tail_cache + 1);
+    const bool cached = t.kind == 1 && t.q.f.R <= p.tail_cache;
+    if (cached && warp >= 2) {
+        const FinalizeParams& f = t.q.f;
+        for (int i = threadIdx.x - kTailThread0; i <= f.R; i += kEpilogueThreads) {
+            off_c[i] = __ldg(f.req_offsets + i);
+            if (i < f.R) tau_c[i] = tau_eval(__ldg(f.load + i), f.tau);
+        }
+    }
+
     if (p.replan) {   // uniform across the grid: every thread reads the same word
         const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
         m_items = (n_valid + kRowsPerItem - 1) / kRowsPerItem;
         if (m_items < p.m_tiles) {
-            if (m_items > 0) {
-                work_items = m_items * plan_splits(p.total_tiles, m_items, p.units).splits;
-            } else {
-                work_items = 0;
-            }
+            work_items = m_items > 0 ? m_items * plan_splits(total_tiles, m_items, p.units).splits : 0;
+        } else {
+            m_items = p.m_tiles;
         }
+        S = m_items > 0 ? work_items / m_items : 1;
     }
     // split sp owns vocabulary tiles sp, sp + S, sp + 2S, ... (ascending: ties keep the lowest index)
-    const int S = m_items > 0 ? work_items / m_items : 1;
-    const int total_tiles = p.total_tiles;
 
     if (warp == 0) {
         // ===================================================================== TMA producer
         // Converged warp, one elected lane issues (see the MMA issuer).
-        {
-            const int k_blocks = p.k_blocks, stages = p.stages;
-            const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);  // leader's barriers
-            int stage = 0;
-            uint32_t phase = 0;
-            for (int w = unit; w < work_items; w += units) {
-                const int mt = w % m_items, sp = w / m_items;
-                const int a_row = mt * kRowsPerItem + static_cast<int>(rank) * kTileM;
-                for (int tile = sp; tile < total_tiles; tile += S) {
-                    const int b_row = tile * BN + static_cast<int>(rank) * b_rows;
-                    for (int kb = 0; kb < k_blocks; ++kb) {
+        const int k_blocks = p.k_blocks, stages = p.stages;
+        const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);  // leader's barriers
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int w = unit; w < work_items; w += units) {
+            const int mt = w % m_items, sp = w / m_items;
+            const int a_row = mt * kRowsPerItem + static_cast<int>(rank) * kTileM;
+            for (int tile = sp; tile < total_tiles; tile += S) {
+                const int b_row = tile * BN + static_cast<int>(rank) * b_rows;
+                for (int kb = 0; kb < k_blocks; ++kb) {
+                    const uint32_t sa = smem + static_cast<uint32_t>(stage) * p.stage_bytes;
+                    const uint32_t fb = full0 + 8u * stage;
+                    if (pre > 0) {
+                        // slot whose W box (and expected byte count) went out ahead of the wait
+                        --pre;
+                        if (ptx::elect_one()) {
+                            if constexpr (kPair)
+                                ptx::tma_load_2d_pair(sa, &tmap_hidden, fb, kb * kBlockK, a_row, ptx::kEvictLast);
+                            else
+                                ptx::tma_load_2d(sa, &tmap_hidden, fb, kb * kBlockK, a_row, ptx::kEvictLast);
+                        }
+                    } else {
                         ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
                         if (ptx::elect_one()) {
-                            const uint32_t sa = smem + static_cast<uint32_t>(stage) * p.stage_bytes;
-                            const uint32_t fb = full0 + 8u * stage;
                             if constexpr (kPair) {
                                 // both CTAs' bytes complete on the leader's barrier
                                 if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2u * p.tx_bytes);
@@ -272,9 +719,9 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                                 ptx::tma_load_2d(sa + kABytes, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
                             }
                         }
-                        __syncwarp();
-                        if (++stage == stages) { stage = 0; phase ^= 1u; }
                     }
+                    __syncwarp();
+                    if (++stage == stages) { stage = 0; phase ^= 1u; }
                 }
             }
         }
@@ -333,8 +780,8 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             if (p.token_ids != nullptr) {
                 const int n = mt * kRowsPerItem + row;
                 if (n < p.n_alloc) {
-                    const int t = __ldg(p.token_ids + n) - p.v_offset;
-                    tok = (t >= 0 && t < p.V) ? t : -1;   // not in this (shard of the) vocabulary
+                    const int tk = __ldg(p.token_ids + n) - p.v_offset;
+                    tok = (tk >= 0 && tk < p.V) ? tk : -1;   // not in this (shard of the) vocabulary
                 }
             }
             for (int tile = sp; tile < total_tiles; tile += S, ++acc) {
@@ -365,272 +812,110 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                     else ptx::mbar_arrive(tempty_bar(buf));
                 }
             }
-            // row-major over splits: the finalize kernel reads a row's partials as contiguous 16-byte
+            // packed row-major over splits: the merge reads a row's partials as contiguous 16-byte
             // records (coalesced); the scattered 16-byte stores here are fire-and-forget
-            const size_t o = (static_cast<size_t>(mt) * kRowsPerItem + row) * p.splits + sp;
-            ptx::pdl_wait();   // the previous call's finalize kernel may still be reading the workspace
+            const size_t o = (static_cast<size_t>(mt) * kRowsPerItem + row) * S + sp;
+            ptx::pdl_wait();   // overlap mode: the previous call's tail may still be reading the workspace
             p.ws[o] = make_float4(m, s, __int_as_float(a), lt);
+        }
+        LASER_TL(t.tl_slot, 3, kTailThread0);   // last record stored
+        // This warp is done with TMEM and the pipeline: tell the teardown below (TMEM deallocation by
+        // warp 1) without waiting for it - the tail that follows needs neither.
+        ptx::tc_fence_before();
+        if constexpr (kPair) ptx::cluster_arrive();
+        else asm volatile("bar.arrive 2, %0;" ::"n"(kFusedThreads) : "memory");
+
+        // ================================================================= tail (epilogue warps only)
+        // The four epilogue warps count this CTA in as soon as their records are stored - the producer
+        // and MMA warps go straight to the teardown - and the LAST F CTAs to arrive run merge + a3-a5
+        // (kind 1) or the shard reduce (kind 2): they are the ones with the least to wait for.
+        if (t.kind != 0) {
+            ptx::pdl_wait();   // outputs are written below (a CTA without work items has not waited yet)
+            const int tid = threadIdx.x - kTailThread0, tw = tid >> 5;
+            constexpr int kTW = kEpilogueThreads / 32;
+            const FinalizeParams& f = t.q.f;
+            const int grid = gridDim.x;
+            const int F = (t.kind == 1) ? min(grid, f.R) : min(grid, (f.n_alloc + kTW - 1) / kTW);
+            // scratch: bytes [192, 232) of the barrier block
+            float* warp_acc = reinterpret_cast<float*>(smem_raw + (smem - raw) + p.stages * p.stage_bytes + 192u);
+            volatile uint32_t* tk = reinterpret_cast<volatile uint32_t*>(warp_acc + kMaxTailWarps);
+            group_sync<1, kEpilogueThreads>();   // every record store of this CTA is ordered before the count
+            if (tid == 0) {
+                if (!p.wait_first) base = ptx::ld_relaxed_gpu_u32(t.ctl + 1);   // overlap: the call ahead is complete only now
+                const uint32_t target = base + static_cast<uint32_t>(grid);
+                LASER_TL(t.tl_slot, 4, kTailThread0);
+                const uint32_t mine = ptx::atom_add_acq_rel_gpu_u32(t.ctl, 1u) + 1u;
+                if (mine == target) t.ctl[1] = target;   // last arrival: every CTA has read `base`
+                tk[0] = mine; tk[1] = target;
+            }
+            group_sync<1, kEpilogueThreads>();
+            const uint32_t mine = tk[0], target = tk[1];
+            const int behind = static_cast<int>(target - mine);    // CTAs still to arrive
+            if (behind >= F) {
+                // not one of the last F: padding rows do not depend on anybody's records
+                if (t.kind == 1) mark_padding_rows(f, blockIdx.x * kEpilogueThreads + tid, grid * kEpilogueThreads);
+            } else {
+                const int fi = F - 1 - behind;    // 0 .. F-1; the last arrival is F-1
+                if (behind > 0) {
+                    if ((tid & 31) == 0) {
+                        const long long t0 = clock64();
+                        while (static_cast<int32_t>(ptx::ld_acquire_gpu_u32(t.ctl) - target) < 0) {
+                            // all CTAs of this grid are resident or become resident as others exit (grid
+                            // <= SMs); a wait of seconds means the device cannot hold the grid: trap
+                            if (clock64() - t0 > 8000000000LL) __trap();
+                        }
+                    }
+                    __syncwarp();
+                }   // (the last arrival's own acq_rel count has acquired everybody's records)
+                LASER_TL(t.tl_slot, 5, kTailThread0);
+                if (t.kind == 1) {
+                    for (int r = fi; r < f.R; r += F) {
+                        const int rb = cached ? off_c[r] : __ldg(f.req_offsets + r);
+                        const int re = cached ? off_c[r + 1] : __ldg(f.req_offsets + r + 1);
+                        float tau = 0.f;
+                        if (tid == kFinalThread) tau = cached ? tau_c[r] : tau_eval(__ldg(f.load + r), f.tau);
+                        finalize_request<1, kEpilogueThreads>(f, tid, r, rb, re, tau, S, warp_acc);
+                        if (r == fi) LASER_TL(t.tl_slot, 6, kTailThread0);
+                    }
+                    mark_padding_rows(f, blockIdx.x * kEpilogueThreads + tid, grid * kEpilogueThreads);
+                } else {
+                    const int n_valid = (f.R > 0) ? min(max(__ldg(f.req_offsets + f.R), 0), f.n_alloc) : 0;
+                    for (int n = fi * kTW + tw; n < f.n_alloc; n += F * kTW) reduce_row(t.q, n, n_valid, S, tid & 31);
+                    __threadfence_system();   // remote (peer) stores of this thread are performed before the count below
+                    group_sync<1, kEpilogueThreads>();
+                    if (tid < 32) {
+                        uint32_t last = 0;
+                        if (tid == 0) {
+                            last = (ptx::atom_add_acq_rel_gpu_u32(t.ctl + 2, 1u) == static_cast<uint32_t>(F - 1)) ? 1u : 0u;
+                            if (last) t.ctl[2] = 0u;
+                        }
+                        last = __shfl_sync(0xffffffffu, last, 0);
+                        if (last) publish_epoch(t.q, tid);   // every tail CTA's rows are on every GPU
+                    }
+                }
+            }
         }
     }
 
     // ------------------------------------------------------------------------- teardown
     __syncwarp();   // reconverge the warps whose lane 0 ran a role loop
+    LASER_TL(t.tl_slot, 7, 0);    // producer done issuing
     // No CTA (not even one without work) completes before the kernel ahead of it in the stream has:
     // completion of this grid then implies completion of everything before it, as stream order demands.
     ptx::pdl_wait();
+    if (warp >= 2) {
+        // epilogue warps arrived before their tail; the cluster barrier wants every arrival waited for
+        if constexpr (kPair) ptx::cluster_wait();
+        return;
+    }
     ptx::tc_fence_before();
-    if constexpr (kPair) ptx::cluster_sync();   // the peer may still read this CTA's shared memory / TMEM
-    else __syncthreads();
+    // all epilogue warps (of both CTAs of a pair: the peer may still read this CTA's shared memory /
+    // TMEM) have finished with TMEM
+    if constexpr (kPair) ptx::cluster_sync();
+    else asm volatile("bar.sync 2, %0;" ::"n"(kFusedThreads) : "memory");
     if (warp == 1) {
         ptx::tc_fence_after();
         ptx::tmem_dealloc_t<kPair>(tmem_base, kTmemCols);
-    }
-}
-
-// ---------------------------------------------------------------------------------- finalize
-struct TauParamsDev {
-    float lambda_base, beta, gamma, l_target, lambda_min, lambda_max;
-};
-
-// a4: Eq. 5 then the clamp.  Shared by the kernel and laser_tau_from_load.
-__host__ __device__ __forceinline__ float tau_eval(float load, const TauParamsDev& t) {
-    float lam = t.lambda_base - t.beta * tanhf(t.gamma * (load - t.l_target) / t.l_target);
-    lam = fmaxf(lam, t.lambda_min);
-    lam = fminf(lam, t.lambda_max);
-    return lam;
-}
-
-// One 16-byte record of online-softmax statistics: what the fused kernel leaves per (row, split) in
-// the workspace, what laser_probe_partial leaves per row of a vocabulary shard, and what
-// laser_probe_combine merges.  Same layout as laser_row_stats in include/laser_probe.h.
-//   x = max logit, y = sum exp(logit - max), z = argmax (int bits), w = logit of the row's token
-struct FinalizeParams {
-    int32_t n_alloc, R, splits, n_pad, agg_mode;
-    int32_t m_tiles, rows_per_item, total_tiles, units, replan;   // see FusedParams
-    // record (n, sp) lives at ws[n * row_stride + sp * split_stride]:
-    //   fused workspace [n_pad, splits]: row_stride = splits, split_stride = 1
-    //   gathered shard statistics [G, N]: row_stride = 1, split_stride = N  (laser_probe_combine)
-    int64_t row_stride, split_stride;
-    int32_t prob_mode;            // 0: row maximum 1/S; 1: the row's token exp(l_tok - m)/S
-    int32_t a_offset;             // added to every argmax (vocabulary shard offset; reduce kernel)
-    // laser_probe_combine over peer-pushed statistics: wait until flags[g] has reached `epoch` for
-    // every g < splits before reading (nullptr: the records are already complete in stream order).
-    const uint32_t* wait_flags;
-    uint32_t epoch;
-    const float4* ws;
-    const int32_t* req_offsets;
-    const float* load;
-    float* out_conf;
-    int32_t* out_argmax;
-    uint8_t* out_exit;
-    float* out_tau;   // nullable
-    float* out_pmax;  // nullable
-    TauParamsDev tau;
-};
-
-// (m,a,s,lt) (+) (m',a',s',lt'): commutative form - on equal maxima the smaller vocabulary index
-// wins; at most one operand carries a finite token logit.
-__device__ __forceinline__ void merge_stats(float& m, int& a, float& s, float& lt, float m2, int a2,
-                                            float s2, float lt2) {
-    const float M = fmaxf(m, m2);
-    const int an = (m > m2) ? a : ((m2 > m) ? a2 : min(a, a2));
-    const float e1 = (m == M) ? 1.f : ptx::ex2_approx((m - M) * kLog2e);
-    const float e2 = (m2 == M) ? 1.f : ptx::ex2_approx((m2 - M) * kLog2e);
-    s = s * e1 + s2 * e2;
-    m = M;
-    a = an;
-    lt = fmaxf(lt, lt2);
-}
-
-constexpr int kFinalizeThreads = 256;
-constexpr int kFinalizeWarps = kFinalizeThreads / 32;
-constexpr int kMergeBatch = 5;  // partials a lane loads before it starts merging (148 splits: one batch)
-
-// Merge the nsplit records of one row across a warp (lanes stride over the records, loads issued in
-// batches so that they overlap; then shuffles).  Every lane returns the merged statistics.
-__device__ __forceinline__ void merge_row(const float4* rec, int64_t split_stride, int nsplit, int lane,
-                                          float& m, int& a, float& s, float& lt) {
-    m = -CUDART_INF_F; s = 0.f; lt = -CUDART_INF_F;
-    a = 0x7fffffff;
-    for (int sp0 = lane; sp0 < nsplit; sp0 += 32 * kMergeBatch) {
-        float4 v[kMergeBatch];
-#pragma unroll
-        for (int j = 0; j < kMergeBatch; ++j) {
-            const int sp = sp0 + 32 * j;
-            v[j] = sp < nsplit ? rec[sp * split_stride]
-                               : make_float4(-CUDART_INF_F, 0.f, __int_as_float(0x7fffffff), -CUDART_INF_F);
-        }
-#pragma unroll
-        for (int j = 0; j < kMergeBatch; ++j)
-            merge_stats(m, a, s, lt, v[j].x, __float_as_int(v[j].z), v[j].y, v[j].w);
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        const float m2 = __shfl_xor_sync(0xffffffffu, m, off);
-        const int a2 = __shfl_xor_sync(0xffffffffu, a, off);
-        const float s2 = __shfl_xor_sync(0xffffffffu, s, off);
-        const float l2 = __shfl_xor_sync(0xffffffffu, lt, off);
-        merge_stats(m, a, s, lt, m2, a2, s2, l2);
-    }
-}
-
-// Records per row the fused kernel wrote for this batch (device-side re-plan, see FusedParams).
-__device__ __forceinline__ int records_per_row(const FinalizeParams& p) {
-    int nsplit = p.splits;
-    if (p.replan) {
-        const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
-        const int m_items = (n_valid + p.rows_per_item - 1) / p.rows_per_item;
-        if (m_items > 0) nsplit = plan_splits(p.total_tiles, min(m_items, p.m_tiles), p.units).splits;
-    }
-    return nsplit;
-}
-
-// Spin until every peer's flag has reached `epoch` (peer GPUs store them with system scope after
-// their statistics have landed here).  One thread per flag, then a block barrier.
-__device__ __forceinline__ void wait_peer_flags(const uint32_t* flags, int G, uint32_t epoch) {
-    if (static_cast<int>(threadIdx.x) < G) {
-        const long long t0 = clock64();
-        while (static_cast<int32_t>(ptx::ld_acquire_sys_u32(flags + threadIdx.x) - epoch) < 0) {
-            __nanosleep(64);
-            // a peer that never signals (crashed rank, mismatched epoch) must not hang the GPU:
-            // after ~5 s the kernel traps and the caller sees a CUDA error instead
-            if (clock64() - t0 > 10000000000LL) __trap();
-        }
-    }
-    __syncthreads();
-}
-
-// Blocks [0, R): one request each.  A warp takes rows b+w, b+w+8, ...: its lanes stride over the
-// records of the row, fold their own, then merge across the warp with shuffles.
-// Blocks [R, R + ceil(n_alloc/256)): mark padding rows (n >= req_offsets[R]).
-// Everything that does not depend on the fused kernel (offsets, load, threshold) is read before
-// griddepcontrol.wait so that under programmatic dependent launch it overlaps the fused kernel.
-// launch_dependents is issued first of all: the next call's fused kernel may then take every SM the
-// current fused kernel vacates and run its prologue there; it still blocks in its own
-// griddepcontrol.wait until this grid (hence, transitively, the current fused kernel) has completed.
-__global__ void __launch_bounds__(kFinalizeThreads)
-laser_probe_finalize_kernel(const FinalizeParams p) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    ptx::pdl_launch_dependents();
-    if (static_cast<int>(blockIdx.x) >= p.R) {
-        const int n = (blockIdx.x - p.R) * kFinalizeThreads + threadIdx.x;
-        const int n_valid = (p.R > 0) ? __ldg(p.req_offsets + p.R) : 0;
-        if (n < p.n_alloc && n >= n_valid) {   // outputs of padding rows: independent of the fused kernel
-            p.out_argmax[n] = -1;
-            if (p.out_pmax) p.out_pmax[n] = CUDART_NAN_F;
-        }
-        return;
-    }
-    __shared__ float warp_acc[kFinalizeWarps];
-    const int r = blockIdx.x;
-    const int b = __ldg(p.req_offsets + r), e = __ldg(p.req_offsets + r + 1);
-    float tau = 0.f;
-    if (threadIdx.x == 0) tau = tau_eval(__ldg(p.load + r), p.tau);   // a4
-    const int nsplit = records_per_row(p);
-
-    ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
-    if (p.wait_flags != nullptr) wait_peer_flags(p.wait_flags, nsplit, p.epoch);
-
-    // running aggregate of this warp's rows: sum (mean), sum of logs (geomean), min
-    float acc = (p.agg_mode == 2) ? CUDART_INF_F : 0.f;
-    bool any_nan = false;
-    for (int n = b + warp; n < e; n += kFinalizeWarps) {
-        float m, s, lt;
-        int a;
-        merge_row(p.ws + static_cast<int64_t>(n) * p.row_stride, p.split_stride, nsplit, lane, m, a, s, lt);
-        // s >= 1 up to the rounding of ex2.approx; a probability does not exceed 1.  NaN stays NaN.
-        float prob;
-        if (p.prob_mode == 0) {
-            prob = (s == s) ? fminf(1.0f / s, 1.0f) : CUDART_NAN_F;
-        } else {   // the row's token: exp(l_tok - m) / S; a token outside the vocabulary has l_tok = -inf -> 0
-            prob = (s == s) ? fminf(ptx::ex2_approx((lt - m) * kLog2e) / s, 1.0f) : CUDART_NAN_F;
-        }
-        if (lane == 0) {
-            p.out_argmax[n] = a;
-            if (p.out_pmax) p.out_pmax[n] = prob;
-        }
-        any_nan |= (prob != prob);
-        if (p.agg_mode == 0) acc += prob;
-        else if (p.agg_mode == 1) acc += logf(prob);
-        else acc = fminf(acc, prob);
-    }
-    if (p.agg_mode == 2 && any_nan) acc = CUDART_NAN_F;
-    if (lane == 0) warp_acc[warp] = acc;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const int len = e - b;
-        float conf = 0.f;
-        if (len > 0) {
-            if (p.agg_mode == 2) {
-                conf = warp_acc[0];
-                bool nan = conf != conf;
-                for (int w = 1; w < kFinalizeWarps; ++w) {
-                    nan |= (warp_acc[w] != warp_acc[w]);
-                    conf = fminf(conf, warp_acc[w]);
-                }
-                if (nan) conf = CUDART_NAN_F;
-            } else {
-                float t = 0.f;
-                for (int w = 0; w < kFinalizeWarps; ++w) t += warp_acc[w];
-                conf = t / static_cast<float>(len);
-                if (p.agg_mode == 1) conf = expf(conf);
-            }
-        }
-        p.out_conf[r] = conf;                  // a3
-        p.out_exit[r] = (conf > tau) ? 1 : 0;  // a5: strict; NaN > tau is false
-        if (p.out_tau) p.out_tau[r] = tau;
-    }
-}
-
-// ---------------------------------------------------------------------------------- vocab-parallel
-// laser_probe_partial: the fused kernel over one vocabulary SHARD, then this kernel: one warp per row
-// merges the row's split records into a single record {m, S, argmax + v_offset, l_tok} and stores it
-//   * to out_stats[n] (local), and
-//   * when peers are given, to slot [rank, n] of every GPU's gathered buffer [G, N] through
-//     peer-mapped pointers (NVLink stores; 16 bytes per row and peer) - the all-gather of the
-//     statistics is done by the producer, no collective call.
-// Rows n >= req_offsets[R] (padding) get the neutral record.
-constexpr int kMaxPeers = 16;
-struct ReduceParams {
-    FinalizeParams f;          // ws, strides, replan fields, req_offsets, R, n_alloc, a_offset
-    float4* out_stats;         // [n_alloc] or nullptr
-    int32_t rank, world;       // world = 0: no peers
-    float4* peer_stats[kMaxPeers];   // peer_stats[g] = base of GPU g's gathered buffer [world, n_alloc]
-};
-
-__global__ void __launch_bounds__(kFinalizeThreads)
-laser_probe_reduce_kernel(const ReduceParams q) {
-    const FinalizeParams& p = q.f;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    ptx::pdl_launch_dependents();
-    const int n = blockIdx.x * kFinalizeWarps + warp;
-    const int n_valid = (p.R > 0) ? min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc) : 0;
-    const int nsplit = records_per_row(p);
-    ptx::pdl_wait();
-    if (n >= p.n_alloc) return;
-    float m = -CUDART_INF_F, s = 0.f, lt = -CUDART_INF_F;
-    int a = 0x7fffffff;
-    if (n < n_valid) {
-        merge_row(p.ws + static_cast<int64_t>(n) * p.row_stride, p.split_stride, nsplit, lane, m, a, s, lt);
-        a += p.a_offset;
-    }
-    const float4 rec = make_float4(m, s, __int_as_float(a), lt);
-    if (lane == 0 && q.out_stats) q.out_stats[n] = rec;
-    if (lane < q.world) q.peer_stats[lane][static_cast<int64_t>(q.rank) * p.n_alloc + n] = rec;
-}
-
-// After the reduce kernel (stream order: its stores, remote ones included, have been performed):
-// publish `epoch` in slot [rank] of every GPU's flag array with a system-scope release store.
-struct SignalParams {
-    int32_t rank, world;
-    uint32_t epoch;
-    uint32_t* peer_flags[kMaxPeers];   // peer_flags[g] = GPU g's flag array [world]
-};
-__global__ void laser_probe_signal_kernel(const SignalParams q) {
-    const int g = threadIdx.x;
-    if (g < q.world) {
-        __threadfence_system();
-        ptx::st_release_sys_u32(q.peer_flags[g] + q.rank, q.epoch);
     }
 }
 

@@ -22,6 +22,11 @@ PMAX_TOL = 2e-4
 TAU_TOL = 2e-6
 
 
+# How run_gpu() calls the library (laser_probe_options fields + which entry point).  Test-side state:
+# the fixtures of the GPU tests switch it to run the same case through every variant.
+CFG = dict(mode=0, tail=0, overlap=False, use_handle=True)
+
+
 @dataclass
 class GpuRun:
     conf: np.ndarray
@@ -47,13 +52,14 @@ def run_gpu(w, dev=None, agg=0, tau_params=None) -> GpuRun:
     import torch
     from paper_2606_31580_b200 import binding as B
     dev = dev or to_device(w)
-    probe = B.Probe(w.N_alloc, w.d, w.V, w.R)
+    probe = B.Probe(w.N_alloc, w.d, w.V, w.R, **CFG)
     # poison outputs so that unwritten entries are caught
     probe.conf.fill_(-7.0); probe.argmax.fill_(-7); probe.exit.fill_(7)
     probe.tau.fill_(-7.0); probe.pmax.fill_(-7.0)
     tp = B.TauParams(**(tau_params or w.tau_params))
     out = probe(dev["hidden"], dev["W"], dev["off"], dev["load"], tp, agg=agg)
     torch.cuda.synchronize()
+    probe.close()
     return GpuRun(out.conf.cpu().numpy(), out.argmax.cpu().numpy(), out.exit.cpu().numpy(),
                   out.tau.cpu().numpy(), out.pmax.cpu().numpy(), probe.plan)
 

@@ -64,9 +64,15 @@ def test_plan_invariants(dims):
     assert p["grid"] == (2 if pair else 1) * min(units, p["work_items"])
     assert 2 <= p["stages"] <= 8
     b_rows = bn // 2 if pair else bn                          # W rows one CTA stages per tile
-    assert p["stages"] * (16384 + b_rows * 128) + 1280 == p["smem_bytes"] <= 227 * 1024
-    assert B.workspace_bytes(*dims) == max(16, 16 * p["ws_splits"] * p["m_tiles"] * tm)
-    assert p["ws_splits"] >= S and (p["ws_splits"] == S or p["m_tiles"] > 1)
+    pipe = p["stages"] * (16384 + b_rows * 128) + 1280        # stages + alignment slack + barrier block
+    assert 0 <= p["tail_cache"] <= 512
+    assert pipe + (8 * (p["tail_cache"] + 1) if p["tail_cache"] else 0) == p["smem_bytes"] <= 227 * 1024
+    # packed records: at least the full batch's, at most 2x it (a re-plan for fewer token items may use
+    # more splits per row, never more than the units allow); one buffer serves both kernel variants
+    full = p["m_tiles"] * tm * S
+    assert full <= p["ws_records"] <= 2 * full and (p["ws_records"] == full or p["m_tiles"] > 1)
+    both = [B.plan_query(*dims, mode=m)["ws_records"] for m in (B.MODE_SINGLE, B.MODE_PAIR)]
+    assert B.workspace_bytes(*dims) == max(16, 16 * max(both)) >= 16 * p["ws_records"]
     # the busiest unit does at most ~8 % more than an even share of W rows (+ one tile of slack)
     busy = min(units, p["work_items"])
     rounds = -(-p["work_items"] // busy)
@@ -74,17 +80,42 @@ def test_plan_invariants(dims):
 
 
 def test_forced_modes_plan():
-    try:
-        B.set_mode(B.MODE_PAIR)
-        p = B.plan_query(32, 64, 1000, 8)
-        assert p["cta_pair"] == 1 and p["tile_m"] == 256 and p["grid"] % 2 == 0 and p["tile_n"] % 32 == 0
-        B.set_mode(B.MODE_SINGLE)
-        p = B.plan_query(4096, 1536, 151936, 512)
-        assert p["cta_pair"] == 0 and p["tile_m"] == 128 and p["m_tiles"] == 32
-        with pytest.raises(B.LaserError):
-            B.set_mode(5)
-    finally:
-        B.set_mode(B.MODE_AUTO)
+    p = B.plan_query(32, 64, 1000, 8, mode=B.MODE_PAIR)
+    assert p["cta_pair"] == 1 and p["tile_m"] == 256 and p["grid"] % 2 == 0 and p["tile_n"] % 32 == 0
+    p = B.plan_query(4096, 1536, 151936, 512, mode=B.MODE_SINGLE)
+    assert p["cta_pair"] == 0 and p["tile_m"] == 128 and p["m_tiles"] == 32
+    with pytest.raises(B.LaserError):
+        B.plan_query(32, 64, 1000, 8, mode=5)
+    # the N = 16384 workspace is tens of MB, not the 77 MB of a max-split stride (round-1 advice)
+    assert B.workspace_bytes(16384, 1536, 151936, 2048) < 40e6
+
+
+def test_options_are_per_call_and_validated():
+    """kernel variant, overlap and tail travel in laser_probe_options (no process-wide setters)."""
+    L = B.lib()
+    o = B.Options(7, 7, None, 7, 1, 7)
+    assert L.laser_probe_options_default(C.byref(o)) == 0
+    assert (o.aggregate_mode, o.prob_mode, o.token_ids, o.kernel_mode, o.overlap, o.tail, o.reserved) == \
+        (0, 0, None, 0, 0, 0, 0)
+    assert not hasattr(L, "laser_probe_set_mode") and not hasattr(L, "laser_probe_set_overlap")
+    buf = (C.c_char * 4096)()
+    a = C.addressof(buf)
+    tp, d = B.TauParams(), B.Dims(32, 64, 1000, 8)
+    call = lambda opt: L.laser_probe_confidence_opt(a, a, a, a, C.byref(tp), a, a, a, C.byref(d), a, 4096, None,
+                                                    None, None, C.byref(opt))
+    for bad in (B.Options(kernel_mode=3), B.Options(tail=3), B.Options(aggregate_mode=3), B.Options(prob_mode=2)):
+        assert call(bad) == -8                                              # LASER_E_MODE
+    o = B.Options(); o.overlap = 2
+    assert call(o) == -8
+    o = B.Options(); o.reserved = 1
+    assert call(o) == -8
+    assert call(B.Options(prob_mode=B.PROB_TOKEN)) == -1                    # token ids missing
+    h = C.c_void_p()
+    assert L.laser_probe_handle_create(C.byref(h), C.byref(B.Dims(32, 60, 1000, 8)), None) == -2
+    assert L.laser_probe_handle_create(C.byref(h), C.byref(d), C.byref(B.Options(tail=9))) == -8
+    assert L.laser_probe_handle_create(None, C.byref(d), None) == -1
+    assert L.laser_probe_handle_run(None, a, a, a, a, C.byref(tp), a, a, a, a, 4096, None, None, None) == -1
+    assert L.laser_probe_handle_destroy(None) == 0 and L.laser_probe_handle_workspace_bytes(None) == 0
 
 
 def test_c2_plan_is_the_documented_one():
@@ -155,13 +186,16 @@ def test_ema_and_budget_match_oracle():
     pt = rng.integers(1, 600, 500)
     Lr = (rng.random(500) * 60).astype(np.float32)
     got = B.allocate_budget(pt, Lr)
-    # same inputs on both sides: the ABI's parameters are floats, so the oracle gets the float32-rounded
-    # defaults (a floor() decides an integer here; both sides then decide it in double)
-    f32 = lambda x: float(np.float32(x))
-    q = oracle.BudgetParams(f_min=f32(0.6), f_max=f32(1.5))
-    want = oracle.budget(pt.astype(np.float64), Lr.astype(np.float64), q)
+    # the ABI's parameters are doubles: the oracle gets the same unrounded defaults
+    want = oracle.budget(pt.astype(np.float64), Lr.astype(np.float64), oracle.BudgetParams())
     assert np.array_equal(got, want)
     assert got.min() >= 2 and got.max() <= 15
+    # the whole integer grid, including the points where the exact product of Eq. 6 is an integer
+    ps, Ls = np.meshgrid(np.arange(1, 600), np.arange(0, 61), indexing="ij")
+    got = B.allocate_budget(ps.ravel(), Ls.ravel().astype(np.float32))
+    want = oracle.budget(ps.ravel().astype(np.float64), Ls.ravel().astype(np.float64), oracle.BudgetParams())
+    assert np.array_equal(got, want)
+    assert list(B.allocate_budget([100, 65], np.asarray([5, 11], np.float32))) == [8, 6]
 
 
 def test_partial_combine_validation_needs_no_gpu():
@@ -170,8 +204,8 @@ def test_partial_combine_validation_needs_no_gpu():
     L = B.lib()
     d = B.Dims(8, 64, 100, 1)
     tp = B.TauParams()
-    assert L.laser_probe_partial(None, None, None, None, C.byref(d), 0, None, None, None, 0, None) == -1
-    assert L.laser_probe_partial(None, None, None, None, C.byref(d), -1, None, None, None, 0, None) == -2
+    assert L.laser_probe_partial(None, None, None, None, C.byref(d), 0, None, None, None, 0, None, None) == -1
+    assert L.laser_probe_partial(None, None, None, None, C.byref(d), -1, None, None, None, 0, None, None) == -2
     assert L.laser_probe_combine(None, 0, None, None, C.byref(tp), None, None, None, C.byref(d), None, None,
                                  None, None, None, 0) == -2
     assert L.laser_probe_combine(None, 17, None, None, C.byref(tp), None, None, None, C.byref(d), None, None,
@@ -215,11 +249,24 @@ def test_headers_are_plain_c_and_link(tmp_path):
 #include "laser_sim.h"
 int main(void) {
     laser_tau_params t; laser_sim_policy sp; laser_probe_dims d = {128, 1536, 151936, 16}; laser_probe_plan pl;
+    laser_probe_options opt; laser_probe_handle* h = 0; laser_budget_params bp; int rc;
+    int32_t prompt[2] = {100, 65}, budget[2]; float L[2] = {5.0f, 11.0f};
     float load[3] = {0.0f, 10.0f, 20.0f}, tau[3];
     if (laser_tau_params_default(&t) != LASER_OK || laser_sim_policy_default(&sp) != LASER_OK) return 1;
     if (laser_tau_from_load(load, 3, &t, tau) != LASER_OK) return 2;
     if (laser_probe_plan_query(&d, &pl) != LASER_OK || laser_probe_workspace_bytes(&d) == 0) return 3;
     if (laser_probe_confidence(0, 0, 0, 0, &t, 0, 0, 0, &d, 0, 0, 0, 0, 0) != LASER_E_NULL) return 4;
+    /* the handle API: per-call options; without a B200 creation must fail loudly, never fall back */
+    if (laser_probe_options_default(&opt) != LASER_OK) return 5;
+    opt.kernel_mode = LASER_MODE_SINGLE; opt.tail = LASER_TAIL_FUSED;
+    rc = laser_probe_handle_create(&h, &d, &opt);
+    if (rc == LASER_OK) {
+        if (laser_probe_handle_plan(h, &pl) != LASER_OK || laser_probe_handle_workspace_bytes(h) == 0) return 6;
+        if (laser_probe_handle_run(h, 0, 0, 0, 0, &t, 0, 0, 0, 0, 0, 0, 0, 0) != LASER_E_NULL) return 7;
+        if (laser_probe_handle_destroy(h) != LASER_OK) return 8;
+    } else if (rc != LASER_E_CUDA && rc != LASER_E_ARCH) return 9;
+    if (laser_budget_params_default(&bp) != LASER_OK) return 10;
+    if (laser_allocate_budget(prompt, L, 2, &bp, budget) != LASER_OK || budget[0] != 8 || budget[1] != 6) return 11;
     printf("%.6f %.6f %.6f %d %s\n", tau[0], tau[1], tau[2], pl.splits, laser_status_string(LASER_E_ARCH));
     return 0;
 }

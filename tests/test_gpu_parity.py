@@ -111,22 +111,33 @@ def test_literal_generator_flat(P):
     (1000, 64, 3, 130, None, None),        # a request longer than one token tile
     (17, 8, 2, 3, None, None),             # V smaller than one tile, d smaller than one k-block
 ])
-def test_scaled_shapes(P, V, d, R, L, n_alloc, var_len):
+def test_scaled_shapes(P, path, V, d, R, L, n_alloc, var_len):
     w = wl.scaled(f"scaled-V{V}-d{d}", V, d, 0.05, R, L, seed=V + d, N_alloc=n_alloc, var_len=var_len)
     st = P.check(w)
-    _log(w.name, st)
+    _log(f"{w.name}/{path}", st)
 
 
 # ------------------------------------------------------------------ both kernel variants on every shape class
 @pytest.fixture
-def force_mode():
-    """Force the single-CTA or the CTA-pair kernel (laser_probe_set_mode); restored afterwards."""
-    from paper_2606_31580_b200 import binding as B
-
+def force_mode(P):
+    """Force the single-CTA or the CTA-pair kernel (laser_probe_options.kernel_mode) for run_gpu()."""
     def _set(mode):
-        B.set_mode(mode)
+        P.CFG["mode"] = mode
     yield _set
-    B.set_mode(B.MODE_AUTO)
+    P.CFG["mode"] = 0
+
+
+PATHS = {"tail-handle": dict(tail=1, use_handle=True),       # a3-a5 in the fused kernel's tail (default)
+         "separate-handle": dict(tail=2, use_handle=True),   # second kernel (LASER_TAIL_SEPARATE)
+         "tail-implicit": dict(tail=0, use_handle=False)}    # handle-less entry point, implicit handle
+
+
+@pytest.fixture(params=list(PATHS))
+def path(P, request):
+    """Run the test once per call path: fused tail / separate finalize kernel / handle-less ABI."""
+    P.CFG.update(PATHS[request.param])
+    yield request.param
+    P.CFG.update(tail=0, use_handle=True)
 
 
 @pytest.mark.parametrize("mode", [1, 2])
@@ -137,7 +148,7 @@ def force_mode():
     (1000, 64, 3, 130, None, None),        # a request that straddles the two CTAs of a pair
     (17, 8, 2, 3, None, None),             # V smaller than half a tile
 ])
-def test_forced_variants(P, force_mode, mode, V, d, R, L, n_alloc, var_len):
+def test_forced_variants(P, force_mode, path, mode, V, d, R, L, n_alloc, var_len):
     force_mode(mode)
     w = wl.scaled(f"mode{mode}-V{V}-d{d}", V, d, 0.05, R, L, seed=V + d + mode, N_alloc=n_alloc, var_len=var_len)
     st = P.check(w)
@@ -165,7 +176,7 @@ def test_forced_variants_c5_512(P, force_mode, c2_W_bits, mode):
     (33, 8, None, 1024),         # 264 valid rows: one row group into the next item
     (5, 0, None, 700),           # every request empty, several token tiles allocated
 ])
-def test_padding_tiles_are_skipped_and_replanned(P, force_mode, mode, R, L, var_len, n_alloc):
+def test_padding_tiles_are_skipped_and_replanned(P, force_mode, path, mode, R, L, var_len, n_alloc):
     """req_offsets[R] < N leaves whole token tiles of padding: the kernels skip them and re-deal the
     vocabulary over the tiles that hold rows (device-side plan_splits); results must not change."""
     force_mode(mode)
@@ -257,12 +268,14 @@ def test_ties_across_tile_and_split_boundaries(P):
         P.compare(w, g, ora, rows, reqs, "ties")
 
 
+@pytest.mark.parametrize("tail", [1, 2])
 @pytest.mark.parametrize("overlap", [True, False])
-def test_back_to_back_calls_share_a_workspace(P, overlap):
+def test_back_to_back_calls_share_a_workspace(P, overlap, tail):
     """Stream order under programmatic dependent launch: calls enqueued back to back on one stream,
     all on ONE workspace, with alternating inputs.  The fused kernel of call k+1 may start while the
-    finalize kernel of call k still reads the workspace (laser_probe_set_overlap); every call must
-    still produce its own batch's result."""
+    tail of call k still reads the workspace (laser_probe_options.overlap), and all calls go through
+    ONE handle, i.e. one control slot whose counters call k resets just before call k+1 counts;
+    every call must still produce its own batch's result."""
     import torch
     from paper_2606_31580_b200 import binding as B
     V, d, R, L = 1000, 64, 48, 8          # short fused kernel, long finalize kernel: the tightest race
@@ -270,19 +283,18 @@ def test_back_to_back_calls_share_a_workspace(P, overlap):
     devs = [P.to_device(w) for w in ws]
     oras = [P.run_oracle(w) for w in ws]
     K = 24
-    probes = [B.Probe(R * L, d, V, R) for _ in range(K)]
+    probes = [B.Probe(R * L, d, V, R, overlap=overlap, tail=tail) for _ in range(K)]
     for p in probes[1:]:
         p.workspace = probes[0].workspace
-    B.set_overlap(overlap)
-    try:
-        tp = B.TauParams(**ws[0].tau_params)
-        torch.cuda.synchronize()
-        for k, p in enumerate(probes):
-            dv = devs[k % 2]
-            p(dv["hidden"], dv["W"], dv["off"], dv["load"], tp)
-        torch.cuda.synchronize()
-    finally:
-        B.set_overlap(False)
+        p._handles = probes[0]._handles          # one handle (one control slot) for all calls
+    tp = B.TauParams(**ws[0].tau_params)
+    torch.cuda.synchronize()
+    n0 = B.kernel_launch_count()
+    for k, p in enumerate(probes):
+        dv = devs[k % 2]
+        p(dv["hidden"], dv["W"], dv["off"], dv["load"], tp)
+    assert B.kernel_launch_count() - n0 == K * (2 if tail == 2 else 1)
+    torch.cuda.synchronize()
     for k, p in enumerate(probes):
         g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),
                      p.tau.cpu().numpy(), p.pmax.cpu().numpy(), p.plan)
@@ -293,9 +305,10 @@ def test_back_to_back_calls_share_a_workspace(P, overlap):
 
 
 def test_c2_in_the_configuration_bench_times(P, c2_W_bits):
-    """The launch configuration of bench.py's timed region at full C2 size: laser_probe_set_overlap(1),
-    calls enqueued back to back on one stream, two resident copies of W alternating between calls,
-    one workspace.  Every call's outputs (kept in separate buffers) are compared with the oracle."""
+    """The launch configuration of bench.py's timed regions at full C2 size: strict (the headline) and
+    overlap, calls enqueued back to back on one stream through one handle, two resident copies of W
+    alternating between calls, one workspace.  Every call's outputs (kept in separate buffers) are
+    compared with the oracle."""
     import torch
     from paper_2606_31580_b200 import binding as B
     w = wl.config_c2(c2_W_bits)
@@ -303,25 +316,26 @@ def test_c2_in_the_configuration_bench_times(P, c2_W_bits):
     Ws = [dev["W"], dev["W"].clone()]
     ora, rows, reqs = P.run_oracle(w)
     K = 6
-    probes = [B.Probe(w.N_alloc, w.d, w.V, w.R) for _ in range(K)]
-    for p in probes[1:]:
-        p.workspace = probes[0].workspace
-    for p in probes:
-        p.conf.fill_(-7.0); p.argmax.fill_(-7); p.exit.fill_(7); p.pmax.fill_(-7.0)
     tp = B.TauParams(**w.tau_params)
-    B.set_overlap(True)
-    try:
+    for overlap in (False, True):
+        probes = [B.Probe(w.N_alloc, w.d, w.V, w.R, overlap=overlap) for _ in range(K)]
+        for p in probes[1:]:
+            p.workspace = probes[0].workspace
+            p._handles = probes[0]._handles
+        for p in probes:
+            p.conf.fill_(-7.0); p.argmax.fill_(-7); p.exit.fill_(7); p.pmax.fill_(-7.0)
         torch.cuda.synchronize()
+        n0 = B.kernel_launch_count()
         for k, p in enumerate(probes):
             p(dev["hidden"], Ws[k % 2], dev["off"], dev["load"], tp)
+        assert B.kernel_launch_count() - n0 == K * probes[0].plan["kernel_launches"]
+        assert probes[0].plan["kernel_launches"] == (2 if overlap else 1)   # strict: one launch per call
         torch.cuda.synchronize()
-    finally:
-        B.set_overlap(False)
-    for k, p in enumerate(probes):
-        g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),
-                     p.tau.cpu().numpy(), p.pmax.cpu().numpy(), p.plan)
-        st = P.compare(w, g, ora, rows, reqs, f"c2 bench configuration, call {k}")
-    _log("c2-bench-config", st)
+        for k, p in enumerate(probes):
+            g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),
+                         p.tau.cpu().numpy(), p.pmax.cpu().numpy(), p.plan)
+            st = P.compare(w, g, ora, rows, reqs, f"c2 bench configuration, overlap={overlap}, call {k}")
+        _log(f"c2-bench-config/overlap={overlap}", st)
 
 
 # ------------------------------------------------------------------ semantics fixed at the boundary
@@ -388,7 +402,7 @@ def test_lower_clamp_and_fixed_threshold(P):
 
 
 @pytest.mark.parametrize("agg", [1, 2])
-def test_aggregate_modes(P, agg):
+def test_aggregate_modes(P, path, agg):
     """NEXT-1: geometric mean / min over the request's tokens in the same fused reduction."""
     w = wl.scaled("agg", 12000, 256, 0.05, 10, None, seed=21, var_len=(1, 9))
     st = P.check(w, agg=agg)
@@ -457,8 +471,8 @@ def test_error_codes_on_device(P):
 
 
 def test_cuda_graph_capture_and_replay(P, c2_W_bits):
-    """A serving engine captures its decode step in a CUDA graph: the probe call (two kernel launches
-    with programmatic-dependent-launch attributes, no synchronisation, no allocation) must be
+    """A serving engine captures its decode step in a CUDA graph: the probe call (one kernel launch
+    with the programmatic-dependent-launch attribute, no synchronisation, no allocation) must be
     capturable, and a replay must read the CURRENT contents of the input buffers."""
     import torch
     from paper_2606_31580_b200 import binding as B
@@ -485,7 +499,7 @@ def test_cuda_graph_capture_and_replay(P, c2_W_bits):
                        probe.tau.cpu().numpy(), probe.pmax.cpu().numpy(), probe.plan)
         ora, rows, reqs = P.run_oracle(w)
         P.compare(w, run, ora, rows, reqs, f"graph replay {w.name}")
-    # replay latency of one captured call (both kernels), for the record
+    # replay latency of one captured call, for the record
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ts = []
     for _ in range(20):

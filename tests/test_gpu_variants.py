@@ -139,7 +139,7 @@ def test_token_mode_needs_token_ids(P):
 
 
 # ------------------------------------------------------------------------------- vocabulary-parallel
-def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False):
+def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False, tail=0):
     """G virtual ranks on one GPU, one after the other on one stream."""
     import torch
     from paper_2606_31580_b200 import binding as B
@@ -152,7 +152,7 @@ def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False):
     shards = []
     for g in range(G):
         v0, v1 = par.shard_vocab(w.V, G, g)
-        sh = B.VocabShardProbe(N, w.d, v1 - v0, w.R, v0, G)
+        sh = B.VocabShardProbe(N, w.d, v1 - v0, w.R, v0, G, tail=tail)
         Wg = dev["W"][v0:v1].contiguous()
         if peer:
             pe = B.Peers()
@@ -164,6 +164,9 @@ def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False):
         else:
             sh.partial(dev["hidden"], Wg, dev["off"], token_ids=tok_d, out=stats_all[g])
         shards.append((sh, Wg))
+    launches = None
+    if tail:    # one kernel per partial with the fused tail; 2 (+1 signal with peers) with a separate reduce
+        launches = B.kernel_launch_count()
     sh = shards[0][0]
     sh.conf.fill_(-7.0); sh.argmax.fill_(-7); sh.exit.fill_(7); sh.pmax.fill_(-7.0)
     out = sh.combine(dev["off"], dev["load"], tp, stats_all=stats_all, agg=agg, token_prob=tok is not None,
@@ -175,15 +178,20 @@ def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False):
                     out.tau.cpu().numpy(), out.pmax.cpu().numpy(), sh.plan), stats_all.cpu().numpy()
 
 
+@pytest.mark.parametrize("tail", [1, 2])       # reduce + push + signal in the fused kernel's tail / as kernels
 @pytest.mark.parametrize("peer", [False, True])
 @pytest.mark.parametrize("G", [1, 2, 3, 8])
 @pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
     (33000, 512, 12, 8, None, None),
     (9001, 256, 40, None, 400, (1, 16)),     # V not divisible by G, several token tiles, padding rows
 ])
-def test_vocab_parallel_matches_oracle(P, G, peer, V, d, R, L, n_alloc, var_len):
+def test_vocab_parallel_matches_oracle(P, G, peer, tail, V, d, R, L, n_alloc, var_len):
+    from paper_2606_31580_b200 import binding as B
     w = wl.scaled(f"vp-V{V}-G{G}", V, d, 0.05, R, L, seed=88, N_alloc=n_alloc, var_len=var_len)
-    g, stats = _run_vocab_parallel(P, w, G, peer=peer)
+    n0 = B.kernel_launch_count()
+    g, stats = _run_vocab_parallel(P, w, G, peer=peer, tail=tail)
+    per_partial = 1 if tail == 1 else (3 if peer else 2)
+    assert B.kernel_launch_count() - n0 == G * per_partial + 1          # + the combine kernel
     ora, rows, reqs = P.run_oracle(w)
     st = P.compare(w, g, ora, rows, reqs, w.name)
     print(w.name, "peer" if peer else "collective", {k: v for k, v in st.items() if k != "plan"})
@@ -291,9 +299,10 @@ def test_fuzz_shapes_modes_aggregates(P, i):
                   N_alloc=w0.N_valid + pad)
     if w.N_alloc == 0:
         pytest.skip("empty batch (covered by test_empty_batches_and_requests)")
-    B.set_mode(mode)
+    tail, use_handle = [(0, True), (2, True), (1, False), (0, False)][i % 4]
+    P.CFG.update(mode=mode, tail=tail, use_handle=use_handle)
     try:
         st = P.check(w, agg=agg)
     finally:
-        B.set_mode(B.MODE_AUTO)
+        P.CFG.update(mode=0, tail=0, use_handle=True)
     print(w.name, {k: v for k, v in st.items() if k != "plan"}, "pair" if st["plan"]["cta_pair"] else "single")
