@@ -2,31 +2,43 @@
 """bench.py — throughput of the LASER confidence probe on B200 (one JSON line on stdout).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--workload C2|C3|C4|C5:<N>|shape:d=<d>,V=<V>,N=<N>] [--no-sweep] [--no-cpu-baseline]
+                    [--workload C2|C3|C4|C5:<N>|shape:d=<d>,V=<V>,N=<N>] [--sharding requests|vocab]
+                    [--exchange peer|collective] [--no-sweep] [--no-cpu-baseline]
 
 A "step" is one pass of the whole hot path (a1-a5 of include/laser_probe.h: projection, online
 softmax, per-request confidence, threshold, exit mask) over one batch of seeded synthetic input —
-one laser_probe_confidence() call, two kernel launches.  Default workload: BASELINE.json configs[1]
-(Qwen-1.5B-shaped, d=1536, V=151936, 16 requests x 8 tokens), the config the metric is quoted on.
+one laser_probe_handle_run() call = ONE kernel launch (merge + a3-a5 run in the fused kernel's tail).
+Default workload: BASELINE.json configs[1] (Qwen-1.5B-shaped, d=1536, V=151936, 16 requests x 8
+tokens), the config the metric is quoted on.
 
-`value`    rows/s with every input already resident in HBM (device-timed, CUDA events on the launch
-           stream, barrier + synchronize either side, max over ranks).
-`e2e`      rows/s through laser_probe_confidence_host_async(): per-step inputs (hidden, req_offsets,
-           load) in pinned HOST memory, H2D + kernels + D2H of conf/argmax/exit inside the timed
-           region, every step's result read on the host; two batches in flight on two streams so the
-           copy of one overlaps the kernels of the other.  e2e.sync_value is the same through the
-           synchronous laser_probe_confidence_host() (one batch at a time).  W, the model's LM-head
-           weight, stays resident (it is not a per-step input).
-`roofline` for the dominant (fused) kernel: algorithmic bytes per launch / its own average duration
-           (events recorded by the library either side of that kernel, second pass of K steps).
+`value`    rows/s with every input already resident in HBM, in the library's DEFAULT (strict) mode:
+           every per-call input is read in stream order behind whatever kernel precedes the call -
+           what a serving loop gets behind the forward pass that writes `hidden` (device-timed, CUDA
+           events on the launch stream, barrier + synchronize either side, max over ranks).
+           `overlap` is the same loop with laser_probe_options.overlap = 1 (secondary figure).
+`e2e`      rows/s through the host-buffer entry point of a handle: per-step inputs (hidden,
+           req_offsets, load) in pinned HOST memory, H2D + kernel + D2H of conf/argmax/exit inside the
+           timed region, every step's result read on the host; two batches in flight on two streams
+           so the copy of one overlaps the kernel of the other.  e2e.sync_value is one batch at a time.
+           W, the model's LM-head weight, stays resident (it is not a per-step input).
+`roofline` for the dominant (fused) kernel: algorithmic bytes (or flops) per launch / that kernel's OWN
+           average duration, bracketed by CUDA events the library records either side of it on the
+           launch stream (second pass of K steps).  frac = achieved / peak reproduces by hand from
+           the line.  frac_strict / frac_isolated / frac_sustained are the same bytes over the strict
+           step, one isolated call and the step after 0.25 s of continuous load (with its SM clock);
+           `sweep` is configs[4].
 `cpu_baseline` the fp64 oracle, as it stands, on this box's host cores (rank 0, N=1 only).
 
 --impl reference times the oracle itself (the reference arm of this tier): each step is the oracle
 on a bounded sample of the same workload.  Under torchrun only rank 0 runs it.
 
-Multi-GPU (--gpus N under torchrun): the probe's batches are independent, so ranks shard requests
-(each rank probes its own batch against its own replica of W) with no data-path collective: weak
-scaling.  torch.distributed is used for the barrier and the max-over-ranks reduction only.
+Multi-GPU (--gpus N under torchrun).  --sharding requests (default): the probe's batches are
+independent, so ranks shard requests (each rank probes its own batch against its own replica of W)
+with no data-path collective: weak scaling.  --sharding vocab: the LM head's tensor-parallel layout
+(parallel.VocabParallelProbe): every rank holds V/N rows of W and the whole batch; the per-row
+statistics meet on every rank through peer stores over NVLink (--exchange peer) or an NCCL
+all-gather (--exchange collective): strong scaling, exchange inside the timed step.
+torch.distributed is otherwise used for the barrier and the max-over-ranks reduction only.
 """
 from __future__ import annotations
 
@@ -154,20 +166,22 @@ def describe(w: wl.Workload) -> str:
             f"polarised synthetic generator (DESIGN.md §4)")
 
 
-def roofline_for(w: wl.Workload, fused_us: float, peaks: dict, sustained: bool):
-    """Slower of (algorithmic bytes / HBM) and (flops / bf16 tensor peak) bounds the path."""
+def roofline_for(w: wl.Workload, us: float, peaks: dict):
+    """Slower of (algorithmic bytes / HBM) and (flops / bf16 tensor peak) bounds the path.  The peak is
+    the burst figure of MEASURED_PEAKS.json (every region timed here is far shorter than a second);
+    for the tensor bound the ratio against cuBLAS's sustained figure is given beside it."""
     by, fl = w.algorithmic_bytes(), w.flops()
-    tc_peak = peaks["bf16_tflops_sustained"] if sustained else peaks["bf16_tflops"]
     t_hbm = by / (peaks["hbm_gbs"] * 1e9)
-    t_tc = fl / (tc_peak * 1e12)
+    t_tc = fl / (peaks["bf16_tflops"] * 1e12)
     if t_hbm >= t_tc:
-        ach = by / (fused_us * 1e-6) / 1e9
+        ach = by / (us * 1e-6) / 1e9
         return dict(bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"],
-                    frac_of_nominal=ach / NOMINAL_HBM_GBS, peak_source=f"of {peaks['source']}")
-    ach = fl / (fused_us * 1e-6) / 1e12
-    return dict(bound="tensor", achieved=ach, peak=tc_peak, unit="TFLOP/s", frac=ach / tc_peak,
-                frac_of_nominal=ach / NOMINAL_BF16_TFLOPS,
-                peak_source=f"of {peaks['source']} ({'sustained' if sustained else 'burst'})")
+                    frac_of_nominal=ach / NOMINAL_HBM_GBS, peak_source=f"{peaks['source']} (copy bandwidth)")
+    ach = fl / (us * 1e-6) / 1e12
+    return dict(bound="tensor", achieved=ach, peak=peaks["bf16_tflops"], unit="TFLOP/s",
+                frac=ach / peaks["bf16_tflops"], frac_of_nominal=ach / NOMINAL_BF16_TFLOPS,
+                frac_vs_sustained_peak=ach / peaks["bf16_tflops_sustained"],
+                peak_source=f"{peaks['source']} (cuBLAS bf16 burst; sustained {peaks['bf16_tflops_sustained']:.0f})")
 
 
 # ----------------------------------------------------------------------------------------- GPU arm
@@ -187,20 +201,24 @@ def settle(case, seconds: float = SETTLE_S):
 
 
 class GpuCase:
-    def __init__(self, w: wl.Workload, device, two_w_copies: bool = False, Ws=None):
+    def __init__(self, w: wl.Workload, device, two_w_copies: bool = False, Ws=None, overlap: bool = False,
+                 share=None):
         import torch
         from paper_2606_31580_b200 import binding as B
         self.torch, self.B, self.w = torch, B, w
-        self.hidden = B.bf16_tensor_from_bits(w.hidden_bits, device)
+        if share is not None:
+            self.hidden, self.off, self.load = share.hidden, share.off, share.load
+        else:
+            self.hidden = B.bf16_tensor_from_bits(w.hidden_bits, device)
+            self.off = torch.from_numpy(w.req_offsets).to(device)
+            self.load = torch.from_numpy(w.load).to(device)
         if Ws is None:
             Ws = [B.bf16_tensor_from_bits(w.W_bits, device)]
             if two_w_copies:
                 Ws.append(Ws[0].clone())
         self.Ws = Ws
-        self.off = torch.from_numpy(w.req_offsets).to(device)
-        self.load = torch.from_numpy(w.load).to(device)
         self.tp = B.TauParams(**w.tau_params)
-        self.probe = B.Probe(w.N_alloc, w.d, w.V, w.R, device=device, debug_outputs=False)
+        self.probe = B.Probe(w.N_alloc, w.d, w.V, w.R, device=device, debug_outputs=False, overlap=overlap)
         self.i = 0
 
     def step(self):
@@ -242,7 +260,7 @@ class GpuCase:
 
     def graph_replay_us(self, calls: int, reps: int = 20):
         """Median duration (us) of replaying a CUDA graph that holds `calls` back-to-back probe calls,
-        captured under the current overlap setting - how a serving engine that captures its step
+        captured with this case's options - how a serving engine that captures its step
         would run the probe (no per-launch host work)."""
         torch = self.torch
         side = torch.cuda.Stream(device=self.hidden.device)
@@ -376,6 +394,102 @@ def serving_sim_bench(device, seeds: int = 128, n_req: int = 1000, with_cpu: boo
     return res
 
 
+def run_vocab_sharded(args, dist, rank, local_rank, world, device):
+    """--sharding vocab: parallel.VocabParallelProbe under torchrun (or alone: a world of one).  Strong
+    scaling: the batch is fixed, W is cut into `world` row ranges, the per-row statistics of all shards
+    meet on every rank inside the timed step (peer stores over NVLink, or an NCCL all-gather)."""
+    import socket
+    import torch
+    from paper_2606_31580_b200 import binding as B, parallel as par
+    os.environ.setdefault("NCCL_DEBUG", "INFO")          # keep the communicator lines (NVLS / P2P) on stderr
+    os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    own_group = False
+    if dist is None:
+        import torch.distributed as dist
+        s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", str(port))
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=device)
+        own_group = True
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    sampler.start()
+    w = wl.by_name(args.workload, {})                    # every rank: the same batch, the same W
+    vp = par.VocabParallelProbe(dist, w.N_alloc, w.d, w.V, w.R, device, exchange=args.exchange)
+    hidden = B.bf16_tensor_from_bits(w.hidden_bits, device)
+    Wg = B.bf16_tensor_from_bits(w.W_bits[vp.v0:vp.v1], device)
+    off = torch.from_numpy(w.req_offsets).to(device)
+    load = torch.from_numpy(w.load).to(device)
+    tp = B.TauParams(**w.tau_params)
+
+    def step():
+        return vp(hidden, Wg, off, load, tp)
+
+    def timed(fn, n):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        dist.barrier(); torch.cuda.synchronize()
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize(); dist.barrier()
+        t = torch.tensor([e0.elapsed_time(e1)], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t[0])
+
+    for _ in range(args.warmup):
+        step()
+    launches0 = B.kernel_launch_count()
+    t0 = time.perf_counter()
+    ms = timed(step, args.steps)
+    clocks = sampler.summary(t0, time.perf_counter())
+    launches = B.kernel_launch_count() - launches0
+
+    # end to end: the step's inputs start in pinned host memory, its results are read on the host
+    hh = B.bf16_tensor_from_bits(w.hidden_bits, pin=True)
+    hoff, hload = torch.from_numpy(w.req_offsets).pin_memory(), torch.from_numpy(w.load).pin_memory()
+    o_conf = torch.empty(w.R, dtype=torch.float32).pin_memory()
+    o_arg = torch.empty(w.N_alloc, dtype=torch.int32).pin_memory()
+    o_exit = torch.empty(w.R, dtype=torch.uint8).pin_memory()
+
+    def e2e_step():
+        hidden.copy_(hh, non_blocking=True); off.copy_(hoff, non_blocking=True); load.copy_(hload, non_blocking=True)
+        out = step()
+        o_conf.copy_(out.conf, non_blocking=True); o_arg.copy_(out.argmax, non_blocking=True)
+        o_exit.copy_(out.exit, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        return int(o_exit.sum())
+
+    for _ in range(args.warmup):
+        e2e_step()
+    e2e_ms = timed(e2e_step, args.steps)
+    sampler.stop()
+    if rank == 0:
+        ms_per_step = ms / args.steps
+        shard_bytes = (vp.v1 - vp.v0) * w.d * 2
+        print(json.dumps(dict(
+            metric=METRIC, value=w.N_valid / (ms_per_step * 1e-3), unit=UNIT, n_gpus=world, steps=args.steps,
+            warmup=args.warmup, ms_per_step=ms_per_step, higher_is_better=True, scaling="strong", vs_baseline=None,
+            dtype="bf16", data="synthetic",
+            config=dict(workload=describe(w), sharding=f"vocabulary: {world} row ranges of W, whole batch on every rank",
+                        exchange=args.exchange, shard_rows=vp.v1 - vp.v0, plan=vp.shard.plan,
+                        l2="each rank's W shard (%.0f MB)%s" % (shard_bytes / 1e6,
+                                                                " exceeds the 126 MB L2" if shard_bytes > 126e6 else
+                                                                " FITS the 126 MB L2: per-rank figure is L2-assisted")),
+            requests_per_sec=w.R / (ms_per_step * 1e-3), clocks=clocks,
+            e2e=dict(value=w.N_valid / (e2e_ms / args.steps * 1e-3), unit=UNIT,
+                     h2d_bytes_per_step=w.N_alloc * w.d * 2 + (w.R + 1) * 4 + w.R * 4,
+                     d2h_bytes_per_step=w.R * 4 + w.N_alloc * 4 + w.R, ms_per_step=e2e_ms / args.steps,
+                     api="torch copies (plumbing) around parallel.VocabParallelProbe, synchronous"),
+            gpu_launches=int(launches) * world,
+            roofline=dict(bound="hbm", achieved=shard_bytes / (ms_per_step * 1e-3) / 1e9, unit="GB/s",
+                          peak=measured_peaks()["hbm_gbs"],
+                          frac=shard_bytes / (ms_per_step * 1e-3) / 1e9 / measured_peaks()["hbm_gbs"],
+                          traffic=None, note="per rank: its W shard over the whole step, exchange included"))), flush=True)
+    dist.barrier()
+    if own_group or world > 1:
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import torch
     from paper_2606_31580_b200 import binding as B
@@ -392,6 +506,8 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=device)
+    if args.sharding == "vocab":
+        return run_vocab_sharded(args, dist, rank, local_rank, world, device)
 
     def barrier():
         if dist is not None:
@@ -402,12 +518,12 @@ def run_ours(args):
     sampler.start()                      # NVML initialises while the workload is generated
     W_cache: dict = {}
     w = make_workload(args.workload, rank, W_cache)
+    # the library default: strict stream order for every per-call input (what a serving loop needs
+    # behind the forward pass that writes `hidden`).  This is the headline configuration.
     case = GpuCase(w, device, two_w_copies=(w.V * w.d * 2 < 2_000_000_000))
+    # laser_probe_options.overlap = 1: consecutive calls of a loop over resident inputs overlap
+    over = GpuCase(w, device, Ws=case.Ws, overlap=True, share=case)
 
-    # The library's default is strict stream order for every input.  The timed region is a loop of
-    # probe calls whose inputs are complete before the loop starts, which is the case
-    # laser_probe_set_overlap(1) exists for; the strict figure is measured too (`strict`).
-    B.set_overlap(True)
     for _ in range(args.warmup):
         case.step()
     torch.cuda.synchronize()
@@ -419,33 +535,30 @@ def run_ours(args):
     launches = B.kernel_launch_count() - launches0
     clocks = sampler.summary(t0, t1)
 
-    # the same K steps under the default strict stream order (griddepcontrol.wait before the first read)
-    B.set_overlap(False)
+    # the same K steps with overlap = 1 (secondary figure)
     for _ in range(3):
-        case.step()
-    strict_ms = case.time_steps(args.steps, barrier)
+        over.step()
+    overlap_ms = over.time_steps(args.steps, barrier)
 
     # CUDA-graph replay under the strict default: one call, and ten calls in one graph
     graph_one_us = case.graph_replay_us(1)
     graph_ten_us = case.graph_replay_us(10) / 10.0
-    B.set_overlap(True)
-    graph_ten_overlap_us = case.graph_replay_us(10) / 10.0
+    graph_ten_overlap_us = over.graph_replay_us(10) / 10.0
 
-    # dominant kernel on its own (second pass, same stream, library-recorded events)
+    # dominant kernel on its own (second pass, same stream, library-recorded events either side of it)
     fused_us, fin_us = case.kernel_times(args.steps)
     isolated_us = case.isolated_call_us()
 
-    # the same K steps once more after SETTLE_S seconds of continuous load: the power-capped steady state
+    # the same K strict steps once more after SETTLE_S seconds of continuous load: the power-capped steady state
     settle(case)
     t2 = time.perf_counter()
     sustained_ms = case.time_steps(args.steps, barrier)
     sustained_clocks = sampler.summary(t2, time.perf_counter())
 
-    # end to end through the host-buffer entry points: per-step inputs in pinned host memory, results
-    # read on the host every step.  Two batches in flight (laser_probe_confidence_host_async on two
-    # streams, one staging/workspace/output set each) so that the H2D copy of batch i+1 overlaps the
-    # kernels of batch i, as a serving loop would run it; the one-batch-at-a-time synchronous call
-    # (laser_probe_confidence_host) is timed as well and reported as e2e.sync_*.
+    # end to end through the host-buffer entry point of a handle: per-step inputs in pinned host memory,
+    # results read on the host every step.  Two batches in flight (two handles, two streams, one
+    # staging/workspace/output set each) so that the H2D copy of batch i+1 overlaps the kernel of batch
+    # i, as a serving loop would run it; one batch at a time (synchronous) is timed as well.
     depth = 2
     slots = [B.HostProbe(w.N_alloc, w.d, w.V, w.R, device=device) for _ in range(depth)]
     streams = [torch.cuda.Stream(device=device) for _ in range(depth)]
@@ -499,9 +612,9 @@ def run_ours(args):
     e2e_sync_ms = e2e_sync(args.steps)
 
     if dist is not None:
-        t = torch.tensor([ms, e2e_ms, sustained_ms, strict_ms], device=device, dtype=torch.float64)
+        t = torch.tensor([ms, e2e_ms, sustained_ms, overlap_ms], device=device, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_ms, sustained_ms, strict_ms = float(t[0]), float(t[1]), float(t[2]), float(t[3])
+        ms, e2e_ms, sustained_ms, overlap_ms = float(t[0]), float(t[1]), float(t[2]), float(t[3])
         rows_t = torch.tensor([w.N_valid, w.R], device=device, dtype=torch.float64)
         dist.all_reduce(rows_t, op=dist.ReduceOp.SUM)
         rows_all, reqs_all = float(rows_t[0]), float(rows_t[1])
@@ -512,29 +625,37 @@ def run_ours(args):
     if rank == 0:
         ms_per_step = ms / args.steps
         value = rows_all / (ms_per_step * 1e-3)
-        # The event-bracketed pass breaks the programmatic-dependent-launch chain and adds the launch
-        # latency after each event to the kernel's interval (ncu: 75 us where events say 85-90); the
-        # fused kernel runs once per step, so the time it costs per launch in the timed region cannot
-        # exceed the step's (consecutive calls overlap: a launch's own span is longer than the step).
-        kernel_us = min(fused_us, ms_per_step * 1e3)
-        roof = roofline_for(w, kernel_us, peaks, sustained=False)
-        roof["traffic"] = ncu_traffic_bytes(args.workload)
+        # roofline of the dominant kernel from ITS OWN duration: events recorded by the library
+        # immediately before and after the fused kernel on the launch stream (no programmatic
+        # dependent launch for those calls, so nothing overlaps the bracket).
+        roof = roofline_for(w, fused_us, peaks)
         roof["kernel"] = "laser_probe_fused_kernel<%d>" % case.probe.plan["cta_pair"]
-        roof["kernel_us"] = kernel_us
-        roof["kernel_us_event_bracketed"] = fused_us
-        # the most conservative reading: the kernel alone between two events (launch latency included)
-        roof["frac_event_bracketed"] = roofline_for(w, fused_us, peaks, sustained=False)["frac"]
-        roof["kernel_us_note"] = ("min(average over K launches bracketed by CUDA events on the launch stream, without "
-                                  "programmatic dependent launch; average step duration of the timed region)")
-        roof["finalize_kernel_us"] = fin_us
-        roof["isolated_call_us"] = isolated_us
-        roof["isolated_call_note"] = ("median of 30 single calls on an idle GPU (both kernels, events either side); "
-                                      "in the timed region consecutive calls overlap (laser_probe_set_overlap), "
-                                      "so a step is shorter than an isolated call")
+        roof["kernel_us"] = fused_us
+        roof["kernel_us_source"] = ("average over K launches, each bracketed on its own by CUDA events on the launch "
+                                    "stream (laser_profile_enable; no programmatic dependent launch for those calls, "
+                                    "so prologue and W pre-issue are inside the bracket); the kernel is the whole hot "
+                                    "path: merge + a3-a5 run in its tail")
+        # the interval between the event after the kernel and the next event, with nothing in between:
+        # what one event pair costs on this stream (it is inside kernel_us as well; not subtracted)
+        roof["event_pair_overhead_us"] = fin_us
         roof["algorithmic_bytes"] = w.algorithmic_bytes()
-        roof["step_frac"] = (w.algorithmic_bytes() / (ms_per_step * 1e-3) / 1e9 / peaks["hbm_gbs"]
-                             if roof["bound"] == "hbm" else
-                             w.flops() / (ms_per_step * 1e-3) / 1e12 / peaks["bf16_tflops"])
+        roof["algorithmic_flops"] = w.flops()
+        roof["traffic"] = ncu_traffic_bytes(args.workload)
+        roof["traffic_source"] = ("profiles/fused_kernel_dram_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum "
+                                  "per launch from a committed ncu --set full capture of this kernel; not measured in this run")
+        roof["step_us_strict"] = ms_per_step * 1e3
+        roof["frac_strict"] = roofline_for(w, ms_per_step * 1e3, peaks)["frac"]
+        roof["isolated_call_us"] = graph_one_us
+        roof["frac_isolated"] = roofline_for(w, graph_one_us, peaks)["frac"]
+        roof["isolated_call_note"] = ("median replay of a CUDA graph holding ONE call on an idle GPU, events either side: "
+                                      "the device-side latency of a single probe; isolated_call_us_python_launch is the "
+                                      "same call launched from Python (ctypes + launch latency inside the bracket)")
+        roof["isolated_call_us_python_launch"] = isolated_us
+        roof["step_us_sustained"] = sustained_ms / args.steps * 1e3
+        roof["frac_sustained"] = roofline_for(w, sustained_ms / args.steps * 1e3, peaks)["frac"]
+        roof["sustained_sm_mhz"] = sustained_clocks.get("sm_mhz")
+        roof["step_us_overlap"] = overlap_ms / args.steps * 1e3
+        roof["step_frac_overlap"] = roofline_for(w, overlap_ms / args.steps * 1e3, peaks)["frac"]
         out = dict(
             metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
             ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None,
@@ -545,20 +666,19 @@ def run_ours(args):
                            "W (%.0f MB) exceeds the 126 MB L2" % (w.V * w.d * 2 / 1e6),
                         sharding="requests sharded across ranks, W replicated, no collective" if world > 1 else "single GPU",
                         e2e_w_resident=True,
-                        overlap="laser_probe_set_overlap(1): consecutive calls of the timed loop overlap "
-                                "(inputs complete before the loop); `strict` is the library default",
-                        ),
-            strict=dict(value=rows_all / (strict_ms / args.steps * 1e-3), unit=UNIT,
-                        ms_per_step=strict_ms / args.steps,
-                        note="the same K steps with laser_probe_set_overlap(0), the library default: every "
-                             "input read waits for the preceding kernel (griddepcontrol.wait first)"),
+                        mode="library default: strict stream order (laser_probe_options.overlap = 0), "
+                             "merge + a3-a5 in the fused kernel's tail (one launch per call)"),
+            overlap=dict(value=rows_all / (overlap_ms / args.steps * 1e-3), unit=UNIT,
+                         ms_per_step=overlap_ms / args.steps,
+                         note="the same K steps with laser_probe_options.overlap = 1: consecutive calls of a loop "
+                              "over resident inputs overlap; not what a loop behind a producer of `hidden` may use"),
             cuda_graph=dict(one_call_us=graph_one_us, per_call_us_ten_calls_strict=graph_ten_us,
                             per_call_us_ten_calls_overlap=graph_ten_overlap_us,
                             note="median replay time of a captured CUDA graph holding 1 / 10 probe calls "
                                  "(rank 0); a call is capturable: no sync, no allocation, no host read"),
             sustained=dict(value=rows_all / (sustained_ms / args.steps * 1e-3), unit=UNIT,
                            ms_per_step=sustained_ms / args.steps, clocks=sustained_clocks,
-                           note=f"the same K steps timed again after {SETTLE_S} s of continuous probing "
+                           note=f"the same K strict steps timed again after {SETTLE_S} s of continuous probing "
                                 "(power-capped steady state)"),
             requests_per_sec=reqs_all / (ms_per_step * 1e-3),
             clocks=clocks,
@@ -566,10 +686,10 @@ def run_ours(args):
                      h2d_bytes_per_step=w.N_valid * w.d * 2 + (w.R + 1) * 4 + w.R * 4,
                      d2h_bytes_per_step=hp.d2h_bytes,
                      ms_per_step=e2e_ms / args.steps, batches_in_flight=depth,
-                     api="laser_probe_confidence_host_async, 2 streams; results read on the host every step",
+                     api="laser_probe_handle_run_host (asynchronous), 2 handles on 2 streams; results read on the host every step",
                      sync_value=float(w.N_valid) * world / (e2e_sync_ms / args.steps * 1e-3),
                      sync_ms_per_step=e2e_sync_ms / args.steps,
-                     sync_api="laser_probe_confidence_host (one batch at a time, rank 0's figure x ranks)"),
+                     sync_api="laser_probe_handle_run_host (synchronous, one batch at a time; rank 0's figure x ranks)"),
             gpu_launches=int(launches) * world,      # every rank enqueues the same calls
             roofline=roof,
             realised=realised_distribution(w, case),
@@ -585,18 +705,20 @@ def run_ours(args):
             for _ in range(3):
                 c.step()
             t_ms = c.time_steps(k) / k
-            f_us, z_us = c.kernel_times(min(k, 64))
-            f_us = min(f_us, t_ms * 1e3)           # see kernel_us_note
-            r = roofline_for(ws, f_us, peaks, sustained=(N >= 4096))
-            sweep.append(dict(N=N, us_per_step=t_ms * 1e3, rows_per_sec=N / (t_ms * 1e-3), fused_us=f_us,
-                              finalize_us=z_us, bound=r["bound"], achieved=r["achieved"], unit=r["unit"],
-                              frac=r["frac"], frac_of_nominal=r["frac_of_nominal"], plan=c.probe.plan))
+            f_us, _z = c.kernel_times(min(k, 64))
+            r = roofline_for(ws, f_us, peaks)
+            sweep.append(dict(N=N, step_us=round(t_ms * 1e3, 2), rows_per_sec=N / (t_ms * 1e-3),
+                              kernel_us=round(f_us, 2), bound=r["bound"], achieved=r["achieved"], unit=r["unit"],
+                              frac=r["frac"], frac_of_nominal=r["frac_of_nominal"],
+                              frac_vs_sustained_peak=r.get("frac_vs_sustained_peak"),
+                              frac_step=roofline_for(ws, t_ms * 1e3, peaks)["frac"],
+                              pair=c.probe.plan["cta_pair"], tile_n=c.probe.plan["tile_n"]))
             del c
-        out["sweep"] = sweep
+        out["roofline"]["sweep"] = sweep
 
     # vocabulary-parallel layout (laser_probe_partial + laser_probe_combine): what ONE rank of G would
-    # execute per step - its 1/G slice of W, then the merge of G records per row.  The exchange itself
-    # needs G GPUs and is not part of this figure.
+    # execute per step - its 1/G slice of W (ONE kernel: reduce and record stores in the fused kernel's
+    # tail), then the merge of G records per row.  The exchange itself needs G GPUs (--sharding vocab).
     if rank == 0 and world == 1 and not args.no_sweep and args.workload == "C2":
         from paper_2606_31580_b200 import parallel as par
         vp = []
@@ -619,7 +741,7 @@ def run_ours(args):
             e1.record()
             torch.cuda.synchronize()
             us = e0.elapsed_time(e1) / k * 1e3
-            vp.append(dict(G=G, shard_rows=v1 - v0, us_per_step_per_rank=us, kernels_per_step=3,
+            vp.append(dict(G=G, shard_rows=v1 - v0, us_per_step_per_rank=us, kernels_per_step=2,
                            shard_gb_per_s=(v1 - v0) * w.d * 2 / (us * 1e-6) / 1e9, plan=sh.plan))
         out["vocab_parallel_per_rank"] = dict(
             note="one rank's work at G-way vocabulary sharding, measured on one GPU: partial over the "
@@ -639,19 +761,28 @@ def run_ours(args):
 
 
 # ----------------------------------------------------------------------------------------- CPU arm
+def oracle_sample(w: wl.Workload, gflop_budget: float):
+    """Whole requests from the front of the batch worth about `gflop_budget` GFLOP of fp64 work (the
+    whole batch if it is smaller): (rows, requests, hidden, offsets, load)."""
+    budget_rows = max(4, int(gflop_budget * 1e9 / (2.0 * w.V * w.d)))
+    reqs = 0
+    while reqs < w.R and int(w.req_offsets[reqs + 1]) <= budget_rows:
+        reqs += 1
+    reqs = max(reqs, 1)
+    rows = int(w.req_offsets[reqs])
+    return rows, reqs, w.hidden_f32()[:rows], w.req_offsets[:reqs + 1], w.load[:reqs]
+
+
+CPU_SAMPLE_GFLOP = 120.0      # C2: the whole 128-row batch (59.7 GFLOP)
+
+
 def cpu_baseline(w: wl.Workload, target_s: float):
     """The fp64 oracle, as it stands, on this box's host cores, on the same workload (a bounded sample
     for the large configs).  bench.py's cpu_baseline / --impl reference legs are, with tests/ and
     smoke(), the only callers of oracle/ in the repo."""
     import oracle
     tp = oracle.TauParams(**w.tau_params)
-    budget_rows = max(8, int(120e9 / (2.0 * w.V * w.d)))   # ~120 GFLOP per repetition
-    reqs = 0
-    while reqs < w.R and int(w.req_offsets[reqs + 1]) <= budget_rows:
-        reqs += 1
-    reqs = max(reqs, 1)
-    rows = int(w.req_offsets[reqs])
-    hid, off, load = w.hidden_f32()[:rows], w.req_offsets[:reqs + 1], w.load[:reqs]
+    rows, reqs, hid, off, load = oracle_sample(w, CPU_SAMPLE_GFLOP)
     Wf = w.W_f32()
     best, spent, reps = None, 0.0, 0
     while spent < target_s and reps < 20:        # about target_s (10 s) of CPU work
@@ -673,17 +804,18 @@ def run_reference(args):
     import oracle
     w = wl.by_name(args.workload, {})
     tp = oracle.TauParams(**w.tau_params)
-    # bounded sample per step: whole requests, about 4 GFLOP of fp64 (a fraction of a second of CPU
-    # time), so that --steps 200 still ends within a minute or two
-    budget_rows = max(4, int(4e9 / (2.0 * w.V * w.d)))
-    reqs = 0
-    while reqs < w.R and int(w.req_offsets[reqs + 1]) <= budget_rows:
-        reqs += 1
-    reqs = max(reqs, 1)
-    rows = int(w.req_offsets[reqs])
-    hid, off, load = w.hidden_f32()[:rows], w.req_offsets[:reqs + 1], w.load[:reqs]
     Wf = w.W_f32()
     steps, warm = args.steps, args.warmup
+    # Each step = the oracle on the sample cpu_baseline times (C2: the whole batch), as long as the
+    # whole --steps/--warmup run then ends within a few minutes; otherwise a smaller sample of whole
+    # requests (stated in `sample`).
+    rows, reqs, hid, off, load = oracle_sample(w, CPU_SAMPLE_GFLOP)
+    t_one = oracle.probe(hid, Wf, off, load, tp).seconds
+    same_sample = True
+    if t_one * (steps + warm) > 150.0:
+        same_sample = False
+        shrink = 150.0 / (t_one * (steps + warm))
+        rows, reqs, hid, off, load = oracle_sample(w, CPU_SAMPLE_GFLOP * shrink * rows / max(rows, 1))
     for _ in range(warm):
         oracle.probe(hid, Wf, off, load, tp)
     t0 = time.perf_counter()
@@ -691,7 +823,8 @@ def run_reference(args):
         oracle.probe(hid, Wf, off, load, tp)
     dt = time.perf_counter() - t0
     value = rows * steps / dt
-    sample = (f"each step = fp64 oracle on the first {reqs} requests ({rows} rows) of {w.name}, full V and d")
+    sample = (f"each step = fp64 oracle on the first {reqs} requests ({rows} rows) of {w.name}, full V and d"
+              + (" (the cpu_baseline sample)" if same_sample else " (smaller than the cpu_baseline sample: time cap)"))
     print(json.dumps(dict(
         impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=steps, warmup=warm,
         ms_per_step=dt / steps * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
@@ -708,6 +841,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2")
+    ap.add_argument("--sharding", default="requests", choices=["requests", "vocab"])
+    ap.add_argument("--exchange", default="peer", choices=["peer", "collective"])
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
