@@ -186,6 +186,16 @@ def roofline_for(w: wl.Workload, us: float, peaks: dict):
 
 # ----------------------------------------------------------------------------------------- GPU arm
 SETTLE_S = 0.25
+COOL_S = 1.0
+
+
+def cool():
+    """Between measurement phases: let the board leave the power-capped state the previous phase drove
+    it into, so that every phase (except `sustained`, which wants that state) starts like the headline."""
+    import torch
+    torch.cuda.synchronize()
+    time.sleep(COOL_S)
+
 
 
 def settle(case, seconds: float = SETTLE_S):
@@ -536,17 +546,21 @@ def run_ours(args):
     clocks = sampler.summary(t0, t1)
 
     # the same K steps with overlap = 1 (secondary figure)
+    cool()
     for _ in range(3):
         over.step()
     overlap_ms = over.time_steps(args.steps, barrier)
 
     # CUDA-graph replay under the strict default: one call, and ten calls in one graph
+    cool()
     graph_one_us = case.graph_replay_us(1)
     graph_ten_us = case.graph_replay_us(10) / 10.0
     graph_ten_overlap_us = over.graph_replay_us(10) / 10.0
 
     # dominant kernel on its own (second pass, same stream, library-recorded events either side of it)
+    cool()
     fused_us, fin_us = case.kernel_times(args.steps)
+    cool()
     isolated_us = case.isolated_call_us()
 
     # the same K strict steps once more after SETTLE_S seconds of continuous load: the power-capped steady state
@@ -604,6 +618,7 @@ def run_ours(args):
         return (time.perf_counter() - tw0) * 1e3
 
     sampler.stop()
+    cool()
     e2e_pipelined(args.warmup)
     e2e_sync(args.warmup)
     barrier()
@@ -629,7 +644,8 @@ def run_ours(args):
         # immediately before and after the fused kernel on the launch stream (no programmatic
         # dependent launch for those calls, so nothing overlaps the bracket).
         roof = roofline_for(w, fused_us, peaks)
-        roof["kernel"] = "laser_probe_fused_kernel<%d>" % case.probe.plan["cta_pair"]
+        roof["kernel"] = ("laser_probe_fused_kernel<1> (CTA pairs) beside laser_probe_fused_kernel<0> (single CTAs): mixed schedule"
+                          if case.probe.plan["mixed"] else "laser_probe_fused_kernel<%d>" % case.probe.plan["cta_pair"])
         roof["kernel_us"] = fused_us
         roof["kernel_us_source"] = ("average over K launches, each bracketed on its own by CUDA events on the launch "
                                     "stream (laser_profile_enable; no programmatic dependent launch for those calls, "
@@ -702,9 +718,11 @@ def run_ours(args):
             ws = wl.config_c5(N, W_cache["C2"])
             c = GpuCase(ws, device, Ws=case.Ws)
             k = max(5, min(args.steps, int(2e5 / max(N, 128))))
+            cool()
             for _ in range(3):
                 c.step()
             t_ms = c.time_steps(k) / k
+            cool()
             f_us, _z = c.kernel_times(min(k, 64))
             r = roofline_for(ws, f_us, peaks)
             sweep.append(dict(N=N, step_us=round(t_ms * 1e3, 2), rows_per_sec=N / (t_ms * 1e-3),

@@ -86,11 +86,21 @@ typedef struct {
     int32_t ws_records;      /* 16-byte workspace records (the most any re-plan of the batch writes)  */
     int32_t tail_cache;      /* requests whose {offset, threshold} the fused kernel's tail keeps in the
                                 shared memory the pipeline leaves over (0: read from global memory)    */
+    /* Mixed schedule (AUTO, N > 128 rows): the fields above describe the CTA-pair kernel (256-row
+     * items); when the number of 128-row tiles that hold rows is odd, the last tile runs on single CTAs
+     * in a second kernel beside it.  The split of the SMs is decided on the device from
+     * req_offsets[R].  kernel_launches = 3: tail-tile kernel, pair kernel, finalize kernel. */
+    int32_t mixed;           /* 1: mixed schedule                                                     */
+    int32_t tail_tile_n;     /* vocab rows per tile of the single-CTA tail-tile kernel                */
+    int32_t tail_stages;     /* its pipeline depth                                                    */
+    int32_t tail_smem_bytes; /* its dynamic shared memory per CTA                                     */
+    int32_t tail_grid;       /* its CTAs (those it does not need exit at once)                        */
 } laser_probe_plan;
 
-/* Kernel variant (laser_probe_options.kernel_mode).  AUTO (default): one CTA per work item for
- * N <= 128 rows and for small odd counts of 128-row tiles (< 10), CTA pairs otherwise.  SINGLE / PAIR
- * force one variant for every shape (tuning and tests; both are exact). */
+/* Kernel variant (laser_probe_options.kernel_mode).  AUTO (default): one single-CTA kernel for
+ * N <= 128 rows; above that the mixed schedule (CTA pairs for the even part of the 128-row tiles that
+ * hold rows, single CTAs for an odd last tile, decided on the device).  SINGLE / PAIR force one
+ * variant for every shape (tuning and tests; both are exact; PAIR pads an odd tile count). */
 enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2 };
 
 /* Where merge + a3-a5 run (laser_probe_options.tail).
@@ -134,6 +144,22 @@ size_t laser_probe_workspace_bytes(const laser_probe_dims* dims);
  * SMs when no device is present). */
 int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan);
 int laser_probe_plan_query_mode(const laser_probe_dims* dims, int kernel_mode, laser_probe_plan* plan);
+
+/* What the mixed schedule does for a batch of dims->N allocated rows of which n_valid (= what
+ * req_offsets[R] will say) hold requests: the entry of the table the kernels look up on the device.
+ * Informational (tests, tuning); host; needs no GPU.  mixed = 0: dims take a single kernel. */
+typedef struct {
+    int32_t mixed;          /* 1: the fields below apply                                              */
+    int32_t schedule;       /* 0 pair items only, 1 pair items + one single-CTA tile, 2 single-CTA tiles only */
+    int32_t k_pair;         /* 256-row items on CTA pairs                                             */
+    int32_t j_single;       /* 128-row tiles on single CTAs (behind the pair items)                   */
+    int32_t u_pair;         /* CTA pairs that take part                                               */
+    int32_t u_single;       /* single CTAs that take part                                             */
+    int32_t splits_pair;    /* vocabulary splits per pair item                                        */
+    int32_t splits_single;  /* vocabulary splits per single-CTA tile                                  */
+    float model_us;         /* the planner's cost-model estimate of the fused kernels, microseconds   */
+} laser_probe_mixed;
+int laser_probe_mixed_query(const laser_probe_dims* dims, int32_t n_valid, laser_probe_mixed* out);
 
 /*
  * The hot path a1-a5.  Asynchronous on `stream`; returns after enqueueing.

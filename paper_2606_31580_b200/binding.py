@@ -27,7 +27,7 @@ EXPORTS = [
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
     "laser_profile_read", "laser_probe_options_default", "laser_probe_plan_query_mode",
     "laser_probe_confidence_opt", "laser_probe_partial", "laser_probe_combine",
-    "laser_probe_handle_create", "laser_probe_handle_destroy", "laser_probe_handle_plan",
+    "laser_probe_mixed_query", "laser_probe_handle_create", "laser_probe_handle_destroy", "laser_probe_handle_plan",
     "laser_probe_handle_workspace_bytes", "laser_probe_handle_run", "laser_probe_handle_run_host",
     "laser_sim_policy_default", "laser_sim_run",
 ]
@@ -60,10 +60,17 @@ class Dims(C.Structure):
 class Plan(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("num_sms", "m_tiles", "splits", "tiles_per_split", "tile_n", "k_blocks", "stages",
-                 "grid", "work_items", "smem_bytes", "kernel_launches", "tile_m", "cta_pair", "ws_records", "tail_cache")]
+                 "grid", "work_items", "smem_bytes", "kernel_launches", "tile_m", "cta_pair", "ws_records", "tail_cache",
+                 "mixed", "tail_tile_n", "tail_stages", "tail_smem_bytes", "tail_grid")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+class Mixed(C.Structure):
+    """laser_probe_mixed: what the mixed schedule does for n_valid rows (laser_probe_mixed_query)."""
+    _fields_ = [(n, C.c_int32) for n in ("mixed", "schedule", "k_pair", "j_single", "u_pair", "u_single",
+                                         "splits_pair", "splits_single")] + [("model_us", C.c_float)]
 
 
 class Options(C.Structure):
@@ -130,6 +137,7 @@ def lib():
         L.laser_probe_plan_query.argtypes = [dp, C.POINTER(Plan)]
         L.laser_probe_plan_query_mode.argtypes = [dp, C.c_int, C.POINTER(Plan)]
         L.laser_probe_options_default.argtypes = [C.POINTER(Options)]
+        L.laser_probe_mixed_query.argtypes = [dp, C.c_int32, C.POINTER(Mixed)]
         L.laser_probe_handle_create.argtypes = [C.POINTER(C.c_void_p), dp, C.POINTER(Options)]
         L.laser_probe_handle_destroy.argtypes = [vp]
         L.laser_probe_handle_plan.argtypes = [vp, C.POINTER(Plan)]
@@ -179,6 +187,12 @@ def plan_query(N, d, V, R, mode=MODE_AUTO) -> dict:
     p = Plan()
     _check(lib().laser_probe_plan_query_mode(C.byref(Dims(N, d, V, R)), mode, C.byref(p)))
     return p.as_dict()
+
+
+def mixed_query(N, d, V, R, n_valid) -> dict:
+    m = Mixed()
+    _check(lib().laser_probe_mixed_query(C.byref(Dims(N, d, V, R)), int(n_valid), C.byref(m)))
+    return {n: getattr(m, n) for n, _ in m._fields_}
 
 
 def workspace_bytes(N, d, V, R) -> int:
@@ -294,7 +308,8 @@ class Probe:
         self.tau = torch.empty(R, dtype=torch.float32, device=self.device) if debug_outputs else None
         self.pmax = torch.empty(N, dtype=torch.float32, device=self.device) if debug_outputs else None
         self.plan = plan_query(N, d, V, R, mode)
-        self.plan["kernel_launches"] = 2 if (tail == TAIL_SEPARATE or (tail == TAIL_AUTO and overlap)) else 1
+        if not self.plan["mixed"]:
+            self.plan["kernel_launches"] = 2 if (tail == TAIL_SEPARATE or (tail == TAIL_AUTO and overlap)) else 1
         self._handles = {}
 
     def _options(self, agg, token_ids) -> Options:

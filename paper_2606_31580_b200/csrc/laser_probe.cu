@@ -8,6 +8,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -156,19 +157,16 @@ double plan_variant(const laser_probe_dims& dm, int units, int tile_m, int bn_st
     return best;
 }
 
-void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_plan* pl) {
-    // CTA pairs (tcgen05 cta_group::2, M = 256) when there is more than one 128-row token tile: each
-    // W tile then enters a pair's shared memory once instead of once per token tile and one issuing
-    // thread feeds two SMs' tensor cores (measured +10..17 % for N >= 256).  An odd count of 128-row
-    // tiles makes the pair kernel compute one padding tile; that costs more than the pair gains
-    // until there are about ten tiles (measured: N = 384 and 640 are faster on single CTAs).
-    const int t128 = ceil_div(dm.N, kTileM);
-    const bool auto_pair = t128 >= 2 && ((t128 % 2) == 0 || t128 >= 10);
-    const bool pair = mode == LASER_MODE_PAIR || (mode == LASER_MODE_AUTO && auto_pair);
+// Plan of one kernel variant: CTA pairs (tcgen05 cta_group::2, M = 256; each W tile enters a pair's
+// shared memory once instead of once per 128-row token tile and one issuing thread feeds two SMs'
+// tensor cores: measured +10..17 % for N >= 256) or single CTAs (M = 128).  bn_force > 0 fixes tile_n.
+void make_variant_plan(const laser_probe_dims& dm, int num_sms, bool pair, int bn_force, laser_probe_plan* pl) {
     const int tile_m = pair ? 2 * kTileM : kTileM;
     const int units = pair ? (num_sms / 2 > 0 ? num_sms / 2 : 1) : num_sms;
     int S, T, BN;
     plan_variant(dm, units, tile_m, pair ? 32 : 16, &S, &T, &BN);   // fixes the tile height BN
+    if (bn_force > 0) BN = bn_force;
+    memset(pl, 0, sizeof *pl);
     pl->num_sms = num_sms;
     pl->m_tiles = dm.N > 0 ? ceil_div(dm.N, tile_m) : 1;
     // The deal of tiles to units comes from the function the kernels also use: with padding rows in
@@ -204,6 +202,103 @@ void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_pl
     pl->kernel_launches = 1;
     pl->tile_m = tile_m;
     pl->cta_pair = pair ? 1 : 0;
+}
+
+// ---- mixed schedule: the host plans every count of 128-row tiles that may hold rows
+// Cost model (B200, measured): a pair CTA spends 2*128*bn*d flop / 10 TFLOP/s on its
+// half of a 256-row item's tile; a single CTA needs 1.2x that for a 128-row tile (it stages a whole W
+// tile instead of half of one: 1.31x at boost clocks, 1.09x under the power cap); every kernel that
+// takes part streams W from HBM once (6.4 TB/s), and the second kernel of a call starts a few
+// microseconds behind the first.
+struct MixedChoice { int sched, u_tail, S_pair, S_tail, k_pair, j_single; double time; };
+MixedChoice plan_mixed_host(int m128, int V, int d, int bn_pair, int bn_tail, int sms) {
+    const int tiles_pair = ceil_div(V, bn_pair), tiles_tail = ceil_div(V, bn_tail);
+    const double t_p = 2.0 * kTileM * bn_pair * d / 10.0e12, t_s = 1.2 * 2.0 * kTileM * bn_tail * d / 10.0e12;
+    const double hbm_pass = 2.0 * V * d / 6.4e12;
+    const int pairs = sms / 2 > 0 ? sms / 2 : 1;
+    auto part = [](int tiles, int items, int units, double t_tile, int* S) {
+        const SplitPlan sp = plan_splits(tiles, items, units);
+        *S = sp.splits;
+        const long rounds = (static_cast<long>(items) * sp.splits + units - 1) / units;
+        return static_cast<double>(rounds) * sp.T * t_tile;
+    };
+    MixedChoice best{0, 0, 1, 1, 0, 0, 1e300};
+    {   // pair items only (an odd count pads half an item)
+        MixedChoice c{0, 0, 1, 1, (m128 + 1) / 2, 0, 0.0};
+        c.time = std::max(part(tiles_pair, c.k_pair, pairs, t_p, &c.S_pair), hbm_pass);
+        best = c;
+    }
+    {   // single-CTA tiles only
+        MixedChoice c{2, sms > 255 ? 255 : sms, 1, 1, 0, m128, 0.0};
+        c.time = std::max(part(tiles_tail, m128, c.u_tail, t_s, &c.S_tail), hbm_pass);
+        if (c.time < best.time) best = c;
+    }
+    if ((m128 & 1) && m128 >= 3) {   // pair items + the odd tile on single CTAs, side by side
+        for (int ut = 2; ut <= sms - 2 && ut <= 254; ut += 2) {   // whole TPCs: see launch_fused
+            MixedChoice c{1, ut, 1, 1, m128 / 2, 1, 0.0};
+            const double ta = part(tiles_pair, c.k_pair, (sms - ut) / 2, t_p, &c.S_pair);
+            const double tb = part(tiles_tail, 1, ut, t_s, &c.S_tail);
+            // two W passes at once do not reach the single-stream rate (5.5 instead of 6.4 TB/s)
+            c.time = std::max(std::max(ta + 4e-6, tb), 2.0 * hbm_pass * (6.4 / 5.5)) + 2e-6;
+            if (c.time < best.time) best = c;
+        }
+    }
+    return best;
+}
+
+// AUTO: one single-CTA kernel for N <= 128 rows; above that the mixed schedule (probe_kernels.cuh):
+// 256-row items on CTA pairs and / or 128-row tiles on single CTAs - which, is looked up on the device
+// from the number of 128-row tiles that hold rows (req_offsets[R]), so a padded batch pays for the
+// rows it holds.  *tail_pl (mixed only) is the plan of the single-CTA kernel.
+// SINGLE / PAIR force one variant (an odd tile count then costs the pair kernel a padding tile).
+void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_plan* pl, laser_probe_plan* tail_pl) {
+    const int t128 = ceil_div(dm.N, kTileM);
+    if (mode == LASER_MODE_SINGLE || (mode == LASER_MODE_AUTO && t128 <= 1)) {
+        make_variant_plan(dm, num_sms, false, 0, pl);
+        return;
+    }
+    make_variant_plan(dm, num_sms, true, 0, pl);
+    if (mode == LASER_MODE_PAIR) return;
+    // ---- mixed
+    laser_probe_dims d1 = dm;
+    d1.N = kTileM;
+    // the single-CTA kernel keeps the tile height that balances one 128-row tile over all SMs (the
+    // case where it works alone); on a fraction of the SMs it has many tiles per CTA anyway
+    laser_probe_plan tp;
+    make_variant_plan(d1, num_sms, false, 0, &tp);
+    tp.grid = num_sms;           // every SM may be needed (single-CTA tiles only)
+    pl->grid = 2 * (num_sms / 2 > 0 ? num_sms / 2 : 1);
+    pl->mixed = 1;
+    pl->tail_tile_n = tp.tile_n;
+    pl->tail_stages = tp.stages;
+    pl->tail_smem_bytes = tp.smem_bytes;
+    pl->tail_grid = tp.grid;
+    pl->kernel_launches = 3;     // single-CTA kernel, pair kernel, finalize kernel
+    long ws_records = 1;
+    for (int m128 = 1; m128 <= t128; ++m128) {
+        long rec;
+        if (m128 < kMixedTabMax) {
+            const MixedChoice c = plan_mixed_host(m128, dm.V, dm.d, pl->tile_n, tp.tile_n, num_sms);
+            rec = 2L * kTileM * c.k_pair * c.S_pair + static_cast<long>(kTileM) * c.j_single * c.S_tail;
+        } else {
+            const int k = (m128 + 1) / 2, up = num_sms / 2 > 0 ? num_sms / 2 : 1;
+            rec = 2L * kTileM * k * plan_splits(ceil_div(dm.V, pl->tile_n), k, up).splits;
+        }
+        if (rec > ws_records) ws_records = rec;
+    }
+    pl->ws_records = static_cast<int32_t>(ws_records);
+    if (tail_pl) *tail_pl = tp;
+}
+
+// The table of PlanDesc (kind 2): one packed plan per count of 128-row tiles.
+void fill_mixed_table(const laser_probe_dims& dm, const laser_probe_plan& pl, int num_sms, uint32_t* tab) {
+    const int t128 = ceil_div(dm.N, kTileM);
+    tab[0] = mixed_pack(0, 0, 1, 1);
+    for (int m128 = 1; m128 < kMixedTabMax; ++m128) {
+        if (m128 > t128) { tab[m128] = tab[t128 < kMixedTabMax ? t128 : kMixedTabMax - 1]; continue; }
+        const MixedChoice c = plan_mixed_host(m128, dm.V, dm.d, pl.tile_n, pl.tail_tile_n, num_sms);
+        tab[m128] = mixed_pack(c.sched, c.u_tail, c.S_pair, c.S_tail);
+    }
 }
 
 size_t workspace_bytes_for(const laser_probe_plan& pl) {
@@ -316,10 +411,12 @@ struct laser_probe_handle_s {
     laser_probe_dims dims;
     laser_probe_options opt;
     laser_probe_plan plan;
+    laser_probe_plan tail_plan;     // mixed schedule: the single-CTA kernel
+    uint32_t mixed_tab[kMixedTabMax] = {};
     DeviceInfo* di = nullptr;
     uint32_t* ctl = nullptr;
     bool debug = false;
-    struct MapEntry { const void* ptr = nullptr; CUtensorMap map; };
+    struct MapEntry { const void* ptr = nullptr; int box_rows = 0; CUtensorMap map; };
     MapEntry hid[2], w[4];
     int hid_rr = 0, w_rr = 0;
     struct HostMap { const void* h = nullptr; void* d = nullptr; };
@@ -334,13 +431,14 @@ typedef laser_probe_handle_s Handle;
 int handle_tensor_map(Handle::MapEntry* tab, int n, int* rr, const void* ptr, int rows, int cols,
                       int box_rows, const CUtensorMap** out) {
     for (int i = 0; i < n; ++i)
-        if (tab[i].ptr == ptr) { *out = &tab[i].map; return LASER_OK; }
+        if (tab[i].ptr == ptr && tab[i].box_rows == box_rows) { *out = &tab[i].map; return LASER_OK; }
     Handle::MapEntry& e = tab[*rr];
     *rr = (*rr + 1) % n;
     e.ptr = nullptr;
     int rc = encode_tensor_map(ptr, rows, cols, box_rows, &e.map);
     if (rc != LASER_OK) return rc;
     e.ptr = ptr;
+    e.box_rows = box_rows;
     *out = &e.map;
     return LASER_OK;
 }
@@ -354,7 +452,8 @@ int make_handle(const laser_probe_dims& dims, const laser_probe_options& opt, Ha
     h->dims = dims;
     h->opt = opt;
     h->di = di;
-    make_plan(dims, di->sms, opt.kernel_mode, &h->plan);
+    make_plan(dims, di->sms, opt.kernel_mode, &h->plan, &h->tail_plan);
+    if (h->plan.mixed) fill_mixed_table(dims, h->plan, di->sms, h->mixed_tab);
     const char* dbg = getenv("LASER_DEBUG");
     h->debug = dbg && dbg[0] && dbg[0] != '0';
     *out = h;
@@ -367,13 +466,31 @@ void free_handle(Handle* h) {
     delete h;
 }
 
+// The decomposition of a call as the kernels see it (PlanDesc, probe_kernels.cuh).
+PlanDesc plan_desc(const Handle* h, const int32_t* req_offsets) {
+    const laser_probe_plan& pl = h->plan;
+    PlanDesc d{};
+    d.n_alloc = h->dims.N; d.R = h->dims.R; d.req_offsets = req_offsets;
+    d.m_tiles = pl.m_tiles; d.rows_per_item = pl.tile_m; d.splits = pl.splits;
+    d.total_tiles = ceil_div(h->dims.V, pl.tile_n);
+    d.units = units_for(h->di, pl.cta_pair != 0);
+    d.kind = pl.mixed ? 2 : (pl.m_tiles > 1 ? 1 : 0);
+    if (pl.mixed) {
+        d.tiles_pair = ceil_div(h->dims.V, pl.tile_n);
+        d.sms = h->di->sms;
+        memcpy(d.mixed_tab, h->mixed_tab, sizeof d.mixed_tab);
+    }
+    return d;
+}
+
 // Enqueue laser_probe_fused_kernel for the handle's dims (W has dims.V rows; v_offset localises
-// token_ids); `tail` says what its last phase does.
-int launch_fused(Handle* h, const void* hidden, const void* W, const int32_t* req_offsets,
+// token_ids); `tail` says what its last phase does.  role: 0 = the call's only fused kernel (plan
+// h->plan); mixed schedule: 2 = the single-CTA tail-tile kernel (h->tail_plan), 1 = the pair kernel.
+int launch_fused(Handle* h, int role, const void* hidden, const void* W, const int32_t* req_offsets,
                  const int32_t* token_ids, int v_offset, float4* ws, cudaStream_t stream, bool allow_pdl,
                  const TailParams& tail) {
     DeviceInfo* di = h->di;
-    const laser_probe_plan& pl = h->plan;
+    const laser_probe_plan& pl = role == 2 ? h->tail_plan : h->plan;
     const laser_probe_dims& dims = h->dims;
     const int N = dims.N;
     const bool pair = pl.cta_pair != 0;
@@ -399,22 +516,20 @@ int launch_fused(Handle* h, const void* hidden, const void* W, const int32_t* re
     rc = handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V, dims.d, b_rows, &tm_w);
     if (rc != LASER_OK) return rc;
 
-    FusedParams fp;
+    FusedParams fp{};
     fp.n_alloc = N; fp.d = dims.d; fp.V = dims.V;
-    fp.m_tiles = pl.m_tiles;
-    fp.req_offsets = req_offsets; fp.R = dims.R;
+    fp.pd = plan_desc(h, req_offsets);
+    fp.role = role;
+    fp.grid_total = h->plan.grid;     // the fused tail exists only where one kernel makes the call
     fp.total_tiles = ceil_div(dims.V, pl.tile_n);
-    fp.units = units_for(di, pair);
-    fp.replan = pl.m_tiles > 1 ? 1 : 0;
     fp.wait_first = h->opt.overlap ? 0 : 1;
     fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
-    fp.work_items = pl.work_items;
     fp.tail_cache = pl.tail_cache;
     fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
     fp.tx_bytes = static_cast<uint32_t>((a_rows + b_rows) * 128);  // OOB rows are zero-filled and still counted
     // W is streamed once when a single token tile exists; with several token tiles the other
     // CTAs re-read the same rows from L2, so do not mark them evict-first.
-    fp.w_policy = (pl.m_tiles == 1) ? ptx::kEvictFirst : ptx::kEvictNormal;
+    fp.w_policy = (h->plan.m_tiles == 1 && !h->plan.mixed) ? ptx::kEvictFirst : ptx::kEvictNormal;
     fp.ws = ws;
     fp.token_ids = token_ids;
     fp.v_offset = v_offset;
@@ -434,7 +549,10 @@ int launch_fused(Handle* h, const void* hidden, const void* W, const int32_t* re
         fattr[na].val.programmaticStreamSerializationAllowed = 1;
         ++na;
     }
-    if (pair) {   // the two CTAs of a pair form a cluster (same TPC)
+    // the two CTAs of a pair form a cluster (same TPC).  The single-CTA kernel of a mixed call is
+    // launched as clusters of two as well - for placement only: its CTAs then fill whole TPCs and leave
+    // whole TPCs to the pair kernel beside it (scattered over the TPCs they starve it of pairs).
+    if (pair || (role == 2 && (pl.grid % 2) == 0)) {
         fattr[na].id = cudaLaunchAttributeClusterDimension;
         fattr[na].val.clusterDim.x = 2;
         fattr[na].val.clusterDim.y = 1;
@@ -443,26 +561,44 @@ int launch_fused(Handle* h, const void* hidden, const void* W, const int32_t* re
     }
     cfg.attrs = fattr;
     cfg.numAttrs = na;
-    cudaError_t e = pair ? cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<true>, *tm_h, *tm_w, fp, tail)
-                         : cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<false>, *tm_h, *tm_w, fp, tail);
+#ifdef LASER_TIMELINE
+    static int tl_launches = 0;      // debug build: one timeline slot per launch
+    TailParams tail_tl = tail;
+    tail_tl.tl_slot = tl_launches++;
+    const TailParams& tail_arg = tail_tl;
+#else
+    const TailParams& tail_arg = tail;
+#endif
+    cudaError_t e = pair ? cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<true>, *tm_h, *tm_w, fp, tail_arg)
+                         : cudaLaunchKernelEx(&cfg, laser_probe_fused_kernel<false>, *tm_h, *tm_w, fp, tail_arg);
     if (e != cudaSuccess) return set_cuda_error("launch laser_probe_fused_kernel", e);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return LASER_OK;
 }
 
-// The fields of FinalizeParams that describe the fused kernel's workspace for the handle's dims.
+// The fields of FinalizeParams that describe the fused kernels' workspace for the handle's dims.
 FinalizeParams finalize_params(const Handle* h, bool run_fused, const int32_t* req_offsets) {
-    const laser_probe_plan& pl = h->plan;
     FinalizeParams fz{};
-    fz.n_alloc = h->dims.N; fz.R = h->dims.R; fz.splits = pl.splits;
-    fz.m_tiles = pl.m_tiles; fz.rows_per_item = pl.tile_m;
-    fz.total_tiles = ceil_div(h->dims.V, pl.tile_n);
-    fz.units = units_for(h->di, pl.cta_pair != 0);
-    fz.replan = (run_fused && pl.m_tiles > 1) ? 1 : 0;
+    fz.n_alloc = h->dims.N; fz.R = h->dims.R;
+    fz.pd = plan_desc(h, req_offsets);
+    if (!run_fused) fz.pd.kind = 0;      // nothing was written: no request holds a row
     fz.req_offsets = req_offsets;
-    fz.row_stride = 0; fz.split_stride = 1;    // packed [rows, nsplit]
+    fz.row_stride = 0; fz.split_stride = 1;    // packed records
     fz.wait_flags = nullptr; fz.epoch = 0; fz.a_offset = 0; fz.prob_mode = 0; fz.agg_mode = 0;
     return fz;
+}
+
+// One call's fused kernel(s): a single launch, or - mixed schedule - the single-CTA tail-tile kernel
+// and, behind it under programmatic dependent launch, the pair kernel.  The two then run side by
+// side (the CTAs either part does not need exit at once); nothing in one waits for the other, so a
+// tool that serialises kernels only costs time.
+int launch_call(Handle* h, const void* hidden, const void* W, const int32_t* req_offsets,
+                const int32_t* token_ids, int v_offset, float4* ws, cudaStream_t stream, bool allow_pdl,
+                const TailParams& tail) {
+    if (!h->plan.mixed) return launch_fused(h, 0, hidden, W, req_offsets, token_ids, v_offset, ws, stream, allow_pdl, tail);
+    int rc = launch_fused(h, 2, hidden, W, req_offsets, token_ids, v_offset, ws, stream, allow_pdl, tail);
+    if (rc != LASER_OK) return rc;
+    return launch_fused(h, 1, hidden, W, req_offsets, token_ids, v_offset, ws, stream, true, tail);
 }
 
 // Enqueue laser_probe_finalize_kernel: blocks [0, R) aggregate, the rest mark padding rows.
@@ -502,6 +638,15 @@ int launch_validate(const Handle* h, const int32_t* req_offsets, cudaStream_t st
 int want_fused_tail(Handle* h, cudaStream_t stream, bool* fused_tail) {
     *fused_tail = false;
     if (h->opt.tail == LASER_TAIL_SEPARATE) return LASER_OK;
+    if (h->plan.mixed) {
+        // two fused kernels: a tail in one would have to wait for the CTAs of the other, which tools
+        // that serialise kernels (profilers) would turn into a hang.  The merge is the third launch.
+        if (h->opt.tail == LASER_TAIL_FUSED) {
+            g_last_error = "LASER_TAIL_FUSED needs a single fused kernel (N <= 128 rows, or kernel_mode SINGLE / PAIR)";
+            return LASER_E_MODE;
+        }
+        return LASER_OK;
+    }
     // AUTO with overlap: calls chained two deep gate each other's CTAs; the tail CTAs would hold SMs
     // the next call could be streaming on, so the second kernel (co-resident, tiny) is the faster form
     if (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap) return LASER_OK;
@@ -559,17 +704,13 @@ int run_probe(Handle* h, const void* hidden, const void* W, const int32_t* req_o
         rc = launch_validate(h, req_offsets, stream);
         if (rc != LASER_OK) return rc;
         TailParams tail{};
-#ifdef LASER_TIMELINE
-        static int tl_calls = 0;
-        tail.tl_slot = tl_calls++;
-#endif
         tail.kind = fused_tail ? 1 : 0;
         tail.ctl = h->ctl;
         tail.q.f = fz;
         if (prof) cudaEventRecord(g_prof.ev[prof_slot][0], stream);
-        rc = launch_fused(h, hidden, W, req_offsets,
-                          h->opt.prob_mode == LASER_PROB_TOKEN ? token_ids : nullptr, 0,
-                          static_cast<float4*>(workspace), stream, !prof && !h->debug, tail);
+        rc = launch_call(h, hidden, W, req_offsets,
+                         h->opt.prob_mode == LASER_PROB_TOKEN ? token_ids : nullptr, 0,
+                         static_cast<float4*>(workspace), stream, !prof && !h->debug, tail);
         if (rc != LASER_OK) return rc;
         if (prof) cudaEventRecord(g_prof.ev[prof_slot][1], stream);
     }
@@ -621,8 +762,8 @@ int run_partial(Handle* h, const void* hidden, const void* W_shard, const int32_
         tail.kind = fused_tail ? 2 : 0;
         tail.ctl = h->ctl;
         tail.q = rq;
-        rc = launch_fused(h, hidden, W_shard, req_offsets, token_ids_opt, v_offset,
-                          static_cast<float4*>(workspace), stream, !h->debug, tail);
+        rc = launch_call(h, hidden, W_shard, req_offsets, token_ids_opt, v_offset,
+                         static_cast<float4*>(workspace), stream, !h->debug, tail);
         if (rc != LASER_OK) return rc;
         if (fused_tail) return LASER_OK;
     }
@@ -827,7 +968,33 @@ int laser_probe_plan_query_mode(const laser_probe_dims* dims, int kernel_mode, l
     if (kernel_mode < LASER_MODE_AUTO || kernel_mode > LASER_MODE_PAIR) return LASER_E_MODE;
     bool ok = false;
     DeviceInfo* di = current_device(&ok);
-    make_plan(*dims, (ok && di) ? di->sms : kDefaultSMs, kernel_mode, plan);
+    make_plan(*dims, (ok && di) ? di->sms : kDefaultSMs, kernel_mode, plan, nullptr);
+    return LASER_OK;
+}
+
+int laser_probe_mixed_query(const laser_probe_dims* dims, int32_t n_valid, laser_probe_mixed* out) {
+    if (!dims || !out) return LASER_E_NULL;
+    if (!dims_valid(dims) || n_valid < 0 || n_valid > dims->N) return LASER_E_DIMS;
+    laser_probe_plan pl;
+    int rc = laser_probe_plan_query_mode(dims, LASER_MODE_AUTO, &pl);
+    if (rc != LASER_OK) return rc;
+    memset(out, 0, sizeof *out);
+    if (!pl.mixed) return LASER_OK;          // one single-CTA kernel: nothing is decided on the device
+    const int m128 = ceil_div(n_valid, kTileM);
+    if (m128 == 0) return LASER_OK;
+    out->mixed = 1;
+    if (m128 < kMixedTabMax) {
+        const MixedChoice c = plan_mixed_host(m128, dims->V, dims->d, pl.tile_n, pl.tail_tile_n, pl.num_sms);
+        const MixedPlan mp = mixed_unpack(mixed_pack(c.sched, c.u_tail, c.S_pair, c.S_tail), m128, pl.num_sms);
+        out->schedule = c.sched; out->k_pair = mp.k_pair; out->j_single = mp.j_single;
+        out->u_pair = mp.u_pair; out->u_single = mp.j_single > 0 ? mp.u_tail : 0;
+        out->splits_pair = mp.S_pair; out->splits_single = mp.S_tail;
+        out->model_us = static_cast<float>(c.time * 1e6);
+    } else {
+        const int k = (m128 + 1) / 2, up = pl.num_sms / 2 > 0 ? pl.num_sms / 2 : 1;
+        out->schedule = 0; out->k_pair = k; out->u_pair = up;
+        out->splits_pair = plan_splits(ceil_div(dims->V, pl.tile_n), k, up).splits;
+    }
     return LASER_OK;
 }
 
@@ -836,12 +1003,15 @@ int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan)
 }
 
 size_t laser_probe_workspace_bytes(const laser_probe_dims* dims) {
-    // enough for either kernel variant, so that one buffer serves every laser_probe_options.kernel_mode
-    laser_probe_plan a, b;
-    if (laser_probe_plan_query_mode(dims, LASER_MODE_SINGLE, &a) != LASER_OK) return 0;
-    if (laser_probe_plan_query_mode(dims, LASER_MODE_PAIR, &b) != LASER_OK) return 0;
-    const size_t wa = workspace_bytes_for(a), wb = workspace_bytes_for(b);
-    return wa > wb ? wa : wb;
+    // enough for every kernel_mode, so that one buffer serves every laser_probe_options setting
+    size_t best = 0;
+    for (int mode = LASER_MODE_AUTO; mode <= LASER_MODE_PAIR; ++mode) {
+        laser_probe_plan pl;
+        if (laser_probe_plan_query_mode(dims, mode, &pl) != LASER_OK) return 0;
+        const size_t w = workspace_bytes_for(pl);
+        if (w > best) best = w;
+    }
+    return best;
 }
 
 // ------------------------------------------------------------------------------ explicit handles
@@ -856,7 +1026,8 @@ int laser_probe_handle_create(laser_probe_handle** out, const laser_probe_dims* 
     Handle* h = nullptr;
     rc = make_handle(*dims, opt, &h);
     if (rc != LASER_OK) return rc;
-    if (opt.tail != LASER_TAIL_SEPARATE) h->ctl = acquire_ctl(h->di, nullptr);   // may stay NULL: retried per call
+    if (opt.tail != LASER_TAIL_SEPARATE && !h->plan.mixed)
+        h->ctl = acquire_ctl(h->di, nullptr);   // may stay NULL: retried per call
     *out = h;
     return LASER_OK;
 }
@@ -869,8 +1040,9 @@ int laser_probe_handle_destroy(laser_probe_handle* h) {
 int laser_probe_handle_plan(const laser_probe_handle* h, laser_probe_plan* plan) {
     if (!h || !plan) return LASER_E_NULL;
     *plan = h->plan;
-    plan->kernel_launches = (h->opt.tail == LASER_TAIL_SEPARATE || !h->ctl ||
-                             (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap)) ? 2 : 1;
+    if (!h->plan.mixed)
+        plan->kernel_launches = (h->opt.tail == LASER_TAIL_SEPARATE || !h->ctl ||
+                                 (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap)) ? 2 : 1;
     return LASER_OK;
 }
 
@@ -1004,8 +1176,9 @@ int laser_probe_combine(const laser_row_stats* stats, int32_t G, const int32_t* 
     rc = require_b200(&di);
     if (rc != LASER_OK) return rc;
     FinalizeParams fz{};
-    fz.n_alloc = N; fz.R = R; fz.splits = G;
-    fz.m_tiles = 1; fz.rows_per_item = kTileM; fz.total_tiles = 1; fz.units = 1; fz.replan = 0;
+    fz.n_alloc = N; fz.R = R;
+    fz.pd.kind = 0; fz.pd.n_alloc = N; fz.pd.R = R; fz.pd.req_offsets = req_offsets;
+    fz.pd.m_tiles = 1; fz.pd.rows_per_item = kTileM; fz.pd.splits = G;
     fz.agg_mode = opt.aggregate_mode;
     fz.prob_mode = opt.prob_mode;
     fz.a_offset = 0;

@@ -73,25 +73,115 @@ __host__ __device__ inline SplitPlan plan_splits(int total_tiles, int m_items, i
     return best;
 }
 
+// ---------------------------------------------------------------------------------- call plans
+// Mixed schedule (N > 128 rows, kernel_mode AUTO): the token rows are cut into 128-row tiles; an even
+// count runs as 256-row items on CTA pairs (cta_group::2); of an odd count the LAST 128-row tile runs
+// on single CTAs (cta_group::1) instead of being padded to a pair item.  cta_group is a property of a
+// kernel, so a call is two launches - the single-CTA ("tail-tile") kernel first, the pair kernel
+// behind it with programmatic dependent launch - whose CTAs look at req_offsets[R] on the device,
+// split the SMs between the two parts in proportion to their work, and exit at once where they have
+// nothing to do; both walk W in the same tile order, so the second reader of a W tile finds it in L2.
+struct MixedPlan {
+    int k_pair, j_single;  // 256-row pair items; 128-row tiles behind them for the single-CTA kernel
+    int u_pair, u_tail;    // CTA pairs / single CTAs that take part
+    int S_pair, S_tail;    // vocabulary splits per item of either part
+};
+// The host plans every count m128 of 128-row tiles that may hold rows (laser_probe.cu, fill_mixed_table)
+// and hands the kernels one packed word per count: looking the plan up on the device costs nothing.
+//   bits [0,2)   schedule: 0 pair items only (an odd count pads half an item), 1 pair items + one
+//                single-CTA tile, 2 single-CTA tiles only
+//   bits [2,10)  u_tail   bits [10,21)  S_pair   bits [21,32)  S_tail
+constexpr int kMixedTabMax = 256;     // counts beyond the table: pair items only, planned on the device
+__host__ __device__ inline uint32_t mixed_pack(int sched, int u_tail, int S_pair, int S_tail) {
+    return static_cast<uint32_t>(sched) | (static_cast<uint32_t>(u_tail) << 2) |
+           (static_cast<uint32_t>(S_pair) << 10) | (static_cast<uint32_t>(S_tail) << 21);
+}
+__host__ __device__ inline MixedPlan mixed_unpack(uint32_t e, int m128, int sms) {
+    MixedPlan mp;
+    const int sched = static_cast<int>(e & 3u);
+    mp.u_tail = static_cast<int>((e >> 2) & 0xFFu);
+    mp.S_pair = static_cast<int>((e >> 10) & 0x7FFu);
+    mp.S_tail = static_cast<int>((e >> 21) & 0x7FFu);
+    mp.k_pair = sched == 0 ? (m128 + 1) / 2 : (sched == 1 ? m128 / 2 : 0);
+    mp.j_single = sched == 0 ? 0 : (sched == 1 ? 1 : m128);
+    mp.u_pair = mp.k_pair > 0 ? (sms - mp.u_tail) / 2 : 0;
+    return mp;
+}
+
+// What fixes a call's decomposition; shared by the fused kernel(s) and the merge.
+struct PlanDesc {
+    int32_t kind;                      // 0 static, 1 re-plan of one variant, 2 mixed (pair + single-CTA tail tile)
+    int32_t n_alloc, R;
+    const int32_t* req_offsets;
+    int32_t m_tiles, rows_per_item, splits;    // kind 0 / 1: the host plan of the variant
+    int32_t total_tiles, units;                // kind 1: vocabulary tiles of the variant, its execution units
+    int32_t tiles_pair, sms;                   // kind 2: vocabulary tiles of the pair kernel, SMs
+    uint32_t mixed_tab[kMixedTabMax];          // kind 2: the plan for every count of 128-row tiles (mixed_pack)
+};
+// Where a call's records are: rows [0, rows_a) have S_a records each from record 0 on; rows >= rows_a
+// have S_b records each from record rows_a * S_a on.
+struct RecLayout {
+    int rows_a, S_a, S_b;
+};
+// The decomposition that actually runs, decided on the device from req_offsets[R] (kind 1, 2).
+struct RunPlan {
+    MixedPlan mp;          // kind 2
+    int m_items, S;        // kind 0 / 1
+    RecLayout lay;
+};
+__device__ __forceinline__ RunPlan resolve_plan(const PlanDesc& d) {
+    RunPlan rp{};
+    rp.m_items = d.m_tiles; rp.S = d.splits;
+    if (d.kind != 0) {   // uniform across the grid: every thread reads the same word
+        const int n_valid = d.R > 0 ? min(max(__ldg(d.req_offsets + d.R), 0), d.n_alloc) : 0;
+        if (d.kind == 1) {
+            const int m = (n_valid + d.rows_per_item - 1) / d.rows_per_item;
+            if (m < d.m_tiles) {
+                rp.m_items = m;
+                rp.S = m > 0 ? plan_splits(d.total_tiles, m, d.units).splits : 1;
+            }
+        } else {
+            const int m128 = (n_valid + kTileM - 1) / kTileM;
+            if (m128 < kMixedTabMax) {
+                rp.mp = mixed_unpack(d.mixed_tab[m128], m128, d.sms);
+            } else {    // very large batches: an odd last tile is noise, pad it
+                const int up = d.sms / 2 > 0 ? d.sms / 2 : 1;
+                rp.mp = MixedPlan{(m128 + 1) / 2, 0, up, 0, plan_splits(d.tiles_pair, (m128 + 1) / 2, up).splits, 1};
+            }
+        }
+    }
+    if (d.kind == 2) rp.lay = RecLayout{2 * kTileM * rp.mp.k_pair, rp.mp.S_pair, rp.mp.S_tail};
+    else rp.lay = RecLayout{0x7fffffff, rp.S, rp.S};
+    return rp;
+}
+__device__ __forceinline__ const float4* row_records(const float4* ws, const RecLayout& L, int n, int& nsplit) {
+    if (n < L.rows_a) { nsplit = L.S_a; return ws + static_cast<int64_t>(n) * L.S_a; }
+    nsplit = L.S_b;
+    return ws + static_cast<int64_t>(L.rows_a) * L.S_a + static_cast<int64_t>(n - L.rows_a) * L.S_b;
+}
+
 struct FusedParams {
     int32_t n_alloc, d, V;
-    int32_t m_tiles, tile_n, k_blocks, stages;
-    int32_t work_items;    // m_tiles * splits of the host plan; m_tiles counts items of 128 (single) / 256 (pair) rows
+    int32_t tile_n, k_blocks, stages;
+    int32_t total_tiles;   // vocabulary tiles of tile_n rows (this kernel's variant)
     uint32_t tx_bytes;     // bytes TMA delivers per stage and CTA (hidden box + W box)
     uint32_t stage_bytes;  // shared-memory stride of a stage: kABytes + (W rows per CTA) * 128
     uint64_t w_policy;     // L2 eviction policy for the W stream
-    float4* ws;            // packed [rows, splits] per (row, split): {max, sum exp(logit - max), argmax bits, token logit}
+    float4* ws;            // packed records {max, sum exp(logit - max), argmax bits, token logit}, see RecLayout
     // LASER_PROB_TOKEN: token_ids[n] - v_offset is the column of W whose logit is kept for row n
     // (nullptr: no token logit is tracked; v_offset = global vocabulary index of W's row 0).
     const int32_t* token_ids;
     int32_t v_offset;
-    // Padding-aware re-planning (m_tiles > 1 only): token items at or beyond req_offsets[R] are
-    // skipped and the vocabulary tiles are re-dealt over the remaining items.
-    const int32_t* req_offsets;
-    int32_t R, total_tiles, units, replan;
+    PlanDesc pd;           // the call's decomposition (padding-aware on the device when pd.kind != 0)
+    // 0: the call's only fused kernel.  Mixed schedule: 2 = the single-CTA tail-tile kernel (launched
+    // first; it alone orders the call against the kernel ahead: griddepcontrol.wait, THEN
+    // launch_dependents), 1 = the pair kernel behind it (never waits before it has counted itself in:
+    // kernel 2 may be waiting for its arrivals).
+    int32_t role;
+    int32_t grid_total;    // CTAs of all fused kernels of the call: what the tail's arrival count waits for
     // 1 (strict, default): griddepcontrol.wait before the first read of hidden / req_offsets /
     //    token_ids; W - model weight, never written by the kernel ahead - is requested for the first
-    //    `stages` pipeline slots before the wait when the plan is static (replan == 0).
+    //    `stages` pipeline slots before the wait when the plan is static (pd.kind == 0).
     // 0 (overlap): only the workspace / output stores wait (laser_probe_options.overlap).
     int32_t wait_first;
     // requests whose {offset, threshold} fit in the shared memory the pipeline leaves over: the
@@ -188,12 +278,10 @@ __host__ __device__ __forceinline__ float tau_eval(float load, const TauParamsDe
 // laser_probe_combine merges.  Same layout as laser_row_stats in include/laser_probe.h.
 //   x = max logit, y = sum exp(logit - max), z = argmax (int bits), w = logit of the row's token
 struct FinalizeParams {
-    int32_t n_alloc, R, splits, agg_mode;
-    int32_t m_tiles, rows_per_item, total_tiles, units, replan;   // see FusedParams
-    // record (n, sp) lives at ws[n * row_stride + sp * split_stride]:
-    //   fused workspace, packed [rows, nsplit]: row_stride = 0 (meaning "the split count that ran"),
-    //                                           split_stride = 1
-    //   gathered shard statistics [G, N]: row_stride = 1, split_stride = N  (laser_probe_combine)
+    int32_t n_alloc, R, agg_mode;
+    PlanDesc pd;      // where the fused kernel(s) left the records (packed workspace: row_stride == 0)
+    // gathered shard statistics [G, N] (laser_probe_combine): record (n, g) at ws[n * row_stride +
+    // g * split_stride] with row_stride = 1, split_stride = N, pd.kind = 0, pd.splits = G
     int64_t row_stride, split_stride;
     int32_t prob_mode;            // 0: row maximum 1/S; 1: the row's token exp(l_tok - m)/S
     int32_t a_offset;             // added to every argmax (vocabulary shard offset; reduce path)
@@ -223,9 +311,12 @@ constexpr int kMergeBatch = 5;  // partials a lane loads before it starts mergin
 // The records may have been written by other CTAs of the running grid (tail of the fused kernel):
 // they are read through L2 (ld.global.cg), never through this SM's L1.
 template <int NR>
-__device__ __forceinline__ void merge_rows(const float4* const (&rec)[NR], int64_t split_stride, int nsplit,
-                                           int lane, float (&m)[NR], int (&a)[NR], float (&s)[NR],
-                                           float (&lt)[NR]) {
+__device__ __forceinline__ void merge_rows(const float4* const (&rec)[NR], int64_t split_stride,
+                                           const int (&ns)[NR], int lane, float (&m)[NR], int (&a)[NR],
+                                           float (&s)[NR], float (&lt)[NR]) {
+    int nsplit = 0;
+#pragma unroll
+    for (int i = 0; i < NR; ++i) nsplit = max(nsplit, rec[i] != nullptr ? ns[i] : 0);
     const float4 neutral = make_float4(-CUDART_INF_F, 0.f, __int_as_float(0x7fffffff), -CUDART_INF_F);
     // 2^{(x - M) log2e} with the convention that equal operands (also -inf, -inf) give exactly 1
     auto scale = [](float x, float M) { return (x == M) ? 1.f : ptx::ex2_approx((x - M) * kLog2e); };
@@ -240,7 +331,7 @@ __device__ __forceinline__ void merge_rows(const float4* const (&rec)[NR], int64
 #pragma unroll
             for (int j = 0; j < kMergeBatch; ++j) {
                 const int sp = sp0 + 32 * j;
-                v[i][j] = (rec[i] != nullptr && sp < nsplit) ? __ldcg(rec[i] + sp * split_stride) : neutral;
+                v[i][j] = (rec[i] != nullptr && sp < ns[i]) ? __ldcg(rec[i] + sp * split_stride) : neutral;
             }
 #pragma unroll
         for (int i = 0; i < NR; ++i) {
@@ -281,21 +372,18 @@ __device__ __forceinline__ void merge_rows(const float4* const (&rec)[NR], int64
 __device__ __forceinline__ void merge_row(const float4* rec, int64_t split_stride, int nsplit, int lane,
                                           float& m, int& a, float& s, float& lt) {
     const float4* const r1[1] = {rec};
+    const int n1[1] = {nsplit};
     float mm[1], ss[1], ll[1];
     int aa[1];
-    merge_rows<1>(r1, split_stride, nsplit, lane, mm, aa, ss, ll);
+    merge_rows<1>(r1, split_stride, n1, lane, mm, aa, ss, ll);
     m = mm[0]; a = aa[0]; s = ss[0]; lt = ll[0];
 }
 
-// Records per row the fused kernel wrote for this batch (device-side re-plan, see FusedParams).
-__device__ __forceinline__ int records_per_row(const FinalizeParams& p) {
-    int nsplit = p.splits;
-    if (p.replan) {
-        const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
-        const int m_items = (n_valid + p.rows_per_item - 1) / p.rows_per_item;
-        if (m_items > 0) nsplit = plan_splits(p.total_tiles, min(m_items, p.m_tiles), p.units).splits;
-    }
-    return nsplit;
+// Records of row n: packed workspace (layout decided on the device) or gathered shard statistics.
+__device__ __forceinline__ const float4* finalize_row(const FinalizeParams& p, const RecLayout& lay, int n,
+                                                      int& nsplit) {
+    if (p.row_stride != 0) { nsplit = lay.S_a; return p.ws + static_cast<int64_t>(n) * p.row_stride; }
+    return row_records(p.ws, lay, n, nsplit);
 }
 
 // Spin until every peer's flag has reached `epoch` (peer GPUs store them with system scope after
@@ -330,21 +418,21 @@ __device__ __forceinline__ void group_sync() {
 constexpr int kFinalThread = 32;   // lane 0 of the group's warp 1 (thread 0 runs the arrival protocol in the tail)
 template <int kBarId, int kThreads>
 __device__ __forceinline__ void finalize_request(const FinalizeParams& p, int tid, int r, int b, int e, float tau,
-                                                 int nsplit, float* warp_acc) {
+                                                 const RecLayout& lay, float* warp_acc) {
     constexpr int nwarps = kThreads / 32;
     const int warp = tid >> 5, lane = tid & 31;
-    const int64_t row_stride = p.row_stride ? p.row_stride : nsplit;
     // running aggregate of this warp's rows: sum (mean), sum of logs (geomean), min.  Two rows per
     // pass (rows n and n + nwarps): their record loads share one L2 round trip.
     float acc = (p.agg_mode == 2) ? CUDART_INF_F : 0.f;
     bool any_nan = false;
     for (int n0 = b + warp; n0 < e; n0 += 2 * nwarps) {
         const int n1 = n0 + nwarps;
-        const float4* const rec[2] = {p.ws + static_cast<int64_t>(n0) * row_stride,
-                                      n1 < e ? p.ws + static_cast<int64_t>(n1) * row_stride : nullptr};
+        int ns[2] = {0, 0};
+        const float4* const rec[2] = {finalize_row(p, lay, n0, ns[0]),
+                                      n1 < e ? finalize_row(p, lay, n1, ns[1]) : nullptr};
         float m[2], s[2], lt[2];
         int a[2];
-        merge_rows<2>(rec, p.split_stride, nsplit, lane, m, a, s, lt);
+        merge_rows<2>(rec, p.split_stride, ns, lane, m, a, s, lt);
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             const int n = i == 0 ? n0 : n1;
@@ -409,7 +497,7 @@ __device__ __forceinline__ void mark_padding_rows(const FinalizeParams& p, int f
 // rows.  Every global store comes after griddepcontrol.wait (the kernel ahead in the stream may be a
 // previous call still writing the same output buffers).
 __global__ void __launch_bounds__(kFinalizeThreads)
-laser_probe_finalize_kernel(const FinalizeParams p) {
+laser_probe_finalize_kernel(const __grid_constant__ FinalizeParams p) {
     __shared__ float warp_acc[kFinalizeWarps];
     ptx::pdl_launch_dependents();
     if (static_cast<int>(blockIdx.x) >= p.R) {
@@ -424,9 +512,9 @@ laser_probe_finalize_kernel(const FinalizeParams p) {
     float tau = 0.f;
     if (threadIdx.x == kFinalThread) tau = tau_eval(__ldg(p.load + r), p.tau);   // a4
     ptx::pdl_wait();  // all of the fused kernel's partials are visible after this
-    const int nsplit = records_per_row(p);
-    if (p.wait_flags != nullptr) wait_peer_flags(p.wait_flags, nsplit, p.epoch);
-    finalize_request<0, kFinalizeThreads>(p, threadIdx.x, r, b, e, tau, nsplit, warp_acc);
+    const RunPlan rp = resolve_plan(p.pd);
+    if (p.wait_flags != nullptr) wait_peer_flags(p.wait_flags, p.pd.splits, p.epoch);
+    finalize_request<0, kFinalizeThreads>(p, threadIdx.x, r, b, e, tau, rp.lay, warp_acc);
 }
 
 // ---------------------------------------------------------------------------------- vocab-parallel
@@ -450,13 +538,15 @@ struct ReduceParams {
 };
 
 // One warp: merged record of row n -> out_stats / peers.
-__device__ __forceinline__ void reduce_row(const ReduceParams& q, int n, int n_valid, int nsplit, int lane) {
+__device__ __forceinline__ void reduce_row(const ReduceParams& q, int n, int n_valid, const RecLayout& lay,
+                                           int lane) {
     const FinalizeParams& p = q.f;
     float m = -CUDART_INF_F, s = 0.f, lt = -CUDART_INF_F;
     int a = 0x7fffffff;
     if (n < n_valid) {
-        const int64_t row_stride = p.row_stride ? p.row_stride : nsplit;
-        merge_row(p.ws + static_cast<int64_t>(n) * row_stride, p.split_stride, nsplit, lane, m, a, s, lt);
+        int nsplit = 0;
+        const float4* rec = finalize_row(p, lay, n, nsplit);
+        merge_row(rec, p.split_stride, nsplit, lane, m, a, s, lt);
         a += p.a_offset;
     }
     const float4 rec = make_float4(m, s, __int_as_float(a), lt);
@@ -472,16 +562,16 @@ __device__ __forceinline__ void publish_epoch(const ReduceParams& q, int lane) {
 }
 
 __global__ void __launch_bounds__(kFinalizeThreads)
-laser_probe_reduce_kernel(const ReduceParams q) {
+laser_probe_reduce_kernel(const __grid_constant__ ReduceParams q) {
     const FinalizeParams& p = q.f;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     ptx::pdl_launch_dependents();
     ptx::pdl_wait();
     const int n = blockIdx.x * kFinalizeWarps + warp;
     const int n_valid = (p.R > 0) ? min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc) : 0;
-    const int nsplit = records_per_row(p);
+    const RunPlan rp = resolve_plan(p.pd);
     if (n >= p.n_alloc) return;
-    reduce_row(q, n, n_valid, nsplit, lane);
+    reduce_row(q, n, n_valid, rp.lay, lane);
 }
 
 // After the reduce kernel (stream order: its stores, remote ones included, have been performed):
@@ -551,7 +641,7 @@ struct TailParams {
 template <bool kPair>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
-                         const __grid_constant__ CUtensorMap tmap_w, const FusedParams p,
+                         const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ FusedParams p,
                          const __grid_constant__ TailParams t) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t raw = ptx::smem_u32(smem_raw);
@@ -578,8 +668,12 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     const int BN = p.tile_n;
     const int b_rows = kPair ? (BN >> 1) : BN;   // W rows this CTA stages per tile
     const int total_tiles = p.total_tiles;
-    int m_items = p.m_tiles, work_items = p.work_items;
-    int S = work_items / m_items;                // static plan; re-planned below when p.replan
+    // static plan (pd.kind == 0); decided on the device further down otherwise
+    int m_items = p.pd.m_tiles, S = p.pd.splits, units_run = units;
+    int work_items = m_items * S;
+    int row0 = 0;          // first token row of this kernel's items
+    int64_t rec0 = 0;      // first workspace record of this kernel's region
+    const bool static_plan = p.pd.kind == 0;
 
     // W ahead of the wait (strict mode, static plan): the producer requests the W boxes of its first
     // `stages` pipeline slots - and asks L2 for the boxes of the `stages` slots after those - before
@@ -588,7 +682,7 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     // include/laser_probe.h).  The hidden boxes of those slots follow after the wait.
     int pre = 0;
     auto preissue_w = [&]() {
-        if (!(p.wait_first && !p.replan && unit < work_items)) return;
+        if (!(p.wait_first && static_plan && unit < work_items)) return;
         const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);
         int tile = unit / m_items, kb = 0;
         for (int slot = 0; slot < 2 * p.stages && tile < total_tiles; ++slot) {
@@ -644,18 +738,22 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
 
     // Programmatic dependent launch: whatever follows in the stream may become resident on the SMs
     // this grid vacates; it must itself wait (griddepcontrol.wait) before it touches our outputs.
-    ptx::pdl_launch_dependents();
+    // Role 2 (the first kernel of a mixed call) orders the whole call against the kernel ahead: it
+    // waits first and only then lets the pair kernel (role 1) in, which therefore never has to wait.
+    if (p.role != 2) ptx::pdl_launch_dependents();
     if constexpr (kPair) { if (warp == 0) preissue_w(); }
     LASER_TL(t.tl_slot, 1, 0);    // prologue + W pre-issue done
 
     // Strict: every read of hidden / req_offsets / token_ids below happens after the kernel ahead of
     // this one in the stream has completed.  Overlap: only the stores wait (further down).
-    if (p.wait_first) ptx::pdl_wait();
+    if ((p.wait_first && p.role == 0) || p.role == 2) ptx::pdl_wait();
+    if (p.role == 2) ptx::pdl_launch_dependents();
     LASER_TL(t.tl_slot, 2, 0);    // strict wait passed
     // tail bookkeeping: the arrival count this call starts from (strict: read here, long before it is
     // needed; the call ahead, which may share the slot, has completed)
     uint32_t base = 0;
-    if (threadIdx.x == kTailThread0 && t.kind != 0 && p.wait_first) base = ptx::ld_relaxed_gpu_u32(t.ctl + 1);
+    const bool base_early = p.wait_first || p.role != 0;   // the call ahead (same slot) has completed by now
+    if (threadIdx.x == kTailThread0 && t.kind != 0 && base_early) base = ptx::ld_relaxed_gpu_u32(t.ctl + 1);
     // a4 ahead of time: {req_offsets, tau(load)} of every request into the shared-memory cache behind
     // the barrier block (any CTA may turn out to be one of the last to arrive)
     int* off_c = reinterpret_cast<int*>(smem_raw + (smem - raw) + p.stages * p.stage_bytes + 256u);
@@ -669,15 +767,23 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         }
     }
 
-    if (p.replan) {   // uniform across the grid: every thread reads the same word
-        const int n_valid = min(max(__ldg(p.req_offsets + p.R), 0), p.n_alloc);
-        m_items = (n_valid + kRowsPerItem - 1) / kRowsPerItem;
-        if (m_items < p.m_tiles) {
-            work_items = m_items > 0 ? m_items * plan_splits(total_tiles, m_items, p.units).splits : 0;
-        } else {
-            m_items = p.m_tiles;
+    RunPlan rp{};
+    if (static_plan) {
+        rp.m_items = m_items; rp.S = S;
+        rp.lay = RecLayout{0x7fffffff, S, S};
+    } else {
+        rp = resolve_plan(p.pd);
+        if (p.pd.kind == 1) {
+            m_items = rp.m_items; S = rp.S;
+        } else if (kPair) {      // mixed schedule, pair part: k_pair items of 256 rows on u_pair pairs
+            m_items = rp.mp.k_pair; S = rp.mp.S_pair; units_run = rp.mp.u_pair;
+        } else {                 // mixed schedule, the 128-row tiles behind the pair items on u_tail single CTAs
+            m_items = rp.mp.j_single; S = rp.mp.S_tail; units_run = rp.mp.u_tail;
+            row0 = 2 * kTileM * rp.mp.k_pair;
+            rec0 = static_cast<int64_t>(row0) * rp.mp.S_pair;
         }
-        S = m_items > 0 ? work_items / m_items : 1;
+        work_items = (unit < units_run) ? m_items * S : 0;    // units beyond units_run: nothing to do
+        if (m_items == 0) { m_items = 1; work_items = 0; }
     }
     // split sp owns vocabulary tiles sp, sp + S, sp + 2S, ... (ascending: ties keep the lowest index)
 
@@ -688,9 +794,9 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);  // leader's barriers
         int stage = 0;
         uint32_t phase = 0;
-        for (int w = unit; w < work_items; w += units) {
+        for (int w = unit; w < work_items; w += units_run) {
             const int mt = w % m_items, sp = w / m_items;
-            const int a_row = mt * kRowsPerItem + static_cast<int>(rank) * kTileM;
+            const int a_row = row0 + mt * kRowsPerItem + static_cast<int>(rank) * kTileM;
             for (int tile = sp; tile < total_tiles; tile += S) {
                 const int b_row = tile * BN + static_cast<int>(rank) * b_rows;
                 for (int kb = 0; kb < k_blocks; ++kb) {
@@ -738,7 +844,7 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             const int k_blocks = p.k_blocks, stages = p.stages;
             int stage = 0;
             uint32_t phase = 0, acc = 0, desc_off = 0;
-            for (int w = unit; w < work_items; w += units) {
+            for (int w = unit; w < work_items; w += units_run) {
                 for (int tile = w / m_items; tile < total_tiles; tile += S, ++acc) {
                     const uint32_t buf = acc & 1u, aphase = (acc >> 1) & 1u;
                     // epilogue (of both CTAs in pair mode) drained this buffer
@@ -773,12 +879,12 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         const int row = static_cast<int>(rank) * kTileM + q * 32 + lane;
         const uint32_t lane_addr = static_cast<uint32_t>(q * 32) << 16;
         uint32_t acc = 0;
-        for (int w = unit; w < work_items; w += units) {
+        for (int w = unit; w < work_items; w += units_run) {
             const int mt = w % m_items, sp = w / m_items;
             float m = -CUDART_INF_F, s = 0.f, lt = -CUDART_INF_F;
             int a = -1, tok = -1;
             if (p.token_ids != nullptr) {
-                const int n = mt * kRowsPerItem + row;
+                const int n = row0 + mt * kRowsPerItem + row;
                 if (n < p.n_alloc) {
                     const int tk = __ldg(p.token_ids + n) - p.v_offset;
                     tok = (tk >= 0 && tk < p.V) ? tk : -1;   // not in this (shard of the) vocabulary
@@ -814,8 +920,10 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             }
             // packed row-major over splits: the merge reads a row's partials as contiguous 16-byte
             // records (coalesced); the scattered 16-byte stores here are fire-and-forget
-            const size_t o = (static_cast<size_t>(mt) * kRowsPerItem + row) * S + sp;
-            ptx::pdl_wait();   // overlap mode: the previous call's tail may still be reading the workspace
+            const int64_t o = rec0 + (static_cast<int64_t>(mt) * kRowsPerItem + row) * S + sp;
+            // overlap mode: the previous call's tail may still be reading the workspace.  (Role 1 must
+            // not wait: the kernel ahead of it is its own call's role-2 kernel, ordered already.)
+            if (p.role != 1) ptx::pdl_wait();
             p.ws[o] = make_float4(m, s, __int_as_float(a), lt);
         }
         LASER_TL(t.tl_slot, 3, kTailThread0);   // last record stored
@@ -830,18 +938,18 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         // and MMA warps go straight to the teardown - and the LAST F CTAs to arrive run merge + a3-a5
         // (kind 1) or the shard reduce (kind 2): they are the ones with the least to wait for.
         if (t.kind != 0) {
-            ptx::pdl_wait();   // outputs are written below (a CTA without work items has not waited yet)
+            if (p.role != 1) ptx::pdl_wait();   // outputs are written below (a CTA without work items has not waited yet)
             const int tid = threadIdx.x - kTailThread0, tw = tid >> 5;
             constexpr int kTW = kEpilogueThreads / 32;
             const FinalizeParams& f = t.q.f;
-            const int grid = gridDim.x;
+            const int grid = p.grid_total;
             const int F = (t.kind == 1) ? min(grid, f.R) : min(grid, (f.n_alloc + kTW - 1) / kTW);
             // scratch: bytes [192, 232) of the barrier block
             float* warp_acc = reinterpret_cast<float*>(smem_raw + (smem - raw) + p.stages * p.stage_bytes + 192u);
             volatile uint32_t* tk = reinterpret_cast<volatile uint32_t*>(warp_acc + kMaxTailWarps);
             group_sync<1, kEpilogueThreads>();   // every record store of this CTA is ordered before the count
             if (tid == 0) {
-                if (!p.wait_first) base = ptx::ld_relaxed_gpu_u32(t.ctl + 1);   // overlap: the call ahead is complete only now
+                if (!base_early) base = ptx::ld_relaxed_gpu_u32(t.ctl + 1);   // overlap: the call ahead is complete only now
                 const uint32_t target = base + static_cast<uint32_t>(grid);
                 LASER_TL(t.tl_slot, 4, kTailThread0);
                 const uint32_t mine = ptx::atom_add_acq_rel_gpu_u32(t.ctl, 1u) + 1u;
@@ -853,7 +961,7 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             const int behind = static_cast<int>(target - mine);    // CTAs still to arrive
             if (behind >= F) {
                 // not one of the last F: padding rows do not depend on anybody's records
-                if (t.kind == 1) mark_padding_rows(f, blockIdx.x * kEpilogueThreads + tid, grid * kEpilogueThreads);
+                if (t.kind == 1) mark_padding_rows(f, blockIdx.x * kEpilogueThreads + tid, gridDim.x * kEpilogueThreads);
             } else {
                 const int fi = F - 1 - behind;    // 0 .. F-1; the last arrival is F-1
                 if (behind > 0) {
@@ -874,13 +982,13 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                         const int re = cached ? off_c[r + 1] : __ldg(f.req_offsets + r + 1);
                         float tau = 0.f;
                         if (tid == kFinalThread) tau = cached ? tau_c[r] : tau_eval(__ldg(f.load + r), f.tau);
-                        finalize_request<1, kEpilogueThreads>(f, tid, r, rb, re, tau, S, warp_acc);
+                        finalize_request<1, kEpilogueThreads>(f, tid, r, rb, re, tau, rp.lay, warp_acc);
                         if (r == fi) LASER_TL(t.tl_slot, 6, kTailThread0);
                     }
-                    mark_padding_rows(f, blockIdx.x * kEpilogueThreads + tid, grid * kEpilogueThreads);
+                    mark_padding_rows(f, blockIdx.x * kEpilogueThreads + tid, gridDim.x * kEpilogueThreads);
                 } else {
                     const int n_valid = (f.R > 0) ? min(max(__ldg(f.req_offsets + f.R), 0), f.n_alloc) : 0;
-                    for (int n = fi * kTW + tw; n < f.n_alloc; n += F * kTW) reduce_row(t.q, n, n_valid, S, tid & 31);
+                    for (int n = fi * kTW + tw; n < f.n_alloc; n += F * kTW) reduce_row(t.q, n, n_valid, rp.lay, tid & 31);
                     __threadfence_system();   // remote (peer) stores of this thread are performed before the count below
                     group_sync<1, kEpilogueThreads>();
                     if (tid < 32) {

@@ -55,24 +55,33 @@ def test_plan_invariants(dims):
     bn, T, S = p["tile_n"], p["tiles_per_split"], p["splits"]
     pair, tm = p["cta_pair"], p["tile_m"]
     t128 = -(-N // 128)
-    assert pair == (1 if t128 >= 2 and (t128 % 2 == 0 or t128 >= 10) else 0) and tm == (256 if pair else 128)
+    mixed = p["mixed"]
+    # AUTO: one single-CTA kernel up to 128 rows, above that the mixed schedule (pair kernel + single-CTA
+    # tail-tile kernel + finalize kernel)
+    assert (pair, mixed) == ((0, 0) if t128 <= 1 else (1, 1)) and tm == (256 if pair else 128)
+    assert p["kernel_launches"] == (3 if mixed else 1)
     assert bn % (32 if pair else 16) == 0 and 16 <= bn <= 256
     assert S * T * bn >= V and (S - 1) * T * bn < V          # splits tile the vocabulary exactly once
     assert p["m_tiles"] == max(1, -(-N // tm)) and p["k_blocks"] == -(-d // 64)
     units = p["num_sms"] // 2 if pair else p["num_sms"]
     assert p["work_items"] == p["m_tiles"] * S
-    assert p["grid"] == (2 if pair else 1) * min(units, p["work_items"])
+    assert p["grid"] == ((2 * units) if mixed else (2 if pair else 1) * min(units, p["work_items"]))
     assert 2 <= p["stages"] <= 8
     b_rows = bn // 2 if pair else bn                          # W rows one CTA stages per tile
     pipe = p["stages"] * (16384 + b_rows * 128) + 1280        # stages + alignment slack + barrier block
     assert 0 <= p["tail_cache"] <= 512
     assert pipe + (8 * (p["tail_cache"] + 1) if p["tail_cache"] else 0) == p["smem_bytes"] <= 227 * 1024
-    # packed records: at least the full batch's, at most 2x it (a re-plan for fewer token items may use
-    # more splits per row, never more than the units allow); one buffer serves both kernel variants
-    full = p["m_tiles"] * tm * S
-    assert full <= p["ws_records"] <= 2 * full and (p["ws_records"] == full or p["m_tiles"] > 1)
+    if mixed:
+        assert p["tail_tile_n"] % 16 == 0 and 16 <= p["tail_tile_n"] <= 256 and p["tail_grid"] == p["num_sms"]
+        assert 2 <= p["tail_stages"] <= 8 and p["tail_smem_bytes"] <= 227 * 1024
+        assert p["ws_records"] >= N                            # at least one record per row
+    else:
+        # packed records: at least the full batch's, at most 2x it (a re-plan for fewer token items may
+        # use more splits per row, never more than the units allow)
+        full = p["m_tiles"] * tm * S
+        assert full <= p["ws_records"] <= 2 * full and (p["ws_records"] == full or p["m_tiles"] > 1)
     both = [B.plan_query(*dims, mode=m)["ws_records"] for m in (B.MODE_SINGLE, B.MODE_PAIR)]
-    assert B.workspace_bytes(*dims) == max(16, 16 * max(both)) >= 16 * p["ws_records"]
+    assert B.workspace_bytes(*dims) >= max(16, 16 * max(both + [p["ws_records"]]))
     # the busiest unit does at most ~8 % more than an even share of W rows (+ one tile of slack)
     busy = min(units, p["work_items"])
     rounds = -(-p["work_items"] // busy)

@@ -155,9 +155,9 @@ def force_mode(P):
     P.CFG["mode"] = 0
 
 
-PATHS = {"tail-handle": dict(tail=1, use_handle=True),       # a3-a5 in the fused kernel's tail (default)
-         "separate-handle": dict(tail=2, use_handle=True),   # second kernel (LASER_TAIL_SEPARATE)
-         "tail-implicit": dict(tail=0, use_handle=False)}    # handle-less entry point, implicit handle
+PATHS = {"auto-handle": dict(tail=0, use_handle=True),       # a3-a5 in the fused kernel's tail where one kernel makes the call
+         "separate-handle": dict(tail=2, use_handle=True),   # finalize kernel (LASER_TAIL_SEPARATE)
+         "auto-implicit": dict(tail=0, use_handle=False)}    # handle-less entry point, implicit handle
 
 
 @pytest.fixture(params=list(PATHS))
@@ -214,6 +214,49 @@ def test_padding_tiles_are_skipped_and_replanned(P, force_mode, path, mode, R, L
     st = P.check(w)
     assert st["plan"]["m_tiles"] > 1
     _log(w.name, st)
+
+
+@pytest.mark.parametrize("R,L,var_len,n_alloc", [
+    (40, 8, None, None),         # N = 320: one pair item + a half-filled tail tile
+    (48, 8, None, None),         # N = 384: one pair item + a full tail tile
+    (80, 8, None, None),         # N = 640: two pair items + a tail tile
+    (9, 8, None, 1024),          # 72 valid rows of 1024: the tail-tile kernel alone, on every SM
+    (32, 8, None, 1024),         # 256 valid rows: the pair kernel alone
+    (33, 8, None, 1024),         # 264 valid rows: one pair item + a tail tile holding 8 rows
+    (74, None, (1, 16), 1024),   # ragged, ~600 valid rows (C4-like)
+    (3, 0, None, 700),           # every request empty: neither part has work
+])
+def test_mixed_schedule_odd_tile_counts(P, path, R, L, var_len, n_alloc):
+    """AUTO above 128 rows: 256-row items on CTA pairs, an odd last 128-row tile on single CTAs in a
+    second kernel beside them; which part takes what is decided on the device from req_offsets[R].
+    Requests that straddle the two parts are merged from both kernels' records."""
+    w = wl.scaled(f"mixed-R{R}-L{L}-N{n_alloc}", 33000, 512, 0.05, R, L, seed=R + 31, N_alloc=n_alloc, var_len=var_len)
+    st = P.check(w)
+    assert st["plan"]["mixed"] == 1 and st["plan"]["kernel_launches"] == 3
+    _log(f"{w.name}/{path}", st)
+
+
+def test_mixed_schedule_ties_across_the_two_kernels(P):
+    """Duplicate W rows whose logits tie exactly, for a row of the pair part and a row of the tail tile:
+    the lowest index must win in both kernels (different tile heights, different split counts)."""
+    from paper_2606_31580_b200 import binding as B
+    V, d, N = 40000, 128, 384
+    plan = B.plan_query(N, d, V, 3)
+    assert plan["mixed"] == 1
+    rng = np.random.default_rng(19)
+    Wf = (rng.standard_normal((V, d)) * 0.05).astype(np.float32)
+    h = rng.standard_normal((N, d)).astype(np.float32)
+    for row in (10, 200, 300):                     # leader CTA, peer CTA, tail-tile kernel
+        big = (h[row] * 0.5).astype(np.float32)
+        for v1, v2 in [(255, 256), (1000, 30000), (plan["tile_n"] - 1, plan["tile_n"])]:
+            W2 = Wf.copy(); W2[v1] = big; W2[v2] = big
+            w = wl.Workload("ties-mixed", wl.bf16_bits(W2), wl.bf16_bits(h), wl.fixed_offsets(3, 128),
+                            np.array([0.3, 0.7, 0.5], np.float32))
+            g = P.run_gpu(w)
+            assert g.argmax[row] == v1, (row, v1, v2, g.argmax[row])
+            ora, rows, reqs = P.run_oracle(w)
+            assert ora.argmax[row] == v1 and ora.gap2[row] == 0.0
+            P.compare(w, g, ora, rows, reqs, "ties-mixed")
 
 
 def test_ties_in_pair_mode(P, force_mode):
@@ -297,9 +340,9 @@ def test_ties_across_tile_and_split_boundaries(P):
         P.compare(w, g, ora, rows, reqs, "ties")
 
 
-@pytest.mark.parametrize("tail", [1, 2])
+@pytest.mark.parametrize("tail,mode", [(1, 1), (1, 2), (2, 0), (0, 0)])   # fused tail on either variant / separate / mixed
 @pytest.mark.parametrize("overlap", [True, False])
-def test_back_to_back_calls_share_a_workspace(P, overlap, tail):
+def test_back_to_back_calls_share_a_workspace(P, overlap, tail, mode):
     """Stream order under programmatic dependent launch: calls enqueued back to back on one stream,
     all on ONE workspace, with alternating inputs.  The fused kernel of call k+1 may start while the
     tail of call k still reads the workspace (laser_probe_options.overlap), and all calls go through
@@ -312,7 +355,7 @@ def test_back_to_back_calls_share_a_workspace(P, overlap, tail):
     devs = [P.to_device(w) for w in ws]
     oras = [P.run_oracle(w) for w in ws]
     K = 24
-    probes = [B.Probe(R * L, d, V, R, overlap=overlap, tail=tail) for _ in range(K)]
+    probes = [B.Probe(R * L, d, V, R, overlap=overlap, tail=tail, mode=mode) for _ in range(K)]
     for p in probes[1:]:
         p.workspace = probes[0].workspace
         p._handles = probes[0]._handles          # one handle (one control slot) for all calls
@@ -322,7 +365,8 @@ def test_back_to_back_calls_share_a_workspace(P, overlap, tail):
     for k, p in enumerate(probes):
         dv = devs[k % 2]
         p(dv["hidden"], dv["W"], dv["off"], dv["load"], tp)
-    assert B.kernel_launch_count() - n0 == K * (2 if tail == 2 else 1)
+    assert B.kernel_launch_count() - n0 == K * probes[0].plan["kernel_launches"]
+    assert probes[0].plan["kernel_launches"] == (3 if mode == 0 else (2 if tail == 2 else 1))
     torch.cuda.synchronize()
     for k, p in enumerate(probes):
         g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),

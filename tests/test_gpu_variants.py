@@ -178,7 +178,7 @@ def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False, tail=0):
                     out.tau.cpu().numpy(), out.pmax.cpu().numpy(), sh.plan), stats_all.cpu().numpy()
 
 
-@pytest.mark.parametrize("tail", [1, 2])       # reduce + push + signal in the fused kernel's tail / as kernels
+@pytest.mark.parametrize("tail", [0, 2])       # reduce + push + signal in the fused kernel's tail (one kernel) / as kernels
 @pytest.mark.parametrize("peer", [False, True])
 @pytest.mark.parametrize("G", [1, 2, 3, 8])
 @pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
@@ -190,7 +190,9 @@ def test_vocab_parallel_matches_oracle(P, G, peer, tail, V, d, R, L, n_alloc, va
     w = wl.scaled(f"vp-V{V}-G{G}", V, d, 0.05, R, L, seed=88, N_alloc=n_alloc, var_len=var_len)
     n0 = B.kernel_launch_count()
     g, stats = _run_vocab_parallel(P, w, G, peer=peer, tail=tail)
-    per_partial = 1 if tail == 1 else (3 if peer else 2)
+    mixed = B.plan_query(w.N_alloc, d, par.shard_vocab(V, G, 0)[1], R)["mixed"]
+    fused = 2 if mixed else 1                                           # fused kernels of one partial
+    per_partial = fused if (tail == 0 and not mixed) else fused + (2 if peer else 1)
     assert B.kernel_launch_count() - n0 == G * per_partial + 1          # + the combine kernel
     ora, rows, reqs = P.run_oracle(w)
     st = P.compare(w, g, ora, rows, reqs, w.name)
@@ -299,7 +301,7 @@ def test_fuzz_shapes_modes_aggregates(P, i):
                   N_alloc=w0.N_valid + pad)
     if w.N_alloc == 0:
         pytest.skip("empty batch (covered by test_empty_batches_and_requests)")
-    tail, use_handle = [(0, True), (2, True), (1, False), (0, False)][i % 4]
+    tail, use_handle = [(0, True), (2, True), (2, False), (0, False)][i % 4]
     P.CFG.update(mode=mode, tail=tail, use_handle=use_handle)
     try:
         st = P.check(w, agg=agg)
