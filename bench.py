@@ -311,6 +311,50 @@ class GpuCase:
         return fused / n * 1e3, fin / n * 1e3
 
 
+def cublas_context(w: wl.Workload, case, steps: int, gpu_index: int) -> dict:
+    """CONTEXT ONLY (not the product path, not part of any reported probe figure): the plain library GEMM
+    logits = hidden[:N_valid] @ W^T in bf16 through torch.matmul (cuBLAS), back to back on the same box
+    with the same clock sampler - what the contraction alone costs a library at this shape.  It WRITES
+    the [N, V] logits (which the probe never does) and computes no softmax / argmax / confidence."""
+    import torch
+    torch.cuda.synchronize()
+    time.sleep(COOL_S)
+    h = case.hidden[:w.N_valid]
+    Wt = [W.t() for W in case.Ws]
+    out = torch.empty((w.N_valid, w.V), dtype=torch.bfloat16, device=h.device)
+    for i in range(5):
+        torch.matmul(h, Wt[i % len(Wt)], out=out)
+
+    def timed(n):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for i in range(n):
+            torch.matmul(h, Wt[i % len(Wt)], out=out)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n * 1e3
+
+    sampler = ClockSampler(gpu_index)
+    sampler.start()
+    time.sleep(0.05)
+    t0 = time.perf_counter()
+    us = timed(steps)
+    clocks = sampler.summary(t0, time.perf_counter())
+    settle_t0 = time.perf_counter()
+    while time.perf_counter() - settle_t0 < SETTLE_S:
+        timed(20)
+    t1 = time.perf_counter()
+    us_sus = timed(steps)
+    clocks_sus = sampler.summary(t1, time.perf_counter())
+    sampler.stop()
+    fl = 2.0 * w.N_valid * w.V * w.d
+    return dict(what="torch.matmul(hidden[:N_valid], W.T) bf16 -> bf16 logits [N_valid, V] (cuBLAS); context only",
+                us_per_call=us, tflops=fl / (us * 1e-6) / 1e12, sm_mhz=clocks.get("sm_mhz"),
+                us_per_call_sustained=us_sus, tflops_sustained=fl / (us_sus * 1e-6) / 1e12,
+                sustained_sm_mhz=clocks_sus.get("sm_mhz"), logits_bytes_written=2 * w.N_valid * w.V, steps=steps)
+
+
 def realised_distribution(w: wl.Workload, case) -> dict:
     """One untimed call with the debug outputs on: the realised shares of rows / requests per
     confidence band (SURVEY §8 d: polarisation must be visible next to every number)."""
@@ -769,6 +813,8 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_sweep and args.workload == "C2":
         out["serving_sim"] = serving_sim_bench(device, with_cpu=not args.no_cpu_baseline)
 
+    if rank == 0 and world == 1 and args.with_cublas:
+        out["cublas_context"] = cublas_context(w, case, args.steps, physical_gpu_index(local_rank))
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, target_s=10.0)
     if dist is not None:
@@ -861,6 +907,8 @@ def main():
     ap.add_argument("--workload", default="C2")
     ap.add_argument("--sharding", default="requests", choices=["requests", "vocab"])
     ap.add_argument("--exchange", default="peer", choices=["peer", "collective"])
+    ap.add_argument("--with-cublas", action="store_true",
+                    help="context only: time the plain cuBLAS GEMM hidden @ W^T of the same shape beside the probe")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -674,6 +674,31 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     int row0 = 0;          // first token row of this kernel's items
     int64_t rec0 = 0;      // first workspace record of this kernel's region
     const bool static_plan = p.pd.kind == 0;
+    RunPlan rp{};
+    if (p.pd.kind == 2) {
+        // Mixed schedule: which part takes what is looked up before anything is set up, so that the
+        // CTAs a part does not need (all of them, for the single-CTA kernel of an even dense batch)
+        // leave within a microsecond or two.  The single-CTA kernel (role 2) orders the whole call
+        // against the kernel ahead - it waits, THEN lets the pair kernel in, which never has to wait.
+        if (p.role == 2) ptx::pdl_wait();
+        rp = resolve_plan(p.pd);
+        if (p.role == 2) ptx::pdl_launch_dependents();
+        if (kPair) {             // pair part: k_pair items of 256 rows on u_pair pairs
+            m_items = rp.mp.k_pair; S = rp.mp.S_pair; units_run = rp.mp.u_pair;
+        } else {                 // the 128-row tiles behind the pair items on u_tail single CTAs
+            m_items = rp.mp.j_single; S = rp.mp.S_tail; units_run = rp.mp.u_tail;
+            row0 = 2 * kTileM * rp.mp.k_pair;
+            rec0 = static_cast<int64_t>(row0) * rp.mp.S_pair;
+        }
+        if (m_items == 0 || unit >= units_run) {
+            // nothing for this CTA.  It still completes only after the kernel ahead of it has (the
+            // merge kernel behind the pair kernel relies on that to see the single-CTA kernel's records)
+            if (p.role != 2) ptx::pdl_launch_dependents();
+            ptx::pdl_wait();
+            return;
+        }
+        work_items = m_items * S;
+    }
 
     // W ahead of the wait (strict mode, static plan): the producer requests the W boxes of its first
     // `stages` pipeline slots - and asks L2 for the boxes of the `stages` slots after those - before
@@ -740,14 +765,13 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     // this grid vacates; it must itself wait (griddepcontrol.wait) before it touches our outputs.
     // Role 2 (the first kernel of a mixed call) orders the whole call against the kernel ahead: it
     // waits first and only then lets the pair kernel (role 1) in, which therefore never has to wait.
-    if (p.role != 2) ptx::pdl_launch_dependents();
+    if (p.pd.kind != 2 || p.role == 1) ptx::pdl_launch_dependents();
     if constexpr (kPair) { if (warp == 0) preissue_w(); }
     LASER_TL(t.tl_slot, 1, 0);    // prologue + W pre-issue done
 
     // Strict: every read of hidden / req_offsets / token_ids below happens after the kernel ahead of
     // this one in the stream has completed.  Overlap: only the stores wait (further down).
-    if ((p.wait_first && p.role == 0) || p.role == 2) ptx::pdl_wait();
-    if (p.role == 2) ptx::pdl_launch_dependents();
+    if (p.wait_first && p.role == 0) ptx::pdl_wait();
     LASER_TL(t.tl_slot, 2, 0);    // strict wait passed
     // tail bookkeeping: the arrival count this call starts from (strict: read here, long before it is
     // needed; the call ahead, which may share the slot, has completed)
@@ -767,22 +791,13 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         }
     }
 
-    RunPlan rp{};
     if (static_plan) {
         rp.m_items = m_items; rp.S = S;
         rp.lay = RecLayout{0x7fffffff, S, S};
-    } else {
+    } else if (p.pd.kind == 1) {
         rp = resolve_plan(p.pd);
-        if (p.pd.kind == 1) {
-            m_items = rp.m_items; S = rp.S;
-        } else if (kPair) {      // mixed schedule, pair part: k_pair items of 256 rows on u_pair pairs
-            m_items = rp.mp.k_pair; S = rp.mp.S_pair; units_run = rp.mp.u_pair;
-        } else {                 // mixed schedule, the 128-row tiles behind the pair items on u_tail single CTAs
-            m_items = rp.mp.j_single; S = rp.mp.S_tail; units_run = rp.mp.u_tail;
-            row0 = 2 * kTileM * rp.mp.k_pair;
-            rec0 = static_cast<int64_t>(row0) * rp.mp.S_pair;
-        }
-        work_items = (unit < units_run) ? m_items * S : 0;    // units beyond units_run: nothing to do
+        m_items = rp.m_items; S = rp.S;
+        work_items = m_items * S;
         if (m_items == 0) { m_items = 1; work_items = 0; }
     }
     // split sp owns vocabulary tiles sp, sp + S, sp + 2S, ... (ascending: ties keep the lowest index)
