@@ -834,9 +834,35 @@ int run_host(Handle* h, const void* h_hidden, const void* W, const int32_t* h_re
     if (R > 0 && h_req_offsets[R] >= 0 && h_req_offsets[R] <= N) n_copy = h_req_offsets[R];
     else if (R == 0) n_copy = 0;
     if (n_copy > 0) {
-        e = cudaMemcpyAsync(base + st.hidden, h_hidden, static_cast<size_t>(n_copy) * dims->d * 2,
-                            cudaMemcpyHostToDevice, stream);
-        if (e != cudaSuccess) return set_cuda_error("H2D hidden", e);
+        const size_t bytes = static_cast<size_t>(n_copy) * dims->d * 2;      // a multiple of 16 (d % 8 == 0)
+        void* m_hidden = mapped_ptr(h, h_hidden);
+        static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
+        if (m_hidden && (reinterpret_cast<uintptr_t>(m_hidden) & 15) == 0 && getenv("LASER_NO_STAGE_KERNEL") == nullptr) {
+            // pinned + mapped: the staging kernel pulls the rows over PCIe as a link of the launch chain
+            const int64_t n16 = static_cast<int64_t>(bytes / 16);
+            int grid = static_cast<int>((n16 + kStageThreads * kStageInFlight - 1) / (kStageThreads * kStageInFlight));
+            const int max_grid = 4 * h->di->sms;
+            if (grid > max_grid) grid = max_grid;
+            if (grid < 1) grid = 1;
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3(grid);
+            cfg.blockDim = dim3(kStageThreads);
+            cfg.stream = stream;
+            cudaLaunchAttribute attr[1];
+            if (use_pdl) {
+                attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+                attr[0].val.programmaticStreamSerializationAllowed = 1;
+                cfg.attrs = attr;
+                cfg.numAttrs = 1;
+            }
+            e = cudaLaunchKernelEx(&cfg, laser_probe_stage_kernel, static_cast<const uint4*>(m_hidden),
+                                   reinterpret_cast<uint4*>(base + st.hidden), n16);
+            if (e != cudaSuccess) return set_cuda_error("launch laser_probe_stage_kernel", e);
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+        } else {
+            e = cudaMemcpyAsync(base + st.hidden, h_hidden, bytes, cudaMemcpyHostToDevice, stream);
+            if (e != cudaSuccess) return set_cuda_error("H2D hidden", e);
+        }
     }
     // Zero-copy for the small tensors: when req_offsets, load and the three outputs all live in
     // pinned, device-mapped host memory (cudaHostAlloc / cudaHostRegister / torch pin_memory), the

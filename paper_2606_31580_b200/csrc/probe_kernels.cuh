@@ -580,6 +580,33 @@ __global__ void laser_probe_signal_kernel(const ReduceParams q) {
     publish_epoch(q, threadIdx.x);
 }
 
+// Host-buffer entry points: `hidden` in pinned, device-mapped host memory is pulled over PCIe by this
+// kernel instead of a copy-engine transfer, so that the copy is a link of the same programmatic
+// dependent launch chain as the probe kernels: its CTAs (no shared memory, few registers) become
+// resident beside the previous call's fused CTAs and read their share of the rows into registers
+// while that call is still running; only the stores into the staging buffer wait for it.
+constexpr int kStageThreads = 256;
+constexpr int kStageInFlight = 8;     // 16-byte loads per thread ahead of the wait
+__global__ void __launch_bounds__(kStageThreads)
+laser_probe_stage_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, int64_t n16) {
+    ptx::pdl_launch_dependents();
+    const int64_t tid = static_cast<int64_t>(blockIdx.x) * kStageThreads + threadIdx.x;
+    const int64_t nthreads = static_cast<int64_t>(gridDim.x) * kStageThreads;
+    uint4 v[kStageInFlight];
+#pragma unroll
+    for (int j = 0; j < kStageInFlight; ++j) {
+        const int64_t i = tid + j * nthreads;
+        v[j] = i < n16 ? ptx::ld_nc_v4(src + i) : make_uint4(0u, 0u, 0u, 0u);
+    }
+    ptx::pdl_wait();    // the kernel ahead may still be reading the staging buffer
+#pragma unroll
+    for (int j = 0; j < kStageInFlight; ++j) {
+        const int64_t i = tid + j * nthreads;
+        if (i < n16) dst[i] = v[j];
+    }
+    for (int64_t i = tid + kStageInFlight * nthreads; i < n16; i += nthreads) dst[i] = ptx::ld_nc_v4(src + i);
+}
+
 // LASER_DEBUG=1: the documented precondition on req_offsets (non-decreasing, [0] == 0, [R] <= N),
 // checked on the device by one warp ahead of the probe; a violation traps (the caller sees a CUDA
 // error at the next synchronisation) instead of silently reading other requests' rows.
