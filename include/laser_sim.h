@@ -74,8 +74,8 @@ int laser_sim_policy_default(laser_sim_policy* out);
  *   out_chunks    device, int32  [n_req, n_rep]  chunks generated
  *   out_exited_opt device, uint8 [n_req, n_rep] or NULL: 1 = confidence exit, 0 = budget exhausted
  *   out_budget_opt device, int32 [n_req, n_rep] or NULL: the budget B (after the cap at K)
- *   out_summary   device, double [n_rep, 5]: mean latency, P95 latency (nearest rank; NaN when
- *                 n_req > LASER_SIM_MAX_P95_REQUESTS), throughput n_req / (last finish - first
+ *   out_summary   device, double [n_rep, 5]: mean latency, P95 latency (nearest rank; a shared-memory sort up to
+ *                 LASER_SIM_MAX_P95_REQUESTS requests per queue, a radix select over global memory above), throughput n_req / (last finish - first
  *                 arrival), share of requests with latency <= deadline, mean chunks generated
  *
  * Out-of-range sample or policy ids are a precondition violation (ids are clamped, never read out

@@ -25,6 +25,7 @@
 namespace {
 
 struct SimParams {
+    int lanes;       // replications per warp (see laser_sim_queue_kernel)
     const double* arrival;
     const int32_t* sample_id;
     const int32_t* policy_id;
@@ -70,9 +71,15 @@ __device__ __forceinline__ int32_t sim_budget(double prompt_tokens, double L, co
 
 constexpr int kSimThreads = 32;   // one warp per block: replications spread over all SMs
 
+// Only the first `lanes` lanes of a warp simulate (lanes = 1, 2, 4, ... 32, chosen by the host so that
+// the warps fill the machine's warp slots): the lanes of a warp walk the request index in lock step and
+// wait for the lane whose request generates the most chunks, so the fewer replications share a warp
+// the less of that wait there is (one per warp: none), and a latency-bound kernel loses nothing by
+// running more, emptier warps.
 __global__ void __launch_bounds__(kSimThreads)
 laser_sim_queue_kernel(const __grid_constant__ SimParams q) {
-    const int r = blockIdx.x * kSimThreads + threadIdx.x;
+    if (static_cast<int>(threadIdx.x) >= q.lanes) return;
+    const int r = blockIdx.x * q.lanes + threadIdx.x;
     if (r >= q.n_rep) return;
     const int n = q.n_req, R = q.n_rep, K = q.K;
     int pid = __ldg(q.policy_id + r);
@@ -210,6 +217,53 @@ laser_sim_p95_kernel(const double* __restrict__ arrival, const double* __restric
     }
 }
 
+// n_req > LASER_SIM_MAX_P95_REQUESTS: the same nearest-rank element by an 8-pass most-significant-byte
+// radix select over the latencies recomputed from global memory (a double's bits, sign-flipped, order
+// like the value).  One block per replication; each pass histograms the byte of the keys that match
+// the prefix found so far.
+__device__ __forceinline__ unsigned long long order_key(double x) {
+    const unsigned long long b = static_cast<unsigned long long>(__double_as_longlong(x));
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__global__ void __launch_bounds__(kP95Threads)
+laser_sim_p95_select_kernel(const double* __restrict__ arrival, const double* __restrict__ finish,
+                            double* __restrict__ out_summary, int n_rep, int n_req) {
+    __shared__ unsigned int hist[256];
+    __shared__ unsigned long long s_prefix;
+    __shared__ unsigned int s_rank;
+    const int r = blockIdx.x;
+    if (threadIdx.x == 0) {
+        int rank = static_cast<int>(ceil(__dmul_rn(0.95, static_cast<double>(n_req))));
+        s_rank = static_cast<unsigned int>(rank < 1 ? 1 : rank);     // 1-based rank still to find
+        s_prefix = 0ull;
+    }
+    for (int pass = 0; pass < 8; ++pass) {
+        const int shift = 56 - 8 * pass;
+        for (int i = threadIdx.x; i < 256; i += kP95Threads) hist[i] = 0u;
+        __syncthreads();
+        const unsigned long long prefix = s_prefix;
+        const unsigned long long mask = pass == 0 ? 0ull : (~0ull << (shift + 8));
+        for (int i = threadIdx.x; i < n_req; i += kP95Threads) {
+            const size_t o = static_cast<size_t>(i) * n_rep + r;
+            const unsigned long long k = order_key(__dsub_rn(finish[o], arrival[o]));
+            if ((k & mask) == prefix) atomicAdd(&hist[(k >> shift) & 0xFFull], 1u);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned int left = s_rank, b = 0;
+            for (; b < 255u && hist[b] < left; ++b) left -= hist[b];
+            s_rank = left;
+            s_prefix = prefix | (static_cast<unsigned long long>(b) << shift);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const unsigned long long k = s_prefix;
+        const unsigned long long b = (k >> 63) ? (k & 0x7FFFFFFFFFFFFFFFull) : ~k;
+        out_summary[static_cast<size_t>(r) * LASER_SIM_SUMMARY_COLS + 1] = __longlong_as_double(static_cast<long long>(b));
+    }
+}
+
 bool policy_valid(const laser_sim_policy& p) {
     return std::isfinite(p.lambda_base) && std::isfinite(p.beta) && std::isfinite(p.gamma) &&
            std::isfinite(p.l_target) && p.l_target > 0.0 && p.lambda_min <= p.lambda_max &&
@@ -266,10 +320,22 @@ int laser_sim_run(const double* arrival, const int32_t* sample_id, const int32_t
     for (int i = 0; i < n_pol; ++i) q.pol[i] = policies[i];
 
     cudaStream_t stream = static_cast<cudaStream_t>(stream_v);
-    const int blocks = (dims->n_rep + kSimThreads - 1) / kSimThreads;
+    // as few replications per warp as keeps the warp count within 16 warps per SM (measured: 8 and 32 are
+    // slower at 3840 and 30720 replications)
+    int sms = 148;
+    (void)cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int lanes = 1;
+    while (lanes < kSimThreads && (dims->n_rep + lanes - 1) / lanes > 16 * sms) lanes <<= 1;
+    q.lanes = lanes;
+    const int blocks = (dims->n_rep + lanes - 1) / lanes;
     laser_sim_queue_kernel<<<blocks, kSimThreads, 0, stream>>>(q);
     if (cudaGetLastError() != cudaSuccess) return LASER_E_CUDA;
-    if (dims->n_req <= LASER_SIM_MAX_P95_REQUESTS) {
+    if (dims->n_req > LASER_SIM_MAX_P95_REQUESTS) {
+        // too many latencies for shared memory: radix select over global memory, one block per queue
+        laser_sim_p95_select_kernel<<<dims->n_rep, kP95Threads, 0, stream>>>(arrival, out_finish, out_summary,
+                                                                         dims->n_rep, dims->n_req);
+        if (cudaGetLastError() != cudaSuccess) return LASER_E_CUDA;
+    } else {
         int n_pow2 = 1;
         while (n_pow2 < dims->n_req) n_pow2 <<= 1;
         const size_t smem = static_cast<size_t>(n_pow2) * sizeof(double);

@@ -176,3 +176,30 @@ def test_sim_fuzz_random_policies():
             s = oracle.sim_summary(arr[:, r], o["finish"], o["chunks"], 30.0)
             assert np.array_equal(g["summary"][r, [0, 1, 2, 4]], s[[0, 1, 2, 4]])
         assert flips <= 1
+
+
+def test_sim_p95_above_the_shared_memory_sort_and_packed_warps():
+    """More than 8192 requests per queue: P95 comes from the radix select over global memory, and must
+    still be the oracle's nearest-rank element bit for bit.  More replications than warp slots: several
+    replications share a warp (lanes > 1), a sample of them against the oracle."""
+    import oracle
+    pool = wl.sim_pool(S=40, K=6, seed=8)
+    names = list(_policies())
+    pols = [_policies()[n] for n in names]
+    # (a) 9001 and 20000 requests per queue
+    for n_req, n_rep in ((9001, 3), (20000, 2)):
+        arr = wl.sim_arrivals_poisson(n_rep, n_req, 2.0, seed=n_req)
+        sid = wl.sim_sample_ids(n_rep, n_req, 40, seed=n_req + 1)
+        pid = (np.arange(n_rep) % len(pols)).astype(np.int32)
+        g = _run_gpu(arr, sid, pid, pols, pool)
+        assert not np.isnan(g["summary"][:, 1]).any()
+        assert _compare(arr, sid, pid, pols, pool, g) == 0
+    # (b) 10000 replications of 40 requests: eight replications per warp (16 warps per SM at most)
+    n_req, n_rep = 40, 10000
+    arr = wl.sim_arrivals_poisson(n_rep, n_req, 4.0, seed=77)
+    sid = wl.sim_sample_ids(n_rep, n_req, 40, seed=78)
+    pid = (np.arange(n_rep) % len(pols)).astype(np.int32)
+    g = _run_gpu(arr, sid, pid, pols, pool)
+    pick = np.r_[0:40, 4990:5030, 9960:10000]
+    sub = {k: v[:, pick] if v.ndim == 2 and v.shape[1] == n_rep else v[pick] for k, v in g.items()}
+    assert _compare(np.ascontiguousarray(arr[:, pick]), np.ascontiguousarray(sid[:, pick]), pid[pick], pols, pool, sub) == 0
