@@ -80,16 +80,17 @@ typedef struct {
     int32_t work_items;      /* m_tiles * splits                                                      */
     int32_t smem_bytes;      /* dynamic shared memory per CTA                                         */
     int32_t kernel_launches; /* kernels one laser_probe_confidence call enqueues: 1 (a3-a5 run in the
-                                fused kernel's tail) or 2 (LASER_TAIL_SEPARATE)                        */
+                                fused kernel's tail; mixed schedule: 2) or one more (LASER_TAIL_SEPARATE) */
     int32_t tile_m;          /* token rows per work item: 128 (one CTA) or 256 (CTA pair)             */
     int32_t cta_pair;        /* 1: clusters of two CTAs, tcgen05 cta_group::2; 0: one CTA per item    */
     int32_t ws_records;      /* 16-byte workspace records (the most any re-plan of the batch writes)  */
     int32_t tail_cache;      /* requests whose {offset, threshold} the fused kernel's tail keeps in the
                                 shared memory the pipeline leaves over (0: read from global memory)    */
-    /* Mixed schedule (AUTO, N > 128 rows): the fields above describe the CTA-pair kernel (256-row
+    /* Mixed schedule (AUTO, N > 256 rows): the fields above describe the CTA-pair kernel (256-row
      * items); when the number of 128-row tiles that hold rows is odd, the last tile runs on single CTAs
      * in a second kernel beside it.  The split of the SMs is decided on the device from
-     * req_offsets[R].  kernel_launches = 3: tail-tile kernel, pair kernel, finalize kernel. */
+     * req_offsets[R].  kernel_launches = 2: tail-tile kernel, pair kernel (a3-a5 in the tail of
+     * whichever of the two has the work; of the pair kernel when both have). */
     int32_t mixed;           /* 1: mixed schedule                                                     */
     int32_t tail_tile_n;     /* vocab rows per tile of the single-CTA tail-tile kernel                */
     int32_t tail_stages;     /* its pipeline depth                                                    */
@@ -98,16 +99,19 @@ typedef struct {
 } laser_probe_plan;
 
 /* Kernel variant (laser_probe_options.kernel_mode).  AUTO (default): one single-CTA kernel for
- * N <= 128 rows; above that the mixed schedule (CTA pairs for the even part of the 128-row tiles that
- * hold rows, single CTAs for an odd last tile, decided on the device).  SINGLE / PAIR force one
- * variant for every shape (tuning and tests; both are exact; PAIR pads an odd tile count). */
+ * N <= 128 rows; one CTA-pair kernel for 129..256 rows (a single 256-row item whatever req_offsets[R]
+ * says); above that the mixed schedule (CTA pairs for the even part of the 128-row tiles that hold
+ * rows, single CTAs for an odd last tile, decided on the device).  SINGLE / PAIR force one variant for
+ * every shape (tuning and tests; both are exact; PAIR pads an odd tile count). */
 enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2 };
 
 /* Where merge + a3-a5 run (laser_probe_options.tail).
  *   FUSED     in the tail of the fused kernel: every CTA counts itself in when its records are in the
- *             workspace, the first min(grid, R) CTAs wait for the count and share the requests.  One
- *             launch per call.  Needs a control slot of the library's per-device control block.
- *   SEPARATE  a second kernel (laser_probe_finalize_kernel) behind the fused one.  Two launches.
+ *             workspace, the last min(grid, R) CTAs to arrive wait for the count and share the
+ *             requests.  One launch per call (mixed schedule: its two fused kernels; the tail runs in
+ *             the one that has the work, in the pair kernel when both have).  Needs a control slot of
+ *             the library's per-device control block.
+ *   SEPARATE  one more kernel (laser_probe_finalize_kernel) behind the fused one(s).
  *   AUTO      FUSED for strict calls when a control slot is available (the only case where none is:
  *             the very first call on a device is made under CUDA stream capture, where nothing can
  *             be allocated); SEPARATE for overlap = 1 calls (measured faster there: the tiny second

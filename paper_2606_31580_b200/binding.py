@@ -308,8 +308,8 @@ class Probe:
         self.tau = torch.empty(R, dtype=torch.float32, device=self.device) if debug_outputs else None
         self.pmax = torch.empty(N, dtype=torch.float32, device=self.device) if debug_outputs else None
         self.plan = plan_query(N, d, V, R, mode)
-        if not self.plan["mixed"]:
-            self.plan["kernel_launches"] = 2 if (tail == TAIL_SEPARATE or (tail == TAIL_AUTO and overlap)) else 1
+        fused = 2 if self.plan["mixed"] else 1
+        self.plan["kernel_launches"] = fused + (1 if (tail == TAIL_SEPARATE or (tail == TAIL_AUTO and overlap)) else 0)
         self._handles = {}
 
     def _options(self, agg, token_ids) -> Options:

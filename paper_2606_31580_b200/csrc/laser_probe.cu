@@ -259,6 +259,10 @@ void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_pl
     }
     make_variant_plan(dm, num_sms, true, 0, pl);
     if (mode == LASER_MODE_PAIR) return;
+    // 129..256 rows: one 256-row pair item whatever req_offsets[R] says - a static plan (one launch, W
+    // requested ahead of the wait, tail in the kernel).  With <= 128 valid rows half the item is padding,
+    // which costs little: that case is bound by the W stream.
+    if (t128 == 2) return;
     // ---- mixed
     laser_probe_dims d1 = dm;
     d1.N = kTileM;
@@ -273,7 +277,7 @@ void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_pl
     pl->tail_stages = tp.stages;
     pl->tail_smem_bytes = tp.smem_bytes;
     pl->tail_grid = tp.grid;
-    pl->kernel_launches = 3;     // single-CTA kernel, pair kernel, finalize kernel
+    pl->kernel_launches = 2;     // single-CTA kernel, pair kernel (+ finalize kernel: LASER_TAIL_SEPARATE)
     long ws_records = 1;
     for (int m128 = 1; m128 <= t128; ++m128) {
         long rec;
@@ -638,15 +642,6 @@ int launch_validate(const Handle* h, const int32_t* req_offsets, cudaStream_t st
 int want_fused_tail(Handle* h, cudaStream_t stream, bool* fused_tail) {
     *fused_tail = false;
     if (h->opt.tail == LASER_TAIL_SEPARATE) return LASER_OK;
-    if (h->plan.mixed) {
-        // two fused kernels: a tail in one would have to wait for the CTAs of the other, which tools
-        // that serialise kernels (profilers) would turn into a hang.  The merge is the third launch.
-        if (h->opt.tail == LASER_TAIL_FUSED) {
-            g_last_error = "LASER_TAIL_FUSED needs a single fused kernel (N <= 128 rows, or kernel_mode SINGLE / PAIR)";
-            return LASER_E_MODE;
-        }
-        return LASER_OK;
-    }
     // AUTO with overlap: calls chained two deep gate each other's CTAs; the tail CTAs would hold SMs
     // the next call could be streaming on, so the second kernel (co-resident, tiny) is the faster form
     if (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap) return LASER_OK;
@@ -1052,7 +1047,7 @@ int laser_probe_handle_create(laser_probe_handle** out, const laser_probe_dims* 
     Handle* h = nullptr;
     rc = make_handle(*dims, opt, &h);
     if (rc != LASER_OK) return rc;
-    if (opt.tail != LASER_TAIL_SEPARATE && !h->plan.mixed)
+    if (opt.tail != LASER_TAIL_SEPARATE)
         h->ctl = acquire_ctl(h->di, nullptr);   // may stay NULL: retried per call
     *out = h;
     return LASER_OK;
@@ -1066,9 +1061,9 @@ int laser_probe_handle_destroy(laser_probe_handle* h) {
 int laser_probe_handle_plan(const laser_probe_handle* h, laser_probe_plan* plan) {
     if (!h || !plan) return LASER_E_NULL;
     *plan = h->plan;
-    if (!h->plan.mixed)
-        plan->kernel_launches = (h->opt.tail == LASER_TAIL_SEPARATE || !h->ctl ||
-                                 (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap)) ? 2 : 1;
+    const int fused = h->plan.mixed ? 2 : 1;    // fused kernels per call
+    plan->kernel_launches = (h->opt.tail == LASER_TAIL_SEPARATE || !h->ctl ||
+                             (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap)) ? fused + 1 : fused;
     return LASER_OK;
 }
 

@@ -178,7 +178,7 @@ struct FusedParams {
     // launch_dependents), 1 = the pair kernel behind it (never waits before it has counted itself in:
     // kernel 2 may be waiting for its arrivals).
     int32_t role;
-    int32_t grid_total;    // CTAs of all fused kernels of the call: what the tail's arrival count waits for
+    int32_t grid_total;    // one fused kernel: its CTAs, what the tail's arrival count waits for (mixed: TailRole)
     // 1 (strict, default): griddepcontrol.wait before the first read of hidden / req_offsets /
     //    token_ids; W - model weight, never written by the kernel ahead - is requested for the first
     //    `stages` pipeline slots before the wait when the plan is static (pd.kind == 0).
@@ -655,6 +655,110 @@ struct TailParams {
     ReduceParams q;
 };
 
+// Who takes part in a call's tail (decided per kernel, uniformly over its CTAs).
+//   count_total  CTAs (of all fused kernels of the call) that count themselves in: the arrival target
+//   fin_mode     0: the LAST F arrivals finalize (they have the least to wait for; fixed finalizers would
+//                   spin for tens of microseconds in overlap mode);  1: CTAs [0, F) of this kernel
+//                   finalize;  2: this kernel's CTAs only count themselves in;  -1: no tail here
+//   part         CTAs of this kernel that take part (blockIdx.x < part): bounds F, strides the padding rows
+struct TailRole {
+    int count_total, fin_mode, part;
+};
+// Mixed schedule (pd.kind 2): only CTAs with work count.  Pair items only / single-CTA tiles only: the
+// kernel that has the work runs the whole tail like a call with one fused kernel, the other stays out
+// of it.  Both parts busy: the busy CTAs of both kernels count themselves in and the first F busy CTAs
+// of the PAIR kernel finalize - it is launched behind the single-CTA kernel, so every CTA it waits
+// for is resident or done (a dependent grid starts only when all CTAs of the grid ahead have
+// started), while the single-CTA kernel never waits for anything launched after it: a tool that
+// serialises the two kernels only costs time.  No row at all (req_offsets[R] == 0): every CTA of the
+// pair kernel takes part, so that conf = 0 / exit = 0 / the padding marks are written.
+__device__ __forceinline__ TailRole mixed_tail_role(const MixedPlan& mp, int role, int grid) {
+    const int busy_pair = mp.k_pair > 0 ? 2 * mp.u_pair : 0;
+    const int busy_single = mp.j_single > 0 ? mp.u_tail : 0;
+    if (busy_pair + busy_single == 0) return role == 1 ? TailRole{grid, 0, grid} : TailRole{0, -1, 0};
+    if (busy_single == 0) return role == 1 ? TailRole{busy_pair, 0, busy_pair} : TailRole{0, -1, 0};
+    if (busy_pair == 0) return role == 2 ? TailRole{busy_single, 0, busy_single} : TailRole{0, -1, 0};
+    return role == 1 ? TailRole{busy_pair + busy_single, 1, busy_pair} : TailRole{busy_pair + busy_single, 2, busy_single};
+}
+
+// The tail, run by the four epilogue warps (threads [kTailThread0, kTailThread0 + 128)) of every CTA
+// that takes part (TailRole) once the CTA's records - if it had any to write - are stored: the CTA
+// counts itself in, and the CTAs chosen as finalizers wait for the count to reach base + count_total
+// and run merge + a3-a5 (kind 1) or the shard reduce (kind 2).
+// base: ctl[1] as read by thread kTailThread0 when base_known (the call ahead, which may share the slot,
+// had completed); otherwise it is read here.  cached: off_c / tau_c hold {req_offsets, tau} of every request.
+__device__ __forceinline__ void fused_tail(const FusedParams& p, const TailParams& t, const RunPlan& rp,
+                                           const TailRole tr, uint32_t base, bool base_known, bool cached,
+                                           const int* off_c, const float* tau_c, float* warp_acc) {
+    if (tr.fin_mode < 0 || static_cast<int>(blockIdx.x) >= tr.part) return;
+    if (p.role != 1) ptx::pdl_wait();   // outputs are written below (a CTA without work items has not waited yet)
+    const int tid = threadIdx.x - kTailThread0, tw = tid >> 5;
+    constexpr int kTW = kEpilogueThreads / 32;
+    const FinalizeParams& f = t.q.f;
+    const int F = (t.kind == 1) ? min(tr.part, f.R) : min(tr.part, (f.n_alloc + kTW - 1) / kTW);
+    // scratch: bytes [192, 232) of the barrier block
+    volatile uint32_t* tk = reinterpret_cast<volatile uint32_t*>(warp_acc + kMaxTailWarps);
+    group_sync<1, kEpilogueThreads>();   // every record store of this CTA is ordered before the count
+    if (tid == 0) {
+        if (!base_known) base = ptx::ld_relaxed_gpu_u32(t.ctl + 1);   // overlap: the call ahead is complete only now
+        const uint32_t target = base + static_cast<uint32_t>(tr.count_total);
+        LASER_TL(t.tl_slot, 4, kTailThread0);
+        const uint32_t mine = ptx::atom_add_acq_rel_gpu_u32(t.ctl, 1u) + 1u;
+        if (mine == target) t.ctl[1] = target;   // last arrival: every CTA that counts has read `base`
+        tk[0] = mine; tk[1] = target;
+    }
+    if (tr.fin_mode == 2) return;        // counted in, nothing else
+    group_sync<1, kEpilogueThreads>();
+    const uint32_t mine = tk[0], target = tk[1];
+    const int behind = static_cast<int>(target - mine);    // CTAs still to arrive
+    int fi;             // finalizer index 0 .. F-1, or -1
+    if (tr.fin_mode == 1) fi = static_cast<int>(blockIdx.x) < F ? static_cast<int>(blockIdx.x) : -1;
+    else fi = behind < F ? F - 1 - behind : -1;     // the last arrival is F-1
+    const int pad_first = blockIdx.x * kEpilogueThreads + tid, pad_step = tr.part * kEpilogueThreads;
+    if (fi < 0) {
+        // not a finalizer: padding rows do not depend on anybody's records
+        if (t.kind == 1) mark_padding_rows(f, pad_first, pad_step);
+        return;
+    }
+    if (behind > 0) {
+        if ((tid & 31) == 0) {
+            const long long t0 = clock64();
+            while (static_cast<int32_t>(ptx::ld_acquire_gpu_u32(t.ctl) - target) < 0) {
+                // every CTA that counts is resident or becomes resident as others exit (grid <= SMs);
+                // a wait of seconds means the device cannot hold the grid: trap
+                if (clock64() - t0 > 8000000000LL) __trap();
+            }
+        }
+        __syncwarp();
+    }   // (the last arrival's own acq_rel count has acquired everybody's records)
+    LASER_TL(t.tl_slot, 5, kTailThread0);
+    if (t.kind == 1) {
+        for (int r = fi; r < f.R; r += F) {
+            const int rb = cached ? off_c[r] : __ldg(f.req_offsets + r);
+            const int re = cached ? off_c[r + 1] : __ldg(f.req_offsets + r + 1);
+            float tau = 0.f;
+            if (tid == kFinalThread) tau = cached ? tau_c[r] : tau_eval(__ldg(f.load + r), f.tau);
+            finalize_request<1, kEpilogueThreads>(f, tid, r, rb, re, tau, rp.lay, warp_acc);
+            if (r == fi) LASER_TL(t.tl_slot, 6, kTailThread0);
+        }
+        mark_padding_rows(f, pad_first, pad_step);
+    } else {
+        const int n_valid = (f.R > 0) ? min(max(__ldg(f.req_offsets + f.R), 0), f.n_alloc) : 0;
+        for (int n = fi * kTW + tw; n < f.n_alloc; n += F * kTW) reduce_row(t.q, n, n_valid, rp.lay, tid & 31);
+        __threadfence_system();   // remote (peer) stores of this thread are performed before the count below
+        group_sync<1, kEpilogueThreads>();
+        if (tid < 32) {
+            uint32_t last = 0;
+            if (tid == 0) {
+                last = (ptx::atom_add_acq_rel_gpu_u32(t.ctl + 2, 1u) == static_cast<uint32_t>(F - 1)) ? 1u : 0u;
+                if (last) t.ctl[2] = 0u;
+            }
+            last = __shfl_sync(0xffffffffu, last, 0);
+            if (last) publish_epoch(t.q, tid);   // every tail CTA's rows are on every GPU
+        }
+    }
+}
+
 // kPair = false: one CTA per SM, tcgen05 cta_group::1, a work item is (128 token rows, vocab split).
 // kPair = true : clusters of two CTAs (the two SMs of a TPC), tcgen05 cta_group::2: one M = 256 MMA
 //                spans both CTAs.  A work item is (256 token rows, vocab split); CTA `rank` of the pair
@@ -702,6 +806,7 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     int64_t rec0 = 0;      // first workspace record of this kernel's region
     const bool static_plan = p.pd.kind == 0;
     RunPlan rp{};
+    TailRole tr{p.grid_total, 0, static_cast<int>(gridDim.x)};   // one fused kernel: every CTA takes part
     if (p.pd.kind == 2) {
         // Mixed schedule: which part takes what is looked up before anything is set up, so that the
         // CTAs a part does not need (all of them, for the single-CTA kernel of an even dense batch)
@@ -717,10 +822,16 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
             row0 = 2 * kTileM * rp.mp.k_pair;
             rec0 = static_cast<int64_t>(row0) * rp.mp.S_pair;
         }
+        tr = mixed_tail_role(rp.mp, p.role, gridDim.x);
         if (m_items == 0 || unit >= units_run) {
-            // nothing for this CTA.  It still completes only after the kernel ahead of it has (the
-            // merge kernel behind the pair kernel relies on that to see the single-CTA kernel's records)
+            // nothing to compute for this CTA.  It takes part in a fused tail only when no CTA of the
+            // call has anything to compute (mixed_tail_role), and it completes only after the kernel
+            // ahead of it has (completion of the pair kernel then implies completion of the whole call).
             if (p.role != 2) ptx::pdl_launch_dependents();
+            if (t.kind != 0 && warp >= 2) {
+                float* scratch = reinterpret_cast<float*>(smem_raw + (smem - raw) + p.stages * p.stage_bytes + 192u);
+                fused_tail(p, t, rp, tr, 0u, false, false, nullptr, nullptr, scratch);
+            }
             ptx::pdl_wait();
             return;
         }
@@ -980,70 +1091,8 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         // and MMA warps go straight to the teardown - and the LAST F CTAs to arrive run merge + a3-a5
         // (kind 1) or the shard reduce (kind 2): they are the ones with the least to wait for.
         if (t.kind != 0) {
-            if (p.role != 1) ptx::pdl_wait();   // outputs are written below (a CTA without work items has not waited yet)
-            const int tid = threadIdx.x - kTailThread0, tw = tid >> 5;
-            constexpr int kTW = kEpilogueThreads / 32;
-            const FinalizeParams& f = t.q.f;
-            const int grid = p.grid_total;
-            const int F = (t.kind == 1) ? min(grid, f.R) : min(grid, (f.n_alloc + kTW - 1) / kTW);
-            // scratch: bytes [192, 232) of the barrier block
-            float* warp_acc = reinterpret_cast<float*>(smem_raw + (smem - raw) + p.stages * p.stage_bytes + 192u);
-            volatile uint32_t* tk = reinterpret_cast<volatile uint32_t*>(warp_acc + kMaxTailWarps);
-            group_sync<1, kEpilogueThreads>();   // every record store of this CTA is ordered before the count
-            if (tid == 0) {
-                if (!base_early) base = ptx::ld_relaxed_gpu_u32(t.ctl + 1);   // overlap: the call ahead is complete only now
-                const uint32_t target = base + static_cast<uint32_t>(grid);
-                LASER_TL(t.tl_slot, 4, kTailThread0);
-                const uint32_t mine = ptx::atom_add_acq_rel_gpu_u32(t.ctl, 1u) + 1u;
-                if (mine == target) t.ctl[1] = target;   // last arrival: every CTA has read `base`
-                tk[0] = mine; tk[1] = target;
-            }
-            group_sync<1, kEpilogueThreads>();
-            const uint32_t mine = tk[0], target = tk[1];
-            const int behind = static_cast<int>(target - mine);    // CTAs still to arrive
-            if (behind >= F) {
-                // not one of the last F: padding rows do not depend on anybody's records
-                if (t.kind == 1) mark_padding_rows(f, blockIdx.x * kEpilogueThreads + tid, gridDim.x * kEpilogueThreads);
-            } else {
-                const int fi = F - 1 - behind;    // 0 .. F-1; the last arrival is F-1
-                if (behind > 0) {
-                    if ((tid & 31) == 0) {
-                        const long long t0 = clock64();
-                        while (static_cast<int32_t>(ptx::ld_acquire_gpu_u32(t.ctl) - target) < 0) {
-                            // all CTAs of this grid are resident or become resident as others exit (grid
-                            // <= SMs); a wait of seconds means the device cannot hold the grid: trap
-                            if (clock64() - t0 > 8000000000LL) __trap();
-                        }
-                    }
-                    __syncwarp();
-                }   // (the last arrival's own acq_rel count has acquired everybody's records)
-                LASER_TL(t.tl_slot, 5, kTailThread0);
-                if (t.kind == 1) {
-                    for (int r = fi; r < f.R; r += F) {
-                        const int rb = cached ? off_c[r] : __ldg(f.req_offsets + r);
-                        const int re = cached ? off_c[r + 1] : __ldg(f.req_offsets + r + 1);
-                        float tau = 0.f;
-                        if (tid == kFinalThread) tau = cached ? tau_c[r] : tau_eval(__ldg(f.load + r), f.tau);
-                        finalize_request<1, kEpilogueThreads>(f, tid, r, rb, re, tau, rp.lay, warp_acc);
-                        if (r == fi) LASER_TL(t.tl_slot, 6, kTailThread0);
-                    }
-                    mark_padding_rows(f, blockIdx.x * kEpilogueThreads + tid, gridDim.x * kEpilogueThreads);
-                } else {
-                    const int n_valid = (f.R > 0) ? min(max(__ldg(f.req_offsets + f.R), 0), f.n_alloc) : 0;
-                    for (int n = fi * kTW + tw; n < f.n_alloc; n += F * kTW) reduce_row(t.q, n, n_valid, rp.lay, tid & 31);
-                    __threadfence_system();   // remote (peer) stores of this thread are performed before the count below
-                    group_sync<1, kEpilogueThreads>();
-                    if (tid < 32) {
-                        uint32_t last = 0;
-                        if (tid == 0) {
-                            last = (ptx::atom_add_acq_rel_gpu_u32(t.ctl + 2, 1u) == static_cast<uint32_t>(F - 1)) ? 1u : 0u;
-                            if (last) t.ctl[2] = 0u;
-                        }
-                        last = __shfl_sync(0xffffffffu, last, 0);
-                        if (last) publish_epoch(t.q, tid);   // every tail CTA's rows are on every GPU
-                    }
-                }
-            }
+            float* scratch = reinterpret_cast<float*>(smem_raw + (smem - raw) + p.stages * p.stage_bytes + 192u);
+            fused_tail(p, t, rp, tr, base, base_early, cached, off_c, tau_c, scratch);
         }
     }
 

@@ -56,10 +56,10 @@ def test_plan_invariants(dims):
     pair, tm = p["cta_pair"], p["tile_m"]
     t128 = -(-N // 128)
     mixed = p["mixed"]
-    # AUTO: one single-CTA kernel up to 128 rows, above that the mixed schedule (pair kernel + single-CTA
-    # tail-tile kernel + finalize kernel)
-    assert (pair, mixed) == ((0, 0) if t128 <= 1 else (1, 1)) and tm == (256 if pair else 128)
-    assert p["kernel_launches"] == (3 if mixed else 1)
+    # AUTO: one single-CTA kernel up to 128 rows, one CTA-pair kernel up to 256, above that the mixed
+    # schedule (single-CTA tail-tile kernel + pair kernel, the tail in whichever has the work)
+    assert (pair, mixed) == ((0, 0) if t128 <= 1 else ((1, 0) if t128 == 2 else (1, 1))) and tm == (256 if pair else 128)
+    assert p["kernel_launches"] == (2 if mixed else 1)
     assert bn % (32 if pair else 16) == 0 and 16 <= bn <= 256
     assert S * T * bn >= V and (S - 1) * T * bn < V          # splits tile the vocabulary exactly once
     assert p["m_tiles"] == max(1, -(-N // tm)) and p["k_blocks"] == -(-d // 64)

@@ -232,7 +232,7 @@ def test_mixed_schedule_odd_tile_counts(P, path, R, L, var_len, n_alloc):
     Requests that straddle the two parts are merged from both kernels' records."""
     w = wl.scaled(f"mixed-R{R}-L{L}-N{n_alloc}", 33000, 512, 0.05, R, L, seed=R + 31, N_alloc=n_alloc, var_len=var_len)
     st = P.check(w)
-    assert st["plan"]["mixed"] == 1 and st["plan"]["kernel_launches"] == 3
+    assert st["plan"]["mixed"] == 1 and st["plan"]["kernel_launches"] == (3 if path == "separate-handle" else 2)
     _log(f"{w.name}/{path}", st)
 
 
@@ -340,7 +340,7 @@ def test_ties_across_tile_and_split_boundaries(P):
         P.compare(w, g, ora, rows, reqs, "ties")
 
 
-@pytest.mark.parametrize("tail,mode", [(1, 1), (1, 2), (2, 0), (0, 0)])   # fused tail on either variant / separate / mixed
+@pytest.mark.parametrize("tail,mode", [(1, 1), (1, 2), (2, 0), (0, 0), (1, 0)])   # fused tail on either variant / mixed: separate, auto, fused
 @pytest.mark.parametrize("overlap", [True, False])
 def test_back_to_back_calls_share_a_workspace(P, overlap, tail, mode):
     """Stream order under programmatic dependent launch: calls enqueued back to back on one stream,
@@ -366,7 +366,9 @@ def test_back_to_back_calls_share_a_workspace(P, overlap, tail, mode):
         dv = devs[k % 2]
         p(dv["hidden"], dv["W"], dv["off"], dv["load"], tp)
     assert B.kernel_launch_count() - n0 == K * probes[0].plan["kernel_launches"]
-    assert probes[0].plan["kernel_launches"] == (3 if mode == 0 else (2 if tail == 2 else 1))
+    # N = 384 rows: AUTO is the mixed schedule (two fused kernels); the merge is one more launch when it
+    # is asked for (tail 2) or when AUTO avoids the fused tail (overlap)
+    assert probes[0].plan["kernel_launches"] == (2 if mode == 0 else 1) + (1 if (tail == 2 or (tail == 0 and overlap)) else 0)
     torch.cuda.synchronize()
     for k, p in enumerate(probes):
         g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),

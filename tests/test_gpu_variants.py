@@ -192,7 +192,7 @@ def test_vocab_parallel_matches_oracle(P, G, peer, tail, V, d, R, L, n_alloc, va
     g, stats = _run_vocab_parallel(P, w, G, peer=peer, tail=tail)
     mixed = B.plan_query(w.N_alloc, d, par.shard_vocab(V, G, 0)[1], R)["mixed"]
     fused = 2 if mixed else 1                                           # fused kernels of one partial
-    per_partial = fused if (tail == 0 and not mixed) else fused + (2 if peer else 1)
+    per_partial = fused if tail == 0 else fused + (2 if peer else 1)    # the tail also runs in the mixed schedule's kernels
     assert B.kernel_launch_count() - n0 == G * per_partial + 1          # + the combine kernel
     ora, rows, reqs = P.run_oracle(w)
     st = P.compare(w, g, ora, rows, reqs, w.name)
