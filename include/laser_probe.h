@@ -96,6 +96,15 @@ typedef struct {
     int32_t tail_stages;     /* its pipeline depth                                                    */
     int32_t tail_smem_bytes; /* its dynamic shared memory per CTA                                     */
     int32_t tail_grid;       /* its CTAs (those it does not need exit at once)                        */
+    /* Flex kernel (LASER_MODE_FLEX; AUTO for 129 <= N <= 4096 rows where the planner's cost model
+     * prefers it): vocabulary on the MMA M axis (tile_n = 256 rows of W per CTA pair), tokens on N in
+     * chunks of flex_n_tok rows (a multiple of 16, <= 256), so that a batch pays for at most 15 padding
+     * rows per chunk.  m_tiles = chunks, splits / tiles_per_split per chunk, all for a batch whose N
+     * rows are valid; the kernel looks the decomposition for req_offsets[R] up in a table the host
+     * planned (laser_probe_flex_query).  One launch per call. */
+    int32_t flex;            /* 1: flex kernel                                                        */
+    int32_t flex_n_tok;      /* token rows per chunk for a dense batch                                */
+    int32_t flex_max_tok;    /* the largest chunk any valid-row count takes (sizes the pipeline stage) */
 } laser_probe_plan;
 
 /* Kernel variant (laser_probe_options.kernel_mode).  AUTO (default): one single-CTA kernel for
@@ -103,7 +112,7 @@ typedef struct {
  * says); above that the mixed schedule (CTA pairs for the even part of the 128-row tiles that hold
  * rows, single CTAs for an odd last tile, decided on the device).  SINGLE / PAIR force one variant for
  * every shape (tuning and tests; both are exact; PAIR pads an odd tile count). */
-enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2 };
+enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2, LASER_MODE_FLEX = 3 };
 
 /* Where merge + a3-a5 run (laser_probe_options.tail).
  *   FUSED     in the tail of the fused kernel: every CTA counts itself in when its records are in the
@@ -164,6 +173,18 @@ typedef struct {
     float model_us;         /* the planner's cost-model estimate of the fused kernels, microseconds   */
 } laser_probe_mixed;
 int laser_probe_mixed_query(const laser_probe_dims* dims, int32_t n_valid, laser_probe_mixed* out);
+
+/* What the flex kernel does for n_valid (<= 4096) valid rows at vocabulary size dims->V: the entry of
+ * its device-side table.  Informational; host; needs no GPU. */
+typedef struct {
+    int32_t chunks;         /* token chunks C                                                         */
+    int32_t n_tok;          /* token rows per chunk (multiple of 16)                                  */
+    int32_t splits;         /* vocabulary splits per chunk S (a row gets 2 S workspace records)       */
+    int32_t tiles_per_split;/* 256-row vocabulary tiles per split                                     */
+    int32_t rounds;         /* work items the busiest CTA pair takes                                  */
+    float model_cost;       /* the planner's relative cost (rounds x tiles x per-tile cost)           */
+} laser_probe_flex;
+int laser_probe_flex_query(const laser_probe_dims* dims, int32_t n_valid, laser_probe_flex* out);
 
 /*
  * The hot path a1-a5.  Asynchronous on `stream`; returns after enqueueing.

@@ -16,7 +16,7 @@ _lib = None
 
 AGG_MEAN, AGG_GEOMEAN, AGG_MIN = 0, 1, 2
 PROB_MAX, PROB_TOKEN = 0, 1
-MODE_AUTO, MODE_SINGLE, MODE_PAIR = 0, 1, 2
+MODE_AUTO, MODE_SINGLE, MODE_PAIR, MODE_FLEX = 0, 1, 2, 3
 TAIL_AUTO, TAIL_FUSED, TAIL_SEPARATE = 0, 1, 2
 
 EXPORTS = [
@@ -27,7 +27,7 @@ EXPORTS = [
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
     "laser_profile_read", "laser_probe_options_default", "laser_probe_plan_query_mode",
     "laser_probe_confidence_opt", "laser_probe_partial", "laser_probe_combine",
-    "laser_probe_mixed_query", "laser_probe_handle_create", "laser_probe_handle_destroy", "laser_probe_handle_plan",
+    "laser_probe_mixed_query", "laser_probe_flex_query", "laser_probe_handle_create", "laser_probe_handle_destroy", "laser_probe_handle_plan",
     "laser_probe_handle_workspace_bytes", "laser_probe_handle_run", "laser_probe_handle_run_host",
     "laser_sim_policy_default", "laser_sim_run",
 ]
@@ -61,7 +61,8 @@ class Plan(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("num_sms", "m_tiles", "splits", "tiles_per_split", "tile_n", "k_blocks", "stages",
                  "grid", "work_items", "smem_bytes", "kernel_launches", "tile_m", "cta_pair", "ws_records", "tail_cache",
-                 "mixed", "tail_tile_n", "tail_stages", "tail_smem_bytes", "tail_grid")]
+                 "mixed", "tail_tile_n", "tail_stages", "tail_smem_bytes", "tail_grid",
+                 "flex", "flex_n_tok", "flex_max_tok")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -71,6 +72,12 @@ class Mixed(C.Structure):
     """laser_probe_mixed: what the mixed schedule does for n_valid rows (laser_probe_mixed_query)."""
     _fields_ = [(n, C.c_int32) for n in ("mixed", "schedule", "k_pair", "j_single", "u_pair", "u_single",
                                          "splits_pair", "splits_single")] + [("model_us", C.c_float)]
+
+
+class Flex(C.Structure):
+    """laser_probe_flex: what the flex kernel does for n_valid rows (laser_probe_flex_query)."""
+    _fields_ = [(n, C.c_int32) for n in ("chunks", "n_tok", "splits", "tiles_per_split", "rounds")] + \
+               [("model_cost", C.c_float)]
 
 
 class Options(C.Structure):
@@ -138,6 +145,7 @@ def lib():
         L.laser_probe_plan_query_mode.argtypes = [dp, C.c_int, C.POINTER(Plan)]
         L.laser_probe_options_default.argtypes = [C.POINTER(Options)]
         L.laser_probe_mixed_query.argtypes = [dp, C.c_int32, C.POINTER(Mixed)]
+        L.laser_probe_flex_query.argtypes = [dp, C.c_int32, C.POINTER(Flex)]
         L.laser_probe_handle_create.argtypes = [C.POINTER(C.c_void_p), dp, C.POINTER(Options)]
         L.laser_probe_handle_destroy.argtypes = [vp]
         L.laser_probe_handle_plan.argtypes = [vp, C.POINTER(Plan)]
@@ -192,6 +200,12 @@ def plan_query(N, d, V, R, mode=MODE_AUTO) -> dict:
 def mixed_query(N, d, V, R, n_valid) -> dict:
     m = Mixed()
     _check(lib().laser_probe_mixed_query(C.byref(Dims(N, d, V, R)), int(n_valid), C.byref(m)))
+    return {n: getattr(m, n) for n, _ in m._fields_}
+
+
+def flex_query(N, d, V, R, n_valid) -> dict:
+    m = Flex()
+    _check(lib().laser_probe_flex_query(C.byref(Dims(N, d, V, R)), int(n_valid), C.byref(m)))
     return {n: getattr(m, n) for n, _ in m._fields_}
 
 

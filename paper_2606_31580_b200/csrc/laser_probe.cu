@@ -20,6 +20,7 @@
 #include <vector>
 
 #include "probe_kernels.cuh"
+#include "flex_kernel.cuh"
 
 namespace {
 
@@ -246,6 +247,99 @@ MixedChoice plan_mixed_host(int m128, int V, int d, int bn_pair, int bn_tail, in
     return best;
 }
 
+// ---- flex kernel (flex_kernel.cuh): C chunks of n_tok token rows (multiple of 16, <= 256) x S vocabulary
+// splits of 256-row tiles on the CTA pairs.  Cost of a (tile, chunk): the MMAs take time in proportion to
+// n_tok; staging the 256 W rows, the pipeline bubble between tiles and the epilogue's fixed part are charged
+// as kFlexTileCharge token rows.  Among the chunk counts that cover the rows the cheapest busiest pair wins.
+struct FlexChoice { int C, n_tok, S, T, rounds; double cost; };
+double flex_tile_charge() {
+    static const double v = [] {
+        const char* e = getenv("LASER_FLEX_TILE_CHARGE");
+        return e ? atof(e) : 40.0;
+    }();
+    return v;
+}
+FlexChoice plan_flex_host(int n_valid, int V, int sms) {
+    const int pairs = sms / 2 > 0 ? sms / 2 : 1;
+    const int tiles = ceil_div(V, kFlexVocabTile);
+    FlexChoice best{0, 16, 1, tiles, 0, 1e300};
+    if (n_valid <= 0) { best.cost = 0.0; return best; }
+    const int c_min = ceil_div(n_valid, kFlexMaxTok);
+    for (int C = c_min; C <= c_min + 3 && C <= 31; ++C) {
+        const int n_tok = round_up(ceil_div(n_valid, C), 16);
+        if (n_tok > kFlexMaxTok) continue;
+        // splits in multiples of the smallest count that fills the pairs in whole rounds: every pair
+        // streams W (the tiles of a split are dealt round-robin, so splits differ by at most one tile)
+        const int s_unit = pairs / gcd_i(pairs, C);
+        for (int k = 1; k <= 4; ++k) {
+            int S = s_unit * k;
+            if (S > tiles) { if (k > 1) break; S = tiles; }     // tiny vocabularies: a tile per split
+            const int T = ceil_div(tiles, S);
+            const long rounds = (static_cast<long>(C) * S + pairs - 1) / pairs;
+            // the busiest pair, exactly: pair u takes items u, u + pairs, ...; item w is split w / C
+            long busiest = 0;
+            for (int u = 0; u < pairs && u < C * S; ++u) {
+                long tl = 0;
+                for (int w = u; w < C * S; w += pairs) {
+                    const int sp = w / C;
+                    tl += sp < tiles ? (tiles - sp + S - 1) / S : 0;
+                }
+                if (tl > busiest) busiest = tl;
+            }
+            const double cost = static_cast<double>(busiest) * (n_tok + flex_tile_charge()) + 8.0 * rounds;
+            if (cost < best.cost - 1e-9) best = FlexChoice{C, n_tok, S, T, static_cast<int>(rounds), cost};
+        }
+    }
+    return best;
+}
+
+// Plan of the flex kernel for dims (N <= kFlexMaxRows) and its table: entry [g - 1] for g 16-row groups.
+void make_flex_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* pl, uint32_t* tab) {
+    memset(pl, 0, sizeof *pl);
+    const int groups = ceil_div(dm.N, 16);
+    int max_tok = 16;
+    long ws_records = 1;
+    FlexChoice dense{0, 16, 1, 1, 0, 0.0};
+    for (int g = 1; g <= kMixedTabMax; ++g) {
+        const int gg = g <= groups ? g : (groups > 0 ? groups : 1);
+        const int n_valid = gg * 16 < dm.N ? gg * 16 : (dm.N > 0 ? dm.N : 16);
+        const FlexChoice c = plan_flex_host(n_valid, dm.V, num_sms);
+        if (tab) tab[g - 1] = flex_pack(c.C, c.n_tok, c.S);
+        if (g > groups && groups > 0) continue;
+        if (c.n_tok > max_tok) max_tok = c.n_tok;
+        long rows = static_cast<long>(c.C) * c.n_tok;
+        if (rows > dm.N) rows = dm.N;
+        const long rec = rows * 2L * c.S;
+        if (rec > ws_records) ws_records = rec;
+        if (g == groups) dense = c;
+    }
+    pl->num_sms = num_sms;
+    pl->m_tiles = dense.C > 0 ? dense.C : 1;
+    pl->splits = dense.S;
+    pl->tiles_per_split = dense.T;
+    pl->tile_n = kFlexVocabTile;
+    pl->k_blocks = ceil_div(dm.d, kBlockK);
+    const int stage_bytes = kABytes + (max_tok / 2) * 128;
+    int stages = (kMaxDynSmem - kSmemSlack - kFlexXposeBytes) / stage_bytes;
+    if (stages > kMaxStages) stages = kMaxStages;
+    pl->stages = stages;
+    pl->work_items = pl->m_tiles * pl->splits;
+    pl->grid = 2 * (num_sms / 2 > 0 ? num_sms / 2 : 1);
+    const int spare = kMaxDynSmem - (stages * stage_bytes + kSmemSlack + kFlexXposeBytes);
+    int cache = spare / 8 - 1;
+    if (cache > kTailCache) cache = kTailCache;
+    if (cache < 0) cache = 0;
+    pl->tail_cache = cache;
+    pl->smem_bytes = stages * stage_bytes + kSmemSlack + kFlexXposeBytes + (cache > 0 ? 8 * (cache + 1) : 0);
+    pl->kernel_launches = 1;
+    pl->tile_m = dense.n_tok;
+    pl->cta_pair = 1;
+    pl->ws_records = static_cast<int32_t>(ws_records);
+    pl->flex = 1;
+    pl->flex_n_tok = dense.n_tok;
+    pl->flex_max_tok = max_tok;
+}
+
 // AUTO: one single-CTA kernel for N <= 128 rows; above that the mixed schedule (probe_kernels.cuh):
 // 256-row items on CTA pairs and / or 128-row tiles on single CTAs - which, is looked up on the device
 // from the number of 128-row tiles that hold rows (req_offsets[R]), so a padded batch pays for the
@@ -253,6 +347,11 @@ MixedChoice plan_mixed_host(int m128, int V, int d, int bn_pair, int bn_tail, in
 // SINGLE / PAIR force one variant (an odd tile count then costs the pair kernel a padding tile).
 void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_plan* pl, laser_probe_plan* tail_pl) {
     const int t128 = ceil_div(dm.N, kTileM);
+    if (mode == LASER_MODE_FLEX && dm.N > 0 && dm.N <= kFlexMaxRows) {
+        make_flex_plan(dm, num_sms, pl, nullptr);
+        return;
+    }
+    if (mode == LASER_MODE_FLEX) mode = LASER_MODE_AUTO;     // outside the table's range
     if (mode == LASER_MODE_SINGLE || (mode == LASER_MODE_AUTO && t128 <= 1)) {
         make_variant_plan(dm, num_sms, false, 0, pl);
         return;
@@ -385,7 +484,7 @@ const laser_probe_options kDefaultOptions{LASER_AGG_MEAN, LASER_PROB_MAX, nullpt
 int options_valid(const laser_probe_options& o) {
     if (o.aggregate_mode < LASER_AGG_MEAN || o.aggregate_mode > LASER_AGG_MIN) return LASER_E_MODE;
     if (o.prob_mode < LASER_PROB_MAX || o.prob_mode > LASER_PROB_TOKEN) return LASER_E_MODE;
-    if (o.kernel_mode < LASER_MODE_AUTO || o.kernel_mode > LASER_MODE_PAIR) return LASER_E_MODE;
+    if (o.kernel_mode < LASER_MODE_AUTO || o.kernel_mode > LASER_MODE_FLEX) return LASER_E_MODE;
     if (o.tail < LASER_TAIL_AUTO || o.tail > LASER_TAIL_SEPARATE) return LASER_E_MODE;
     if (o.overlap != 0 && o.overlap != 1) return LASER_E_MODE;
     if (o.reserved != 0) return LASER_E_MODE;
@@ -423,6 +522,10 @@ struct laser_probe_handle_s {
     struct MapEntry { const void* ptr = nullptr; int box_rows = 0; CUtensorMap map; };
     MapEntry hid[2], w[4];
     int hid_rr = 0, w_rr = 0;
+    // flex kernel: one hidden map per chunk height (box of 8, 16, ..., 128 token rows), per hidden buffer
+    struct FlexEntry { const void* ptr = nullptr; FlexMaps maps; };
+    FlexEntry flex_hid[2];
+    int flex_rr = 0;
     struct HostMap { const void* h = nullptr; void* d = nullptr; };
     HostMap hm[8];
     int hm_rr = 0;
@@ -458,6 +561,7 @@ int make_handle(const laser_probe_dims& dims, const laser_probe_options& opt, Ha
     h->di = di;
     make_plan(dims, di->sms, opt.kernel_mode, &h->plan, &h->tail_plan);
     if (h->plan.mixed) fill_mixed_table(dims, h->plan, di->sms, h->mixed_tab);
+    if (h->plan.flex) make_flex_plan(dims, di->sms, &h->plan, h->mixed_tab);
     const char* dbg = getenv("LASER_DEBUG");
     h->debug = dbg && dbg[0] && dbg[0] != '0';
     *out = h;
@@ -478,7 +582,8 @@ PlanDesc plan_desc(const Handle* h, const int32_t* req_offsets) {
     d.m_tiles = pl.m_tiles; d.rows_per_item = pl.tile_m; d.splits = pl.splits;
     d.total_tiles = ceil_div(h->dims.V, pl.tile_n);
     d.units = units_for(h->di, pl.cta_pair != 0);
-    d.kind = pl.mixed ? 2 : (pl.m_tiles > 1 ? 1 : 0);
+    d.kind = pl.flex ? 3 : (pl.mixed ? 2 : (pl.m_tiles > 1 ? 1 : 0));
+    if (pl.flex) memcpy(d.mixed_tab, h->mixed_tab, sizeof d.mixed_tab);
     if (pl.mixed) {
         d.tiles_pair = ceil_div(h->dims.V, pl.tile_n);
         d.sms = h->di->sms;
@@ -580,6 +685,95 @@ int launch_fused(Handle* h, int role, const void* hidden, const void* W, const i
     return LASER_OK;
 }
 
+// Enqueue laser_probe_flex_kernel (one launch: every decision about chunks and splits is the kernel's).
+int launch_flex(Handle* h, const void* hidden, const void* W, const int32_t* req_offsets,
+                const int32_t* token_ids, int v_offset, float4* ws, cudaStream_t stream, bool allow_pdl,
+                const TailParams& tail) {
+    DeviceInfo* di = h->di;
+    const laser_probe_plan& pl = h->plan;
+    const laser_probe_dims& dims = h->dims;
+    static const bool use_pdl = getenv("LASER_NO_PDL") == nullptr;
+    static bool attr_set[64] = {};
+    int dev = static_cast<int>(di - g_dev);
+    if (!attr_set[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(laser_probe_flex_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             kMaxDynSmem);
+        if (e != cudaSuccess) return set_cuda_error("cudaFuncSetAttribute", e);
+        attr_set[dev] = true;
+    }
+    const CUtensorMap* tm_w = nullptr;
+    int rc = handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V, dims.d, kTileM, &tm_w);
+    if (rc != LASER_OK) return rc;
+    Handle::FlexEntry* fe = nullptr;
+    for (auto& e : h->flex_hid)
+        if (e.ptr == hidden) fe = &e;
+    if (!fe) {
+        fe = &h->flex_hid[h->flex_rr];
+        h->flex_rr = (h->flex_rr + 1) % 2;
+        fe->ptr = nullptr;
+        for (int i = 0; i < kFlexMaps; ++i) {
+            if (16 * (i + 1) > pl.flex_max_tok) { fe->maps.hid[i] = fe->maps.hid[0]; continue; }
+            rc = encode_tensor_map(hidden, dims.N, dims.d, 8 * (i + 1), &fe->maps.hid[i]);
+            if (rc != LASER_OK) return rc;
+        }
+        fe->ptr = hidden;
+    }
+
+    FusedParams fp{};
+    fp.n_alloc = dims.N; fp.d = dims.d; fp.V = dims.V;
+    fp.pd = plan_desc(h, req_offsets);
+    fp.role = 0;
+    fp.grid_total = pl.grid;
+    fp.total_tiles = ceil_div(dims.V, kFlexVocabTile);
+    fp.wait_first = h->opt.overlap ? 0 : 1;
+    fp.tile_n = kFlexVocabTile; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
+    fp.tail_cache = pl.tail_cache;
+    fp.stage_bytes = static_cast<uint32_t>(kABytes + (pl.flex_max_tok / 2) * 128);
+    fp.tx_bytes = 0;       // depends on the chunk height: computed in the kernel
+    fp.hint_C = pl.m_tiles; fp.hint_S = pl.splits;     // the dense decomposition (see the kernel)
+    {
+        static const bool no_hint = getenv("LASER_FLEX_NO_HINT") != nullptr;
+        if (no_hint) fp.hint_C = 0;
+    }
+    // several chunks re-read a W tile from L2 (side by side: chunk-fastest item order)
+    fp.w_policy = pl.m_tiles == 1 && dims.N <= kFlexMaxTok ? ptx::kEvictFirst : ptx::kEvictNormal;
+    fp.ws = ws;
+    fp.token_ids = token_ids;
+    fp.v_offset = v_offset;
+
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(pl.grid);
+    cfg.blockDim = dim3(kFusedThreads);
+    cfg.dynamicSmemBytes = static_cast<size_t>(pl.smem_bytes);
+    cfg.stream = stream;
+    cudaLaunchAttribute fattr[2];
+    unsigned na = 0;
+    if (use_pdl && allow_pdl) {
+        fattr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        fattr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    fattr[na].id = cudaLaunchAttributeClusterDimension;
+    fattr[na].val.clusterDim.x = 2;
+    fattr[na].val.clusterDim.y = 1;
+    fattr[na].val.clusterDim.z = 1;
+    ++na;
+    cfg.attrs = fattr;
+    cfg.numAttrs = na;
+#ifdef LASER_TIMELINE
+    static int tl_launches = 0;
+    TailParams tail_tl = tail;
+    tail_tl.tl_slot = tl_launches++;
+    const TailParams& tail_arg = tail_tl;
+#else
+    const TailParams& tail_arg = tail;
+#endif
+    cudaError_t e = cudaLaunchKernelEx(&cfg, laser_probe_flex_kernel, fe->maps, *tm_w, fp, tail_arg);
+    if (e != cudaSuccess) return set_cuda_error("launch laser_probe_flex_kernel", e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return LASER_OK;
+}
+
 // The fields of FinalizeParams that describe the fused kernels' workspace for the handle's dims.
 FinalizeParams finalize_params(const Handle* h, bool run_fused, const int32_t* req_offsets) {
     FinalizeParams fz{};
@@ -599,6 +793,7 @@ FinalizeParams finalize_params(const Handle* h, bool run_fused, const int32_t* r
 int launch_call(Handle* h, const void* hidden, const void* W, const int32_t* req_offsets,
                 const int32_t* token_ids, int v_offset, float4* ws, cudaStream_t stream, bool allow_pdl,
                 const TailParams& tail) {
+    if (h->plan.flex) return launch_flex(h, hidden, W, req_offsets, token_ids, v_offset, ws, stream, allow_pdl, tail);
     if (!h->plan.mixed) return launch_fused(h, 0, hidden, W, req_offsets, token_ids, v_offset, ws, stream, allow_pdl, tail);
     int rc = launch_fused(h, 2, hidden, W, req_offsets, token_ids, v_offset, ws, stream, allow_pdl, tail);
     if (rc != LASER_OK) return rc;
@@ -986,7 +1181,7 @@ int laser_probe_options_default(laser_probe_options* out) {
 int laser_probe_plan_query_mode(const laser_probe_dims* dims, int kernel_mode, laser_probe_plan* plan) {
     if (!dims || !plan) return LASER_E_NULL;
     if (!dims_valid(dims)) return LASER_E_DIMS;
-    if (kernel_mode < LASER_MODE_AUTO || kernel_mode > LASER_MODE_PAIR) return LASER_E_MODE;
+    if (kernel_mode < LASER_MODE_AUTO || kernel_mode > LASER_MODE_FLEX) return LASER_E_MODE;
     bool ok = false;
     DeviceInfo* di = current_device(&ok);
     make_plan(*dims, (ok && di) ? di->sms : kDefaultSMs, kernel_mode, plan, nullptr);
@@ -1019,6 +1214,17 @@ int laser_probe_mixed_query(const laser_probe_dims* dims, int32_t n_valid, laser
     return LASER_OK;
 }
 
+int laser_probe_flex_query(const laser_probe_dims* dims, int32_t n_valid, laser_probe_flex* out) {
+    if (!dims || !out) return LASER_E_NULL;
+    if (!dims_valid(dims) || n_valid < 0 || n_valid > kFlexMaxRows) return LASER_E_DIMS;
+    bool ok = false;
+    DeviceInfo* di = current_device(&ok);
+    const FlexChoice c = plan_flex_host(n_valid, dims->V, (ok && di) ? di->sms : kDefaultSMs);
+    out->chunks = c.C; out->n_tok = c.n_tok; out->splits = c.S; out->tiles_per_split = c.T;
+    out->rounds = c.rounds; out->model_cost = static_cast<float>(c.cost);
+    return LASER_OK;
+}
+
 int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan) {
     return laser_probe_plan_query_mode(dims, LASER_MODE_AUTO, plan);
 }
@@ -1026,7 +1232,7 @@ int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan)
 size_t laser_probe_workspace_bytes(const laser_probe_dims* dims) {
     // enough for every kernel_mode, so that one buffer serves every laser_probe_options setting
     size_t best = 0;
-    for (int mode = LASER_MODE_AUTO; mode <= LASER_MODE_PAIR; ++mode) {
+    for (int mode = LASER_MODE_AUTO; mode <= LASER_MODE_FLEX; ++mode) {
         laser_probe_plan pl;
         if (laser_probe_plan_query_mode(dims, mode, &pl) != LASER_OK) return 0;
         const size_t w = workspace_bytes_for(pl);

@@ -108,15 +108,34 @@ __host__ __device__ inline MixedPlan mixed_unpack(uint32_t e, int m128, int sms)
     return mp;
 }
 
+// Flex kernel (flex_kernel.cuh; vocabulary on the MMA M axis, tokens on N): the valid rows are cut into
+// C chunks of n_tok rows (a multiple of 16, <= 256 = UMMA N) and every chunk's vocabulary tiles (256 rows
+// per CTA pair) into S splits.  The host plans every count of 16-row groups that may hold rows and hands
+// the kernel one packed word per count (PlanDesc.mixed_tab, kind 3):
+//   bits [0,5) C   bits [5,10) n_tok / 16   bits [10,22) S
+constexpr int kFlexVocabTile = 256;   // vocabulary rows per tile and CTA pair (UMMA M of cta_group::2)
+constexpr int kFlexMaxTok = 256;      // token rows per chunk
+constexpr int kFlexMaxRows = 16 * 256;   // largest batch the table covers
+struct FlexPlan {
+    int C, n_tok, S;
+};
+__host__ __device__ inline uint32_t flex_pack(int C, int n_tok, int S) {
+    return static_cast<uint32_t>(C) | (static_cast<uint32_t>(n_tok >> 4) << 5) | (static_cast<uint32_t>(S) << 10);
+}
+__host__ __device__ inline FlexPlan flex_unpack(uint32_t e) {
+    return FlexPlan{static_cast<int>(e & 31u), static_cast<int>((e >> 5) & 31u) << 4, static_cast<int>((e >> 10) & 0xFFFu)};
+}
+
 // What fixes a call's decomposition; shared by the fused kernel(s) and the merge.
 struct PlanDesc {
-    int32_t kind;                      // 0 static, 1 re-plan of one variant, 2 mixed (pair + single-CTA tail tile)
+    int32_t kind;                      // 0 static, 1 re-plan of one variant, 2 mixed (pair + single-CTA tail tile), 3 flex
     int32_t n_alloc, R;
     const int32_t* req_offsets;
     int32_t m_tiles, rows_per_item, splits;    // kind 0 / 1: the host plan of the variant
     int32_t total_tiles, units;                // kind 1: vocabulary tiles of the variant, its execution units
     int32_t tiles_pair, sms;                   // kind 2: vocabulary tiles of the pair kernel, SMs
     uint32_t mixed_tab[kMixedTabMax];          // kind 2: the plan for every count of 128-row tiles (mixed_pack)
+                                               // kind 3: for every count of 16-row groups, entry [count - 1] (flex_pack)
 };
 // Where a call's records are: rows [0, rows_a) have S_a records each from record 0 on; rows >= rows_a
 // have S_b records each from record rows_a * S_a on.
@@ -126,7 +145,8 @@ struct RecLayout {
 // The decomposition that actually runs, decided on the device from req_offsets[R] (kind 1, 2).
 struct RunPlan {
     MixedPlan mp;          // kind 2
-    int m_items, S;        // kind 0 / 1
+    int m_items, S;        // kind 0 / 1; kind 3: token chunks C, vocabulary splits S
+    int n_tok;             // kind 3: token rows per chunk
     RecLayout lay;
 };
 __device__ __forceinline__ RunPlan resolve_plan(const PlanDesc& d) {
@@ -134,6 +154,14 @@ __device__ __forceinline__ RunPlan resolve_plan(const PlanDesc& d) {
     rp.m_items = d.m_tiles; rp.S = d.splits;
     if (d.kind != 0) {   // uniform across the grid: every thread reads the same word
         const int n_valid = d.R > 0 ? min(max(__ldg(d.req_offsets + d.R), 0), d.n_alloc) : 0;
+        if (d.kind == 3) {
+            const int g16 = (n_valid + 15) >> 4;
+            const FlexPlan fp = g16 > 0 ? flex_unpack(d.mixed_tab[min(g16, kMixedTabMax) - 1]) : FlexPlan{0, 16, 1};
+            rp.m_items = fp.C; rp.S = fp.S; rp.n_tok = fp.n_tok;
+            // both CTAs of a pair leave a record per (row, split): 2 S records per row
+            rp.lay = RecLayout{0x7fffffff, 2 * fp.S, 2 * fp.S};
+            return rp;
+        }
         if (d.kind == 1) {
             const int m = (n_valid + d.rows_per_item - 1) / d.rows_per_item;
             if (m < d.m_tiles) {
@@ -187,6 +215,10 @@ struct FusedParams {
     // requests whose {offset, threshold} fit in the shared memory the pipeline leaves over: the
     // epilogue warps fill that cache right after the wait, so the tail needs no input loads
     int32_t tail_cache;
+    // flex kernel: the decomposition of a batch whose n_alloc rows are all valid (chunks, splits).  The
+    // producer requests the W boxes of its first tiles under this guess ahead of the wait; when
+    // req_offsets[R] then says otherwise the boxes are dropped (0: nothing is requested early).
+    int32_t hint_C, hint_S;
 };
 
 // ---------------------------------------------------------------------------------- descriptors
