@@ -185,6 +185,7 @@ def roofline_for(w: wl.Workload, us: float, peaks: dict):
 
 
 # ----------------------------------------------------------------------------------------- GPU arm
+KERNEL_MODES = ["auto", "single", "pair", "flex", "mixed"]     # laser_probe_options.kernel_mode, by value
 SETTLE_S = 0.25
 COOL_S = 1.0
 
@@ -212,7 +213,7 @@ def settle(case, seconds: float = SETTLE_S):
 
 class GpuCase:
     def __init__(self, w: wl.Workload, device, two_w_copies: bool = False, Ws=None, overlap: bool = False,
-                 share=None):
+                 share=None, mode: int = 0):
         import torch
         from paper_2606_31580_b200 import binding as B
         self.torch, self.B, self.w = torch, B, w
@@ -228,7 +229,7 @@ class GpuCase:
                 Ws.append(Ws[0].clone())
         self.Ws = Ws
         self.tp = B.TauParams(**w.tau_params)
-        self.probe = B.Probe(w.N_alloc, w.d, w.V, w.R, device=device, debug_outputs=False, overlap=overlap)
+        self.probe = B.Probe(w.N_alloc, w.d, w.V, w.R, device=device, debug_outputs=False, overlap=overlap, mode=mode)
         self.i = 0
 
     def step(self):
@@ -574,9 +575,10 @@ def run_ours(args):
     w = make_workload(args.workload, rank, W_cache)
     # the library default: strict stream order for every per-call input (what a serving loop needs
     # behind the forward pass that writes `hidden`).  This is the headline configuration.
-    case = GpuCase(w, device, two_w_copies=(w.V * w.d * 2 < 2_000_000_000))
+    kmode = KERNEL_MODES.index(args.kernel_mode)
+    case = GpuCase(w, device, two_w_copies=(w.V * w.d * 2 < 2_000_000_000), mode=kmode)
     # laser_probe_options.overlap = 1: consecutive calls of a loop over resident inputs overlap
-    over = GpuCase(w, device, Ws=case.Ws, overlap=True, share=case)
+    over = GpuCase(w, device, Ws=case.Ws, overlap=True, share=case, mode=kmode)
 
     for _ in range(args.warmup):
         case.step()
@@ -618,7 +620,7 @@ def run_ours(args):
     # staging/workspace/output set each) so that the H2D copy of batch i+1 overlaps the kernel of batch
     # i, as a serving loop would run it; one batch at a time (synchronous) is timed as well.
     depth = 2
-    slots = [B.HostProbe(w.N_alloc, w.d, w.V, w.R, device=device) for _ in range(depth)]
+    slots = [B.HostProbe(w.N_alloc, w.d, w.V, w.R, device=device, mode=kmode) for _ in range(depth)]
     streams = [torch.cuda.Stream(device=device) for _ in range(depth)]
     hp = slots[0]
     hh = B.bf16_tensor_from_bits(w.hidden_bits, pin=True)
@@ -698,7 +700,8 @@ def run_ours(args):
         # immediately before and after the fused kernel on the launch stream (no programmatic
         # dependent launch for those calls, so nothing overlaps the bracket).
         roof = roofline_for(w, fused_us, peaks)
-        roof["kernel"] = ("laser_probe_fused_kernel<1> (CTA pairs) beside laser_probe_fused_kernel<0> (single CTAs): mixed schedule"
+        roof["kernel"] = ("laser_probe_flex_kernel" if case.probe.plan["flex"] else
+                          "laser_probe_fused_kernel<1> (CTA pairs) beside laser_probe_fused_kernel<0> (single CTAs): mixed schedule"
                           if case.probe.plan["mixed"] else "laser_probe_fused_kernel<%d>" % case.probe.plan["cta_pair"])
         roof["kernel_us"] = fused_us
         roof["kernel_us_source"] = ("average over K launches, each bracketed on its own by CUDA events on the launch "
@@ -735,7 +738,7 @@ def run_ours(args):
                            % (w.V * w.d * 2 / 1e6) if len(case.Ws) > 1 else
                            "W (%.0f MB) exceeds the 126 MB L2" % (w.V * w.d * 2 / 1e6),
                         sharding="requests sharded across ranks, W replicated, no collective" if world > 1 else "single GPU",
-                        e2e_w_resident=True,
+                        e2e_w_resident=True, kernel_mode=args.kernel_mode,
                         mode="library default: strict stream order (laser_probe_options.overlap = 0), "
                              "merge + a3-a5 in the fused kernel's tail (one launch per call)"),
             overlap=dict(value=rows_all / (overlap_ms / args.steps * 1e-3), unit=UNIT,
@@ -923,6 +926,8 @@ def main():
     ap.add_argument("--exchange", default="peer", choices=["peer", "collective"])
     ap.add_argument("--with-cublas", action="store_true",
                     help="context only: time the plain cuBLAS GEMM hidden @ W^T of the same shape beside the probe")
+    ap.add_argument("--kernel-mode", default="auto", choices=KERNEL_MODES,
+                    help="laser_probe_options.kernel_mode (auto = the library default; the others force a variant)")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

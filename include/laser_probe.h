@@ -108,11 +108,14 @@ typedef struct {
 } laser_probe_plan;
 
 /* Kernel variant (laser_probe_options.kernel_mode).  AUTO (default): one single-CTA kernel for
- * N <= 128 rows; one CTA-pair kernel for 129..256 rows (a single 256-row item whatever req_offsets[R]
- * says); above that the mixed schedule (CTA pairs for the even part of the 128-row tiles that hold
- * rows, single CTAs for an odd last tile, decided on the device).  SINGLE / PAIR force one variant for
- * every shape (tuning and tests; both are exact; PAIR pads an odd tile count). */
-enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2, LASER_MODE_FLEX = 3 };
+ * N <= 128 rows; the flex kernel (vocabulary on the MMA M axis, token chunks of a multiple of 16 rows on
+ * N, decided on the device from req_offsets[R]) for 129..1024 rows except exactly 256; one CTA-pair
+ * kernel for N = 256 (a single 256-row item); above 1024 rows the mixed schedule (CTA pairs for the
+ * even part of the 128-row tiles that hold rows, single CTAs for an odd last tile, decided on the
+ * device).  SINGLE / PAIR force one variant for every shape (tuning and tests; both are exact; PAIR
+ * pads an odd tile count); FLEX forces the flex kernel up to 4096 rows, MIXED the schedule AUTO uses
+ * above 1024 rows for every N > 128. */
+enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2, LASER_MODE_FLEX = 3, LASER_MODE_MIXED = 4 };
 
 /* Where merge + a3-a5 run (laser_probe_options.tail).
  *   FUSED     in the tail of the fused kernel: every CTA counts itself in when its records are in the

@@ -16,7 +16,7 @@ _lib = None
 
 AGG_MEAN, AGG_GEOMEAN, AGG_MIN = 0, 1, 2
 PROB_MAX, PROB_TOKEN = 0, 1
-MODE_AUTO, MODE_SINGLE, MODE_PAIR, MODE_FLEX = 0, 1, 2, 3
+MODE_AUTO, MODE_SINGLE, MODE_PAIR, MODE_FLEX, MODE_MIXED = 0, 1, 2, 3, 4
 TAIL_AUTO, TAIL_FUSED, TAIL_SEPARATE = 0, 1, 2
 
 EXPORTS = [

@@ -255,7 +255,7 @@ struct FlexChoice { int C, n_tok, S, T, rounds; double cost; };
 double flex_tile_charge() {
     static const double v = [] {
         const char* e = getenv("LASER_FLEX_TILE_CHARGE");
-        return e ? atof(e) : 40.0;
+        return e ? atof(e) : 110.0;
     }();
     return v;
 }
@@ -347,11 +347,16 @@ void make_flex_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* p
 // SINGLE / PAIR force one variant (an odd tile count then costs the pair kernel a padding tile).
 void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_plan* pl, laser_probe_plan* tail_pl) {
     const int t128 = ceil_div(dm.N, kTileM);
-    if (mode == LASER_MODE_FLEX && dm.N > 0 && dm.N <= kFlexMaxRows) {
+    // AUTO takes the flex kernel for 129..1024 allocated rows except exactly 256 (measured at the C2 / C3 /
+    // C4 shapes: it wins wherever the rows do not fill 256-row items - N = 320: 130 vs 151 us,
+    // C4's 590 of 1024 rows: 456 vs 508 us - and ties at 512 / 768 / 1024; a dense 256-row batch is the
+    // one case where its fixed 256-row vocabulary tiles quantise worse than the pair kernel's).
+    const bool auto_flex = mode == LASER_MODE_AUTO && dm.N > kTileM && dm.N <= 1024 && dm.N != 2 * kTileM;
+    if ((mode == LASER_MODE_FLEX && dm.N > 0 && dm.N <= kFlexMaxRows) || auto_flex) {
         make_flex_plan(dm, num_sms, pl, nullptr);
         return;
     }
-    if (mode == LASER_MODE_FLEX) mode = LASER_MODE_AUTO;     // outside the table's range
+    if (mode == LASER_MODE_FLEX || mode == LASER_MODE_MIXED) mode = LASER_MODE_AUTO;     // the schedule AUTO had before
     if (mode == LASER_MODE_SINGLE || (mode == LASER_MODE_AUTO && t128 <= 1)) {
         make_variant_plan(dm, num_sms, false, 0, pl);
         return;
@@ -484,7 +489,7 @@ const laser_probe_options kDefaultOptions{LASER_AGG_MEAN, LASER_PROB_MAX, nullpt
 int options_valid(const laser_probe_options& o) {
     if (o.aggregate_mode < LASER_AGG_MEAN || o.aggregate_mode > LASER_AGG_MIN) return LASER_E_MODE;
     if (o.prob_mode < LASER_PROB_MAX || o.prob_mode > LASER_PROB_TOKEN) return LASER_E_MODE;
-    if (o.kernel_mode < LASER_MODE_AUTO || o.kernel_mode > LASER_MODE_FLEX) return LASER_E_MODE;
+    if (o.kernel_mode < LASER_MODE_AUTO || o.kernel_mode > LASER_MODE_MIXED) return LASER_E_MODE;
     if (o.tail < LASER_TAIL_AUTO || o.tail > LASER_TAIL_SEPARATE) return LASER_E_MODE;
     if (o.overlap != 0 && o.overlap != 1) return LASER_E_MODE;
     if (o.reserved != 0) return LASER_E_MODE;
@@ -1181,7 +1186,7 @@ int laser_probe_options_default(laser_probe_options* out) {
 int laser_probe_plan_query_mode(const laser_probe_dims* dims, int kernel_mode, laser_probe_plan* plan) {
     if (!dims || !plan) return LASER_E_NULL;
     if (!dims_valid(dims)) return LASER_E_DIMS;
-    if (kernel_mode < LASER_MODE_AUTO || kernel_mode > LASER_MODE_FLEX) return LASER_E_MODE;
+    if (kernel_mode < LASER_MODE_AUTO || kernel_mode > LASER_MODE_MIXED) return LASER_E_MODE;
     bool ok = false;
     DeviceInfo* di = current_device(&ok);
     make_plan(*dims, (ok && di) ? di->sms : kDefaultSMs, kernel_mode, plan, nullptr);
@@ -1232,7 +1237,7 @@ int laser_probe_plan_query(const laser_probe_dims* dims, laser_probe_plan* plan)
 size_t laser_probe_workspace_bytes(const laser_probe_dims* dims) {
     // enough for every kernel_mode, so that one buffer serves every laser_probe_options setting
     size_t best = 0;
-    for (int mode = LASER_MODE_AUTO; mode <= LASER_MODE_FLEX; ++mode) {
+    for (int mode = LASER_MODE_AUTO; mode <= LASER_MODE_MIXED; ++mode) {
         laser_probe_plan pl;
         if (laser_probe_plan_query_mode(dims, mode, &pl) != LASER_OK) return 0;
         const size_t w = workspace_bytes_for(pl);

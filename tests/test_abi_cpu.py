@@ -52,12 +52,18 @@ def test_library_is_sm100a_with_tcgen05_and_tma():
 def test_plan_invariants(dims):
     N, d, V, R = dims
     p = B.plan_query(*dims)
+    # AUTO: the flex kernel for 129..1024 rows except exactly 256 (checked in test_flex_plan_invariants)
+    assert p["flex"] == (1 if (128 < N <= 1024 and N != 256) else 0)
+    if p["flex"]:
+        p = B.plan_query(*dims, mode=B.MODE_MIXED)
+    assert p["flex"] == 0
     bn, T, S = p["tile_n"], p["tiles_per_split"], p["splits"]
     pair, tm = p["cta_pair"], p["tile_m"]
     t128 = -(-N // 128)
     mixed = p["mixed"]
-    # AUTO: one single-CTA kernel up to 128 rows, one CTA-pair kernel up to 256, above that the mixed
-    # schedule (single-CTA tail-tile kernel + pair kernel, the tail in whichever has the work)
+    # AUTO outside the flex range / MIXED: one single-CTA kernel up to 128 rows, one CTA-pair kernel up to
+    # 256, above that the mixed schedule (single-CTA tail-tile kernel + pair kernel, the tail in whichever
+    # has the work)
     assert (pair, mixed) == ((0, 0) if t128 <= 1 else ((1, 0) if t128 == 2 else (1, 1))) and tm == (256 if pair else 128)
     assert p["kernel_launches"] == (2 if mixed else 1)
     assert bn % (32 if pair else 16) == 0 and 16 <= bn <= 256
@@ -88,6 +94,36 @@ def test_plan_invariants(dims):
     assert rounds * T * bn <= 1.08 * (p["m_tiles"] * V / busy) + bn
 
 
+@pytest.mark.parametrize("dims", [(136, 1536, 151936, 17), (256, 3584, 152064, 32), (320, 1536, 151936, 40),
+                                  (1024, 4096, 128256, 64), (400, 512, 33000, 40), (130, 64, 1000, 3),
+                                  (4096, 1536, 151936, 512), (17, 8, 17, 2), (2000, 256, 300, 9)])
+def test_flex_plan_invariants(dims):
+    """The flex kernel's plan and its device-side table (one entry per count of 16-row groups)."""
+    N, d, V, R = dims
+    p = B.plan_query(*dims, mode=B.MODE_FLEX)
+    assert p["flex"] == 1 and p["mixed"] == 0 and p["cta_pair"] == 1 and p["kernel_launches"] == 1
+    assert p["tile_n"] == 256 and p["grid"] == 2 * (p["num_sms"] // 2) and p["k_blocks"] == -(-d // 64)
+    pairs, tiles = p["num_sms"] // 2, -(-V // 256)
+    assert p["flex_n_tok"] % 16 == 0 and 16 <= p["flex_n_tok"] <= p["flex_max_tok"] <= 256
+    assert p["m_tiles"] * p["flex_n_tok"] >= N and p["splits"] * p["tiles_per_split"] >= tiles
+    assert 2 <= p["stages"] <= 8 and 0 <= p["tail_cache"] <= 512
+    pipe = p["stages"] * (16384 + p["flex_max_tok"] // 2 * 128) + 1280 + 16384   # ring + slack + transpose blocks
+    assert pipe + (8 * (p["tail_cache"] + 1) if p["tail_cache"] else 0) == p["smem_bytes"] <= 227 * 1024
+    assert B.workspace_bytes(*dims) >= 16 * p["ws_records"]
+    for n_valid in sorted({1, 15, 16, 17, 128, 129, 255, 256, 257, N // 2, N - 1, N} & set(range(1, N + 1))):
+        f = B.flex_query(*dims, n_valid)
+        C_, nt, S = f["chunks"], f["n_tok"], f["splits"]
+        assert nt % 16 == 0 and 16 <= nt <= p["flex_max_tok"]
+        assert C_ * nt >= n_valid and (C_ - 1) * nt < n_valid + 16 * C_   # the chunks cover the rows, padding < 16 per chunk
+        assert S * f["tiles_per_split"] >= tiles and 1 <= S <= max(4 * pairs, 1)
+        assert (C_ * S) % pairs == 0 or S == tiles or C_ * S < pairs      # whole rounds unless V is tiny
+        assert min(C_ * nt, N) * 2 * S <= p["ws_records"]                  # 2 S records per row fit the workspace
+        assert f["rounds"] == -(-C_ * S // pairs)
+    # outside the table's range FLEX falls back to what AUTO does
+    if N <= 4096:
+        assert B.plan_query(5000, d, V, R, mode=B.MODE_FLEX)["flex"] == 0
+
+
 def test_forced_modes_plan():
     p = B.plan_query(32, 64, 1000, 8, mode=B.MODE_PAIR)
     assert p["cta_pair"] == 1 and p["tile_m"] == 256 and p["grid"] % 2 == 0 and p["tile_n"] % 32 == 0
@@ -112,7 +148,7 @@ def test_options_are_per_call_and_validated():
     tp, d = B.TauParams(), B.Dims(32, 64, 1000, 8)
     call = lambda opt: L.laser_probe_confidence_opt(a, a, a, a, C.byref(tp), a, a, a, C.byref(d), a, 4096, None,
                                                     None, None, C.byref(opt))
-    for bad in (B.Options(kernel_mode=3), B.Options(tail=3), B.Options(aggregate_mode=3), B.Options(prob_mode=2)):
+    for bad in (B.Options(kernel_mode=5), B.Options(tail=3), B.Options(aggregate_mode=3), B.Options(prob_mode=2)):
         assert call(bad) == -8                                              # LASER_E_MODE
     o = B.Options(); o.overlap = 2
     assert call(o) == -8

@@ -56,23 +56,33 @@ def test_c2_qwen15b_full(P, c2_W_bits):
     assert st["rows"] == 128 and st["requests"] == 16 and 0 < st["exits"] < 16
 
 
-def test_c3_qwen7b_full(P):
-    """Every row and request of C3 against the oracle (pair kernel, one 256-row item per split)."""
+@pytest.mark.parametrize("mode", [0, 3])
+def test_c3_qwen7b_full(P, force_mode, mode):
+    """Every row and request of C3 against the oracle: AUTO (pair kernel, one 256-row item per split) and
+    the flex kernel (one 256-token chunk)."""
+    force_mode(mode)
     w = wl.config_c3()
-    st = P.check(w)
-    _log("C3", st)
+    g = P.run_gpu(w)
+    assert g.plan["flex"] == (1 if mode == 3 else 0)
+    ora, rows, reqs = _oracle_once(P, "C3", w)
+    st = P.compare(w, g, ora, rows, reqs, f"C3/mode{mode}")
+    _log(f"C3/mode{mode}", st)
     assert st["rows"] == w.N_valid == 256 and st["requests"] == 32
 
 
-def test_c4_llama8b_full(P):
-    """Every valid row and every request of C4 (variable lengths, padded allocation, device-side
-    re-plan of the pair kernel) against the oracle."""
+@pytest.mark.parametrize("mode", [0, 4])
+def test_c4_llama8b_full(P, force_mode, mode):
+    """Every valid row and every request of C4 (variable lengths, padded allocation) against the oracle:
+    AUTO (the flex kernel: chunks and splits decided on the device from req_offsets[R], the W boxes
+    requested under the dense guess dropped) and the mixed schedule (device-side split of the SMs)."""
+    force_mode(mode)
     w = wl.config_c4()
     assert w.N_alloc == 1024 and w.N_valid < 1024
     g = P.run_gpu(w)
-    ora, rows, reqs = P.run_oracle(w)
-    st = P.compare(w, g, ora, rows, reqs, "C4")
-    _log("C4", st)
+    assert g.plan["flex"] == (1 if mode == 0 else 0) and g.plan["mixed"] == (1 if mode == 4 else 0)
+    ora, rows, reqs = _oracle_once(P, "C4", w)
+    st = P.compare(w, g, ora, rows, reqs, f"C4/mode{mode}")
+    _log(f"C4/mode{mode}", st)
     assert st["rows"] == w.N_valid and st["requests"] == w.R == 64
     assert np.all(g.argmax[w.N_valid:] == -1)                 # padding rows (DESIGN A11)
     assert np.all(g.argmax[:w.N_valid] >= 0)
@@ -112,6 +122,18 @@ def test_c5_sweep(P, c2_W_bits, N):
     assert np.all(g.argmax[pl] == w.planted[pl])
     assert np.all((g.conf >= 0) & (g.conf <= 1.0 + 1e-6))
     assert np.all((g.pmax > 0) & (g.pmax <= 1.0))
+
+
+def test_c5_4096_flex(P, force_mode, c2_W_bits):
+    """The flex kernel at the top of its range (16 chunks of 256 tokens), every row against the oracle."""
+    force_mode(3)
+    w = wl.config_c5(4096, c2_W_bits)
+    g = P.run_gpu(w)
+    assert g.plan["flex"] == 1 and g.plan["m_tiles"] == 16
+    ora, rows, reqs = _oracle_once(P, "C5:4096", w)
+    st = P.compare(w, g, ora, rows, reqs, "C5:4096/flex")
+    _log("C5:4096/flex", st)
+    assert st["rows"] == 4096
 
 
 # ------------------------------------------------------------------ stress inputs (not timed)
@@ -168,7 +190,7 @@ def path(P, request):
     P.CFG.update(tail=0, use_handle=True)
 
 
-@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("mode", [1, 2, 3])
 @pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
     (5000, 256, 12, 8, None, None),        # N = 96: the pair's second CTA holds only padding rows
     (33000, 512, 40, None, 400, (1, 16)),  # N = 400: two 256-row items, second one ragged
@@ -180,16 +202,17 @@ def test_forced_variants(P, force_mode, path, mode, V, d, R, L, n_alloc, var_len
     force_mode(mode)
     w = wl.scaled(f"mode{mode}-V{V}-d{d}", V, d, 0.05, R, L, seed=V + d + mode, N_alloc=n_alloc, var_len=var_len)
     st = P.check(w)
-    assert st["plan"]["cta_pair"] == (1 if mode == 2 else 0)
+    assert st["plan"]["cta_pair"] == (1 if mode >= 2 else 0) and st["plan"]["flex"] == (1 if mode == 3 else 0)
     _log(w.name, st)
 
 
-@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("mode", [1, 2, 3, 4])
 def test_forced_variants_c5_512(P, force_mode, c2_W_bits, mode):
     force_mode(mode)
     w = wl.config_c5(512, c2_W_bits)
     g = P.run_gpu(w)
-    assert g.plan["cta_pair"] == (1 if mode == 2 else 0)
+    assert g.plan["cta_pair"] == (1 if mode >= 2 else 0) and g.plan["flex"] == (1 if mode == 3 else 0)
+    assert g.plan["mixed"] == (1 if mode == 4 else 0)
     ora, rows, reqs = _oracle_once(P, "C5:512", w)
     st = P.compare(w, g, ora, rows, reqs, f"C5:512/mode{mode}")
     assert st["rows"] == 512
@@ -198,7 +221,7 @@ def test_forced_variants_c5_512(P, force_mode, c2_W_bits, mode):
     assert np.all(g.argmax[pl] == w.planted[pl])
 
 
-@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("R,L,var_len,n_alloc", [
     (20, None, (1, 16), 1000),   # ~170 valid rows of 1000: most token tiles are padding
     (32, 8, None, 1024),         # exactly 256 valid rows: boundary of a pair item
@@ -226,22 +249,25 @@ def test_padding_tiles_are_skipped_and_replanned(P, force_mode, path, mode, R, L
     (74, None, (1, 16), 1024),   # ragged, ~600 valid rows (C4-like)
     (3, 0, None, 700),           # every request empty: neither part has work
 ])
-def test_mixed_schedule_odd_tile_counts(P, path, R, L, var_len, n_alloc):
-    """AUTO above 128 rows: 256-row items on CTA pairs, an odd last 128-row tile on single CTAs in a
-    second kernel beside them; which part takes what is decided on the device from req_offsets[R].
-    Requests that straddle the two parts are merged from both kernels' records."""
+def test_mixed_schedule_odd_tile_counts(P, force_mode, path, R, L, var_len, n_alloc):
+    """Mixed schedule (AUTO above 1024 rows, LASER_MODE_MIXED anywhere above 256): 256-row items on CTA
+    pairs, an odd last 128-row tile on single CTAs in a second kernel beside them; which part takes what
+    is decided on the device from req_offsets[R].  Requests that straddle the two parts are merged from
+    both kernels' records."""
+    force_mode(4)
     w = wl.scaled(f"mixed-R{R}-L{L}-N{n_alloc}", 33000, 512, 0.05, R, L, seed=R + 31, N_alloc=n_alloc, var_len=var_len)
     st = P.check(w)
     assert st["plan"]["mixed"] == 1 and st["plan"]["kernel_launches"] == (3 if path == "separate-handle" else 2)
     _log(f"{w.name}/{path}", st)
 
 
-def test_mixed_schedule_ties_across_the_two_kernels(P):
+def test_mixed_schedule_ties_across_the_two_kernels(P, force_mode):
     """Duplicate W rows whose logits tie exactly, for a row of the pair part and a row of the tail tile:
     the lowest index must win in both kernels (different tile heights, different split counts)."""
     from paper_2606_31580_b200 import binding as B
+    force_mode(4)
     V, d, N = 40000, 128, 384
-    plan = B.plan_query(N, d, V, 3)
+    plan = B.plan_query(N, d, V, 3, mode=B.MODE_MIXED)
     assert plan["mixed"] == 1
     rng = np.random.default_rng(19)
     Wf = (rng.standard_normal((V, d)) * 0.05).astype(np.float32)
@@ -264,8 +290,8 @@ def test_ties_in_pair_mode(P, force_mode):
     from paper_2606_31580_b200 import binding as B
     force_mode(2)
     V, d, N = 20000, 128, 200
-    plan = B.plan_query(N, d, V, 2)
-    assert plan["cta_pair"] == 1
+    plan = B.plan_query(N, d, V, 2, mode=B.MODE_PAIR)
+    assert plan["cta_pair"] == 1 and plan["flex"] == 0
     bn, T, S = plan["tile_n"], plan["tiles_per_split"], plan["splits"]
     assert T >= 2 and S >= 2
     rng = np.random.default_rng(9)
@@ -283,6 +309,33 @@ def test_ties_in_pair_mode(P, force_mode):
             ora, rows, reqs = P.run_oracle(w)
             assert ora.argmax[row] == v1 and ora.gap2[row] == 0.0
             P.compare(w, g, ora, rows, reqs, "ties-pair")
+
+
+def test_ties_in_flex_mode(P, force_mode):
+    """Flex kernel: duplicate W rows across the vocabulary quarters of the four epilogue warps (31 | 32),
+    the two CTAs of a pair (127 | 128), tiles, consecutive tiles of one split and different splits - for a
+    row of the first chunk, of the second chunk, and of a chunk's last 16-token group."""
+    from paper_2606_31580_b200 import binding as B
+    force_mode(3)
+    V, d, N = 20000, 128, 304
+    f = B.flex_query(N, d, V, 2, N)
+    C_, nt, S = f["chunks"], f["n_tok"], f["splits"]
+    assert C_ == 2 and nt == 160 and S >= 2 and f["tiles_per_split"] >= 2
+    rng = np.random.default_rng(10)
+    Wf = (rng.standard_normal((V, d)) * 0.05).astype(np.float32)
+    h = rng.standard_normal((N, d)).astype(np.float32)
+    for row in (3, 150, 170, 300):                  # chunk 0 (first / last 16-token group), chunk 1 (first / last group)
+        big = (h[row] * 0.5).astype(np.float32)
+        for v1, v2 in [(31, 32), (127, 128), (255, 256), (5, S * 256 + 7), (5, 3 * 256 + 7), (200, 19999)]:
+            W2 = Wf.copy(); W2[v1] = big; W2[v2] = big
+            w = wl.Workload("ties-flex", wl.bf16_bits(W2), wl.bf16_bits(h), wl.fixed_offsets(2, 152),
+                            np.array([0.3, 0.7], np.float32))
+            g = P.run_gpu(w)
+            assert g.plan["flex"] == 1
+            assert g.argmax[row] == v1, (row, v1, v2, g.argmax[row], f)
+            ora, rows, reqs = P.run_oracle(w)
+            assert ora.argmax[row] == v1 and ora.gap2[row] == 0.0
+            P.compare(w, g, ora, rows, reqs, "ties-flex")
 
 
 # ------------------------------------------------------------------ closed forms on the GPU
@@ -340,7 +393,7 @@ def test_ties_across_tile_and_split_boundaries(P):
         P.compare(w, g, ora, rows, reqs, "ties")
 
 
-@pytest.mark.parametrize("tail,mode", [(1, 1), (1, 2), (2, 0), (0, 0), (1, 0)])   # fused tail on either variant / mixed: separate, auto, fused
+@pytest.mark.parametrize("tail,mode", [(1, 1), (1, 2), (2, 4), (0, 4), (1, 4), (2, 3), (0, 0), (1, 3)])   # fused tail on either variant / mixed: separate, auto, fused / flex
 @pytest.mark.parametrize("overlap", [True, False])
 def test_back_to_back_calls_share_a_workspace(P, overlap, tail, mode):
     """Stream order under programmatic dependent launch: calls enqueued back to back on one stream,
@@ -366,9 +419,10 @@ def test_back_to_back_calls_share_a_workspace(P, overlap, tail, mode):
         dv = devs[k % 2]
         p(dv["hidden"], dv["W"], dv["off"], dv["load"], tp)
     assert B.kernel_launch_count() - n0 == K * probes[0].plan["kernel_launches"]
-    # N = 384 rows: AUTO is the mixed schedule (two fused kernels); the merge is one more launch when it
-    # is asked for (tail 2) or when AUTO avoids the fused tail (overlap)
-    assert probes[0].plan["kernel_launches"] == (2 if mode == 0 else 1) + (1 if (tail == 2 or (tail == 0 and overlap)) else 0)
+    # N = 384 rows: MIXED is two fused kernels, AUTO the flex kernel (one); the merge is one more launch
+    # when it is asked for (tail 2) or when AUTO avoids the fused tail (overlap)
+    assert probes[0].plan["flex"] == (1 if mode in (0, 3) else 0)
+    assert probes[0].plan["kernel_launches"] == (2 if mode == 4 else 1) + (1 if (tail == 2 or (tail == 0 and overlap)) else 0)
     torch.cuda.synchronize()
     for k, p in enumerate(probes):
         g = P.GpuRun(p.conf.cpu().numpy(), p.argmax.cpu().numpy(), p.exit.cpu().numpy(),

@@ -139,7 +139,7 @@ def test_token_mode_needs_token_ids(P):
 
 
 # ------------------------------------------------------------------------------- vocabulary-parallel
-def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False, tail=0):
+def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False, tail=0, mode=0):
     """G virtual ranks on one GPU, one after the other on one stream."""
     import torch
     from paper_2606_31580_b200 import binding as B
@@ -152,7 +152,7 @@ def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False, tail=0):
     shards = []
     for g in range(G):
         v0, v1 = par.shard_vocab(w.V, G, g)
-        sh = B.VocabShardProbe(N, w.d, v1 - v0, w.R, v0, G, tail=tail)
+        sh = B.VocabShardProbe(N, w.d, v1 - v0, w.R, v0, G, tail=tail, mode=mode)
         Wg = dev["W"][v0:v1].contiguous()
         if peer:
             pe = B.Peers()
@@ -181,16 +181,18 @@ def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False, tail=0):
 @pytest.mark.parametrize("tail", [0, 2])       # reduce + push + signal in the fused kernel's tail (one kernel) / as kernels
 @pytest.mark.parametrize("peer", [False, True])
 @pytest.mark.parametrize("G", [1, 2, 3, 8])
-@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
-    (33000, 512, 12, 8, None, None),
-    (9001, 256, 40, None, 400, (1, 16)),     # V not divisible by G, several token tiles, padding rows
+@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len,mode", [
+    (33000, 512, 12, 8, None, None, 0),
+    (9001, 256, 40, None, 400, (1, 16), 0),  # V not divisible by G, several token chunks, padding rows: the flex kernel
+    (9001, 256, 40, None, 400, (1, 16), 4),  # the same through the mixed schedule (two fused kernels per partial)
 ])
-def test_vocab_parallel_matches_oracle(P, G, peer, tail, V, d, R, L, n_alloc, var_len):
+def test_vocab_parallel_matches_oracle(P, G, peer, tail, V, d, R, L, n_alloc, var_len, mode):
     from paper_2606_31580_b200 import binding as B
     w = wl.scaled(f"vp-V{V}-G{G}", V, d, 0.05, R, L, seed=88, N_alloc=n_alloc, var_len=var_len)
     n0 = B.kernel_launch_count()
-    g, stats = _run_vocab_parallel(P, w, G, peer=peer, tail=tail)
-    mixed = B.plan_query(w.N_alloc, d, par.shard_vocab(V, G, 0)[1], R)["mixed"]
+    g, stats = _run_vocab_parallel(P, w, G, peer=peer, tail=tail, mode=mode)
+    mixed = B.plan_query(w.N_alloc, d, par.shard_vocab(V, G, 0)[1], R, mode=mode)["mixed"]
+    assert mixed == (1 if mode == 4 else 0)
     fused = 2 if mixed else 1                                           # fused kernels of one partial
     per_partial = fused if tail == 0 else fused + (2 if peer else 1)    # the tail also runs in the mixed schedule's kernels
     assert B.kernel_launch_count() - n0 == G * per_partial + 1          # + the combine kernel
@@ -287,6 +289,8 @@ def _fuzz_case(i):
     pad = int(rng.choice([0, 0, 1, 7, 130, 300]))
     mode = int(rng.integers(0, 3))
     agg = int(rng.integers(0, 3))
+    if i % 3 == 2:
+        mode = 3 + (i % 2)          # flex / mixed
     return V, d, R, (lo, hi), pad, mode, agg
 
 
@@ -307,7 +311,8 @@ def test_fuzz_shapes_modes_aggregates(P, i):
         st = P.check(w, agg=agg)
     finally:
         P.CFG.update(mode=0, tail=0, use_handle=True)
-    print(w.name, {k: v for k, v in st.items() if k != "plan"}, "pair" if st["plan"]["cta_pair"] else "single")
+    print(w.name, {k: v for k, v in st.items() if k != "plan"},
+          "flex" if st["plan"]["flex"] else ("mixed" if st["plan"]["mixed"] else ("pair" if st["plan"]["cta_pair"] else "single")))
 
 
 # ------------------------------------------------------------------------------- boundary: handles, options, debug
