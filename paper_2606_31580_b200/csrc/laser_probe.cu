@@ -1421,7 +1421,10 @@ int laser_probe_combine(const laser_row_stats* stats, int32_t G, const int32_t* 
     fz.out_conf = out_conf; fz.out_argmax = out_argmax; fz.out_exit = out_exit;
     fz.out_tau = out_tau_opt; fz.out_pmax = out_pmax_opt;
     fz.tau = to_dev(tau_params);
-    return launch_finalize(fz, static_cast<cudaStream_t>(stream_v), false);
+    // Programmatic dependent launch: the blocks become resident while the kernel ahead (the partial, or a
+    // collective that never triggers early - then this is an ordinary launch) still runs; they read
+    // offsets / load, wait for its completion (griddepcontrol.wait), then for the peers' flags.
+    return launch_finalize(fz, static_cast<cudaStream_t>(stream_v), true);
 }
 
 size_t laser_probe_staging_bytes(const laser_probe_dims* dims) {
