@@ -18,6 +18,7 @@ AGG_MEAN, AGG_GEOMEAN, AGG_MIN = 0, 1, 2
 PROB_MAX, PROB_TOKEN = 0, 1
 MODE_AUTO, MODE_SINGLE, MODE_PAIR, MODE_FLEX, MODE_MIXED = 0, 1, 2, 3, 4
 TAIL_AUTO, TAIL_FUSED, TAIL_SEPARATE = 0, 1, 2
+W_ROWMAJOR, W_KBLOCKED = 0, 1
 
 EXPORTS = [
     "laser_tau_params_default", "laser_probe_workspace_bytes", "laser_probe_plan_query",
@@ -27,7 +28,8 @@ EXPORTS = [
     "laser_last_error", "laser_kernel_launch_count", "laser_shutdown", "laser_profile_enable",
     "laser_profile_read", "laser_probe_options_default", "laser_probe_plan_query_mode",
     "laser_probe_confidence_opt", "laser_probe_partial", "laser_probe_combine",
-    "laser_probe_mixed_query", "laser_probe_flex_query", "laser_probe_handle_create", "laser_probe_handle_destroy", "laser_probe_handle_plan",
+    "laser_probe_mixed_query", "laser_probe_flex_query", "laser_probe_packed_w_bytes", "laser_probe_pack_w",
+    "laser_probe_handle_create", "laser_probe_handle_destroy", "laser_probe_handle_plan",
     "laser_probe_handle_workspace_bytes", "laser_probe_handle_run", "laser_probe_handle_run_host",
     "laser_sim_policy_default", "laser_sim_run",
 ]
@@ -84,11 +86,11 @@ class Options(C.Structure):
     """laser_probe_options (per call: aggregate, probability, kernel variant, overlap, tail)."""
     _fields_ = [("aggregate_mode", C.c_int32), ("prob_mode", C.c_int32), ("token_ids", C.c_void_p),
                 ("kernel_mode", C.c_int32), ("overlap", C.c_int32), ("tail", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("w_layout", C.c_int32)]
 
     def __init__(self, aggregate_mode=AGG_MEAN, prob_mode=PROB_MAX, token_ids=None, kernel_mode=MODE_AUTO,
-                 overlap=0, tail=TAIL_AUTO):
-        super().__init__(aggregate_mode, prob_mode, token_ids, kernel_mode, int(bool(overlap)), tail, 0)
+                 overlap=0, tail=TAIL_AUTO, w_layout=0):
+        super().__init__(aggregate_mode, prob_mode, token_ids, kernel_mode, int(bool(overlap)), tail, w_layout)
 
 
 MAX_PEERS = 16
@@ -146,6 +148,9 @@ def lib():
         L.laser_probe_options_default.argtypes = [C.POINTER(Options)]
         L.laser_probe_mixed_query.argtypes = [dp, C.c_int32, C.POINTER(Mixed)]
         L.laser_probe_flex_query.argtypes = [dp, C.c_int32, C.POINTER(Flex)]
+        L.laser_probe_packed_w_bytes.argtypes = [C.c_int32, C.c_int32]
+        L.laser_probe_packed_w_bytes.restype = C.c_size_t
+        L.laser_probe_pack_w.argtypes = [vp, C.c_int32, C.c_int32, vp, vp]
         L.laser_probe_handle_create.argtypes = [C.POINTER(C.c_void_p), dp, C.POINTER(Options)]
         L.laser_probe_handle_destroy.argtypes = [vp]
         L.laser_probe_handle_plan.argtypes = [vp, C.POINTER(Plan)]
@@ -207,6 +212,21 @@ def flex_query(N, d, V, R, n_valid) -> dict:
     m = Flex()
     _check(lib().laser_probe_flex_query(C.byref(Dims(N, d, V, R)), int(n_valid), C.byref(m)))
     return {n: getattr(m, n) for n, _ in m._fields_}
+
+
+def pack_w(W, stream=None):
+    """laser_probe_pack_w: bf16 [V, d] device tensor -> its K-block-major copy (a flat bf16 tensor of
+    laser_probe_packed_w_bytes(V, d) / 2 elements) for calls with w_layout=W_KBLOCKED.  Once per model."""
+    import torch
+    assert W.is_cuda and W.dtype == torch.bfloat16 and W.dim() == 2 and W.is_contiguous()
+    V, d = W.shape
+    nbytes = int(lib().laser_probe_packed_w_bytes(V, d))
+    if nbytes == 0:
+        raise LaserError(-2, "invalid W shape")
+    out = torch.empty(nbytes // 2, dtype=torch.bfloat16, device=W.device)
+    s = (stream or torch.cuda.current_stream(W.device)).cuda_stream
+    _check(lib().laser_probe_pack_w(W.data_ptr(), V, d, out.data_ptr(), s))
+    return out
 
 
 def workspace_bytes(N, d, V, R) -> int:
@@ -306,12 +326,13 @@ class Probe:
     laser_probe_confidence_opt."""
 
     def __init__(self, N, d, V, R, device="cuda", debug_outputs=True, mode=MODE_AUTO, overlap=False,
-                 tail=TAIL_AUTO, use_handle=True):
+                 tail=TAIL_AUTO, use_handle=True, w_layout=W_ROWMAJOR):
         import torch
         self.torch = torch
         self.dims = Dims(N, d, V, R)
         self.device = torch.device(device)
         self.mode, self.overlap, self.tail, self.use_handle = mode, bool(overlap), tail, use_handle
+        self.w_layout = w_layout           # W_KBLOCKED: every call's W is a pack_w() copy
         wb = workspace_bytes(N, d, V, R)
         if wb == 0:
             raise LaserError(-2, "invalid dimensions")
@@ -329,9 +350,9 @@ class Probe:
     def _options(self, agg, token_ids) -> Options:
         torch = self.torch
         if token_ids is None:
-            return Options(agg, PROB_MAX, None, self.mode, self.overlap, self.tail)
+            return Options(agg, PROB_MAX, None, self.mode, self.overlap, self.tail, self.w_layout)
         assert token_ids.dtype == torch.int32 and token_ids.numel() == self.dims.N and token_ids.is_contiguous()
-        return Options(agg, PROB_TOKEN, token_ids.data_ptr(), self.mode, self.overlap, self.tail)
+        return Options(agg, PROB_TOKEN, token_ids.data_ptr(), self.mode, self.overlap, self.tail, self.w_layout)
 
     def __call__(self, hidden, W, req_offsets, load, params: TauParams, stream=None, agg=AGG_MEAN,
                  token_ids=None):
@@ -343,7 +364,11 @@ class Probe:
         d = self.dims
         assert hidden.dtype == torch.bfloat16 and W.dtype == torch.bfloat16
         assert hidden.is_contiguous() and W.is_contiguous()
-        assert tuple(hidden.shape) == (d.N, d.d) and tuple(W.shape) == (d.V, d.d)
+        assert tuple(hidden.shape) == (d.N, d.d)
+        if self.w_layout == W_KBLOCKED:
+            assert W.numel() * 2 == lib().laser_probe_packed_w_bytes(d.V, d.d)    # a pack_w() copy
+        else:
+            assert tuple(W.shape) == (d.V, d.d)
         assert req_offsets.dtype == torch.int32 and req_offsets.numel() == d.R + 1
         assert load.dtype == torch.float32 and load.numel() == d.R
         s = (stream or torch.cuda.current_stream(self.device)).cuda_stream
@@ -383,10 +408,10 @@ class VocabShardProbe:
     pushes the records into every rank's gathered buffer itself and combine waits for the flags."""
 
     def __init__(self, N, d, V_shard, R, v_offset, world, device="cuda", debug_outputs=True, mode=MODE_AUTO,
-                 overlap=False, tail=TAIL_AUTO):
+                 overlap=False, tail=TAIL_AUTO, w_layout=W_ROWMAJOR):
         import torch
         self.torch = torch
-        self.options = Options(AGG_MEAN, PROB_MAX, None, mode, overlap, tail)
+        self.options = Options(AGG_MEAN, PROB_MAX, None, mode, overlap, tail, w_layout)
         self.dims = Dims(N, d, V_shard, R)
         self.v_offset, self.world = int(v_offset), int(world)
         self.device = torch.device(device)
@@ -411,7 +436,11 @@ class VocabShardProbe:
         torch, d = self.torch, self.dims
         assert hidden.dtype == torch.bfloat16 and W_shard.dtype == torch.bfloat16
         assert hidden.is_contiguous() and W_shard.is_contiguous()
-        assert tuple(hidden.shape) == (d.N, d.d) and tuple(W_shard.shape) == (d.V, d.d)
+        assert tuple(hidden.shape) == (d.N, d.d)
+        if self.options.w_layout == W_KBLOCKED:
+            assert W_shard.numel() * 2 == lib().laser_probe_packed_w_bytes(d.V, d.d)   # pack_w() of the shard
+        else:
+            assert tuple(W_shard.shape) == (d.V, d.d)
         assert req_offsets.dtype == torch.int32 and req_offsets.numel() == d.R + 1
         if token_ids is not None:
             assert token_ids.dtype == torch.int32 and token_ids.numel() == d.N
@@ -444,7 +473,8 @@ class HostProbe:
     """Host-buffer entry points: per-step tensors in pinned HOST memory, W resident on device.
     use_handle=True: laser_probe_handle_run_host; False: laser_probe_confidence_host[_async]."""
 
-    def __init__(self, N, d, V, R, device="cuda", use_handle=True, mode=MODE_AUTO, tail=TAIL_AUTO):
+    def __init__(self, N, d, V, R, device="cuda", use_handle=True, mode=MODE_AUTO, tail=TAIL_AUTO,
+                 w_layout=W_ROWMAJOR):
         import torch
         self.torch = torch
         self.dims = Dims(N, d, V, R)
@@ -456,7 +486,8 @@ class HostProbe:
         self.exit = torch.empty(R, dtype=torch.uint8).pin_memory()
         self.h2d_bytes = N * d * 2 + (R + 1) * 4 + R * 4   # upper bound: only valid rows are copied
         self.d2h_bytes = R * 4 + N * 4 + R
-        self.handle = Handle(self.dims, Options(kernel_mode=mode, tail=tail)) if use_handle else None
+        assert use_handle or w_layout == W_ROWMAJOR      # the handle-less host entry points take row-major W
+        self.handle = Handle(self.dims, Options(kernel_mode=mode, tail=tail, w_layout=w_layout)) if use_handle else None
 
     def _call(self, sync, h_hidden, W, h_req_offsets, h_load, params, stream):
         torch = self.torch

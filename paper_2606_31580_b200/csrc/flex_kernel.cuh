@@ -99,9 +99,9 @@ laser_probe_flex_kernel(const __grid_constant__ FlexMaps tm_hid, const __grid_co
                 if (slot < p.stages) {
                     if (rank == 0) ptx::mbar_expect_tx(full_bar(slot), 2u * kABytes);
                     ptx::tma_load_2d_pair(smem + static_cast<uint32_t>(slot) * p.stage_bytes, &tmap_w,
-                                          full0 + 8u * slot, kb * kBlockK, a_row, p.w_policy);
+                                          full0 + 8u * slot, w_c0(p, kb), w_c1(p, kb, a_row), p.w_policy);
                 } else {
-                    ptx::tma_prefetch_2d(&tmap_w, kb * kBlockK, a_row);
+                    ptx::tma_prefetch_2d(&tmap_w, w_c0(p, kb), w_c1(p, kb, a_row));
                 }
             }
             __syncwarp();
@@ -180,7 +180,7 @@ laser_probe_flex_kernel(const __grid_constant__ FlexMaps tm_hid, const __grid_co
                         ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
                         if (ptx::elect_one()) {
                             if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), tx2);
-                            ptx::tma_load_2d_pair(sa, &tmap_w, fb, kb * kBlockK, a_row, p.w_policy);
+                            ptx::tma_load_2d_pair(sa, &tmap_w, fb, w_c0(p, kb), w_c1(p, kb, a_row), p.w_policy);
                             ptx::tma_load_2d_pair(sa + kABytes, tmap_h, fb, kb * kBlockK, b_row, ptx::kEvictLast);
                         }
                     }

@@ -492,7 +492,7 @@ int options_valid(const laser_probe_options& o) {
     if (o.kernel_mode < LASER_MODE_AUTO || o.kernel_mode > LASER_MODE_MIXED) return LASER_E_MODE;
     if (o.tail < LASER_TAIL_AUTO || o.tail > LASER_TAIL_SEPARATE) return LASER_E_MODE;
     if (o.overlap != 0 && o.overlap != 1) return LASER_E_MODE;
-    if (o.reserved != 0) return LASER_E_MODE;
+    if (o.w_layout != LASER_W_ROWMAJOR && o.w_layout != LASER_W_KBLOCKED) return LASER_E_MODE;
     return LASER_OK;
 }
 
@@ -627,10 +627,14 @@ int launch_fused(Handle* h, int role, const void* hidden, const void* W, const i
     const CUtensorMap *tm_h = nullptr, *tm_w = nullptr;
     int rc = handle_tensor_map(h->hid, 2, &h->hid_rr, hidden, N, dims.d, a_rows, &tm_h);
     if (rc != LASER_OK) return rc;
-    rc = handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V, dims.d, b_rows, &tm_w);
+    // K-block-major W: k_blocks * V rows of 64 columns (one handle = one layout, so the cache key holds)
+    const bool w_kblocked = h->opt.w_layout == LASER_W_KBLOCKED;
+    if (w_kblocked) rc = handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V * ceil_div(dims.d, kBlockK), kBlockK, b_rows, &tm_w);
+    else rc = handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V, dims.d, b_rows, &tm_w);
     if (rc != LASER_OK) return rc;
 
     FusedParams fp{};
+    fp.w_kb_rows = w_kblocked ? dims.V : 0;
     fp.n_alloc = N; fp.d = dims.d; fp.V = dims.V;
     fp.pd = plan_desc(h, req_offsets);
     fp.role = role;
@@ -707,7 +711,9 @@ int launch_flex(Handle* h, const void* hidden, const void* W, const int32_t* req
         attr_set[dev] = true;
     }
     const CUtensorMap* tm_w = nullptr;
-    int rc = handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V, dims.d, kTileM, &tm_w);
+    const bool w_kblocked = h->opt.w_layout == LASER_W_KBLOCKED;
+    int rc = w_kblocked ? handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V * ceil_div(dims.d, kBlockK), kBlockK, kTileM, &tm_w)
+                        : handle_tensor_map(h->w, 4, &h->w_rr, W, dims.V, dims.d, kTileM, &tm_w);
     if (rc != LASER_OK) return rc;
     Handle::FlexEntry* fe = nullptr;
     for (auto& e : h->flex_hid)
@@ -725,6 +731,7 @@ int launch_flex(Handle* h, const void* hidden, const void* W, const int32_t* req
     }
 
     FusedParams fp{};
+    fp.w_kb_rows = w_kblocked ? dims.V : 0;
     fp.n_alloc = dims.N; fp.d = dims.d; fp.V = dims.V;
     fp.pd = plan_desc(h, req_offsets);
     fp.role = 0;
@@ -1116,12 +1123,12 @@ int run_host(Handle* h, const void* h_hidden, const void* W, const int32_t* h_re
 struct ImplicitKey {
     int device;
     laser_probe_dims dims;
-    int32_t agg, prob, mode, overlap, tail;
+    int32_t agg, prob, mode, overlap, tail, w_layout;
     const void* workspace;
     bool operator==(const ImplicitKey& o) const {
         return device == o.device && dims.N == o.dims.N && dims.d == o.dims.d && dims.V == o.dims.V &&
                dims.R == o.dims.R && agg == o.agg && prob == o.prob && mode == o.mode &&
-               overlap == o.overlap && tail == o.tail && workspace == o.workspace;
+               overlap == o.overlap && tail == o.tail && w_layout == o.w_layout && workspace == o.workspace;
     }
 };
 struct ImplicitCache {
@@ -1147,7 +1154,7 @@ int implicit_handle(const laser_probe_dims& dims, const laser_probe_options& opt
         g_cache_seen = gen;
     }
     const ImplicitKey key{dev, dims, opt.aggregate_mode, opt.prob_mode, opt.kernel_mode, opt.overlap, opt.tail,
-                          workspace};
+                          opt.w_layout, workspace};
     for (auto& e : c.entries)
         if (e.key == key) { e.stamp = ++c.clock; *out = e.h; return LASER_OK; }
     Handle* h = nullptr;
@@ -1174,6 +1181,31 @@ extern "C" {
 int laser_tau_params_default(laser_tau_params* out) {
     if (!out) return LASER_E_NULL;
     *out = laser_tau_params{0.95f, 0.04f, 1.0f, 10.0f, 0.88f, 0.97f};
+    return LASER_OK;
+}
+
+size_t laser_probe_packed_w_bytes(int32_t V, int32_t d) {
+    if (V <= 0 || d <= 0 || (d % 8) != 0) return 0;
+    return static_cast<size_t>(ceil_div(d, kBlockK)) * static_cast<size_t>(V) * 128u;
+}
+
+int laser_probe_pack_w(const void* W, int32_t V, int32_t d, void* W_packed, void* stream_v) {
+    if (!W || !W_packed) return LASER_E_NULL;
+    if (V <= 0 || d <= 0 || (d % 8) != 0) return LASER_E_DIMS;
+    if ((reinterpret_cast<uintptr_t>(W) & 15) || (reinterpret_cast<uintptr_t>(W_packed) & 15)) return LASER_E_ALIGN;
+    DeviceInfo* di = nullptr;
+    int rc = require_b200(&di);
+    if (rc != LASER_OK) return rc;
+    const int k_blocks = ceil_div(d, kBlockK);
+    const int64_t total = static_cast<int64_t>(k_blocks) * V * 8;
+    int64_t blocks = (total + 255) / 256;
+    const int64_t cap = static_cast<int64_t>(di->sms) * 16;
+    if (blocks > cap) blocks = cap;
+    laser_probe_pack_w_kernel<<<static_cast<unsigned>(blocks), 256, 0, static_cast<cudaStream_t>(stream_v)>>>(
+        static_cast<const uint4*>(W), static_cast<uint4*>(W_packed), V, d, k_blocks);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return set_cuda_error("launch laser_probe_pack_w_kernel", e);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
     return LASER_OK;
 }
 

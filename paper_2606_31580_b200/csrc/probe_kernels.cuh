@@ -219,7 +219,13 @@ struct FusedParams {
     // producer requests the W boxes of its first tiles under this guess ahead of the wait; when
     // req_offsets[R] then says otherwise the boxes are dropped (0: nothing is requested early).
     int32_t hint_C, hint_S;
+    // W layout (laser_probe_options.w_layout).  0: row-major [V, d].  V (> 0): K-block-major
+    // [ceil(d/64)][V][64] (laser_probe_pack_w): the tensor map sees k_blocks * V rows of 64 columns, the box
+    // of (k-block kb, W row r) is at row kb * V + r and is ONE contiguous run of bytes in HBM.
+    int32_t w_kb_rows;
 };
+__device__ __forceinline__ int w_c0(const FusedParams& p, int kb) { return p.w_kb_rows ? 0 : kb * kBlockK; }
+__device__ __forceinline__ int w_c1(const FusedParams& p, int kb, int row) { return row + kb * p.w_kb_rows; }
 
 // ---------------------------------------------------------------------------------- descriptors
 // Shared-memory matrix descriptor, K-major operand, 128-byte swizzle: rows of 128 B, 8-row groups
@@ -639,6 +645,22 @@ laser_probe_stage_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst,
     for (int64_t i = tid + kStageInFlight * nthreads; i < n16; i += nthreads) dst[i] = ptx::ld_nc_v4(src + i);
 }
 
+// laser_probe_pack_w: [V, d] row-major -> [ceil(d/64)][V][64] (K-block-major), 16 bytes per thread and step;
+// columns past d are zero.  Reads are 128-byte runs per row, writes are fully contiguous.
+__global__ void __launch_bounds__(256)
+laser_probe_pack_w_kernel(const uint4* __restrict__ W, uint4* __restrict__ out, int V, int d, int k_blocks) {
+    const int64_t total = static_cast<int64_t>(k_blocks) * V * 8;     // 16-byte chunks of the packed buffer
+    const int d16 = d >> 3;                                           // 16-byte chunks per row of W
+    for (int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < total;
+         i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+        const int c = static_cast<int>(i & 7);
+        const int64_t r = i >> 3;                 // kb * V + v
+        const int kb = static_cast<int>(r / V), v = static_cast<int>(r - static_cast<int64_t>(kb) * V);
+        const int col16 = kb * 8 + c;
+        out[i] = col16 < d16 ? W[static_cast<int64_t>(v) * d16 + col16] : make_uint4(0u, 0u, 0u, 0u);
+    }
+}
+
 // LASER_DEBUG=1: the documented precondition on req_offsets (non-decreasing, [0] == 0, [R] <= N),
 // checked on the device by one warp ahead of the probe; a violation traps (the caller sees a CUDA
 // error at the next synchronisation) instead of silently reading other requests' rows.
@@ -888,13 +910,13 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                     const uint32_t fb = full0 + 8u * slot;
                     if constexpr (kPair) {
                         if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(slot), 2u * p.tx_bytes);
-                        ptx::tma_load_2d_pair(sb, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
+                        ptx::tma_load_2d_pair(sb, &tmap_w, fb, w_c0(p, kb), w_c1(p, kb, b_row), p.w_policy);
                     } else {
                         ptx::mbar_arrive_expect_tx(fb, p.tx_bytes);
-                        ptx::tma_load_2d(sb, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
+                        ptx::tma_load_2d(sb, &tmap_w, fb, w_c0(p, kb), w_c1(p, kb, b_row), p.w_policy);
                     }
                 } else {
-                    ptx::tma_prefetch_2d(&tmap_w, kb * kBlockK, b_row);
+                    ptx::tma_prefetch_2d(&tmap_w, w_c0(p, kb), w_c1(p, kb, b_row));
                 }
             }
             __syncwarp();
@@ -1003,11 +1025,11 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
                                 // both CTAs' bytes complete on the leader's barrier
                                 if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), 2u * p.tx_bytes);
                                 ptx::tma_load_2d_pair(sa, &tmap_hidden, fb, kb * kBlockK, a_row, ptx::kEvictLast);
-                                ptx::tma_load_2d_pair(sa + kABytes, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
+                                ptx::tma_load_2d_pair(sa + kABytes, &tmap_w, fb, w_c0(p, kb), w_c1(p, kb, b_row), p.w_policy);
                             } else {
                                 ptx::mbar_arrive_expect_tx(fb, p.tx_bytes);
                                 ptx::tma_load_2d(sa, &tmap_hidden, fb, kb * kBlockK, a_row, ptx::kEvictLast);
-                                ptx::tma_load_2d(sa + kABytes, &tmap_w, fb, kb * kBlockK, b_row, p.w_policy);
+                                ptx::tma_load_2d(sa + kABytes, &tmap_w, fb, w_c0(p, kb), w_c1(p, kb, b_row), p.w_policy);
                             }
                         }
                     }

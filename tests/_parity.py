@@ -24,7 +24,7 @@ TAU_TOL = 2e-6
 
 # How run_gpu() calls the library (laser_probe_options fields + which entry point).  Test-side state:
 # the fixtures of the GPU tests switch it to run the same case through every variant.
-CFG = dict(mode=0, tail=0, overlap=False, use_handle=True)
+CFG = dict(mode=0, tail=0, overlap=False, use_handle=True, w_layout=0)
 
 
 @dataclass
@@ -52,6 +52,8 @@ def run_gpu(w, dev=None, agg=0, tau_params=None) -> GpuRun:
     import torch
     from paper_2606_31580_b200 import binding as B
     dev = dev or to_device(w)
+    if CFG["w_layout"] == B.W_KBLOCKED:         # the K-block-major copy of W (laser_probe_pack_w)
+        dev = dict(dev, W=B.pack_w(dev["W"]))
     probe = B.Probe(w.N_alloc, w.d, w.V, w.R, **CFG)
     # poison outputs so that unwritten entries are caught
     probe.conf.fill_(-7.0); probe.argmax.fill_(-7); probe.exit.fill_(7)

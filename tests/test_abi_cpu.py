@@ -124,6 +124,19 @@ def test_flex_plan_invariants(dims):
         assert B.plan_query(5000, d, V, R, mode=B.MODE_FLEX)["flex"] == 0
 
 
+def test_packed_w_size_and_argument_checks():
+    """K-block-major W (laser_probe_pack_w): size formula and argument validation (no GPU needed)."""
+    L = B.lib()
+    assert L.laser_probe_packed_w_bytes(151936, 1536) == 24 * 151936 * 128 == 151936 * 1536 * 2
+    assert L.laser_probe_packed_w_bytes(1000, 72) == 2 * 1000 * 128          # d padded to the next 64 columns
+    assert L.laser_probe_packed_w_bytes(0, 64) == 0 and L.laser_probe_packed_w_bytes(10, 60) == 0
+    buf = (C.c_char * 4096)()
+    a = C.addressof(buf)
+    assert L.laser_probe_pack_w(None, 10, 64, a, None) == -1 and L.laser_probe_pack_w(a, 10, 64, None, None) == -1
+    assert L.laser_probe_pack_w(a, 10, 60, a + 2048, None) == -2 and L.laser_probe_pack_w(a, 0, 64, a + 2048, None) == -2
+    assert L.laser_probe_pack_w(a + 4, 10, 64, a + 2048, None) == -3
+
+
 def test_forced_modes_plan():
     p = B.plan_query(32, 64, 1000, 8, mode=B.MODE_PAIR)
     assert p["cta_pair"] == 1 and p["tile_m"] == 256 and p["grid"] % 2 == 0 and p["tile_n"] % 32 == 0
@@ -140,7 +153,7 @@ def test_options_are_per_call_and_validated():
     L = B.lib()
     o = B.Options(7, 7, None, 7, 1, 7)
     assert L.laser_probe_options_default(C.byref(o)) == 0
-    assert (o.aggregate_mode, o.prob_mode, o.token_ids, o.kernel_mode, o.overlap, o.tail, o.reserved) == \
+    assert (o.aggregate_mode, o.prob_mode, o.token_ids, o.kernel_mode, o.overlap, o.tail, o.w_layout) == \
         (0, 0, None, 0, 0, 0, 0)
     assert not hasattr(L, "laser_probe_set_mode") and not hasattr(L, "laser_probe_set_overlap")
     buf = (C.c_char * 4096)()
@@ -152,7 +165,7 @@ def test_options_are_per_call_and_validated():
         assert call(bad) == -8                                              # LASER_E_MODE
     o = B.Options(); o.overlap = 2
     assert call(o) == -8
-    o = B.Options(); o.reserved = 1
+    o = B.Options(); o.w_layout = 2
     assert call(o) == -8
     assert call(B.Options(prob_mode=B.PROB_TOKEN)) == -1                    # token ids missing
     h = C.c_void_p()

@@ -48,11 +48,19 @@ def test_c1_tiny(P):
     assert st["exits"] >= 1                                   # the mask is exercised (DESIGN A16)
 
 
-def test_c2_qwen15b_full(P, c2_W_bits):
-    """The graded config, every row and request, in the launch configuration bench.py times."""
+@pytest.mark.parametrize("w_layout", [0, 1])
+def test_c2_qwen15b_full(P, c2_W_bits, w_layout):
+    """The graded config, every row and request, in the launch configuration bench.py times (W row-major,
+    and its K-block-major copy from laser_probe_pack_w)."""
     w = wl.config_c2(c2_W_bits)
-    st = P.check(w)
-    _log("C2", st)
+    P.CFG["w_layout"] = w_layout
+    try:
+        g = P.run_gpu(w)
+    finally:
+        P.CFG["w_layout"] = 0
+    ora, rows, reqs = _oracle_once(P, "C2", w)
+    st = P.compare(w, g, ora, rows, reqs, f"C2/w_layout{w_layout}")
+    _log("C2" if w_layout == 0 else "C2/kblocked", st)
     assert st["rows"] == 128 and st["requests"] == 16 and 0 < st["exits"] < 16
 
 

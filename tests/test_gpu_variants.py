@@ -278,6 +278,68 @@ def test_vocab_parallel_process_group_world1(P, exchange):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------- K-block-major W
+@pytest.mark.parametrize("V,d", [(1000, 64), (33000, 512), (70001, 72), (17, 8), (5000, 200)])
+def test_pack_w_layout(V, d):
+    """laser_probe_pack_w against the layout's definition, bit for bit: out[kb][v][c] = W[v][64 kb + c],
+    zero where 64 kb + c >= d."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    g = torch.Generator(device="cuda").manual_seed(V + d)
+    W = torch.randn((V, d), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
+    packed = B.pack_w(W)
+    kb = -(-d // 64)
+    assert packed.numel() == kb * V * 64
+    ref = torch.zeros((V, kb * 64), dtype=torch.bfloat16, device="cuda")
+    ref[:, :d] = W
+    ref = ref.view(V, kb, 64).permute(1, 0, 2).contiguous().view(-1)
+    torch.cuda.synchronize()
+    assert torch.equal(packed.view(torch.int16), ref.view(torch.int16))
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
+    (33000, 512, 40, None, 400, (1, 16)),   # several token tiles / chunks, padding rows
+    (70001, 72, 12, 8, None, None),         # d not a multiple of 64: zero columns in the packed copy, odd V
+    (5000, 200, 3, 60, None, None),         # N = 180, V not a multiple of the tile heights
+])
+def test_kblocked_w_matches_oracle(P, mode, V, d, R, L, n_alloc, var_len):
+    """Every kernel variant with W given K-block-major (laser_probe_options.w_layout): boxes that run past
+    row V of a k-block slab read the next slab's rows, which the epilogue masks like TMA's zero fill."""
+    from paper_2606_31580_b200 import binding as B
+    w = wl.scaled(f"kblocked-m{mode}-V{V}-d{d}", V, d, 0.05, R, L, seed=V + d + 3, N_alloc=n_alloc, var_len=var_len)
+    P.CFG.update(mode=mode, w_layout=B.W_KBLOCKED)
+    try:
+        st = P.check(w)
+    finally:
+        P.CFG.update(mode=0, w_layout=0)
+    print(w.name, {k: v for k, v in st.items() if k != "plan"})
+
+
+def test_kblocked_w_ties_at_the_slab_boundary(P):
+    """Duplicate winning rows at the very end of the vocabulary (the last box runs into the next k-block
+    slab) and across a tile boundary, K-block-major W: the lowest index wins, rows past V never do."""
+    from paper_2606_31580_b200 import binding as B
+    V, d, N = 9001, 128, 16
+    rng = np.random.default_rng(21)
+    Wf = (rng.standard_normal((V, d)) * 0.05).astype(np.float32)
+    h = rng.standard_normal((N, d)).astype(np.float32)
+    big = (h[0] * 0.5).astype(np.float32)
+    P.CFG.update(w_layout=B.W_KBLOCKED)
+    try:
+        for v1, v2 in [(V - 2, V - 1), (207, 208), (3, V - 1)]:
+            W2 = Wf.copy(); W2[v1] = big; W2[v2] = big
+            w = wl.Workload("ties-kblocked", wl.bf16_bits(W2), wl.bf16_bits(h), wl.fixed_offsets(2, 8),
+                            np.array([0.3, 0.7], np.float32))
+            g = P.run_gpu(w)
+            assert g.argmax[0] == v1, (v1, v2, g.argmax[0])
+            ora, rows, reqs = P.run_oracle(w)
+            assert ora.argmax[0] == v1 and ora.gap2[0] == 0.0
+            P.compare(w, g, ora, rows, reqs, "ties-kblocked")
+    finally:
+        P.CFG.update(w_layout=0)
+
+
 # ------------------------------------------------------------------------------- seeded shape fuzz
 def _fuzz_case(i):
     rng = np.random.default_rng(4242 + i)
