@@ -93,7 +93,7 @@ laser_probe_flex_kernel(const __grid_constant__ FlexMaps tm_hid, const __grid_co
     if (warp == 0 && p.wait_first && p.hint_C > 0 && unit < p.hint_C * p.hint_S) {
         const uint32_t full0 = ptx::mapa(full_bar(0), 0u);
         int tile = unit / p.hint_C, kb = 0;
-        for (int slot = 0; slot < 2 * p.stages && tile < total_tiles; ++slot) {
+        for (int slot = 0; slot < p.stages + p.prefetch_slots && tile < total_tiles; ++slot) {
             if (ptx::elect_one()) {
                 const int a_row = tile * kFlexVocabTile + static_cast<int>(rank) * kTileM;
                 if (slot < p.stages) {

@@ -223,6 +223,8 @@ struct FusedParams {
     // [ceil(d/64)][V][64] (laser_probe_pack_w): the tensor map sees k_blocks * V rows of 64 columns, the box
     // of (k-block kb, W row r) is at row kb * V + r and is ONE contiguous run of bytes in HBM.
     int32_t w_kb_rows;
+    // W boxes the producer asks L2 for ahead of the wait, behind the `stages` boxes it requests into shared memory
+    int32_t prefetch_slots;
 };
 __device__ __forceinline__ int w_c0(const FusedParams& p, int kb) { return p.w_kb_rows ? 0 : kb * kBlockK; }
 __device__ __forceinline__ int w_c1(const FusedParams& p, int kb, int row) { return row + kb * p.w_kb_rows; }
@@ -902,7 +904,7 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
         if (!(p.wait_first && static_plan && unit < work_items)) return;
         const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);
         int tile = unit / m_items, kb = 0;
-        for (int slot = 0; slot < 2 * p.stages && tile < total_tiles; ++slot) {
+        for (int slot = 0; slot < p.stages + p.prefetch_slots && tile < total_tiles; ++slot) {
             if (ptx::elect_one()) {
                 const int b_row = tile * BN + static_cast<int>(rank) * b_rows;
                 if (slot < p.stages) {
