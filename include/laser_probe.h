@@ -86,7 +86,7 @@ typedef struct {
     int32_t ws_records;      /* 16-byte workspace records (the most any re-plan of the batch writes)  */
     int32_t tail_cache;      /* requests whose {offset, threshold} the fused kernel's tail keeps in the
                                 shared memory the pipeline leaves over (0: read from global memory)    */
-    /* Mixed schedule (AUTO, N > 256 rows): the fields above describe the CTA-pair kernel (256-row
+    /* Mixed schedule (AUTO for N > 1024 rows, LASER_MODE_MIXED for N > 256): the fields above describe the CTA-pair kernel (256-row
      * items); when the number of 128-row tiles that hold rows is odd, the last tile runs on single CTAs
      * in a second kernel beside it.  The split of the SMs is decided on the device from
      * req_offsets[R].  kernel_launches = 2: tail-tile kernel, pair kernel (a3-a5 in the tail of
@@ -96,9 +96,8 @@ typedef struct {
     int32_t tail_stages;     /* its pipeline depth                                                    */
     int32_t tail_smem_bytes; /* its dynamic shared memory per CTA                                     */
     int32_t tail_grid;       /* its CTAs (those it does not need exit at once)                        */
-    /* Flex kernel (LASER_MODE_FLEX; AUTO for 129 <= N <= 4096 rows where the planner's cost model
-     * prefers it): vocabulary on the MMA M axis (tile_n = 256 rows of W per CTA pair), tokens on N in
-     * chunks of flex_n_tok rows (a multiple of 16, <= 256), so that a batch pays for at most 15 padding
+    /* Flex kernel (LASER_MODE_FLEX up to 4096 rows; AUTO for 129 <= N <= 1024 rows except exactly
+     * 256): vocabulary on the MMA M axis (tile_n = 256 rows of W per CTA pair), tokens on N in chunks of flex_n_tok rows (a multiple of 16, <= 256), so that a batch pays for at most 15 padding
      * rows per chunk.  m_tiles = chunks, splits / tiles_per_split per chunk, all for a batch whose N
      * rows are valid; the kernel looks the decomposition for req_offsets[R] up in a table the host
      * planned (laser_probe_flex_query).  One launch per call. */

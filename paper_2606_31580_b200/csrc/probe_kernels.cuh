@@ -1,4 +1,5 @@
-// probe_kernels.cuh — the two kernels of the LASER confidence probe (sm_100a).
+// probe_kernels.cuh — kernels of the LASER confidence probe (sm_100a) and what they share with
+// flex_kernel.cuh (laser_probe_flex_kernel: the same path with the vocabulary on the MMA M axis).
 //
 //  laser_probe_fused_kernel   a1 + a2 of include/laser_probe.h: LM-head projection on tcgen05 tensor
 //                             cores with the online-softmax statistics (max, lowest-index argmax,
@@ -74,7 +75,7 @@ __host__ __device__ inline SplitPlan plan_splits(int total_tiles, int m_items, i
 }
 
 // ---------------------------------------------------------------------------------- call plans
-// Mixed schedule (N > 128 rows, kernel_mode AUTO): the token rows are cut into 128-row tiles; an even
+// Mixed schedule (kernel_mode AUTO above 1024 rows, MIXED above 256): the token rows are cut into 128-row tiles; an even
 // count runs as 256-row items on CTA pairs (cta_group::2); of an odd count the LAST 128-row tile runs
 // on single CTAs (cta_group::1) instead of being padded to a pair item.  cta_group is a property of a
 // kernel, so a call is two launches - the single-CTA ("tail-tile") kernel first, the pair kernel
