@@ -251,7 +251,7 @@ MixedChoice plan_mixed_host(int m128, int V, int d, int bn_pair, int bn_tail, in
 // splits of 256-row tiles on the CTA pairs.  Cost of a (tile, chunk): the MMAs take time in proportion to
 // n_tok; staging the 256 W rows, the pipeline bubble between tiles and the epilogue's fixed part are charged
 // as kFlexTileCharge token rows.  Among the chunk counts that cover the rows the cheapest busiest pair wins.
-struct FlexChoice { int C, n_tok, S, T, rounds; double cost; };
+struct FlexChoice { int C, n_tok, S, T, rounds; double cost; long busiest; };
 double flex_tile_charge() {
     static const double v = [] {
         const char* e = getenv("LASER_FLEX_TILE_CHARGE");
@@ -262,7 +262,7 @@ double flex_tile_charge() {
 FlexChoice plan_flex_host(int n_valid, int V, int sms) {
     const int pairs = sms / 2 > 0 ? sms / 2 : 1;
     const int tiles = ceil_div(V, kFlexVocabTile);
-    FlexChoice best{0, 16, 1, tiles, 0, 1e300};
+    FlexChoice best{0, 16, 1, tiles, 0, 1e300, 0};
     if (n_valid <= 0) { best.cost = 0.0; return best; }
     const int c_min = ceil_div(n_valid, kFlexMaxTok);
     for (int C = c_min; C <= c_min + 3 && C <= 31; ++C) {
@@ -287,7 +287,7 @@ FlexChoice plan_flex_host(int n_valid, int V, int sms) {
                 if (tl > busiest) busiest = tl;
             }
             const double cost = static_cast<double>(busiest) * (n_tok + flex_tile_charge()) + 8.0 * rounds;
-            if (cost < best.cost - 1e-9) best = FlexChoice{C, n_tok, S, T, static_cast<int>(rounds), cost};
+            if (cost < best.cost - 1e-9) best = FlexChoice{C, n_tok, S, T, static_cast<int>(rounds), cost, busiest};
         }
     }
     return best;
@@ -299,7 +299,7 @@ void make_flex_plan(const laser_probe_dims& dm, int num_sms, laser_probe_plan* p
     const int groups = ceil_div(dm.N, 16);
     int max_tok = 16;
     long ws_records = 1;
-    FlexChoice dense{0, 16, 1, 1, 0, 0.0};
+    FlexChoice dense{0, 16, 1, 1, 0, 0.0, 0};
     for (int g = 1; g <= kMixedTabMax; ++g) {
         const int gg = g <= groups ? g : (groups > 0 ? groups : 1);
         const int n_valid = gg * 16 < dm.N ? gg * 16 : (dm.N > 0 ? dm.N : 16);
@@ -351,7 +351,18 @@ void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_pl
     // C4 shapes: it wins wherever the rows do not fill 256-row items - N = 320: 130 vs 151 us,
     // C4's 590 of 1024 rows: 456 vs 508 us - and ties at 512 / 768 / 1024; a dense 256-row batch is the
     // one case where its fixed 256-row vocabulary tiles quantise worse than the pair kernel's).
-    const bool auto_flex = mode == LASER_MODE_AUTO && dm.N > kTileM && dm.N <= 1024 && dm.N != 2 * kTileM;
+    bool auto_flex = mode == LASER_MODE_AUTO && dm.N > kTileM && dm.N <= 1024 && dm.N != 2 * kTileM;
+    if (auto_flex) {
+        // The flex kernel's vocabulary tiles are 256 rows whatever V is: with few tiles per pair (a small
+        // vocabulary, a vocabulary shard) whole-tile quantisation can leave the busiest pair far above the
+        // average - V = 18992 rows are 75 tiles for 74 pairs, one pair takes two.  The pair kernel picks its
+        // tile height to fit, so AUTO keeps the former schedule when the busiest pair would carry more than
+        // 15 % above an even share (C2's shape: 9 tiles against 8.03, 12 %).
+        const FlexChoice c = plan_flex_host(dm.N, dm.V, num_sms);
+        const int pairs = num_sms / 2 > 0 ? num_sms / 2 : 1;
+        const double even = static_cast<double>(ceil_div(dm.V, kFlexVocabTile)) * c.C / pairs;
+        if (static_cast<double>(c.busiest) > 1.15 * (even > 1.0 ? even : 1.0)) auto_flex = false;
+    }
     if ((mode == LASER_MODE_FLEX && dm.N > 0 && dm.N <= kFlexMaxRows) || auto_flex) {
         make_flex_plan(dm, num_sms, pl, nullptr);
         return;

@@ -53,6 +53,7 @@ def test_plan_invariants(dims):
     N, d, V, R = dims
     p = B.plan_query(*dims)
     # AUTO: the flex kernel for 129..1024 rows except exactly 256 (checked in test_flex_plan_invariants)
+    # unless its fixed 256-row vocabulary tiles quantise badly (test_auto_avoids_flex_for_badly_quantised_vocabularies)
     assert p["flex"] == (1 if (128 < N <= 1024 and N != 256) else 0)
     if p["flex"]:
         p = B.plan_query(*dims, mode=B.MODE_MIXED)
@@ -135,6 +136,17 @@ def test_packed_w_size_and_argument_checks():
     assert L.laser_probe_pack_w(None, 10, 64, a, None) == -1 and L.laser_probe_pack_w(a, 10, 64, None, None) == -1
     assert L.laser_probe_pack_w(a, 10, 60, a + 2048, None) == -2 and L.laser_probe_pack_w(a, 0, 64, a + 2048, None) == -2
     assert L.laser_probe_pack_w(a + 4, 10, 64, a + 2048, None) == -3
+
+
+def test_auto_avoids_flex_for_badly_quantised_vocabularies():
+    """AUTO keeps the pair / mixed schedule when whole 256-row tiles would leave the busiest pair more than
+    15 % above an even share: a G = 8 vocabulary shard of C2 is 75 tiles for 74 pairs."""
+    for N in (200, 400, 640, 1024):
+        p = B.plan_query(N, 1536, 18992, 16)
+        assert p["flex"] == 0 and p["cta_pair"] == 1, (N, p)
+        assert B.plan_query(N, 1536, 18992, 16, mode=B.MODE_FLEX)["flex"] == 1        # still available when forced
+        assert B.plan_query(N, 1536, 151936, 16)["flex"] == 1                          # the whole vocabulary: 12 % at worst
+        assert B.plan_query(N, 64, 1000, 16)["flex"] == 1                              # fewer tiles than pairs: nothing to balance
 
 
 def test_forced_modes_plan():
