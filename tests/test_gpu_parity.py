@@ -643,3 +643,42 @@ def test_cuda_graph_capture_and_replay(P, c2_W_bits):
         torch.cuda.synchronize(); e0.record(); g.replay(); e1.record(); torch.cuda.synchronize()
         ts.append(e0.elapsed_time(e1) * 1e3)
     print("graph replay, one call: median %.1f us" % sorted(ts)[len(ts) // 2])
+
+
+def test_cuda_graph_replay_replans_the_flex_kernel(P):
+    """The flex kernel decides chunks and splits from req_offsets[R] on the device, so ONE captured graph
+    serves batches with different numbers of valid rows in the same allocation: a dense batch (the guess
+    its W boxes are requested under holds), a half-empty one and a nearly empty one (the guess is dropped)."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    V, d, n_alloc = 33000, 512, 640
+    w0 = wl.scaled("graph-flex-dense", V, d, 0.05, 80, 8, seed=61, N_alloc=n_alloc)
+    mk = lambda name, seed, var_len: wl._qwen_like(name, V, d, 0.05, 80, None, 0.9, seed, "uniform", W_bits=w0.W_bits,
+                                                   N_alloc=n_alloc, var_len=var_len)     # the same W: it is in the graph
+    ws = [w0, mk("graph-flex-half", 62, (1, 8)), mk("graph-flex-few", 63, (0, 1))]
+    assert ws[0].N_valid == n_alloc and ws[1].N_valid < 400 and ws[2].N_valid < 100
+    chunks = {B.flex_query(n_alloc, d, V, 80, w.N_valid)["chunks"] for w in ws}
+    assert len(chunks) >= 2                                   # the replays really take different decompositions
+    devs = [P.to_device(w) for w in ws]
+    hidden, off, load = devs[0]["hidden"].clone(), devs[0]["off"].clone(), devs[0]["load"].clone()
+    probe = B.Probe(n_alloc, d, V, 80)
+    assert probe.plan["flex"] == 1
+    tp = B.TauParams(**ws[0].tau_params)
+    probe(hidden, devs[0]["W"], off, load, tp)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            probe(hidden, devs[0]["W"], off, load, tp, stream=side)
+    for k in (0, 1, 2, 1, 0):
+        w, dv = ws[k], devs[k]
+        hidden.copy_(dv["hidden"]); off.copy_(dv["off"]); load.copy_(dv["load"])
+        probe.conf.fill_(-7.0); probe.argmax.fill_(-7); probe.exit.fill_(7); probe.pmax.fill_(-7.0)
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        run = P.GpuRun(probe.conf.cpu().numpy(), probe.argmax.cpu().numpy(), probe.exit.cpu().numpy(),
+                       probe.tau.cpu().numpy(), probe.pmax.cpu().numpy(), probe.plan)
+        ora, rows, reqs = P.run_oracle(w)
+        P.compare(w, run, ora, rows, reqs, f"flex graph replay {w.name}")

@@ -65,12 +65,14 @@ def _compare_token_mode(P, w, g, ora, pt, conf, ex, margin, label):
 
 
 @pytest.mark.parametrize("agg", [0, 1])
-@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len", [
-    (33000, 512, 12, 8, None, None),          # one token tile, several vocabulary tiles, ragged V
-    (9000, 256, 40, None, 400, (1, 16)),      # several token tiles (pair variant), padding rows
-    (1000, 64, 8, 4, None, None),             # C1 shape
+@pytest.mark.parametrize("V,d,R,L,n_alloc,var_len,mode", [
+    (33000, 512, 12, 8, None, None, 0),       # one token tile, several vocabulary tiles, ragged V
+    (9000, 256, 40, None, 400, (1, 16), 0),   # several token chunks (flex kernel), padding rows
+    (9000, 256, 40, None, 400, (1, 16), 4),   # the same through the mixed schedule (pair + single-CTA kernels)
+    (9000, 256, 40, None, 400, (1, 16), 2),   # ... and the pair kernel alone
+    (1000, 64, 8, 4, None, None, 0),          # C1 shape
 ])
-def test_token_prob_mode(P, V, d, R, L, n_alloc, var_len, agg):
+def test_token_prob_mode(P, V, d, R, L, n_alloc, var_len, mode, agg):
     """LASER_PROB_TOKEN: conf aggregates softmax(logits)[token_ids[n]] instead of the row maximum."""
     import torch
     from paper_2606_31580_b200 import binding as B
@@ -79,7 +81,8 @@ def test_token_prob_mode(P, V, d, R, L, n_alloc, var_len, agg):
     tok = _token_ids(w, ora, seed=5)
     pt, conf, ex, margin = _oracle_token_mode(w, ora, tok, agg)
     dev = P.to_device(w)
-    probe = B.Probe(w.N_alloc, w.d, w.V, w.R)
+    probe = B.Probe(w.N_alloc, w.d, w.V, w.R, mode=mode)
+    assert probe.plan["flex"] == (1 if (mode == 0 and w.N_alloc > 128) else 0)
     probe.conf.fill_(-7.0); probe.argmax.fill_(-7); probe.exit.fill_(7); probe.pmax.fill_(-7.0)
     out = probe(dev["hidden"], dev["W"], dev["off"], dev["load"], B.TauParams(**w.tau_params), agg=agg,
                 token_ids=torch.from_numpy(tok).cuda())
