@@ -682,3 +682,52 @@ def test_cuda_graph_replay_replans_the_flex_kernel(P):
                        probe.tau.cpu().numpy(), probe.pmax.cpu().numpy(), probe.plan)
         ora, rows, reqs = P.run_oracle(w)
         P.compare(w, run, ora, rows, reqs, f"flex graph replay {w.name}")
+
+
+def test_flex_back_to_back_with_changing_row_counts(P):
+    """Stress of the flex kernel's guess-and-drop protocol under programmatic dependent launch: 10 x 48 calls
+    enqueued back to back through ONE handle and ONE workspace, cycling over batches whose valid-row count
+    makes the kernel keep (dense) or drop (padded) the W boxes it requested ahead of the wait, with a
+    different decomposition from one call to the next.  Every call's outputs must be bit-identical to those
+    of the same batch run alone, which are checked against the oracle."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    V, d, n_alloc, R = 33000, 512, 640, 80
+    w0 = wl.scaled("stress-flex-dense", V, d, 0.05, R, 8, seed=71, N_alloc=n_alloc)
+    mk = lambda name, seed, var_len: wl._qwen_like(name, V, d, 0.05, R, None, 0.9, seed, "uniform", W_bits=w0.W_bits,
+                                                   N_alloc=n_alloc, var_len=var_len)
+    ws = [w0, mk("stress-flex-half", 72, (1, 8)), mk("stress-flex-few", 73, (0, 2)), mk("stress-flex-most", 74, (4, 8))]
+    devs = [P.to_device(w) for w in ws]
+    tp = B.TauParams(**ws[0].tau_params)
+    ref = []
+    for w, dv in zip(ws, devs):                  # each batch alone, against the oracle
+        pr = B.Probe(n_alloc, d, V, R)
+        assert pr.plan["flex"] == 1
+        out = pr(dv["hidden"], devs[0]["W"], dv["off"], dv["load"], tp)
+        torch.cuda.synchronize()
+        g = P.GpuRun(out.conf.cpu().numpy(), out.argmax.cpu().numpy(), out.exit.cpu().numpy(),
+                     out.tau.cpu().numpy(), out.pmax.cpu().numpy(), pr.plan)
+        ora, rows, reqs = P.run_oracle(w)
+        P.compare(w, g, ora, rows, reqs, w.name)
+        ref.append((out.conf.clone(), out.argmax.clone(), out.exit.clone()))
+    K = 48
+    probes = [B.Probe(n_alloc, d, V, R, debug_outputs=False) for _ in range(K)]
+    for p in probes[1:]:
+        p.workspace = probes[0].workspace
+        p._handles = probes[0]._handles
+    rng = np.random.default_rng(5)
+    for rnd in range(10):
+        order = rng.integers(0, len(ws), size=K)
+        for p in probes:
+            p.conf.fill_(-7.0); p.argmax.fill_(-7); p.exit.fill_(7)
+        torch.cuda.synchronize()
+        for k, p in enumerate(probes):
+            dv = devs[order[k]]
+            p(dv["hidden"], devs[0]["W"], dv["off"], dv["load"], tp)
+        torch.cuda.synchronize()
+        for k, p in enumerate(probes):
+            c, a, e = ref[order[k]]
+            nv = ws[order[k]].N_valid
+            assert torch.equal(p.conf, c) and torch.equal(p.exit, e), (rnd, k, int(order[k]))
+            assert torch.equal(p.argmax, a), (rnd, k, int(order[k]), nv)
+
