@@ -731,3 +731,25 @@ def test_flex_back_to_back_with_changing_row_counts(P):
             assert torch.equal(p.conf, c) and torch.equal(p.exit, e), (rnd, k, int(order[k]))
             assert torch.equal(p.argmax, a), (rnd, k, int(order[k]), nv)
 
+
+@pytest.mark.parametrize("n_valid", [1, 13, 16, 17, 29, 45, 64, 77, 96, 109, 125, 141, 157, 173, 192, 205, 221, 237, 253, 256,
+                                     257, 300, 511, 513, 769, 1000, 1024])
+def test_flex_every_chunk_height(P, force_mode, n_valid):
+    """The flex kernel at every chunk height (16 ... 256 token rows: 16 hidden tensor maps, the 16-token
+    last group of a chunk, one to four chunks) in one 1024-row allocation: n_valid rows in a single request
+    plus empty ones, so that the decomposition comes from req_offsets[R] alone."""
+    from paper_2606_31580_b200 import binding as B
+    force_mode(3)
+    V, d, n_alloc, R = 5000, 64, 1024, 3
+    rng = np.random.default_rng(1000 + n_valid)
+    W_bits = wl.make_W(V, d, 0.05, 4321)                       # one W for the whole sweep
+    hb = np.zeros((n_alloc, d), np.uint16)
+    hb[:n_valid] = wl.bf16_bits(rng.standard_normal((n_valid, d)).astype(np.float32) * 2.0)
+    off = np.array([0, n_valid // 2, n_valid // 2, n_valid], np.int32)    # a request, an empty one, a request
+    w = wl.Workload(f"flex-height-{n_valid}", W_bits, hb, off, rng.random(R).astype(np.float32))
+    f = B.flex_query(n_alloc, d, V, R, n_valid)
+    assert f["chunks"] * f["n_tok"] >= n_valid > (f["chunks"] - 1) * f["n_tok"] - 16 * f["chunks"]
+    st = P.check(w)
+    assert st["plan"]["flex"] == 1 and st["rows"] == n_valid
+    print(w.name, f["chunks"], f["n_tok"], f["splits"], {k: v for k, v in st.items() if k != "plan"})
+
