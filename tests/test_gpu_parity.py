@@ -476,13 +476,20 @@ def test_c2_in_the_configuration_bench_times(P, c2_W_bits):
 
 
 # ------------------------------------------------------------------ semantics fixed at the boundary
-def test_nan_row_poisons_only_its_request(P):
-    w = wl.scaled("nan", 3000, 64, 0.05, 3, 4, seed=11)
-    hf = w.hidden_f32().copy(); hf[5, 7] = np.nan
+@pytest.mark.parametrize("L,mode", [(4, 0), (60, 3), (60, 4), (60, 2)])   # single kernel / flex / mixed / pair
+def test_nan_row_poisons_only_its_request(P, force_mode, L, mode):
+    """DESIGN A12 through every kernel: a NaN in one row makes that row's pmax and its request's conf NaN
+    (exit 0) and leaves the other requests alone."""
+    force_mode(mode)
+    w = wl.scaled("nan", 3000, 64, 0.05, 3, L, seed=11)
+    row = L + 1                                      # a row of request 1
+    hf = w.hidden_f32().copy(); hf[row, 7] = np.nan
     w.hidden_bits = wl.bf16_bits(hf)
     g = P.run_gpu(w)
-    assert np.isnan(g.conf[1]) and g.exit[1] == 0
+    assert g.plan["flex"] == (1 if mode == 3 else 0)
+    assert np.isnan(g.conf[1]) and g.exit[1] == 0 and np.isnan(g.pmax[row])
     assert np.isfinite(g.conf[0]) and np.isfinite(g.conf[2])
+    assert np.isfinite(np.delete(g.pmax, row)).all()
     ora, _, _ = P.run_oracle(w)
     np.testing.assert_allclose(g.conf[[0, 2]], ora.conf[[0, 2]], atol=2e-3)
 
