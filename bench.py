@@ -186,6 +186,7 @@ def roofline_for(w: wl.Workload, us: float, peaks: dict):
 
 # ----------------------------------------------------------------------------------------- GPU arm
 KERNEL_MODES = ["auto", "single", "pair", "flex", "mixed"]     # laser_probe_options.kernel_mode, by value
+W_LAYOUTS = ["rowmajor", "kblocked"]                           # laser_probe_options.w_layout, by value
 SETTLE_S = 0.25
 COOL_S = 1.0
 
@@ -362,7 +363,8 @@ def realised_distribution(w: wl.Workload, case) -> dict:
     confidence band (SURVEY §8 d: polarisation must be visible next to every number)."""
     import torch
     B = case.B
-    probe = B.Probe(w.N_alloc, w.d, w.V, w.R, device=case.hidden.device, debug_outputs=True)
+    probe = B.Probe(w.N_alloc, w.d, w.V, w.R, device=case.hidden.device, debug_outputs=True,
+                    w_layout=case.probe.w_layout)
     out = probe(case.hidden, case.Ws[0], case.off, case.load, case.tp)
     torch.cuda.synchronize()
     nv = w.N_valid
@@ -470,9 +472,12 @@ def run_vocab_sharded(args, dist, rank, local_rank, world, device):
     sampler = ClockSampler(physical_gpu_index(local_rank))
     sampler.start()
     w = wl.by_name(args.workload, {})                    # every rank: the same batch, the same W
-    vp = par.VocabParallelProbe(dist, w.N_alloc, w.d, w.V, w.R, device, exchange=args.exchange)
+    wlay = W_LAYOUTS.index(args.w_layout)
+    vp = par.VocabParallelProbe(dist, w.N_alloc, w.d, w.V, w.R, device, exchange=args.exchange, w_layout=wlay)
     hidden = B.bf16_tensor_from_bits(w.hidden_bits, device)
     Wg = B.bf16_tensor_from_bits(w.W_bits[vp.v0:vp.v1], device)
+    if wlay:
+        Wg = B.pack_w(Wg)                                # once per model: this rank's rows, K-block-major
     off = torch.from_numpy(w.req_offsets).to(device)
     load = torch.from_numpy(w.load).to(device)
     tp = B.TauParams(**w.tau_params)
@@ -527,7 +532,7 @@ def run_vocab_sharded(args, dist, rank, local_rank, world, device):
             warmup=args.warmup, ms_per_step=ms_per_step, higher_is_better=True, scaling="strong", vs_baseline=None,
             dtype="bf16", data="synthetic",
             config=dict(workload=describe(w), sharding=f"vocabulary: {world} row ranges of W, whole batch on every rank",
-                        exchange=args.exchange, shard_rows=vp.v1 - vp.v0, plan=vp.shard.plan,
+                        exchange=args.exchange, w_layout=args.w_layout, shard_rows=vp.v1 - vp.v0, plan=vp.shard.plan,
                         l2="each rank's W shard (%.0f MB)%s" % (shard_bytes / 1e6,
                                                                 " exceeds the 126 MB L2" if shard_bytes > 126e6 else
                                                                 " FITS the 126 MB L2: per-rank figure is L2-assisted")),
@@ -577,9 +582,13 @@ def run_ours(args):
     # the library default: strict stream order for every per-call input (what a serving loop needs
     # behind the forward pass that writes `hidden`).  This is the headline configuration.
     kmode = KERNEL_MODES.index(args.kernel_mode)
+    wlay = W_LAYOUTS.index(args.w_layout)
     case = GpuCase(w, device, two_w_copies=(w.V * w.d * 2 < 2_000_000_000), mode=kmode)
+    if wlay:      # --w-layout kblocked: every timed call gets the packed copies (made here, once, untimed)
+        case = GpuCase(w, device, Ws=[B.pack_w(Wc) for Wc in case.Ws], share=case, mode=kmode, w_layout=wlay)
+        torch.cuda.empty_cache()
     # laser_probe_options.overlap = 1: consecutive calls of a loop over resident inputs overlap
-    over = GpuCase(w, device, Ws=case.Ws, overlap=True, share=case, mode=kmode)
+    over = GpuCase(w, device, Ws=case.Ws, overlap=True, share=case, mode=kmode, w_layout=wlay)
 
     for _ in range(args.warmup):
         case.step()
@@ -620,7 +629,7 @@ def run_ours(args):
     # strict steps and bracketed launches, secondary figure.  Only where W is streamed from HBM once per
     # call and two packed copies fit beside the row-major ones.
     kblocked = None
-    if rank == 0 and w.N_alloc <= 256 and w.V * w.d * 2 < 2_000_000_000:
+    if rank == 0 and wlay == 0 and w.N_alloc <= 256 and w.V * w.d * 2 < 2_000_000_000:
         cool()
         Wp = [B.pack_w(Wc) for Wc in case.Ws]
         kb_case = GpuCase(w, device, Ws=Wp, share=case, mode=kmode, w_layout=B.W_KBLOCKED)
@@ -645,7 +654,7 @@ def run_ours(args):
     # staging/workspace/output set each) so that the H2D copy of batch i+1 overlaps the kernel of batch
     # i, as a serving loop would run it; one batch at a time (synchronous) is timed as well.
     depth = 2
-    slots = [B.HostProbe(w.N_alloc, w.d, w.V, w.R, device=device, mode=kmode) for _ in range(depth)]
+    slots = [B.HostProbe(w.N_alloc, w.d, w.V, w.R, device=device, mode=kmode, w_layout=wlay) for _ in range(depth)]
     streams = [torch.cuda.Stream(device=device) for _ in range(depth)]
     hp = slots[0]
     hh = B.bf16_tensor_from_bits(w.hidden_bits, pin=True)
@@ -768,7 +777,7 @@ def run_ours(args):
                            % (w.V * w.d * 2 / 1e6) if len(case.Ws) > 1 else
                            "W (%.0f MB) exceeds the 126 MB L2" % (w.V * w.d * 2 / 1e6),
                         sharding="requests sharded across ranks, W replicated, no collective" if world > 1 else "single GPU",
-                        e2e_w_resident=True, kernel_mode=args.kernel_mode,
+                        e2e_w_resident=True, kernel_mode=args.kernel_mode, w_layout=args.w_layout,
                         mode="library default: strict stream order (laser_probe_options.overlap = 0), "
                              "merge + a3-a5 in the fused kernel's tail (one launch per call)"),
             overlap=dict(value=rows_all / (overlap_ms / args.steps * 1e-3), unit=UNIT,
@@ -809,7 +818,7 @@ def run_ours(args):
         sweep = []
         for N in wl.C5_NS:
             ws = wl.config_c5(N, W_cache["C2"])
-            c = GpuCase(ws, device, Ws=case.Ws)
+            c = GpuCase(ws, device, Ws=case.Ws, w_layout=wlay)
             k = max(5, min(args.steps, int(2e5 / max(N, 128))))
             cool()
             for _ in range(3):
@@ -830,7 +839,7 @@ def run_ours(args):
     # vocabulary-parallel layout (laser_probe_partial + laser_probe_combine): what ONE rank of G would
     # execute per step - its 1/G slice of W (ONE kernel: reduce and record stores in the fused kernel's
     # tail), then the merge of G records per row.  The exchange itself needs G GPUs (--sharding vocab).
-    if rank == 0 and world == 1 and not args.no_sweep and args.workload == "C2":
+    if rank == 0 and world == 1 and not args.no_sweep and args.workload == "C2" and wlay == 0:
         from paper_2606_31580_b200 import parallel as par
         vp = []
         for G in (2, 4, 8):
@@ -862,7 +871,7 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_sweep and args.workload == "C2":
         out["serving_sim"] = serving_sim_bench(device, with_cpu=not args.no_cpu_baseline)
 
-    if rank == 0 and world == 1 and args.with_cublas:
+    if rank == 0 and world == 1 and args.with_cublas and wlay == 0:
         out["cublas_context"] = cublas_context(w, case, args.steps, physical_gpu_index(local_rank))
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, target_s=10.0)
@@ -960,6 +969,9 @@ def main():
                     help="context only: time the plain cuBLAS GEMM hidden @ W^T of the same shape beside the probe")
     ap.add_argument("--kernel-mode", default="auto", choices=KERNEL_MODES,
                     help="laser_probe_options.kernel_mode (auto = the library default; the others force a variant)")
+    ap.add_argument("--w-layout", default="rowmajor", choices=W_LAYOUTS,
+                    help="rowmajor (default: W as the model stores it) or kblocked (W packed once by "
+                         "laser_probe_pack_w; the timed calls get the packed copy)")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -80,13 +80,15 @@ class VocabParallelProbe:
     (NCCL); exchange="peer" pushes the records from the reduce kernel into every rank's buffer over
     NVLink (PeerExchange: symmetric memory, no collective call on the data path)."""
 
-    def __init__(self, dist, N, d, V, R, device, exchange="collective", group=None, debug_outputs=False):
+    def __init__(self, dist, N, d, V, R, device, exchange="collective", group=None, debug_outputs=False,
+                 w_layout=0):
+        """w_layout = binding.W_KBLOCKED: every call's W_shard is binding.pack_w() of this rank's rows."""
         from . import binding as B
         self.dist, self.group = dist, group
         self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
         self.v0, self.v1 = shard_vocab(V, self.world, self.rank)
         self.shard = B.VocabShardProbe(N, d, self.v1 - self.v0, R, self.v0, self.world, device=device,
-                                       debug_outputs=debug_outputs)
+                                       debug_outputs=debug_outputs, w_layout=w_layout)
         self.exchange = exchange
         self.peers = PeerExchange(dist, N, self.world, self.rank, device, group) if exchange == "peer" else None
 
