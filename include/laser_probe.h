@@ -108,7 +108,9 @@ typedef struct {
 
 /* Kernel variant (laser_probe_options.kernel_mode).  AUTO (default): one single-CTA kernel for
  * N <= 128 rows; the flex kernel (vocabulary on the MMA M axis, token chunks of a multiple of 16 rows on
- * N, decided on the device from req_offsets[R]) for 129..1024 rows except exactly 256; one CTA-pair
+ * N, decided on the device from req_offsets[R]) for 129..1024 rows except exactly 256 (and not where it
+ * measures slower: hidden sizes below 1280 above 384 rows / below 768 at all; vocabularies whose 256-row
+ * tiles would leave the busiest CTA pair more than 15 % above an even share); one CTA-pair
  * kernel for N = 256 (a single 256-row item); above 1024 rows the mixed schedule (CTA pairs for the
  * even part of the 128-row tiles that hold rows, single CTAs for an odd last tile, decided on the
  * device).  SINGLE / PAIR force one variant for every shape (tuning and tests; both are exact; PAIR

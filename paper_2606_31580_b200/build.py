@@ -14,7 +14,7 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 SO = HERE / "liblaser_probe.so"
 SOURCES = [CSRC / "laser_probe.cu", CSRC / "laser_sim.cu"]
-DEPS = SOURCES + [CSRC / "probe_kernels.cuh", CSRC / "ptx.cuh", HERE.parent / "include" / "laser_probe.h",
+DEPS = SOURCES + [CSRC / "probe_kernels.cuh", CSRC / "flex_kernel.cuh", CSRC / "ptx.cuh", HERE.parent / "include" / "laser_probe.h",
                   HERE.parent / "include" / "laser_sim.h"]
 
 NVCC_FLAGS = [

@@ -347,6 +347,12 @@ void make_plan(const laser_probe_dims& dm, int num_sms, int mode, laser_probe_pl
     // C4's 590 of 1024 rows: 456 vs 508 us - and ties at 512 / 768 / 1024; a dense 256-row batch is the
     // one case where its fixed 256-row vocabulary tiles quantise worse than the pair kernel's).
     bool auto_flex = mode == LASER_MODE_AUTO && dm.N > kTileM && dm.N <= 1024 && dm.N != 2 * kTileM;
+    // Narrow hidden sizes: a tile's MMAs shrink with d, its epilogue does not, and the flex epilogue is ~30 %
+    // heavier (the 32 x 32 transposes).  Measured at V = 151936 (flex vs mixed, strict step): d = 1024 N = 320
+    // 96 vs 103 us but N = 512 132 vs 121; d = 512 N = 320 72 vs 59.  Below d = 1280 AUTO takes the flex
+    // kernel only where the mixed schedule pays for padding tiles (N <= 384), below d = 768 not at all.
+    const int kb_d = ceil_div(dm.d, kBlockK);
+    if (auto_flex && (kb_d < 12 || (kb_d < 20 && dm.N > 384))) auto_flex = false;
     if (auto_flex) {
         // The flex kernel's vocabulary tiles are 256 rows whatever V is: with few tiles per pair (a small
         // vocabulary, a vocabulary shard) whole-tile quantisation can leave the busiest pair far above the

@@ -67,7 +67,7 @@ def _compare_token_mode(P, w, g, ora, pt, conf, ex, margin, label):
 @pytest.mark.parametrize("agg", [0, 1])
 @pytest.mark.parametrize("V,d,R,L,n_alloc,var_len,mode", [
     (33000, 512, 12, 8, None, None, 0),       # one token tile, several vocabulary tiles, ragged V
-    (9000, 256, 40, None, 400, (1, 16), 0),   # several token chunks (flex kernel), padding rows
+    (9000, 256, 40, None, 400, (1, 16), 3),   # several token chunks (flex kernel), padding rows
     (9000, 256, 40, None, 400, (1, 16), 4),   # the same through the mixed schedule (pair + single-CTA kernels)
     (9000, 256, 40, None, 400, (1, 16), 2),   # ... and the pair kernel alone
     (1000, 64, 8, 4, None, None, 0),          # C1 shape
@@ -82,7 +82,7 @@ def test_token_prob_mode(P, V, d, R, L, n_alloc, var_len, mode, agg):
     pt, conf, ex, margin = _oracle_token_mode(w, ora, tok, agg)
     dev = P.to_device(w)
     probe = B.Probe(w.N_alloc, w.d, w.V, w.R, mode=mode)
-    assert probe.plan["flex"] == (1 if (mode == 0 and w.N_alloc > 128) else 0)
+    assert probe.plan["flex"] == (1 if mode == 3 else 0)
     probe.conf.fill_(-7.0); probe.argmax.fill_(-7); probe.exit.fill_(7); probe.pmax.fill_(-7.0)
     out = probe(dev["hidden"], dev["W"], dev["off"], dev["load"], B.TauParams(**w.tau_params), agg=agg,
                 token_ids=torch.from_numpy(tok).cuda())
@@ -186,7 +186,7 @@ def _run_vocab_parallel(P, w, G, tok=None, agg=0, peer=False, tail=0, mode=0):
 @pytest.mark.parametrize("G", [1, 2, 3, 8])
 @pytest.mark.parametrize("V,d,R,L,n_alloc,var_len,mode", [
     (33000, 512, 12, 8, None, None, 0),
-    (9001, 256, 40, None, 400, (1, 16), 0),  # V not divisible by G, several token chunks, padding rows: the flex kernel
+    (9001, 256, 40, None, 400, (1, 16), 3),  # V not divisible by G, several token chunks, padding rows: the flex kernel
     (9001, 256, 40, None, 400, (1, 16), 4),  # the same through the mixed schedule (two fused kernels per partial)
 ])
 def test_vocab_parallel_matches_oracle(P, G, peer, tail, V, d, R, L, n_alloc, var_len, mode):
@@ -194,8 +194,9 @@ def test_vocab_parallel_matches_oracle(P, G, peer, tail, V, d, R, L, n_alloc, va
     w = wl.scaled(f"vp-V{V}-G{G}", V, d, 0.05, R, L, seed=88, N_alloc=n_alloc, var_len=var_len)
     n0 = B.kernel_launch_count()
     g, stats = _run_vocab_parallel(P, w, G, peer=peer, tail=tail, mode=mode)
-    mixed = B.plan_query(w.N_alloc, d, par.shard_vocab(V, G, 0)[1], R, mode=mode)["mixed"]
-    assert mixed == (1 if mode == 4 else 0)
+    pl = B.plan_query(w.N_alloc, d, par.shard_vocab(V, G, 0)[1], R, mode=mode)
+    mixed = pl["mixed"]
+    assert mixed == (1 if mode == 4 else 0) and pl["flex"] == (1 if mode == 3 else 0)
     fused = 2 if mixed else 1                                           # fused kernels of one partial
     per_partial = fused if tail == 0 else fused + (2 if peer else 1)    # the tail also runs in the mixed schedule's kernels
     assert B.kernel_launch_count() - n0 == G * per_partial + 1          # + the combine kernel
