@@ -347,25 +347,31 @@ def test_ties_in_flex_mode(P, force_mode):
 
 
 # ------------------------------------------------------------------ closed forms on the GPU
-def test_uniform_logits_gpu(P):
+@pytest.mark.parametrize("R,mode", [(4, 0), (40, 3), (40, 4)])      # single kernel / flex (N = 320) / mixed
+def test_uniform_logits_gpu(P, force_mode, R, mode):
     """P1 on the device: hidden = 0 -> pmax = 1/V, argmax 0 (lowest index), conf = 1/V."""
-    w = wl.scaled("uniform", 40000, 256, 0.05, 4, 8, seed=5)
+    force_mode(mode)
+    w = wl.scaled("uniform", 40000, 256, 0.05, R, 8, seed=5)
     w.hidden_bits[:] = 0
     g = P.run_gpu(w)
+    assert g.plan["flex"] == (1 if mode == 3 else 0)
     assert np.all(g.argmax == 0)
     np.testing.assert_allclose(g.pmax, 1.0 / w.V, rtol=2e-5)
     np.testing.assert_allclose(g.conf, 1.0 / w.V, rtol=2e-5)
     assert np.all(g.exit == 0)
 
 
-def test_one_hot_confidence_one(P):
+@pytest.mark.parametrize("reps,mode", [(1, 0), (20, 3), (20, 4)])    # N = 8: single kernel; N = 160: flex / mixed
+def test_one_hot_confidence_one(P, force_mode, reps, mode):
     """P2 on the device: W = 40*I, hidden = e_j -> conf = 1 (to fp32), argmax = j, exit."""
+    force_mode(mode)
     V = d = 256
     W = wl.bf16_bits((40.0 * np.eye(V)).astype(np.float32))
-    js = np.array([0, 17, 255, 128, 127, 31, 32, 200])
+    js = np.tile(np.array([0, 17, 255, 128, 127, 31, 32, 200]), reps)
     w = wl.Workload("onehot", W, wl.bf16_bits(np.eye(V, dtype=np.float32)[js]),
-                    wl.fixed_offsets(2, 4), np.array([0.0, 1.0], np.float32))
+                    wl.fixed_offsets(2 * reps, 4), np.tile(np.array([0.0, 1.0], np.float32), reps))
     g = P.run_gpu(w)
+    assert g.plan["flex"] == (1 if mode == 3 else 0)
     assert np.array_equal(g.argmax, js)
     np.testing.assert_allclose(g.conf, 1.0, atol=1e-6)
     assert np.all(g.exit == 1)
