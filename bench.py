@@ -832,7 +832,9 @@ def run_ours(args):
                               frac=r["frac"], frac_of_nominal=r["frac_of_nominal"],
                               frac_vs_sustained_peak=r.get("frac_vs_sustained_peak"),
                               frac_step=roofline_for(ws, t_ms * 1e3, peaks)["frac"],
-                              pair=c.probe.plan["cta_pair"], tile_n=c.probe.plan["tile_n"]))
+                              pair=c.probe.plan["cta_pair"], tile_n=c.probe.plan["tile_n"],
+                              kernel="flex" if c.probe.plan["flex"] else ("mixed" if c.probe.plan["mixed"] else
+                                                                          ("pair" if c.probe.plan["cta_pair"] else "single"))))
             del c
         out["roofline"]["sweep"] = sweep
 
