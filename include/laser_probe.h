@@ -44,7 +44,9 @@ enum {
     LASER_E_WORKSPACE = -5, /* workspace NULL or smaller than laser_probe_workspace_bytes()           */
     LASER_E_ARCH = -6,      /* current device is not compute capability 10.0 (B200)                   */
     LASER_E_CUDA = -7,      /* a CUDA runtime / driver call failed; see laser_last_error()            */
-    LASER_E_MODE = -8       /* unknown aggregate / probability / kernel mode                          */
+    LASER_E_MODE = -8,      /* unknown aggregate / probability / kernel mode                          */
+    LASER_E_STATIC_LIMIT = -9 /* laser_probe_confidence_static: the batch needs more scratch than the
+                                 built-in LASER_STATIC_SCRATCH_BYTES array holds                       */
 };
 
 /* Hyper-parameters of Eq. 5; defaults are the paper's.  `l_target` and load[] share
@@ -283,6 +285,59 @@ int laser_probe_confidence_opt(const void* hidden, const void* W, const int32_t*
                                const laser_probe_dims* dims, void* workspace,
                                size_t workspace_bytes, void* stream, float* out_tau_opt,
                                float* out_pmax_opt, const laser_probe_options* options);
+
+/*
+ * The probe for callers that cannot allocate device memory.
+ *
+ * Who this is for.  Every other entry point needs a device `workspace` from the caller, and the
+ * default tail additionally makes the library cudaMalloc its per-device control block on first use.
+ * Some callers can do neither: a plug-in that runs inside an inference engine whose memory pool
+ * owns the whole GPU (a cudaMalloc there fails or fragments the pool, and the pool's allocator is not
+ * reachable from C), a process started with nearly all of the GPU's memory already reserved by its
+ * host application, or a latency-critical serving loop that must not take the driver's allocation
+ * lock (cudaMalloc / cudaFree serialise against every other thread's CUDA calls and may synchronise
+ * the device).  Such a caller has its inputs and outputs - the engine gave it those - and nothing
+ * else.
+ *
+ * What it does.  Same a1-a5 as laser_probe_confidence, same kernels, same results.  The only scratch
+ * the path needs - the 16-byte per-row statistics records the vocabulary splits hand to the merge -
+ * goes to a fixed array of LASER_STATIC_SCRATCH_BYTES that is part of the library's device image
+ * instead of a caller workspace, and merge + a3-a5 run as the second small kernel
+ * (LASER_TAIL_SEPARATE), which needs no control block.  The call makes no cudaMalloc / cudaFree /
+ * cudaMemset / cudaMemcpy and calls no library routine that allocates device memory; it enqueues its
+ * kernels on `stream` and returns.
+ *
+ * Limit.  The array is LASER_STATIC_SCRATCH_BYTES (4 MiB) per GPU, resident on every GPU the library's
+ * device code is loaded on from that load until the process exits, used or not.  A batch is accepted
+ * iff laser_probe_workspace_bytes(dims) <= LASER_STATIC_SCRATCH_BYTES (checkable ahead of time, on the
+ * host, without a GPU): at the paper's model shapes that is every batch up to about 1024 rows
+ * (C4: 2.5 MB); 4096 rows at V = 151936 need 13.6 MB and are refused with LASER_E_STATIC_LIMIT
+ * (laser_last_error() names both numbers).  Nothing is launched in that case.  Larger batches need
+ * laser_probe_confidence with a workspace.
+ *
+ * First call on a device.  It looks the array's device address up (cudaGetSymbolAddress, once per
+ * device, with that device current; this may make the CUDA runtime load the library's device code,
+ * which is the runtime's allocation, not a call of ours), raises the kernels' shared-memory limit
+ * and encodes the TMA descriptors.  Make that first call ahead of any stream capture, on every
+ * device you will use; later calls with the same dims only launch.
+ *
+ * Sharing.  There is ONE array per GPU and every call on that GPU uses it.  Nothing in it has to start
+ * at zero and nothing is cleared: a call writes every record it later reads, and what the previous
+ * call left behind is never looked at.  But two calls whose kernels can be on the GPU at the same time
+ * - different streams, or different threads, on one device - overwrite each other's records and return
+ * wrong results without any error.  Keep all calls of this entry point on one device in ONE stream
+ * order (one stream, or streams joined by events); calls with a caller workspace are not affected.
+ *
+ * Arguments: as laser_probe_confidence without workspace / workspace_bytes; options NULL = defaults.
+ * options->tail is ignored (always SEPARATE); kernel_mode, overlap, aggregate, token_ids, w_layout
+ * apply as usual.
+ */
+#define LASER_STATIC_SCRATCH_BYTES (4u << 20)
+int laser_probe_confidence_static(const void* hidden, const void* W, const int32_t* req_offsets,
+                                  const float* load, const laser_tau_params* tau_params,
+                                  float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+                                  const laser_probe_dims* dims, void* stream, float* out_tau_opt,
+                                  float* out_pmax_opt, const laser_probe_options* options);
 
 /*
  * Probe handles.  A handle fixes dims and options once and caches what does not change between

@@ -31,7 +31,7 @@ EXPORTS = [
     "laser_probe_mixed_query", "laser_probe_flex_query", "laser_probe_packed_w_bytes", "laser_probe_pack_w",
     "laser_probe_handle_create", "laser_probe_handle_destroy", "laser_probe_handle_plan",
     "laser_probe_handle_workspace_bytes", "laser_probe_handle_run", "laser_probe_handle_run_host",
-    "laser_sim_policy_default", "laser_sim_run",
+    "laser_sim_policy_default", "laser_sim_run", "laser_probe_confidence_static",
 ]
 
 
@@ -163,6 +163,8 @@ def lib():
         L.laser_probe_confidence.argtypes = common
         L.laser_probe_confidence_agg.argtypes = common + [C.c_int]
         L.laser_probe_confidence_opt.argtypes = common + [C.POINTER(Options)]
+        L.laser_probe_confidence_static.argtypes = [vp, vp, i32p, fp, tp, fp, i32p, u8p, dp, vp, fp, fp,
+                                                    C.POINTER(Options)]
         L.laser_probe_partial.argtypes = [vp, vp, i32p, i32p, dp, C.c_int32, vp, C.POINTER(Peers), vp,
                                           C.c_size_t, vp, C.POINTER(Options)]
         L.laser_probe_combine.argtypes = [vp, C.c_int32, i32p, fp, tp, fp, i32p, u8p, dp, vp, fp, fp,
@@ -191,7 +193,7 @@ def _check(rc):
     if rc != 0:
         L = lib()
         txt = L.laser_status_string(rc).decode()
-        if rc == -7:
+        if rc in (-7, -9):
             txt += " — " + L.laser_last_error().decode()
         raise LaserError(rc, txt)
 
@@ -396,6 +398,44 @@ class Probe:
         for h in self._handles.values():
             h.close()
         self._handles = {}
+
+
+STATIC_SCRATCH_BYTES = 4 << 20     # LASER_STATIC_SCRATCH_BYTES
+
+
+def probe_static(hidden, W, req_offsets, load, params: TauParams, out_conf, out_argmax, out_exit,
+                 stream=None, out_tau=None, out_pmax=None, options: Options | None = None):
+    """laser_probe_confidence_static: the probe for callers that have their input and output tensors
+    and nothing else - no device workspace to pass and no way to allocate one (a plug-in inside an engine
+    whose memory pool owns the GPU, a serving loop that must stay off the driver's allocation lock).
+
+    The statistics records go to a 4 MiB array built into the library (STATIC_SCRATCH_BYTES per GPU,
+    held until the process exits); a batch whose workspace_bytes(N, d, V, R) is larger raises LaserError
+    with status -9 and launches nothing.  This wrapper allocates nothing either: every tensor, outputs
+    included, is the caller's.  All calls on one GPU share that array - keep them in one stream order,
+    calls that overlap on the GPU corrupt each other silently.  The first call on a device sets the
+    array's address up; make it before any stream capture.  Asynchronous on `stream`."""
+    import torch
+    assert hidden.is_cuda and hidden.dtype == torch.bfloat16 and hidden.dim() == 2 and hidden.is_contiguous()
+    assert W.dtype == torch.bfloat16 and W.is_contiguous()
+    N, d = hidden.shape
+    R = load.numel()
+    w_layout = options.w_layout if options is not None else W_ROWMAJOR
+    V = W.shape[0] if w_layout == W_ROWMAJOR else W.numel() // (64 * ((d + 63) // 64))
+    assert req_offsets.dtype == torch.int32 and req_offsets.numel() == R + 1
+    assert load.dtype == torch.float32
+    assert out_conf.dtype == torch.float32 and out_conf.numel() == R
+    assert out_argmax.dtype == torch.int32 and out_argmax.numel() == N
+    assert out_exit.dtype == torch.uint8 and out_exit.numel() == R
+    assert out_tau is None or (out_tau.dtype == torch.float32 and out_tau.numel() == R)
+    assert out_pmax is None or (out_pmax.dtype == torch.float32 and out_pmax.numel() == N)
+    s = (stream or torch.cuda.current_stream(hidden.device)).cuda_stream
+    _check(lib().laser_probe_confidence_static(
+        hidden.data_ptr(), W.data_ptr(), req_offsets.data_ptr(), load.data_ptr(), C.byref(params),
+        out_conf.data_ptr(), out_argmax.data_ptr(), out_exit.data_ptr(), C.byref(Dims(N, d, V, R)), s,
+        out_tau.data_ptr() if out_tau is not None else None,
+        out_pmax.data_ptr() if out_pmax is not None else None,
+        C.byref(options) if options is not None else None))
 
 
 class VocabShardProbe:

@@ -1190,6 +1190,46 @@ int implicit_handle(const laser_probe_dims& dims, const laser_probe_options& opt
 
 }  // namespace
 
+// ============================================================================================ static scratch
+// Scratch of laser_probe_confidence_static (include/laser_probe.h): the per-row statistics records of
+// the vocabulary splits, for callers that have no device workspace to give and cannot allocate one.
+// Part of the device image: each GPU that loads this library's device code holds these bytes until the
+// process exits.  In HOST code the name below is only a handle for the runtime's symbol table, not a
+// device address - a kernel handed `laser_static_scratch` itself would fault (or, where the GPU can
+// reach host memory, scribble over the wrong bytes).  static_scratch_ptr() asks the runtime for the
+// array's address on the current device, once per device, and that address is what the kernels get.
+static __device__ __align__(256) unsigned char laser_static_scratch[LASER_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+std::mutex g_static_mu;
+void* g_static_ptr[64] = {};       // device address of laser_static_scratch, per device ordinal
+
+// Device address of the array on the CURRENT device (looked up on the first call per device, which
+// should therefore be made outside any stream capture), or nullptr with g_last_error set.
+void* static_scratch_ptr() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+        (void)cudaGetLastError();
+        g_last_error = "laser_probe_confidence_static: no current CUDA device";
+        return nullptr;
+    }
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, laser_static_scratch);
+        if (e != cudaSuccess || !p) {
+            (void)cudaGetLastError();
+            g_last_error = std::string("cudaGetSymbolAddress(laser_static_scratch): ") + cudaGetErrorString(e);
+            return nullptr;
+        }
+        g_static_ptr[dev] = p;
+    }
+    return g_static_ptr[dev];
+}
+
+}  // namespace
+
 // ============================================================================================ ABI
 extern "C" {
 
@@ -1400,6 +1440,54 @@ int laser_probe_confidence(const void* hidden, const void* W, const int32_t* req
                                       out_pmax_opt, nullptr);
 }
 
+// ------------------------------------------------------------------------------ no device allocation
+// laser_probe_confidence_opt with the library's static array as the workspace and the separate tail (no
+// control block).  Between entry and return: no cudaMalloc / cudaFree / memset / memcpy; host-side `new`
+// of the implicit handle on the first call per (dims, options) only.
+int laser_probe_confidence_static(const void* hidden, const void* W, const int32_t* req_offsets,
+                                  const float* load, const laser_tau_params* tau_params,
+                                  float* out_conf, int32_t* out_argmax, uint8_t* out_exit,
+                                  const laser_probe_dims* dims, void* stream_v, float* out_tau_opt,
+                                  float* out_pmax_opt, const laser_probe_options* options) {
+    if (!dims || !tau_params) return LASER_E_NULL;
+    if (!dims_valid(dims)) return LASER_E_DIMS;
+    if (!params_valid(tau_params)) return LASER_E_PARAMS;
+    laser_probe_options opt = options ? *options : kDefaultOptions;
+    int rc = options_valid(opt);
+    if (rc != LASER_OK) return rc;
+    opt.tail = LASER_TAIL_SEPARATE;        // the fused tail needs the cudaMalloc'ed control block
+    const int N = dims->N, R = dims->R;
+    if (opt.prob_mode == LASER_PROB_TOKEN && N > 0 && !opt.token_ids) return LASER_E_NULL;
+    if (N == 0 && R == 0) return LASER_OK;
+    if (N > 0 && (!hidden || !W || !out_argmax)) return LASER_E_NULL;
+    if (R > 0 && (!req_offsets || !load || !out_conf || !out_exit)) return LASER_E_NULL;
+    if ((reinterpret_cast<uintptr_t>(hidden) & 15) || (reinterpret_cast<uintptr_t>(W) & 15))
+        return LASER_E_ALIGN;
+    // the documented rule: what laser_probe_workspace_bytes says (any kernel_mode) must fit the array
+    const size_t need = laser_probe_workspace_bytes(dims);
+    if (need == 0) return LASER_E_DIMS;
+    if (need > static_cast<size_t>(LASER_STATIC_SCRATCH_BYTES)) {
+        char buf[256];
+        snprintf(buf, sizeof buf,
+                 "laser_probe_confidence_static: N=%d d=%d V=%d R=%d needs %zu bytes of scratch, the built-in "
+                 "array holds %u (LASER_STATIC_SCRATCH_BYTES); use laser_probe_confidence with a workspace",
+                 dims->N, dims->d, dims->V, dims->R, need, static_cast<unsigned>(LASER_STATIC_SCRATCH_BYTES));
+        g_last_error = buf;
+        return LASER_E_STATIC_LIMIT;
+    }
+    DeviceInfo* di = nullptr;
+    rc = require_b200(&di);
+    if (rc != LASER_OK) return rc;
+    void* scratch = static_scratch_ptr();
+    if (!scratch) return LASER_E_CUDA;
+    Handle* h = nullptr;
+    rc = implicit_handle(*dims, opt, scratch, &h);
+    if (rc != LASER_OK) return rc;
+    return run_probe(h, hidden, W, req_offsets, load, tau_params, out_conf, out_argmax, out_exit, scratch,
+                     static_cast<size_t>(LASER_STATIC_SCRATCH_BYTES), stream_v, out_tau_opt, out_pmax_opt,
+                     opt.token_ids);
+}
+
 // ------------------------------------------------------------------------------ vocabulary-parallel
 int laser_probe_partial(const void* hidden, const void* W_shard, const int32_t* req_offsets,
                         const int32_t* token_ids_opt, const laser_probe_dims* dims, int32_t v_offset,
@@ -1568,6 +1656,8 @@ const char* laser_status_string(int status) {
         case LASER_E_ARCH: return "device is not sm_100 (B200); this library has no fallback path";
         case LASER_E_CUDA: return "CUDA call failed (see laser_last_error)";
         case LASER_E_MODE: return "unknown aggregate / probability / kernel / tail mode or option";
+        case LASER_E_STATIC_LIMIT:
+            return "batch needs more scratch than the library's built-in array holds (see laser_last_error)";
         default: return "unknown status";
     }
 }

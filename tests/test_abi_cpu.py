@@ -214,7 +214,7 @@ def test_argument_validation_needs_no_gpu():
     bad = list(args(B.Dims(32, 64, 1000, 8))); bad[0] = None
     assert L.laser_probe_confidence_agg(*bad) == -1                                     # LASER_E_NULL
     assert L.laser_probe_confidence_agg(*args(B.Dims(32, 64, 1000, 8))[:0], *[a + 2] + list(args(B.Dims(32, 64, 1000, 8)))[1:]) == -3
-    for code in range(-8, 1):
+    for code in range(-9, 1):
         assert L.laser_status_string(code)
 
 
