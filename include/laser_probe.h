@@ -122,15 +122,21 @@ enum { LASER_MODE_AUTO = 0, LASER_MODE_SINGLE = 1, LASER_MODE_PAIR = 2, LASER_MO
 
 /* Where merge + a3-a5 run (laser_probe_options.tail).
  *   FUSED     in the tail of the fused kernel: every CTA counts itself in when its records are in the
- *             workspace, the last min(grid, R) CTAs to arrive wait for the count and share the
+ *             workspace, the last min(grid, R, 32) CTAs to arrive wait for the count and share the
  *             requests.  One launch per call (mixed schedule: its two fused kernels; the tail runs in
  *             the one that has the work, in the pair kernel when both have).  Needs a control slot of
- *             the library's per-device control block.
- *   SEPARATE  one more kernel (laser_probe_finalize_kernel) behind the fused one(s).
- *   AUTO      FUSED for strict calls when a control slot is available (the only case where none is:
- *             the very first call on a device is made under CUDA stream capture, where nothing can
- *             be allocated); SEPARATE for overlap = 1 calls (measured faster there: the tiny second
- *             kernel runs beside the next call's CTAs instead of holding their SMs). */
+ *             the library's per-device control block.  The waiting CTAs hold their SMs; with at most
+ *             32 of them per call, up to FOUR fused-tail calls may be in flight on one device at the
+ *             same time (different streams) and the CTAs they wait for always find a free SM.  Callers
+ *             that run more probe calls than that concurrently, or beside other kernels that pin most
+ *             of the SMs, use SEPARATE (a call that does starve traps after ~4 s rather than hang).
+ *   SEPARATE  one more kernel (laser_probe_finalize_kernel) behind the fused one(s).  Nothing waits.
+ *   AUTO      FUSED for strict calls of at most 64 requests when a control slot is available (the only
+ *             case where none is: the very first call on a device is made under CUDA stream capture,
+ *             where nothing can be allocated); SEPARATE for more requests (32 finalizers would take
+ *             them several apiece; a block per request is faster) and for overlap = 1 calls (measured
+ *             faster there: the tiny second kernel runs beside the next call's CTAs instead of holding
+ *             their SMs). */
 enum { LASER_TAIL_AUTO = 0, LASER_TAIL_FUSED = 1, LASER_TAIL_SEPARATE = 2 };
 
 /* Ordering against the kernel ahead of the call on the stream (laser_probe_options.overlap).  The
@@ -141,7 +147,8 @@ enum { LASER_TAIL_AUTO = 0, LASER_TAIL_FUSED = 1, LASER_TAIL_SEPARATE = 2 };
  *    writes `hidden` (Algorithm 1).  W IS READ EARLIER: it is the model's LM-head
  *    weight, and the call requires that the kernel ahead of it on the stream does not write W.  The
  *    kernel requests the first W tiles of every CTA ahead of the wait, so the head of the W stream
- *    overlaps the tail of the preceding kernel.
+ *    overlaps the tail of the preceding kernel.  laser_probe_options.w_ordered = 1 turns this off for
+ *    callers whose W is written on the stream (then W too is read after the wait).
  * 1 (overlap): every input may be read while the kernel ahead is still running; only the kernel's
  *    stores (workspace, outputs) wait for it.  Exact whenever hidden, W, req_offsets, load are
  *    complete when the preceding kernel STARTS - true for a loop of probe calls over resident
@@ -222,6 +229,10 @@ int laser_probe_flex_query(const laser_probe_dims* dims, int32_t n_valid, laser_
  *                precondition: the library never reads device data on the host.  With the
  *                environment variable LASER_DEBUG=1 a one-warp kernel checks it on the device ahead
  *                of every call and traps on a violation - the call then surfaces as a CUDA error).
+ *                Two more debugging switches are read from the environment, once per process:
+ *                LASER_NO_PDL=1 launches every kernel without programmatic dependent launch (full
+ *                stream order, slower), LASER_NO_STAGE_KERNEL=1 makes the *_host entry points copy
+ *                `hidden` with cudaMemcpyAsync instead of their staging kernel.  Same results.
  *                Rows >= req_offsets[R] are padding.
  *   load         device, float [R]: smoothed load Lbar of each request's probe point, unit of l_target.
  *   tau_params   HOST pointer; copied by value into the launch.
@@ -273,6 +284,15 @@ typedef struct {
     int32_t overlap;           /* 0 strict (default) / 1 overlap, see above                          */
     int32_t tail;              /* LASER_TAIL_*                                                       */
     int32_t w_layout;          /* LASER_W_*: how the buffer passed as W is laid out (default row-major) */
+    int32_t w_ordered;         /* 0 (default): strict calls read W AHEAD of the kernel ahead's completion (see
+                                  `overlap` above) - right for resident weights.  1: W is read in stream order
+                                  like every other input.  Set it when W is PRODUCED on the stream just ahead of
+                                  the call by a kernel that lets its dependents start early (a dequantise / cast /
+                                  LoRA-merge kernel launched with programmatic dependent launch, a weight swap):
+                                  such a W would otherwise be read stale, silently.  Costs the overlap of the head
+                                  of the W stream with the preceding kernel's tail (a few us per call).  Applies to
+                                  laser_probe_partial's W_shard as well.  laser_probe_pack_w is an ordinary launch:
+                                  it reads W in stream order and its output is complete before the next kernel. */
 } laser_probe_options;
 int laser_probe_options_default(laser_probe_options* out);
 
@@ -348,9 +368,20 @@ int laser_probe_confidence_static(const void* hidden, const void* W, const int32
  * above use implicit handles from a small per-thread cache keyed by (device, dims, options,
  * workspace).
  *
- * Thread safety: any number of handles may be used concurrently; ONE handle must be used by one
+ * Thread safety: any number of handles may be used concurrently from any number of threads and
+ * streams with LASER_TAIL_SEPARATE, and up to four calls in flight at once per device with the fused
+ * tail (see LASER_TAIL_FUSED above: its finalizer CTAs wait on the GPU); ONE handle must be used by one
  * thread at a time, and the calls made through it must be stream-ordered with respect to each other
  * (they share the handle's control slot, like calls that share a workspace).
+ *
+ * Lifetime: a handle - explicit, or the implicit one behind a handle-less call - owns a control slot
+ * whose address is baked into the launches made through it.  Destroy a handle (and call laser_shutdown,
+ * which drops the implicit ones) only after the work enqueued through it has completed, and keep it
+ * alive as long as a CUDA graph captured through it may be replayed: the slot goes back to a free list
+ * and a later handle may be given it.  Implicit handles are keyed by (device, dims, options, workspace),
+ * 16 per thread, least recently used evicted: a serving loop whose N or R change from step to step
+ * should hold explicit handles of the capacity (N_alloc, R_max) instead - padding rows and empty
+ * requests cost nothing - rather than churn implicit ones.
  *
  * laser_probe_handle_create   host; the current device must be a B200 (else LASER_E_ARCH).  options
  *                             NULL = defaults; options->token_ids (LASER_PROB_TOKEN) is remembered.
@@ -513,8 +544,11 @@ const char* laser_status_string(int status);
 const char* laser_last_error(void);
 /* Number of kernels this library has enqueued since load (all threads). */
 uint64_t laser_kernel_launch_count(void);
-/* Drops the implicit handles (each thread frees its own at its next call).  Explicit handles are the
- * caller's to destroy.  The control block stays until process exit. */
+/* Drops the implicit handles (the calling thread's at once, every other thread's at that thread's next
+ * call) with their cached TMA descriptors, and frees a device's control block once no handle holds a slot
+ * of it any more (explicit handles are the caller's to destroy first).  Call it when the work enqueued
+ * through the library has completed.  The library stays usable: the next call builds what it needs again.
+ * The 4 MiB array of laser_probe_confidence_static is part of the device image and stays. */
 int laser_shutdown(void);
 
 #ifdef __cplusplus

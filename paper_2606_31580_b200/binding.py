@@ -11,7 +11,10 @@ import ctypes as C
 from dataclasses import dataclass
 from pathlib import Path
 
-_SO = Path(__file__).resolve().parent / "liblaser_probe.so"
+import os
+
+# LASER_PROBE_LIB: another build of the SAME library (the -DLASER_TIMELINE debug build, bench.py --timeline)
+_SO = Path(os.environ.get("LASER_PROBE_LIB") or Path(__file__).resolve().parent / "liblaser_probe.so")
 _lib = None
 
 AGG_MEAN, AGG_GEOMEAN, AGG_MIN = 0, 1, 2
@@ -86,11 +89,12 @@ class Options(C.Structure):
     """laser_probe_options (per call: aggregate, probability, kernel variant, overlap, tail)."""
     _fields_ = [("aggregate_mode", C.c_int32), ("prob_mode", C.c_int32), ("token_ids", C.c_void_p),
                 ("kernel_mode", C.c_int32), ("overlap", C.c_int32), ("tail", C.c_int32),
-                ("w_layout", C.c_int32)]
+                ("w_layout", C.c_int32), ("w_ordered", C.c_int32)]
 
     def __init__(self, aggregate_mode=AGG_MEAN, prob_mode=PROB_MAX, token_ids=None, kernel_mode=MODE_AUTO,
-                 overlap=0, tail=TAIL_AUTO, w_layout=0):
-        super().__init__(aggregate_mode, prob_mode, token_ids, kernel_mode, int(bool(overlap)), tail, w_layout)
+                 overlap=0, tail=TAIL_AUTO, w_layout=0, w_ordered=0):
+        super().__init__(aggregate_mode, prob_mode, token_ids, kernel_mode, int(bool(overlap)), tail, w_layout,
+                         int(bool(w_ordered)))
 
 
 MAX_PEERS = 16
@@ -328,12 +332,13 @@ class Probe:
     laser_probe_confidence_opt."""
 
     def __init__(self, N, d, V, R, device="cuda", debug_outputs=True, mode=MODE_AUTO, overlap=False,
-                 tail=TAIL_AUTO, use_handle=True, w_layout=W_ROWMAJOR):
+                 tail=TAIL_AUTO, use_handle=True, w_layout=W_ROWMAJOR, w_ordered=False):
         import torch
         self.torch = torch
         self.dims = Dims(N, d, V, R)
         self.device = torch.device(device)
         self.mode, self.overlap, self.tail, self.use_handle = mode, bool(overlap), tail, use_handle
+        self.w_ordered = bool(w_ordered)   # W is produced on the stream: read it in stream order too
         self.w_layout = w_layout           # W_KBLOCKED: every call's W is a pack_w() copy
         wb = workspace_bytes(N, d, V, R)
         if wb == 0:
@@ -346,15 +351,17 @@ class Probe:
         self.pmax = torch.empty(N, dtype=torch.float32, device=self.device) if debug_outputs else None
         self.plan = plan_query(N, d, V, R, mode)
         fused = 2 if self.plan["mixed"] else 1
-        self.plan["kernel_launches"] = fused + (1 if (tail == TAIL_SEPARATE or (tail == TAIL_AUTO and overlap)) else 0)
+        # TAIL_AUTO: the fused tail for strict calls of up to 64 requests, else the finalize kernel (want_fused_tail)
+        self.plan["kernel_launches"] = fused + (1 if (tail == TAIL_SEPARATE or (tail == TAIL_AUTO and (overlap or R > 64))) else 0)
         self._handles = {}
 
     def _options(self, agg, token_ids) -> Options:
         torch = self.torch
         if token_ids is None:
-            return Options(agg, PROB_MAX, None, self.mode, self.overlap, self.tail, self.w_layout)
+            return Options(agg, PROB_MAX, None, self.mode, self.overlap, self.tail, self.w_layout, self.w_ordered)
         assert token_ids.dtype == torch.int32 and token_ids.numel() == self.dims.N and token_ids.is_contiguous()
-        return Options(agg, PROB_TOKEN, token_ids.data_ptr(), self.mode, self.overlap, self.tail, self.w_layout)
+        return Options(agg, PROB_TOKEN, token_ids.data_ptr(), self.mode, self.overlap, self.tail, self.w_layout,
+                       self.w_ordered)
 
     def __call__(self, hidden, W, req_offsets, load, params: TauParams, stream=None, agg=AGG_MEAN,
                  token_ids=None):
@@ -514,7 +521,7 @@ class HostProbe:
     use_handle=True: laser_probe_handle_run_host; False: laser_probe_confidence_host[_async]."""
 
     def __init__(self, N, d, V, R, device="cuda", use_handle=True, mode=MODE_AUTO, tail=TAIL_AUTO,
-                 w_layout=W_ROWMAJOR):
+                 w_layout=W_ROWMAJOR, overlap=False, w_ordered=False):
         import torch
         self.torch = torch
         self.dims = Dims(N, d, V, R)
@@ -527,7 +534,10 @@ class HostProbe:
         self.h2d_bytes = N * d * 2 + (R + 1) * 4 + R * 4   # upper bound: only valid rows are copied
         self.d2h_bytes = R * 4 + N * 4 + R
         assert use_handle or w_layout == W_ROWMAJOR      # the handle-less host entry points take row-major W
-        self.handle = Handle(self.dims, Options(kernel_mode=mode, tail=tail, w_layout=w_layout)) if use_handle else None
+        assert use_handle or not overlap
+        self.handle = (Handle(self.dims, Options(kernel_mode=mode, tail=tail, w_layout=w_layout, overlap=overlap,
+                                                 w_ordered=w_ordered))
+                       if use_handle else None)
 
     def _call(self, sync, h_hidden, W, h_req_offsets, h_load, params, stream):
         torch = self.torch

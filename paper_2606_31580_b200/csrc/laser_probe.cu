@@ -93,14 +93,35 @@ uint32_t* acquire_ctl(DeviceInfo* di, cudaStream_t stream) {
     std::lock_guard<std::mutex> lk(g_mu);
     if (!di->ctl_base) {
         if (di->ctl_failed) return nullptr;
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
-            (void)cudaGetLastError();
-            return nullptr;   // retried by the next call outside a capture
+        // The caller's stream may be under capture (nothing can be allocated then).  The legacy stream
+        // (nullptr: laser_probe_handle_create, or a caller on the default stream) cannot be captured, and
+        // merely querying it while ANOTHER thread captures in global mode would invalidate that capture.
+        if (stream != nullptr) {
+            cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+            if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+                (void)cudaGetLastError();
+                return nullptr;   // retried by the next call outside a capture
+            }
         }
+        // One-time allocation.  This thread's capture mode is relaxed for its duration, so that the calls
+        // below do not break a capture some other thread has open; the zeroes are on the device before any
+        // kernel of any stream (torch's streams do not synchronise with the legacy stream) can read them.
+        cudaStreamCaptureMode cmode = cudaStreamCaptureModeRelaxed;
+        const bool exchanged = cudaThreadExchangeStreamCaptureMode(&cmode) == cudaSuccess;
         void* p = nullptr;
-        if (cudaMalloc(&p, sizeof(uint32_t) * kCtlWords * kCtlSlots) != cudaSuccess ||
-            cudaMemset(p, 0, sizeof(uint32_t) * kCtlWords * kCtlSlots) != cudaSuccess) {
+        bool ok = cudaMalloc(&p, sizeof(uint32_t) * kCtlWords * kCtlSlots) == cudaSuccess;
+        if (ok) {
+            cudaStream_t zs = nullptr;
+            ok = cudaStreamCreateWithFlags(&zs, cudaStreamNonBlocking) == cudaSuccess;
+            if (ok) {
+                ok = cudaMemsetAsync(p, 0, sizeof(uint32_t) * kCtlWords * kCtlSlots, zs) == cudaSuccess &&
+                     cudaStreamSynchronize(zs) == cudaSuccess;
+                (void)cudaStreamDestroy(zs);
+            }
+            if (!ok) (void)cudaFree(p);
+        }
+        if (exchanged) (void)cudaThreadExchangeStreamCaptureMode(&cmode);
+        if (!ok) {
             (void)cudaGetLastError();
             di->ctl_failed = true;
             return nullptr;
@@ -495,7 +516,7 @@ Staging staging_layout(const laser_probe_dims& d) {
 }
 
 const laser_probe_options kDefaultOptions{LASER_AGG_MEAN, LASER_PROB_MAX, nullptr, LASER_MODE_AUTO, 0,
-                                          LASER_TAIL_AUTO, 0};
+                                          LASER_TAIL_AUTO, 0, 0};
 
 // Everything but token_ids (checked per call: it may be supplied at run time).
 int options_valid(const laser_probe_options& o) {
@@ -505,6 +526,7 @@ int options_valid(const laser_probe_options& o) {
     if (o.tail < LASER_TAIL_AUTO || o.tail > LASER_TAIL_SEPARATE) return LASER_E_MODE;
     if (o.overlap != 0 && o.overlap != 1) return LASER_E_MODE;
     if (o.w_layout != LASER_W_ROWMAJOR && o.w_layout != LASER_W_KBLOCKED) return LASER_E_MODE;
+    if (o.w_ordered != 0 && o.w_ordered != 1) return LASER_E_MODE;
     return LASER_OK;
 }
 
@@ -551,6 +573,10 @@ struct laser_probe_handle_s {
     struct HostMap { const void* h = nullptr; void* d = nullptr; };
     HostMap hm[8];
     int hm_rr = 0;
+    // set by run_host around its probe call: `hidden` is produced on the stream just ahead (the staging
+    // kernel or the H2D copy), so the fused kernel must not read it before that work has completed,
+    // whatever opt.overlap says
+    bool strict_inputs = false;
 };
 
 namespace {
@@ -658,7 +684,8 @@ int launch_fused(Handle* h, int role, const void* hidden, const void* W, const i
     fp.role = role;
     fp.grid_total = h->plan.grid;     // the fused tail exists only where one kernel makes the call
     fp.total_tiles = ceil_div(dims.V, pl.tile_n);
-    fp.wait_first = h->opt.overlap ? 0 : 1;
+    fp.wait_first = (h->opt.overlap && !h->strict_inputs) ? 0 : 1;
+    fp.early_w = (fp.wait_first && !h->opt.w_ordered) ? 1 : 0;   // W ahead of the wait unless it is produced on the stream
     fp.tile_n = pl.tile_n; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
     fp.tail_cache = pl.tail_cache;
     fp.stage_bytes = static_cast<uint32_t>(kABytes + b_rows * 128);
@@ -756,12 +783,13 @@ int launch_flex(Handle* h, const void* hidden, const void* W, const int32_t* req
     fp.role = 0;
     fp.grid_total = pl.grid;
     fp.total_tiles = ceil_div(dims.V, kFlexVocabTile);
-    fp.wait_first = h->opt.overlap ? 0 : 1;
+    fp.wait_first = (h->opt.overlap && !h->strict_inputs) ? 0 : 1;
     fp.tile_n = kFlexVocabTile; fp.k_blocks = pl.k_blocks; fp.stages = pl.stages;
     fp.tail_cache = pl.tail_cache;
     fp.stage_bytes = static_cast<uint32_t>(kABytes + (pl.flex_max_tok / 2) * 128);
     fp.tx_bytes = 0;       // depends on the chunk height: computed in the kernel
     fp.hint_C = pl.m_tiles; fp.hint_S = pl.splits;     // the dense decomposition (see the kernel)
+    if (h->opt.w_ordered) fp.hint_C = 0;               // no guess, no W box ahead of the wait
     // several chunks re-read a W tile from L2 (side by side: chunk-fastest item order)
     fp.w_policy = pl.m_tiles == 1 && dims.N <= kFlexMaxTok ? ptx::kEvictFirst : ptx::kEvictNormal;
     fp.ws = ws;
@@ -867,6 +895,10 @@ int want_fused_tail(Handle* h, cudaStream_t stream, bool* fused_tail) {
     // AUTO with overlap: calls chained two deep gate each other's CTAs; the tail CTAs would hold SMs
     // the next call could be streaming on, so the second kernel (co-resident, tiny) is the faster form
     if (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap) return LASER_OK;
+    // AUTO with many requests: the fused tail has at most kMaxFinalizers CTAs (see fused_tail), each of which
+    // would take R / kMaxFinalizers requests one after the other; beyond two apiece the second kernel - a
+    // block per request, a few microseconds behind kernels of hundreds - is the faster and the simpler form
+    if (h->opt.tail == LASER_TAIL_AUTO && h->dims.R > 2 * kMaxFinalizers) return LASER_OK;
     if (!h->ctl) h->ctl = acquire_ctl(h->di, stream);
     if (h->ctl) { *fused_tail = true; return LASER_OK; }
     if (h->opt.tail == LASER_TAIL_FUSED) {
@@ -1092,11 +1124,15 @@ int run_host(Handle* h, const void* h_hidden, const void* W, const int32_t* h_re
     void* m_arg = N > 0 ? mapped_ptr(h, h_out_argmax) : nullptr;
     const bool zero_copy = (R == 0 || (m_off && m_load && m_conf && m_exit)) && (N == 0 || m_arg);
     int rc;
+    // The staging buffer is written on this stream just ahead of the probe: an overlap = 1 handle must not let
+    // the fused kernel read `hidden` (or the staged offsets / load) before that work has completed.
+    h->strict_inputs = true;
     if (zero_copy) {
         rc = run_probe(h, base + st.hidden, W, static_cast<int32_t*>(m_off), static_cast<float*>(m_load),
                        tau_params, static_cast<float*>(m_conf), static_cast<int32_t*>(m_arg),
                        static_cast<uint8_t*>(m_exit), workspace, workspace_bytes, stream_v, nullptr, nullptr,
                        h->opt.token_ids);
+        h->strict_inputs = false;
         if (rc != LASER_OK) return rc;
     } else {
         if (R > 0) {
@@ -1111,6 +1147,7 @@ int run_host(Handle* h, const void* h_hidden, const void* W, const int32_t* h_re
                        reinterpret_cast<float*>(base + st.conf), reinterpret_cast<int32_t*>(base + st.argmax),
                        base + st.exit_, workspace, workspace_bytes, stream_v, nullptr, nullptr,
                        h->opt.token_ids);
+        h->strict_inputs = false;
         if (rc != LASER_OK) return rc;
         if (R > 0) {
             e = cudaMemcpyAsync(h_out_conf, base + st.conf, static_cast<size_t>(R) * 4, cudaMemcpyDeviceToHost, stream);
@@ -1138,12 +1175,13 @@ int run_host(Handle* h, const void* h_hidden, const void* W, const int32_t* h_re
 struct ImplicitKey {
     int device;
     laser_probe_dims dims;
-    int32_t agg, prob, mode, overlap, tail, w_layout;
+    int32_t agg, prob, mode, overlap, tail, w_layout, w_ordered;
     const void* workspace;
     bool operator==(const ImplicitKey& o) const {
         return device == o.device && dims.N == o.dims.N && dims.d == o.dims.d && dims.V == o.dims.V &&
                dims.R == o.dims.R && agg == o.agg && prob == o.prob && mode == o.mode &&
-               overlap == o.overlap && tail == o.tail && w_layout == o.w_layout && workspace == o.workspace;
+               overlap == o.overlap && tail == o.tail && w_layout == o.w_layout && w_ordered == o.w_ordered &&
+               workspace == o.workspace;
     }
 };
 struct ImplicitCache {
@@ -1169,7 +1207,7 @@ int implicit_handle(const laser_probe_dims& dims, const laser_probe_options& opt
         g_cache_seen = gen;
     }
     const ImplicitKey key{dev, dims, opt.aggregate_mode, opt.prob_mode, opt.kernel_mode, opt.overlap, opt.tail,
-                          opt.w_layout, workspace};
+                          opt.w_layout, opt.w_ordered, workspace};
     for (auto& e : c.entries)
         if (e.key == key) { e.stamp = ++c.clock; *out = e.h; return LASER_OK; }
     Handle* h = nullptr;
@@ -1361,7 +1399,8 @@ int laser_probe_handle_plan(const laser_probe_handle* h, laser_probe_plan* plan)
     *plan = h->plan;
     const int fused = h->plan.mixed ? 2 : 1;    // fused kernels per call
     plan->kernel_launches = (h->opt.tail == LASER_TAIL_SEPARATE || !h->ctl ||
-                             (h->opt.tail == LASER_TAIL_AUTO && h->opt.overlap)) ? fused + 1 : fused;
+                             (h->opt.tail == LASER_TAIL_AUTO && (h->opt.overlap || h->dims.R > 2 * kMaxFinalizers)))
+                                ? fused + 1 : fused;
     return LASER_OK;
 }
 
@@ -1703,8 +1742,22 @@ const char* laser_last_error(void) { return g_last_error.c_str(); }
 uint64_t laser_kernel_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 int laser_shutdown(void) {
-    // implicit handles are per thread: each thread drops its own at its next call
-    g_cache_generation.fetch_add(1, std::memory_order_relaxed);
+    // implicit handles are per thread: this thread's go now, every other thread drops its own at its next call
+    const uint64_t gen = g_cache_generation.fetch_add(1, std::memory_order_relaxed) + 1;
+    for (auto& e : g_implicit.entries) free_handle(e.h);
+    g_implicit.entries.clear();
+    g_cache_seen = gen;
+    // a device's control block is freed once no handle - explicit, or another thread's implicit one - holds a
+    // slot of it (the caller has made sure that the work enqueued through the handles has completed); the next
+    // fused-tail call allocates a new one
+    std::lock_guard<std::mutex> lk(g_mu);
+    for (DeviceInfo& d : g_dev) {
+        if (d.ctl_base && static_cast<int>(d.ctl_free.size()) == kCtlSlots) {
+            if (cudaFree(d.ctl_base) != cudaSuccess) (void)cudaGetLastError();
+            d.ctl_base = nullptr;
+            d.ctl_free.clear();
+        }
+    }
     return LASER_OK;
 }
 

@@ -43,6 +43,7 @@ constexpr int kTmemCols = 512;    // two 256-column accumulators (double buffere
 constexpr int kFusedThreads = 192;  // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-5 epilogue
 constexpr int kEpilogueThreads = 128;
 constexpr int kTailThread0 = 64;    // first epilogue thread: runs the arrival protocol of the tail
+constexpr int kMaxFinalizers = 32;  // CTAs of one call that may wait for the arrival count (fused tail)
 constexpr int kTailCache = 512;     // requests whose offsets / loads a CTA keeps in shared memory for its tail
 constexpr float kLog2e = 1.4426950408889634f;
 
@@ -226,6 +227,7 @@ struct FusedParams {
     int32_t w_kb_rows;
     // W boxes the producer asks L2 for ahead of the wait, behind the `stages` boxes it requests into shared memory
     int32_t prefetch_slots;
+    int32_t early_w;          // 1: W boxes may be requested ahead of griddepcontrol.wait (strict calls whose W is not produced on the stream)
 };
 __device__ __forceinline__ int w_c0(const FusedParams& p, int kb) { return p.w_kb_rows ? 0 : kb * kBlockK; }
 __device__ __forceinline__ int w_c1(const FusedParams& p, int kb, int row) { return row + kb * p.w_kb_rows; }
@@ -684,7 +686,7 @@ __global__ void laser_probe_validate_kernel(const int32_t* req_offsets, int R, i
 // ---------------------------------------------------------------------------------- fused kernel
 // What the tail of the fused kernel does once every CTA's records are in the workspace.
 //   kind 0: nothing (a second kernel follows: LASER_TAIL_SEPARATE)
-//   kind 1: merge + a3-a5 (q.f), CTA b takes requests b, b + F, ... with F = min(grid, R)
+//   kind 1: merge + a3-a5 (q.f), finalizer i takes requests i, i + F, ... with F = min(grid, R, kMaxFinalizers)
 //   kind 2: vocabulary-parallel reduce (q): CTA b takes rows, the last CTA to finish publishes the epoch
 // ctl: four device words owned by the library (never the caller's workspace):
 //   ctl[0] counts CTA arrivals and only ever grows (wrap-safe compares); ctl[1] is the count at which
@@ -752,7 +754,12 @@ __device__ __forceinline__ void fused_tail(const FusedParams& p, const TailParam
     const int tid = threadIdx.x - kTailThread0, tw = tid >> 5;
     constexpr int kTW = kEpilogueThreads / 32;
     const FinalizeParams& f = t.q.f;
-    const int F = (t.kind == 1) ? min(tr.part, f.R) : min(tr.part, (f.n_alloc + kTW - 1) / kTW);
+    // At most kMaxFinalizers CTAs of a call ever spin on the arrival count.  A finalizer holds its SM while
+    // it waits for CTAs that may not be resident yet (grids of other streams can be interleaved with this
+    // one); were every CTA a finalizer, two such calls could each hold part of the SMs and wait for CTAs
+    // that have nowhere to run.  With the cap, 148 - 32 k SMs stay free for the CTAs still to come when k
+    // calls are in their tails at once (include/laser_probe.h: up to four fused-tail calls in flight).
+    const int F = min((t.kind == 1) ? min(tr.part, f.R) : min(tr.part, (f.n_alloc + kTW - 1) / kTW), kMaxFinalizers);
     // scratch: bytes [192, 232) of the barrier block
     volatile uint32_t* tk = reinterpret_cast<volatile uint32_t*>(warp_acc + kMaxTailWarps);
     group_sync<1, kEpilogueThreads>();   // every record store of this CTA is ordered before the count
@@ -902,7 +909,7 @@ laser_probe_fused_kernel(const __grid_constant__ CUtensorMap tmap_hidden,
     // include/laser_probe.h).  The hidden boxes of those slots follow after the wait.
     int pre = 0;
     auto preissue_w = [&]() {
-        if (!(p.wait_first && static_plan && unit < work_items)) return;
+        if (!(p.early_w && static_plan && unit < work_items)) return;
         const uint32_t full0 = kPair ? ptx::mapa(full_bar(0), 0u) : full_bar(0);
         int tile = unit / m_items, kb = 0;
         for (int slot = 0; slot < p.stages + p.prefetch_slots && tile < total_tiles; ++slot) {

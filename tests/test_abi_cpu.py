@@ -167,10 +167,10 @@ def test_forced_modes_plan():
 def test_options_are_per_call_and_validated():
     """kernel variant, overlap and tail travel in laser_probe_options (no process-wide setters)."""
     L = B.lib()
-    o = B.Options(7, 7, None, 7, 1, 7)
+    o = B.Options(7, 7, None, 7, 1, 7, 1, 1)
     assert L.laser_probe_options_default(C.byref(o)) == 0
-    assert (o.aggregate_mode, o.prob_mode, o.token_ids, o.kernel_mode, o.overlap, o.tail, o.w_layout) == \
-        (0, 0, None, 0, 0, 0, 0)
+    assert (o.aggregate_mode, o.prob_mode, o.token_ids, o.kernel_mode, o.overlap, o.tail, o.w_layout, o.w_ordered) == \
+        (0, 0, None, 0, 0, 0, 0, 0)
     assert not hasattr(L, "laser_probe_set_mode") and not hasattr(L, "laser_probe_set_overlap")
     buf = (C.c_char * 4096)()
     a = C.addressof(buf)
@@ -182,6 +182,8 @@ def test_options_are_per_call_and_validated():
     o = B.Options(); o.overlap = 2
     assert call(o) == -8
     o = B.Options(); o.w_layout = 2
+    assert call(o) == -8
+    o = B.Options(); o.w_ordered = 2
     assert call(o) == -8
     assert call(B.Options(prob_mode=B.PROB_TOKEN)) == -1                    # token ids missing
     h = C.c_void_p()

@@ -441,6 +441,44 @@ def test_two_threads_with_different_options(P):
         P.compare(w, g, ora, rows, reqs, name)
 
 
+@pytest.mark.parametrize("n_streams", [2, 3])
+@pytest.mark.parametrize("N,R,mode", [(4096, 512, 0),      # R far above the grid: without the cap every CTA was a finalizer
+                                      (1152, 144, 4)])     # nine 128-row tiles: both kernels of the mixed schedule busy, fixed finalizers
+def test_concurrent_fused_tails_on_several_streams(P, n_streams, N, R, mode):
+    """Fused-tail calls with more requests than the grid has CTAs, issued on two / three streams at once
+    (one of them high priority), 200 calls per stream.  The CTAs of the grids interleave on the SMs; the
+    finalizers of each call (at most 32) spin for CTAs that may not be resident yet, which is safe only
+    while enough SMs stay free for those - the reason for the cap (include/laser_probe.h, thread-safety
+    paragraph).  Every stream's result must equal the one the same handle gives alone, no trap."""
+    import torch
+    from paper_2606_31580_b200 import binding as B
+    w = wl.scaled(f"conc-N{N}", 5000, 64, 0.05, R, N // R, seed=71 + N)
+    dev = P.to_device(w)
+    tp = B.TauParams(**w.tau_params)
+    ora, rows, reqs = P.run_oracle(w)
+    streams = [torch.cuda.Stream(priority=-1 if i == 0 else 0) for i in range(n_streams)]    # -1: high priority
+    probes = [B.Probe(w.N_alloc, w.d, w.V, w.R, tail=B.TAIL_FUSED, mode=mode) for _ in range(n_streams)]
+    assert probes[0].plan["kernel_launches"] == (2 if probes[0].plan["mixed"] else 1)      # fused tail: no finalize kernel
+    # serial reference through the first probe
+    ref = probes[0](dev["hidden"], dev["W"], dev["off"], dev["load"], tp)
+    torch.cuda.synchronize()
+    want = [t.cpu().numpy().copy() for t in (ref.conf, ref.argmax, ref.exit, ref.pmax)]
+    g = P.GpuRun(want[0], want[1], want[2], ref.tau.cpu().numpy(), want[3], probes[0].plan)
+    P.compare(w, g, ora, rows, reqs, w.name)
+    for p in probes:
+        p.conf.fill_(-7.0); p.argmax.fill_(-7); p.exit.fill_(7); p.pmax.fill_(-7.0)
+    torch.cuda.synchronize()
+    for _ in range(200):
+        for p, st in zip(probes, streams):
+            p(dev["hidden"], dev["W"], dev["off"], dev["load"], tp, stream=st)
+    torch.cuda.synchronize()          # a trap (the 4 s watchdog of a starved finalizer) would surface here
+    for i, p in enumerate(probes):
+        got = [t.cpu().numpy() for t in (p.conf, p.argmax, p.exit, p.pmax)]
+        for a, b, name in zip(got, want, ("conf", "argmax", "exit", "pmax")):
+            assert np.array_equal(a, b, equal_nan=(name in ("conf", "pmax"))), f"stream {i}: {name}"
+        p.close()
+
+
 def test_debug_build_checks_req_offsets():
     """LASER_DEBUG=1: a non-monotone req_offsets makes the validation kernel trap (the call surfaces
     as a CUDA error); a valid one passes.  Run in child processes: a trap kills the CUDA context."""
