@@ -1,7 +1,7 @@
 """Build csrc/ -> paper_2606_31580_b200/liblaser_probe.so with nvcc, for sm_100a only.
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box in-tree.
-Usage: python -m paper_2606_31580_b200.build [--force] [--verbose]
+Usage: python -m paper_2606_31580_b200.build [--force] [--verbose] [--timeline]
 """
 from __future__ import annotations
 
@@ -31,12 +31,18 @@ def nvcc_path() -> str:
     return "nvcc"
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
+# Debug build with per-CTA %globaltimer stamps in the fused kernels (-DLASER_TIMELINE): never the shipped
+# library; `bench.py --timeline` loads it through LASER_PROBE_LIB.
+TIMELINE_SO = HERE / "liblaser_probe_timeline.so"
+
+
+def build(force: bool = False, verbose: bool = False, timeline: bool = False) -> Path:
+    SO = TIMELINE_SO if timeline else globals()["SO"]
     newest = max(p.stat().st_mtime for p in DEPS)
     if not force and SO.exists() and SO.stat().st_mtime >= newest:
         return SO
     tmp = SO.with_suffix(f".so.tmp{os.getpid()}")
-    cmd = [nvcc_path(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []),
+    cmd = [nvcc_path(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), *(["-DLASER_TIMELINE"] if timeline else []),
            "-o", str(tmp), *map(str, SOURCES)]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
@@ -48,4 +54,4 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, timeline="--timeline" in sys.argv))
