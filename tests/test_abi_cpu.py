@@ -220,6 +220,16 @@ def test_argument_validation_needs_no_gpu():
         assert L.laser_status_string(code)
 
 
+def test_shutdown_is_idempotent_and_leaves_the_host_side_usable():
+    """laser_shutdown drops cached handles / control blocks (nothing to drop without a GPU) and the
+    library stays usable: the host-side queries answer as before."""
+    L = B.lib()
+    before = B.plan_query(128, 1536, 151936, 16)
+    assert L.laser_shutdown() == 0 and L.laser_shutdown() == 0
+    assert B.plan_query(128, 1536, 151936, 16) == before
+    assert B.workspace_bytes(128, 1536, 151936, 16) > 0
+
+
 def test_no_cpu_fallback():
     """Without a B200 the compute entry point must fail loudly, never compute."""
     import torch
